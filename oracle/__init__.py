@@ -1,0 +1,279 @@
+"""CPU ORACLE for the network-construction hot path of arXiv 2306.09855 -- TEST INFRASTRUCTURE.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and the ``cpu_baseline`` / ``--impl reference`` legs
+of ``bench.py`` may import this package.  It never imports the product package
+(``paper_2306_09855_b200``) and the product never imports it.
+
+``oracle.cpp`` is the oracle itself (plain single-threaded fp64 C++, written from PAPER.md);
+this module only compiles it with g++ and marshals arguments through ctypes.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import math
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_LIB_PATH = _HERE / "liboracle.so"
+
+ONE_TO_ONE, ALL_TO_ALL, FIXED_INDEGREE, FIXED_OUTDEGREE, FIXED_TOTAL_NUMBER, PAIRWISE_BERNOULLI = range(6)
+RULES = {
+    "one_to_one": ONE_TO_ONE,
+    "all_to_all": ALL_TO_ALL,
+    "fixed_indegree": FIXED_INDEGREE,
+    "fixed_outdegree": FIXED_OUTDEGREE,
+    "fixed_total_number": FIXED_TOTAL_NUMBER,
+    "pairwise_bernoulli": PAIRWISE_BERNOULLI,
+}
+OK, ERR_INVALID_ARG, ERR_STATE, ERR_CAPACITY, ERR_OOM = 0, -1, -2, -3, -4
+
+
+def build(force: bool = False) -> Path:
+    """Compile oracle.cpp -> liboracle.so (g++ -O2 -ffp-contract=off, one translation unit)."""
+    srcs = [_HERE / "oracle.cpp", _HERE / "oracle.h"]
+    if not force and _LIB_PATH.exists() and all(_LIB_PATH.stat().st_mtime >= s.stat().st_mtime for s in srcs):
+        return _LIB_PATH
+    tmp = _LIB_PATH.with_suffix(f".so.tmp{os.getpid()}")
+    cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-Wall", "-Wextra",
+           "-o", str(tmp), str(_HERE / "oracle.cpp")]
+    subprocess.run(cmd, check=True)
+    os.replace(tmp, _LIB_PATH)
+    return _LIB_PATH
+
+
+class _Config(C.Structure):
+    _fields_ = [("block_size", C.c_uint64), ("dt_ms", C.c_double)]
+
+
+class _RuleParams(C.Structure):
+    _fields_ = [("degree_or_total", C.c_uint64), ("p", C.c_double)]
+
+
+class _Dist(C.Structure):
+    _fields_ = [("mean", C.c_double), ("sd", C.c_double), ("lo", C.c_double), ("hi", C.c_double)]
+
+
+class _SynSpec(C.Structure):
+    _fields_ = [("weight", _Dist), ("delay_ms", _Dist)]
+
+
+class _Range(C.Structure):
+    _fields_ = [("first", C.c_uint32), ("count", C.c_uint32)]
+
+
+class _ConnView(C.Structure):
+    _fields_ = [("source", C.POINTER(C.c_uint32)), ("target", C.POINTER(C.c_uint32)),
+                ("weight", C.POINTER(C.c_float)), ("delay", C.POINTER(C.c_uint16)),
+                ("perm", C.POINTER(C.c_uint32)), ("boundary", C.POINTER(C.c_uint8)), ("n", C.c_uint64)]
+
+
+class _IndexView(C.Structure):
+    _fields_ = [("src_offsets", C.POINTER(C.c_uint32)), ("group_count", C.POINTER(C.c_uint32)),
+                ("group_ptr", C.POINTER(C.c_uint32)), ("group_start", C.POINTER(C.c_uint32)),
+                ("group_delay", C.POINTER(C.c_uint16)), ("n_nodes", C.c_uint32), ("total_groups", C.c_uint32)]
+
+
+class _Synapse(C.Structure):
+    _fields_ = [("source", C.c_uint32), ("target", C.c_uint32), ("weight", C.c_float),
+                ("delay", C.c_uint16), ("boundary", C.c_uint8), ("accepted", C.c_uint8),
+                ("z0", C.c_double), ("z1", C.c_double), ("x", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(str(build()))
+        P = C.POINTER
+        L.oc_create.argtypes = [P(_Config), P(C.c_void_p)]
+        L.oc_destroy.argtypes = [C.c_void_p]
+        L.oc_create_population.argtypes = [C.c_void_p, C.c_uint32, P(C.c_uint32)]
+        L.oc_connect.argtypes = [C.c_void_p, _Range, _Range, C.c_int, P(_RuleParams), P(_SynSpec), C.c_uint64]
+        L.oc_finalize.argtypes = [C.c_void_p]
+        L.oc_num_connections.argtypes = [C.c_void_p, P(C.c_uint64)]
+        L.oc_num_nodes.argtypes = [C.c_void_p, P(C.c_uint32)]
+        L.oc_num_blocks.argtypes = [C.c_void_p, P(C.c_uint64)]
+        L.oc_block_slot.argtypes = [C.c_void_p, C.c_uint64, P(C.c_uint64), P(C.c_uint64)]
+        L.oc_get_connections.argtypes = [C.c_void_p, C.c_int, P(_ConnView)]
+        L.oc_get_index.argtypes = [C.c_void_p, P(_IndexView)]
+        L.oc_degree_histogram.argtypes = [C.c_void_p, C.c_int, P(P(C.c_uint32)), P(C.c_uint32)]
+        L.oc_philox4x32_10.argtypes = [P(C.c_uint32), P(C.c_uint32), P(C.c_uint32)]
+        L.oc_philox4x32_10.restype = None
+        L.oc_bounded.argtypes = [C.c_uint32, C.c_uint32]
+        L.oc_bounded.restype = C.c_uint32
+        L.oc_bernoulli_threshold.argtypes = [C.c_double]
+        L.oc_bernoulli_threshold.restype = C.c_uint64
+        L.oc_bernoulli_trial_word.argtypes = [C.c_uint64, C.c_uint32, C.c_uint64]
+        L.oc_bernoulli_trial_word.restype = C.c_uint32
+        L.oc_eval_synapse.argtypes = [_Range, _Range, C.c_int, P(_RuleParams), P(_SynSpec), C.c_uint64,
+                                      C.c_uint32, C.c_double, C.c_uint64, P(_Synapse)]
+        _lib = L
+    return _lib
+
+
+def _dist(d) -> _Dist:
+    mean, sd, lo, hi = d
+    return _Dist(float(mean), float(sd), float(lo), float(hi))
+
+
+def _syn(weight, delay_ms) -> _SynSpec:
+    return _SynSpec(_dist(weight), _dist(delay_ms))
+
+
+def _np(ptr, n, dtype):
+    if n == 0:
+        return np.zeros(0, dtype=dtype)
+    return np.ctypeslib.as_array(ptr, shape=(int(n),)).view(dtype)
+
+
+class OracleError(RuntimeError):
+    def __init__(self, code):
+        super().__init__(f"oracle error {code}")
+        self.code = code
+
+
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*ctr)
+    k = (C.c_uint32 * 2)(*key)
+    o = (C.c_uint32 * 4)()
+    lib().oc_philox4x32_10(c, k, o)
+    return tuple(int(v) for v in o)
+
+
+def bounded(word: int, n: int) -> int:
+    return int(lib().oc_bounded(word, n))
+
+
+def bernoulli_threshold(p: float) -> int:
+    return int(lib().oc_bernoulli_threshold(p))
+
+
+def bernoulli_trial_word(seed: int, projection_id: int, q: int) -> int:
+    return int(lib().oc_bernoulli_trial_word(seed, projection_id, q))
+
+
+def eval_synapse(src, tgt, rule, degree_or_total, p, weight, delay_ms, seed, projection_id, dt_ms, idx):
+    """One synapse as a pure function of (seed, projection_id, idx); returns a dict."""
+    rp = _RuleParams(int(degree_or_total), float(p))
+    sp = _syn(weight, delay_ms)
+    out = _Synapse()
+    rc = lib().oc_eval_synapse(_Range(*src), _Range(*tgt), int(rule), C.byref(rp), C.byref(sp), int(seed),
+                               int(projection_id), float(dt_ms), int(idx), C.byref(out))
+    if rc != 0:
+        raise OracleError(rc)
+    return {f: getattr(out, f) for f, _ in _Synapse._fields_}
+
+
+class Oracle:
+    """Same call sequence as the nc_ ABI (create_population / connect / finalize / getters)."""
+
+    def __init__(self, dt_ms: float = 0.1, block_size: int = 0):
+        self._h = C.c_void_p()
+        cfg = _Config(int(block_size), float(dt_ms))
+        rc = lib().oc_create(C.byref(cfg), C.byref(self._h))
+        if rc != 0:
+            raise OracleError(rc)
+
+    def close(self):
+        if self._h:
+            lib().oc_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def create_population(self, n: int) -> int:
+        first = C.c_uint32()
+        rc = lib().oc_create_population(self._h, int(n), C.byref(first))
+        if rc != 0:
+            raise OracleError(rc)
+        return first.value
+
+    def connect_rc(self, src, tgt, rule, degree_or_total=0, p=0.0, weight=(1.0, 0.0, -math.inf, math.inf),
+                   delay_ms=(1.0, 0.0, -math.inf, math.inf), seed=0) -> int:
+        rp = _RuleParams(int(degree_or_total), float(p))
+        sp = _syn(weight, delay_ms)
+        return int(lib().oc_connect(self._h, _Range(*src), _Range(*tgt), int(rule), C.byref(rp), C.byref(sp),
+                                    int(seed)))
+
+    def connect(self, *a, **k):
+        rc = self.connect_rc(*a, **k)
+        if rc != 0:
+            raise OracleError(rc)
+
+    def finalize(self):
+        rc = lib().oc_finalize(self._h)
+        if rc != 0:
+            raise OracleError(rc)
+
+    def num_connections(self) -> int:
+        n = C.c_uint64()
+        lib().oc_num_connections(self._h, C.byref(n))
+        return n.value
+
+    def num_nodes(self) -> int:
+        n = C.c_uint32()
+        lib().oc_num_nodes(self._h, C.byref(n))
+        return n.value
+
+    def num_blocks(self) -> int:
+        n = C.c_uint64()
+        lib().oc_num_blocks(self._h, C.byref(n))
+        return n.value
+
+    def block_slot(self, pos: int):
+        b, s = C.c_uint64(), C.c_uint64()
+        lib().oc_block_slot(self._h, int(pos), C.byref(b), C.byref(s))
+        return b.value, s.value
+
+    def connections(self, sorted: bool = False) -> dict:
+        """Arrays are COPIES (safe to keep after further calls)."""
+        v = _ConnView()
+        rc = lib().oc_get_connections(self._h, 1 if sorted else 0, C.byref(v))
+        if rc != 0:
+            raise OracleError(rc)
+        n = v.n
+        out = {
+            "source": _np(v.source, n, np.uint32).copy(),
+            "target": _np(v.target, n, np.uint32).copy(),
+            "weight": _np(v.weight, n, np.float32).copy(),
+            "delay": _np(v.delay, n, np.uint16).copy(),
+            "boundary": _np(v.boundary, n, np.uint8).copy(),
+            "n": int(n),
+        }
+        if sorted:
+            out["perm"] = _np(v.perm, n, np.uint32).copy()
+        return out
+
+    def index(self) -> dict:
+        v = _IndexView()
+        rc = lib().oc_get_index(self._h, C.byref(v))
+        if rc != 0:
+            raise OracleError(rc)
+        N, G = v.n_nodes, v.total_groups
+        return {
+            "src_offsets": _np(v.src_offsets, N + 1, np.uint32).copy(),
+            "group_count": _np(v.group_count, N, np.uint32).copy(),
+            "group_ptr": _np(v.group_ptr, N + 1, np.uint32).copy(),
+            "group_start": _np(v.group_start, G, np.uint32).copy(),
+            "group_delay": _np(v.group_delay, G, np.uint16).copy(),
+            "n_nodes": int(N),
+            "total_groups": int(G),
+        }
+
+    def degree_histogram(self, kind: int):
+        p = C.POINTER(C.c_uint32)()
+        mx = C.c_uint32()
+        rc = lib().oc_degree_histogram(self._h, int(kind), C.byref(p), C.byref(mx))
+        if rc != 0:
+            raise OracleError(rc)
+        return _np(p, self.num_nodes(), np.uint32).copy(), mx.value

@@ -1,0 +1,139 @@
+/*
+ * oracle.h -- C interface of the CPU ORACLE for the network-construction hot path of
+ * arXiv 2306.09855 (Golosio, Villamar, Tiddia et al., "Runtime Construction of Large-Scale
+ * Spiking Neuronal Network Models on GPU Devices").
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and the
+ * cpu_baseline / --impl reference legs of bench.py may load it.  It is a plain, slow,
+ * single-threaded fp64 restatement of what the path computes, written from the paper
+ * (/root/reference/PAPER.md, cited below as PAPER.md:<line>) and from the readings D1-D12 /
+ * Q1-Q20 listed in DESIGN.md.  It shares no code, header, table or helper with the CUDA path
+ * under paper_2306_09855_b200/csrc: the struct definitions below are its own.
+ *
+ * All pointers are HOST pointers.  Every function returns 0 (OC_OK) or a negative error code.
+ *
+ * Parity status: every function here is pinned by tests/test_oracle_*.py (-m "not gpu") against
+ * known-answer vectors, closed forms, invariants, library routines and brute force; the one
+ * thing that stays "parity unpinned" is agreement with the PAPER'S OWN implementation, whose
+ * RNG (cuRAND) mapping is unspecified and which prints no output values.
+ */
+#ifndef ORACLE_H_
+#define ORACLE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  OC_OK = 0,
+  OC_ERR_INVALID_ARG = -1,
+  OC_ERR_STATE = -2,
+  OC_ERR_CAPACITY = -3,
+  OC_ERR_OOM = -4
+};
+
+/* Connection rules of PAPER.md:73-115 (Eqs. 4-13) plus pairwise_bernoulli. */
+enum {
+  OC_ONE_TO_ONE = 0,
+  OC_ALL_TO_ALL = 1,
+  OC_FIXED_INDEGREE = 2,
+  OC_FIXED_OUTDEGREE = 3,
+  OC_FIXED_TOTAL_NUMBER = 4,
+  OC_PAIRWISE_BERNOULLI = 5
+};
+
+typedef struct oc_context oc_context;
+
+typedef struct {
+  uint64_t block_size; /* B, connections per block; 0 -> 1<<24 */
+  double dt_ms;        /* simulation time resolution in ms */
+} oc_config;
+
+typedef struct {
+  uint64_t degree_or_total; /* K (fixed_in/outdegree) or N (fixed_total_number) */
+  double p;                 /* pairwise_bernoulli connection probability */
+} oc_rule_params;
+
+/* normal(mean, sd) clamped to [lo, hi]; sd = 0 -> constant; lo/hi may be -inf/+inf */
+typedef struct {
+  double mean, sd, lo, hi;
+} oc_dist;
+
+typedef struct {
+  oc_dist weight;
+  oc_dist delay_ms;
+} oc_syn_spec;
+
+typedef struct {
+  uint32_t first, count;
+} oc_range;
+
+typedef struct {
+  const uint32_t* source;
+  const uint32_t* target;
+  const float* weight;
+  const uint16_t* delay;   /* integer time steps, >= 1 */
+  const uint32_t* perm;    /* sorted view only: creation position of sorted entry j; else NULL */
+  const uint8_t* boundary; /* 1 where the delay sits at a rounding/clip boundary (reading D8) */
+  uint64_t n;
+} oc_connections_view;
+
+typedef struct {
+  const uint32_t* src_offsets; /* [n_nodes+1] exclusive scan of out_degree */
+  const uint32_t* group_count; /* [n_nodes]   G_i of PAPER.md:121 */
+  const uint32_t* group_ptr;   /* [n_nodes+1] p_i of Eq. 14 */
+  const uint32_t* group_start; /* [total_groups] sorted position of each group's first connection */
+  const uint16_t* group_delay; /* [total_groups] delay (steps) of each group */
+  uint32_t n_nodes;
+  uint32_t total_groups;
+} oc_index_view;
+
+/* ---- the path (same call sequence as the nc_ ABI of include/nc.h) ---- */
+int oc_create(const oc_config* cfg, oc_context** out);
+int oc_destroy(oc_context* ctx);
+int oc_create_population(oc_context* ctx, uint32_t n, uint32_t* first_id);
+int oc_connect(oc_context* ctx, oc_range src, oc_range tgt, int rule, const oc_rule_params* params,
+               const oc_syn_spec* syn, uint64_t seed);
+int oc_finalize(oc_context* ctx);
+int oc_num_connections(oc_context* ctx, uint64_t* n);
+int oc_num_nodes(oc_context* ctx, uint32_t* n);
+int oc_num_blocks(oc_context* ctx, uint64_t* n_blocks);          /* Eq. 1 */
+int oc_block_slot(oc_context* ctx, uint64_t pos, uint64_t* block, uint64_t* slot); /* reading D9 */
+int oc_get_connections(oc_context* ctx, int sorted, oc_connections_view* out);
+int oc_get_index(oc_context* ctx, oc_index_view* out);
+int oc_degree_histogram(oc_context* ctx, int kind /*0=in,1=out*/, const uint32_t** per_node,
+                        uint32_t* max_degree);
+
+/* ---- single steps, exposed so the tests can pin them one by one ---- */
+/* Philox4x32-10 (Salmon et al., SC'11): reading D2. */
+void oc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+/* rand(N) of PAPER.md:95 as multiply-high: reading D3. */
+uint32_t oc_bounded(uint32_t word, uint32_t n);
+/* Bernoulli acceptance threshold T = floor(p * 2^32) as u64: reading D4/Q14. */
+uint64_t oc_bernoulli_threshold(double p);
+/* Trial word of pair q on the trial stream (stream 1): reading D2/D4. */
+uint32_t oc_bernoulli_trial_word(uint64_t seed, uint32_t projection_id, uint64_t q);
+
+/* One synapse as a pure function of (seed, projection_id, idx).  idx is i_newconns for every
+ * rule except pairwise_bernoulli, where it is the pair index q (and *accepted says whether the
+ * pair exists at all).  Used for sampled parity at sizes the full oracle cannot hold. */
+typedef struct {
+  uint32_t source, target;
+  float weight;
+  uint16_t delay;
+  uint8_t boundary;
+  uint8_t accepted;
+  double z0, z1; /* Box-Muller pair, reading D6 */
+  double x;      /* clamp(mean_d + sd_d z1) * inv_dt, the value that is rounded (reading D8) */
+} oc_synapse;
+int oc_eval_synapse(oc_range src, oc_range tgt, int rule, const oc_rule_params* params,
+                    const oc_syn_spec* syn, uint64_t seed, uint32_t projection_id, double dt_ms,
+                    uint64_t idx, oc_synapse* out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ORACLE_H_ */
