@@ -1,0 +1,225 @@
+/*
+ * nc.h -- C ABI of the B200-native network-construction library (libnc.so).
+ *
+ * The library builds the connectivity of a spiking network directly in GPU memory from high-level
+ * connection rules and organises it for spike delivery: the hot path of arXiv 2306.09855 (Golosio,
+ * Villamar, Tiddia et al., "Runtime Construction of Large-Scale Spiking Neuronal Network Models on
+ * GPU Devices").  Citations "PAPER.md:<line>" refer to /root/reference/PAPER.md; "D<n>"/"Q<n>" to the
+ * readings listed in DESIGN.md.
+ *
+ * Call sequence (node creation -> node connection -> calibration):
+ *     nc_create -> nc_create_population* -> nc_connect* -> nc_finalize -> nc_get_* / nc_read_* -> nc_destroy
+ *
+ * Conventions
+ *  - Every function returns NC_OK (0) or a negative nc_status; no exception crosses the ABI.
+ *    nc_last_error() gives a human-readable message for the last failure on that context.
+ *  - One context = one GPU and one CUDA stream.  All kernels are enqueued on that stream; results are
+ *    valid for work enqueued later on the same stream, or after nc_synchronize().  Functions that
+ *    return host values (nc_num_connections, nc_read_*, nc_degree_histogram's max) synchronise.
+ *  - The library owns every device buffer.  It obtains them through nc_config.mem (PyTorch's caching
+ *    allocator in the Python binding; cudaMalloc/cudaFree when mem.alloc is NULL) and releases them in
+ *    nc_destroy.  Pointers returned by nc_get_* are BORROWED device pointers, valid until nc_destroy;
+ *    the caller never frees them.  nc_read_* take HOST pointers owned by the caller.
+ *  - There is no CPU fallback: if no CUDA device is usable nc_create fails with NC_ERR_CUDA.
+ *  - A failed nc_connect leaves the context unchanged and does not consume a projection id.
+ *  - Limits: total connections <= 2^32 - 1, nodes <= 2^32 - 1, delay <= 65535 steps.
+ */
+#ifndef NC_H_
+#define NC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  NC_OK = 0,
+  NC_ERR_INVALID_ARG = -1, /* range outside created nodes, count 0, N_src != N_tgt for one_to_one
+                              (PAPER.md:79), p outside [0,1], sd < 0, lo > hi, dt <= 0, NULL pointer */
+  NC_ERR_STATE = -2,       /* connect/create after finalize, sorted view or index before finalize */
+  NC_ERR_CAPACITY = -3,    /* > 2^32-1 connections or nodes, or a delay that can exceed 65535 steps */
+  NC_ERR_OOM = -4,         /* the allocator returned NULL */
+  NC_ERR_CUDA = -5         /* a CUDA call failed or no device is present */
+} nc_status;
+
+/* Connection rules: Eqs. 4-13, names as in Senk et al. 2022.
+ * Autapses and multapses are always allowed. */
+typedef enum {
+  NC_ONE_TO_ONE = 0,         /* Eqs. 4-5:   s = s0 + i,            t = t0 + i            N = N_src = N_tgt */
+  NC_ALL_TO_ALL = 1,         /* Eqs. 6-7:   s = s0 + i / N_tgt,    t = t0 + i % N_tgt    N = N_src N_tgt  */
+  NC_FIXED_INDEGREE = 2,     /* Eqs. 10-11: s = s0 + rand(N_src),  t = t0 + i / K        N = N_tgt K      */
+  NC_FIXED_OUTDEGREE = 3,    /* Eqs. 8-9:   s = s0 + i / K,        t = t0 + rand(N_tgt)  N = N_src K      */
+  NC_FIXED_TOTAL_NUMBER = 4, /* Eqs. 12-13: s = s0 + rand(N_src),  t = t0 + rand(N_tgt)  N given          */
+  NC_PAIRWISE_BERNOULLI = 5  /* not in the paper's code; every ordered pair (s,t) of the two
+                                ranges is tried once with probability p, pairs kept in ascending
+                                q = (s-s0) N_tgt + (t-t0) (readings D4, Q13, Q14) */
+} nc_rule;
+
+typedef struct nc_context nc_context; /* opaque */
+
+/* Device-memory provider.  alloc returns a DEVICE pointer aligned to >= 256 bytes or NULL; free releases
+ * it.  Both are called on the thread that calls into the library, never from a CUDA callback. */
+typedef struct {
+  void* (*alloc)(void* user, size_t bytes);
+  void (*free)(void* user, void* ptr);
+  void* user;
+} nc_allocator;
+
+enum {
+  NC_FLAG_TIMING = 1u << 0,     /* record CUDA events around every phase (nc_get_timings) */
+  NC_FLAG_EXACT_FP64 = 1u << 1, /* debug: draw every delay on the fp64 path (no fp32 fast path) */
+  NC_FLAG_CARRY_PAYLOAD = 1u << 2 /* sort carries (target, weight) through the passes instead of
+                                     gathering them by the permutation afterwards */
+};
+
+typedef struct {
+  uint64_t block_size; /* B: connections per storage block.  0 -> 2^24.  Any B >= 1 works;
+                          the paper's default 10^7 too (Q10). */
+  double dt_ms;        /* simulation time resolution in ms; delays are stored in units of it */
+  nc_allocator mem;    /* device memory provider; mem.alloc == NULL -> cudaMalloc / cudaFree */
+  void* cuda_stream;   /* cudaStream_t all work is enqueued on (NULL = the legacy default stream) */
+  int32_t device;      /* CUDA device ordinal; -1 = the calling thread's current device */
+  uint32_t flags;      /* NC_FLAG_* */
+} nc_config;
+
+typedef struct {
+  uint64_t degree_or_total; /* K for fixed_indegree / fixed_outdegree, N for fixed_total_number */
+  double p;                 /* connection probability for pairwise_bernoulli, in [0, 1] */
+} nc_rule_params;
+
+/* Normal(mean, sd) clamped to [lo, hi] (never redrawn, Q4).  sd = 0 -> the constant `mean`
+ * ("identical values for all connections").  lo / hi may be -INFINITY / +INFINITY. */
+typedef struct {
+  double mean, sd, lo, hi;
+} nc_dist;
+
+/* Per-connection parameters: weight, and delay in ms which is converted to integer time
+ * steps by dividing by dt, rounding half up and clamping to [1, 65535] (readings D8, Q5, Q6). */
+typedef struct {
+  nc_dist weight;
+  nc_dist delay_ms;
+} nc_syn_spec;
+
+typedef struct {
+  uint32_t first, count; /* nodes first .. first+count-1 (consecutive indexes) */
+} nc_range;
+
+/* Connections, either in creation order (sorted = 0) or organised for delivery (sorted = 1).
+ *  sorted = 1: source/target/weight/delay/perm are flat device arrays of n entries ordered by
+ *              (source, delay, creation position) (D10); perm[j] = creation position.
+ *  sorted = 0: the connections live in n_blocks storage blocks of block_size entries.
+ *              blocks is a HOST array of n_blocks device base pointers; inside a block the four arrays
+ *              start at byte offsets off_source/off_target/off_weight/off_delay.  Creation position pos
+ *              is entry pos % block_size of block pos / block_size (D9).  The flat pointers are NULL
+ *              unless n_blocks == 1, in which case they point into that single block. */
+typedef struct {
+  const uint32_t* source;
+  const uint32_t* target;
+  const float* weight;
+  const uint16_t* delay;
+  const uint32_t* perm;
+  uint64_t n;
+  uint64_t block_size;
+  uint64_t n_blocks;
+  void* const* blocks;
+  uint64_t off_source, off_target, off_weight, off_delay;
+} nc_connections_view;
+
+/* Index over the sorted connections (D11).  All device pointers.
+ *  src_offsets[s] .. src_offsets[s+1]: sorted positions of the connections of source s   [n_nodes+1]
+ *  group_count[s]  = G_s, number of distinct delays of source s            [n_nodes]
+ *  group_ptr[s]    = p_s = sum_{j<s} G_j (Eq. 14), group_ptr[n_nodes] = total_groups      [n_nodes+1]
+ *  group_start[g]  = sorted position of the first connection of group g    [total_groups]
+ *  group_delay[g]  = delay in steps shared by the connections of group g                  [total_groups] */
+typedef struct {
+  const uint32_t* src_offsets;
+  const uint32_t* group_count;
+  const uint32_t* group_ptr;
+  const uint32_t* group_start;
+  const uint16_t* group_delay;
+  uint32_t n_nodes;
+  uint32_t total_groups;
+} nc_index_view;
+
+typedef enum {
+  NC_PHASE_GENERATE = 0, /* rule expansion + draws + append (nc_connect) */
+  NC_PHASE_HISTOGRAM = 1, /* sort: digit histograms over the packed (source, delay) key */
+  NC_PHASE_SORT = 2,     /* sort: onesweep digit passes */
+  NC_PHASE_PERMUTE = 3,  /* materialise sorted source/target/weight/delay */
+  NC_PHASE_INDEX = 4,    /* head flags, scans, group compaction */
+  NC_PHASE_DEGREE = 5,   /* nc_degree_histogram */
+  NC_PHASE_COUNT = 6
+} nc_phase;
+
+typedef struct {
+  double ms[NC_PHASE_COUNT];          /* device time per phase, summed over the context's life */
+  uint32_t launches[NC_PHASE_COUNT];  /* kernels launched per phase */
+  double sort_pass_ms;                /* device time of the onesweep pass kernels alone */
+  uint32_t sort_passes;               /* how many onesweep pass kernels ran */
+} nc_timings;
+
+typedef struct {
+  uint64_t kernel_launches;   /* kernels this context launched so far */
+  uint64_t bytes_in_use;      /* device bytes currently held */
+  uint64_t bytes_peak;        /* high-water mark of bytes_in_use */
+  uint64_t n_blocks;          /* storage blocks allocated (Eq. 1) */
+  uint32_t n_projections;     /* successful nc_connect calls */
+  uint32_t key_bits;          /* width of the packed (source, delay) sort key, set by nc_finalize */
+  uint32_t sort_passes;       /* digit passes nc_finalize used */
+  uint32_t delay_bits;        /* bits of the key that hold the delay */
+} nc_stats;
+
+/* ---- lifecycle ---- */
+int nc_create(const nc_config* cfg, nc_context** out);
+int nc_destroy(nc_context* ctx);
+const char* nc_last_error(nc_context* ctx);
+int nc_synchronize(nc_context* ctx);
+
+/* ---- node creation (D1): ids are contiguous, *first_id = nodes created so far ---- */
+int nc_create_population(nc_context* ctx, uint32_t n, uint32_t* first_id);
+
+/* ---- node connection.  Appends N_newconns connections at creation positions
+ * N_conns .. N_conns+N_newconns-1, allocating floor((N_conns+N_newconns+B-1)/B) - N_blocks new blocks (Eq. 1).
+ * Connection i draws its randomness from Philox4x32-10 keyed by (seed, projection_id, i) (D2), where
+ * projection_id = number of earlier successful nc_connect calls, so the result does not depend on thread
+ * order.  Asynchronous except for pairwise_bernoulli, which waits for its exact count. ---- */
+int nc_connect(nc_context* ctx, nc_range src, nc_range tgt, nc_rule rule, const nc_rule_params* params,
+               const nc_syn_spec* syn, uint64_t seed);
+
+/* ---- calibration: stable sort by (source, delay), then the group index ---- */
+int nc_finalize(nc_context* ctx);
+
+/* ---- queries ---- */
+int nc_num_connections(nc_context* ctx, uint64_t* n);
+int nc_num_nodes(nc_context* ctx, uint32_t* n);
+int nc_get_connections(nc_context* ctx, int sorted, nc_connections_view* out);
+int nc_get_index(nc_context* ctx, nc_index_view* out);
+/* kind 0 = in-degree (counted over targets), 1 = out-degree (counted over sources); *per_node_degree is a
+ * borrowed device array of n_nodes entries; *max_degree is written to host (synchronises).  Either may be NULL. */
+int nc_degree_histogram(nc_context* ctx, int kind, const uint32_t** per_node_degree, uint32_t* max_degree);
+int nc_get_stats(nc_context* ctx, nc_stats* out);
+/* Needs NC_FLAG_TIMING; synchronises the stream. */
+int nc_get_timings(nc_context* ctx, nc_timings* out);
+
+/* ---- host-buffer reads (device -> host copies; every destination is a HOST pointer and may be NULL) ----
+ * nc_read_connections copies entries first .. first+count-1 of the chosen view (gathering across storage
+ * blocks for the creation-order view).  perm is only written for sorted = 1. */
+int nc_read_connections(nc_context* ctx, int sorted, uint64_t first, uint64_t count, uint32_t* source,
+                        uint32_t* target, float* weight, uint16_t* delay, uint32_t* perm);
+int nc_read_index(nc_context* ctx, uint32_t* src_offsets, uint32_t* group_count, uint32_t* group_ptr,
+                  uint32_t* group_start, uint16_t* group_delay);
+int nc_read_degree_histogram(nc_context* ctx, int kind, uint32_t* per_node_degree, uint32_t* max_degree);
+
+/* ---- device self-tests used by the GPU test-suite (each runs a small kernel on the context's stream) ----
+ * nc_selftest_philox: out[4*k..4*k+3] = Philox4x32-10(ctr[4*k..], key[2*k..]) computed on the device (D2).
+ * nc_selftest_fastpath: exhaustive error of the fp32 Box-Muller fast path against fp64 on the device over
+ *   all 2^24 values of u1 and of u2 (D5, D6): max |r32 - r64| / r64, max |sin32 - sin64|, max |cos32 - cos64|. */
+int nc_selftest_philox(nc_context* ctx, uint32_t n, const uint32_t* ctr, const uint32_t* key, uint32_t* out);
+int nc_selftest_fastpath(nc_context* ctx, double* max_rel_err_r, double* max_abs_err_sin, double* max_abs_err_cos);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NC_H_ */

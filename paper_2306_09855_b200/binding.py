@@ -1,0 +1,306 @@
+"""Thin ctypes binding over libnc.so (C ABI: include/nc.h) -- argument marshalling only.
+
+Every step of the path (rule expansion, draws, append, sort, index) runs in the CUDA kernels of the
+library.  PyTorch is used for two things: device memory (the library's nc_allocator callbacks are backed by
+torch's caching allocator) and the CUDA stream the work is enqueued on.  There is no CPU fallback: without
+the built library or without a GPU, creating a context raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import math
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+LIB_PATH = _HERE / "libnc.so"
+
+OK, ERR_INVALID_ARG, ERR_STATE, ERR_CAPACITY, ERR_OOM, ERR_CUDA = 0, -1, -2, -3, -4, -5
+ONE_TO_ONE, ALL_TO_ALL, FIXED_INDEGREE, FIXED_OUTDEGREE, FIXED_TOTAL_NUMBER, PAIRWISE_BERNOULLI = range(6)
+FLAG_TIMING, FLAG_EXACT_FP64, FLAG_CARRY_PAYLOAD = 1, 2, 4
+PHASES = ("generate", "histogram", "sort", "permute", "index", "degree")
+
+# every symbol include/nc.h declares (checked by tests/test_abi.py against the header and the library)
+SYMBOLS = (
+    "nc_create", "nc_destroy", "nc_last_error", "nc_synchronize", "nc_create_population", "nc_connect",
+    "nc_finalize", "nc_num_connections", "nc_num_nodes", "nc_get_connections", "nc_get_index",
+    "nc_degree_histogram", "nc_get_stats", "nc_get_timings", "nc_read_connections", "nc_read_index",
+    "nc_read_degree_histogram", "nc_selftest_philox", "nc_selftest_fastpath",
+)
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_void_p, C.c_size_t)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p, C.c_void_p)
+
+
+class Allocator(C.Structure):
+    _fields_ = [("alloc", ALLOC_FN), ("free", FREE_FN), ("user", C.c_void_p)]
+
+
+class Config(C.Structure):
+    _fields_ = [("block_size", C.c_uint64), ("dt_ms", C.c_double), ("mem", Allocator),
+                ("cuda_stream", C.c_void_p), ("device", C.c_int32), ("flags", C.c_uint32)]
+
+
+class RuleParams(C.Structure):
+    _fields_ = [("degree_or_total", C.c_uint64), ("p", C.c_double)]
+
+
+class Dist(C.Structure):
+    _fields_ = [("mean", C.c_double), ("sd", C.c_double), ("lo", C.c_double), ("hi", C.c_double)]
+
+
+class SynSpec(C.Structure):
+    _fields_ = [("weight", Dist), ("delay_ms", Dist)]
+
+
+class Range(C.Structure):
+    _fields_ = [("first", C.c_uint32), ("count", C.c_uint32)]
+
+
+class ConnectionsView(C.Structure):
+    _fields_ = [("source", C.c_void_p), ("target", C.c_void_p), ("weight", C.c_void_p), ("delay", C.c_void_p),
+                ("perm", C.c_void_p), ("n", C.c_uint64), ("block_size", C.c_uint64), ("n_blocks", C.c_uint64),
+                ("blocks", C.POINTER(C.c_void_p)), ("off_source", C.c_uint64), ("off_target", C.c_uint64),
+                ("off_weight", C.c_uint64), ("off_delay", C.c_uint64)]
+
+
+class IndexView(C.Structure):
+    _fields_ = [("src_offsets", C.c_void_p), ("group_count", C.c_void_p), ("group_ptr", C.c_void_p),
+                ("group_start", C.c_void_p), ("group_delay", C.c_void_p), ("n_nodes", C.c_uint32),
+                ("total_groups", C.c_uint32)]
+
+
+class Timings(C.Structure):
+    _fields_ = [("ms", C.c_double * 6), ("launches", C.c_uint32 * 6), ("sort_pass_ms", C.c_double),
+                ("sort_passes", C.c_uint32)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("kernel_launches", C.c_uint64), ("bytes_in_use", C.c_uint64), ("bytes_peak", C.c_uint64),
+                ("n_blocks", C.c_uint64), ("n_projections", C.c_uint32), ("key_bits", C.c_uint32),
+                ("sort_passes", C.c_uint32), ("delay_bits", C.c_uint32)]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libnc.so and declare the argument types of every entry point.  Raises if it is not built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not LIB_PATH.exists():
+        raise RuntimeError(f"{LIB_PATH} is not built: run `python -m paper_2306_09855_b200.build` "
+                           "(there is no CPU fallback)")
+    L = C.CDLL(str(LIB_PATH))
+    P, vp = C.POINTER, C.c_void_p
+    L.nc_create.argtypes = [P(Config), P(vp)]
+    L.nc_destroy.argtypes = [vp]
+    L.nc_last_error.argtypes = [vp]
+    L.nc_last_error.restype = C.c_char_p
+    L.nc_synchronize.argtypes = [vp]
+    L.nc_create_population.argtypes = [vp, C.c_uint32, P(C.c_uint32)]
+    L.nc_connect.argtypes = [vp, Range, Range, C.c_int, P(RuleParams), P(SynSpec), C.c_uint64]
+    L.nc_finalize.argtypes = [vp]
+    L.nc_num_connections.argtypes = [vp, P(C.c_uint64)]
+    L.nc_num_nodes.argtypes = [vp, P(C.c_uint32)]
+    L.nc_get_connections.argtypes = [vp, C.c_int, P(ConnectionsView)]
+    L.nc_get_index.argtypes = [vp, P(IndexView)]
+    L.nc_degree_histogram.argtypes = [vp, C.c_int, P(vp), P(C.c_uint32)]
+    L.nc_get_stats.argtypes = [vp, P(Stats)]
+    L.nc_get_timings.argtypes = [vp, P(Timings)]
+    L.nc_read_connections.argtypes = [vp, C.c_int, C.c_uint64, C.c_uint64, vp, vp, vp, vp, vp]
+    L.nc_read_index.argtypes = [vp, vp, vp, vp, vp, vp]
+    L.nc_read_degree_histogram.argtypes = [vp, C.c_int, vp, P(C.c_uint32)]
+    L.nc_selftest_philox.argtypes = [vp, C.c_uint32, vp, vp, vp]
+    L.nc_selftest_fastpath.argtypes = [vp, P(C.c_double), P(C.c_double), P(C.c_double)]
+    for name in SYMBOLS:
+        if name != "nc_last_error":
+            getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+class NCError(RuntimeError):
+    def __init__(self, code, msg=""):
+        super().__init__(f"nc error {code}: {msg}")
+        self.code = code
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+class TorchAllocator:
+    """nc_allocator backed by torch's caching allocator on the current device/stream."""
+
+    def __init__(self):
+        import torch
+        self._torch = torch
+        self._held = {}
+        self.alloc_cb = ALLOC_FN(self._alloc)
+        self.free_cb = FREE_FN(self._free)
+
+    def _alloc(self, _user, nbytes):
+        try:
+            t = self._torch.empty(int(nbytes), dtype=self._torch.uint8, device="cuda")
+        except Exception:  # torch.cuda.OutOfMemoryError and friends -> NULL -> NC_ERR_OOM
+            return None
+        p = t.data_ptr()
+        self._held[p] = t
+        return p
+
+    def _free(self, _user, p):
+        self._held.pop(p, None)
+
+    def struct(self):
+        return Allocator(self.alloc_cb, self.free_cb, None)
+
+
+class NC:
+    """One construction context.  Method names and order follow the C ABI one to one."""
+
+    def __init__(self, dt_ms: float = 0.1, block_size: int = 0, flags: int = 0, use_torch_allocator: bool = True,
+                 stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the construction path only exists as CUDA kernels (no CPU fallback)")
+        self._L = load_library()
+        self._alloc = TorchAllocator() if use_torch_allocator else None
+        cfg = Config()
+        cfg.block_size = int(block_size)
+        cfg.dt_ms = float(dt_ms)
+        if self._alloc is not None:
+            cfg.mem = self._alloc.struct()
+        s = stream if stream is not None else torch.cuda.current_stream()
+        self._stream = s
+        cfg.cuda_stream = s.cuda_stream
+        cfg.device = torch.cuda.current_device()
+        cfg.flags = int(flags)
+        self._h = C.c_void_p()
+        rc = self._L.nc_create(C.byref(cfg), C.byref(self._h))
+        if rc != 0:
+            raise NCError(rc, "nc_create failed")
+
+    # -- plumbing --
+    def _check(self, rc):
+        if rc != 0:
+            raise NCError(rc, (self._L.nc_last_error(self._h) or b"").decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.nc_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    # -- the ABI --
+    def synchronize(self):
+        self._check(self._L.nc_synchronize(self._h))
+
+    def create_population(self, n: int) -> int:
+        first = C.c_uint32()
+        self._check(self._L.nc_create_population(self._h, int(n), C.byref(first)))
+        return first.value
+
+    def connect_rc(self, src, tgt, rule, degree_or_total=0, p=0.0, weight=(1.0, 0.0, -math.inf, math.inf),
+                   delay_ms=(1.0, 0.0, -math.inf, math.inf), seed=0) -> int:
+        rp = RuleParams(int(degree_or_total), float(p))
+        sp = SynSpec(Dist(*map(float, weight)), Dist(*map(float, delay_ms)))
+        return int(self._L.nc_connect(self._h, Range(*src), Range(*tgt), int(rule), C.byref(rp), C.byref(sp), int(seed)))
+
+    def connect(self, *a, **k):
+        self._check(self.connect_rc(*a, **k))
+
+    def finalize(self):
+        self._check(self._L.nc_finalize(self._h))
+
+    def num_connections(self) -> int:
+        n = C.c_uint64()
+        self._check(self._L.nc_num_connections(self._h, C.byref(n)))
+        return n.value
+
+    def num_nodes(self) -> int:
+        n = C.c_uint32()
+        self._check(self._L.nc_num_nodes(self._h, C.byref(n)))
+        return n.value
+
+    def get_connections(self, sorted: bool = False) -> ConnectionsView:
+        v = ConnectionsView()
+        self._check(self._L.nc_get_connections(self._h, 1 if sorted else 0, C.byref(v)))
+        return v
+
+    def get_index(self) -> IndexView:
+        v = IndexView()
+        self._check(self._L.nc_get_index(self._h, C.byref(v)))
+        return v
+
+    def stats(self) -> dict:
+        s = Stats()
+        self._check(self._L.nc_get_stats(self._h, C.byref(s)))
+        return {f: getattr(s, f) for f, _ in Stats._fields_}
+
+    def timings(self) -> dict:
+        t = Timings()
+        self._check(self._L.nc_get_timings(self._h, C.byref(t)))
+        out = {f"{name}_ms": t.ms[i] for i, name in enumerate(PHASES)}
+        out["sort_pass_ms"] = t.sort_pass_ms
+        out["sort_passes"] = t.sort_passes
+        return out
+
+    # -- host-buffer reads --
+    def read_connections(self, sorted: bool = False, first: int = 0, count: int | None = None,
+                         fields=("source", "target", "weight", "delay", "perm")) -> dict:
+        n = self.num_connections()
+        if count is None:
+            count = n - first
+        out = {"n": int(count)}
+        bufs = {"source": np.uint32, "target": np.uint32, "weight": np.float32, "delay": np.uint16, "perm": np.uint32}
+        arr = {k: (np.empty(count, dtype=dt) if (k in fields and (k != "perm" or sorted)) else None)
+               for k, dt in bufs.items()}
+        self._check(self._L.nc_read_connections(self._h, 1 if sorted else 0, int(first), int(count), _ptr(arr["source"]),
+                                                _ptr(arr["target"]), _ptr(arr["weight"]), _ptr(arr["delay"]),
+                                                _ptr(arr["perm"])))
+        out.update({k: v for k, v in arr.items() if v is not None})
+        return out
+
+    def read_index(self) -> dict:
+        v = self.get_index()
+        N, G = v.n_nodes, v.total_groups
+        a = {"src_offsets": np.empty(N + 1, np.uint32), "group_count": np.empty(N, np.uint32),
+             "group_ptr": np.empty(N + 1, np.uint32), "group_start": np.empty(G, np.uint32),
+             "group_delay": np.empty(G, np.uint16)}
+        self._check(self._L.nc_read_index(self._h, _ptr(a["src_offsets"]), _ptr(a["group_count"]), _ptr(a["group_ptr"]),
+                                          _ptr(a["group_start"]), _ptr(a["group_delay"])))
+        a["n_nodes"], a["total_groups"] = int(N), int(G)
+        return a
+
+    def read_degree_histogram(self, kind: int):
+        deg = np.empty(self.num_nodes(), np.uint32)
+        mx = C.c_uint32()
+        self._check(self._L.nc_read_degree_histogram(self._h, int(kind), _ptr(deg), C.byref(mx)))
+        return deg, mx.value
+
+    # -- device self-tests --
+    def selftest_philox(self, ctr: np.ndarray, key: np.ndarray) -> np.ndarray:
+        ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+        key = np.ascontiguousarray(key, dtype=np.uint32).reshape(-1, 2)
+        out = np.empty_like(ctr)
+        self._check(self._L.nc_selftest_philox(self._h, ctr.shape[0], _ptr(ctr), _ptr(key), _ptr(out)))
+        return out
+
+    def selftest_fastpath(self):
+        a, b, c = C.c_double(), C.c_double(), C.c_double()
+        self._check(self._L.nc_selftest_fastpath(self._h, C.byref(a), C.byref(b), C.byref(c)))
+        return a.value, b.value, c.value

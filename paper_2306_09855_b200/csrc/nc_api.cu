@@ -1,0 +1,971 @@
+// nc_api.cu -- host side of libnc: context, planner (Eq. 1 block reservation, key-width plan),
+// kernel launches and the C ABI of include/nc.h.  No torch types, no CPU compute path.
+#include "../../include/nc.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <unordered_map>
+#include <vector>
+
+#include "nc_common.cuh"
+#include "nc_generate.cuh"
+#include "nc_index.cuh"
+#include "nc_sort.cuh"
+
+using namespace nc;
+
+namespace {
+
+constexpr uint64_t kMaxConns = 0xffffffffull;
+constexpr double kZMax = 5.769;  // |z| <= sqrt(48 ln 2) = 5.7681 (D5/D6), rounded up (Q6)
+constexpr int kSortThreads = 512;
+constexpr int kSortItems = 16;
+
+struct Span {
+  int phase;
+  bool is_pass;
+  cudaEvent_t a, b;
+};
+
+inline uint64_t align_up(uint64_t v, uint64_t a) { return (v + a - 1) / a * a; }
+inline uint32_t bit_width_u64(uint64_t v) {
+  uint32_t b = 0;
+  while (v) {
+    ++b;
+    v >>= 1;
+  }
+  return b;
+}
+
+}  // namespace
+
+struct nc_context {
+  nc_config cfg{};
+  cudaStream_t stream = nullptr;
+  int device = 0;
+  uint64_t B = 0;
+  double dt = 0, inv_dt = 0;
+  std::string err;
+
+  uint32_t n_nodes = 0;
+  uint32_t n_proj = 0;
+  uint64_t n_conns = 0;
+  bool finalized = false;
+  uint32_t max_delay_steps = 1;  // bound over all projections (Q6), sets the key's delay bits
+
+  // storage blocks (D9)
+  std::vector<void*> blocks;
+  uint64_t* d_table = nullptr;
+  size_t table_cap = 0;
+  uint64_t off_tgt = 0, off_w = 0, off_d = 0, block_bytes = 0;
+
+  // allocations
+  std::unordered_map<void*, size_t> live;
+  std::vector<void*> deferred;  // scratch to release at the next point the stream is known idle
+  uint64_t bytes_in_use = 0, bytes_peak = 0;
+
+  // sorted view + index
+  uint32_t *s_src = nullptr, *s_tgt = nullptr, *perm = nullptr;
+  float* s_w = nullptr;
+  uint16_t* s_d = nullptr;
+  uint32_t *src_offsets = nullptr, *group_count = nullptr, *group_ptr = nullptr, *group_start = nullptr;
+  uint16_t* group_delay = nullptr;
+  uint32_t total_groups = 0;
+  uint32_t *out_degree = nullptr, *in_degree = nullptr, *d_max = nullptr;  // d_max: [2] device scalars
+  bool have_in = false, have_out = false;
+  uint32_t max_in = 0, max_out = 0;
+
+  // stats / timing
+  uint64_t launches = 0;
+  uint32_t key_bits = 0, delay_bits = 0, sort_passes = 0;
+  std::vector<Span> spans;
+  nc_timings acc{};
+};
+
+namespace {
+
+int fail(nc_context* c, int code, const std::string& msg) {
+  if (c) c->err = msg;
+  return code;
+}
+
+#define NC_CUDA(ctx, call)                                                                      \
+  do {                                                                                          \
+    cudaError_t e_ = (call);                                                                    \
+    if (e_ != cudaSuccess)                                                                      \
+      return fail(ctx, NC_ERR_CUDA, std::string(#call) + ": " + cudaGetErrorString(e_));        \
+  } while (0)
+
+#define NC_LAUNCH_CHECK(ctx, name)                                                              \
+  do {                                                                                          \
+    (ctx)->launches++;                                                                          \
+    cudaError_t e_ = cudaPeekAtLastError();                                                     \
+    if (e_ != cudaSuccess)                                                                      \
+      return fail(ctx, NC_ERR_CUDA, std::string("launch ") + name + ": " + cudaGetErrorString(e_)); \
+  } while (0)
+
+void* dev_alloc(nc_context* c, size_t bytes) {
+  if (bytes == 0) bytes = 256;
+  void* p = nullptr;
+  if (c->cfg.mem.alloc) {
+    p = c->cfg.mem.alloc(c->cfg.mem.user, bytes);
+  } else {
+    if (cudaMalloc(&p, bytes) != cudaSuccess) {
+      cudaGetLastError();
+      p = nullptr;
+    }
+  }
+  if (p) {
+    c->live[p] = bytes;
+    c->bytes_in_use += bytes;
+    c->bytes_peak = std::max(c->bytes_peak, c->bytes_in_use);
+  }
+  return p;
+}
+
+void dev_free(nc_context* c, void* p) {
+  if (!p) return;
+  auto it = c->live.find(p);
+  if (it != c->live.end()) {
+    c->bytes_in_use -= it->second;
+    c->live.erase(it);
+  }
+  if (c->cfg.mem.alloc) {
+    c->cfg.mem.free(c->cfg.mem.user, p);
+  } else {
+    cudaFree(p);
+  }
+}
+
+// scratch that may still be read by enqueued kernels: released once the stream has been synchronised
+void dev_free_later(nc_context* c, void* p) {
+  if (p) c->deferred.push_back(p);
+}
+void release_deferred(nc_context* c) {
+  for (void* p : c->deferred) dev_free(c, p);
+  c->deferred.clear();
+}
+
+int sync_stream(nc_context* c) {
+  NC_CUDA(c, cudaStreamSynchronize(c->stream));
+  release_deferred(c);
+  return NC_OK;
+}
+
+struct Scope {  // CUDA-event span around a phase (NC_FLAG_TIMING)
+  nc_context* c;
+  Span s{};
+  bool on;
+  Scope(nc_context* c_, int phase, bool is_pass = false) : c(c_), on((c_->cfg.flags & NC_FLAG_TIMING) != 0) {
+    if (!on) return;
+    s.phase = phase;
+    s.is_pass = is_pass;
+    cudaEventCreate(&s.a);
+    cudaEventCreate(&s.b);
+    cudaEventRecord(s.a, c->stream);
+  }
+  ~Scope() {
+    if (!on) return;
+    cudaEventRecord(s.b, c->stream);
+    c->spans.push_back(s);
+  }
+};
+
+BlockMap make_map(const nc_context* c) {
+  BlockMap m{};
+  m.table = c->d_table;
+  m.B = c->B;
+  m.off_tgt = c->off_tgt;
+  m.off_w = c->off_w;
+  m.off_d = c->off_d;
+  if ((c->B & (c->B - 1)) == 0) {
+    m.shift = bit_width_u64(c->B) - 1;
+    m.magic = 0;
+  } else {
+    m.shift = 0xffffffffu;
+    m.magic = (uint64_t)(((unsigned __int128)1 << 64) / c->B) + 1;
+  }
+  return m;
+}
+
+bool dist_ok(const nc_dist& d) {
+  if (std::isnan(d.mean) || std::isnan(d.sd) || std::isnan(d.lo) || std::isnan(d.hi)) return false;
+  if (std::isinf(d.mean) || std::isinf(d.sd)) return false;
+  return d.sd >= 0.0 && d.lo <= d.hi;
+}
+
+// Q6: largest number of steps a projection's delay can take.
+double delay_bound_steps(const nc_dist& d, double inv_dt) {
+  double top = d.mean + kZMax * d.sd;
+  if (top > d.hi) top = d.hi;
+  if (top < d.lo) top = d.lo;
+  return std::floor(top * inv_dt + 0.5);
+}
+
+SynConst make_syn(const nc_context* c, const nc_syn_spec& s) {
+  SynConst k{};
+  k.w_mean = (float)s.weight.mean;
+  k.w_sd = (float)s.weight.sd;
+  k.w_lo = (float)s.weight.lo;
+  k.w_hi = (float)s.weight.hi;
+  k.d_mean = (float)s.delay_ms.mean;
+  k.d_sd = (float)s.delay_ms.sd;
+  k.d_lo = (float)s.delay_ms.lo;
+  k.d_hi = (float)s.delay_ms.hi;
+  k.inv_dt = (float)c->inv_dt;
+  // Guard band: 32 fp32 ulps of the largest |sd z1| / dt term, 32 relative
+  // ulps of x itself (covers the fp32 roundings of mean, sd, bounds, 1/dt and of the products), and a floor.
+  const double ulp32 = 1.0 / 16777216.0 * 32.0;
+  k.eps_abs = (float)(std::fabs(s.delay_ms.sd) * c->inv_dt * kZMax * ulp32 + 1e-6);
+  k.eps_rel = (float)ulp32;
+  k.exact = (c->cfg.flags & NC_FLAG_EXACT_FP64) ? 1 : 0;
+  k.dd_mean = s.delay_ms.mean;
+  k.dd_sd = s.delay_ms.sd;
+  k.dd_lo = s.delay_ms.lo;
+  k.dd_hi = s.delay_ms.hi;
+  k.dinv_dt = c->inv_dt;
+  return k;
+}
+
+// Eq. 1: allocate floor((N_conns + N_newconns + B - 1) / B) - N_blocks new blocks and refresh
+// the device-side table.  On failure nothing is kept.
+int reserve_blocks(nc_context* c, uint64_t n_new) {
+  const uint64_t want = (c->n_conns + n_new + c->B - 1) / c->B;
+  const size_t have = c->blocks.size();
+  if (want <= have) return NC_OK;
+  std::vector<void*> fresh;
+  for (uint64_t b = have; b < want; ++b) {
+    void* p = dev_alloc(c, c->block_bytes);
+    if (!p) {
+      for (void* q : fresh) dev_free(c, q);
+      return fail(c, NC_ERR_OOM, "out of device memory allocating a connection block");
+    }
+    fresh.push_back(p);
+  }
+  if (want > c->table_cap) {
+    const size_t cap = std::max<size_t>(1024, (size_t)want * 2);
+    uint64_t* t = (uint64_t*)dev_alloc(c, cap * sizeof(uint64_t));
+    if (!t) {
+      for (void* q : fresh) dev_free(c, q);
+      return fail(c, NC_ERR_OOM, "out of device memory allocating the block table");
+    }
+    dev_free_later(c, c->d_table);  // earlier kernels may still read the old table
+    c->d_table = t;
+    c->table_cap = cap;
+    c->blocks.insert(c->blocks.end(), fresh.begin(), fresh.end());
+    NC_CUDA(c, cudaMemcpyAsync(c->d_table, c->blocks.data(), c->blocks.size() * sizeof(uint64_t),
+                               cudaMemcpyHostToDevice, c->stream));
+  } else {
+    c->blocks.insert(c->blocks.end(), fresh.begin(), fresh.end());
+    NC_CUDA(c, cudaMemcpyAsync(c->d_table + have, c->blocks.data() + have, (want - have) * sizeof(uint64_t),
+                               cudaMemcpyHostToDevice, c->stream));
+  }
+  return NC_OK;
+}
+
+template <int RULE>
+void launch_generate(nc_context* c, const GenParams& p, bool vec) {
+  const uint64_t first_group = p.pos0 >> 2;
+  const uint64_t last_group = (p.pos0 + p.n + 3) >> 2;
+  const uint64_t groups = last_group - first_group;
+  const uint64_t per_cta = (uint64_t)kGenThreads * kGenGroups;
+  const unsigned grid = (unsigned)((groups + per_cta - 1) / per_cta);
+  if (vec) {
+    generate_kernel<RULE, true><<<grid, kGenThreads, 0, c->stream>>>(p);
+  } else {
+    generate_kernel<RULE, false><<<grid, kGenThreads, 0, c->stream>>>(p);
+  }
+}
+
+int device_scan(nc_context* c, const uint32_t* in, uint32_t* out, uint64_t n, uint32_t* partial, uint64_t* total) {
+  const uint64_t chunks = (n + kScanChunk - 1) / kScanChunk;
+  scan_reduce_kernel<<<(unsigned)chunks, kScanThreads, 0, c->stream>>>(in, n, partial);
+  NC_LAUNCH_CHECK(c, "scan_reduce");
+  scan_partials_kernel<<<1, kScanThreads, 0, c->stream>>>(partial, chunks, total);
+  NC_LAUNCH_CHECK(c, "scan_partials");
+  scan_downsweep_kernel<<<(unsigned)chunks, kScanThreads, 0, c->stream>>>(in, n, partial, out);
+  NC_LAUNCH_CHECK(c, "scan_downsweep");
+  return NC_OK;
+}
+
+int connect_bernoulli(nc_context* c, GenParams gp, double p) {
+  const uint64_t n_pairs = (uint64_t)gp.n_src * gp.n_tgt;
+  const uint64_t T = (uint64_t)std::floor(std::ldexp(p, 32));  // Q14
+  if (T == 0) return NC_OK;                                    // realised probability 0: nothing to create
+  const uint64_t n_tiles = (n_pairs + kBernTile - 1) / kBernTile;
+  if (n_tiles > 0x7fffffffull) return fail(c, NC_ERR_CAPACITY, "pairwise_bernoulli: too many pairs for one call");
+  const uint64_t n_words = (n_pairs + 31) / 32;
+  const uint64_t chunks = (n_tiles + kScanChunk - 1) / kScanChunk;
+  uint32_t* mask = (uint32_t*)dev_alloc(c, n_words * 4);
+  uint32_t* tile_count = (uint32_t*)dev_alloc(c, n_tiles * 4);
+  uint32_t* tile_off = (uint32_t*)dev_alloc(c, n_tiles * 4);
+  uint32_t* partial = (uint32_t*)dev_alloc(c, chunks * 4);
+  uint64_t* d_total = (uint64_t*)dev_alloc(c, 8);
+  auto drop = [&]() {
+    dev_free_later(c, mask); dev_free_later(c, tile_count); dev_free_later(c, tile_off);
+    dev_free_later(c, partial); dev_free_later(c, d_total);
+  };
+  if (!mask || !tile_count || !tile_off || !partial || !d_total) {
+    drop();
+    return fail(c, NC_ERR_OOM, "out of device memory for pairwise_bernoulli scratch");
+  }
+  uint64_t total = 0;
+  {
+    Scope sc(c, NC_PHASE_GENERATE);
+    BernParams bp{};
+    bp.n_pairs = n_pairs;
+    bp.threshold = T;
+    bp.seed_lo = gp.seed_lo;
+    bp.seed_hi = gp.seed_hi;
+    bp.projection_id = gp.projection_id;
+    bp.mask = mask;
+    bp.tile_count = tile_count;
+    bernoulli_trials_kernel<<<(unsigned)n_tiles, kBernThreads, 0, c->stream>>>(bp);
+    NC_LAUNCH_CHECK(c, "bernoulli_trials");
+    int rc = device_scan(c, tile_count, tile_off, n_tiles, partial, d_total);
+    if (rc != NC_OK) return rc;
+    NC_CUDA(c, cudaMemcpyAsync(&total, d_total, 8, cudaMemcpyDeviceToHost, c->stream));
+  }
+  NC_CUDA(c, cudaStreamSynchronize(c->stream));  // the exact count decides the allocation
+  if (c->n_conns + total > kMaxConns) {
+    drop();
+    return fail(c, NC_ERR_CAPACITY, "more than 2^32-1 connections");
+  }
+  int rc = reserve_blocks(c, total);
+  if (rc != NC_OK) {
+    drop();
+    return rc;
+  }
+  if (total > 0) {
+    Scope sc(c, NC_PHASE_GENERATE);
+    BernWriteParams wp{};
+    wp.g = gp;
+    wp.g.map = make_map(c);
+    wp.g.pos0 = c->n_conns;
+    wp.g.n = total;
+    wp.n_pairs = n_pairs;
+    wp.mask = mask;
+    wp.tile_offset = tile_off;
+    bernoulli_write_kernel<<<(unsigned)n_tiles, kBernThreads, 0, c->stream>>>(wp);
+    NC_LAUNCH_CHECK(c, "bernoulli_write");
+  }
+  drop();
+  c->n_conns += total;
+  return NC_OK;
+}
+
+PassPlan plan_passes(uint32_t key_bits) {
+  PassPlan pl{};
+  pl.n_passes = (key_bits + kRadixBits - 1) / kRadixBits;
+  uint32_t left = key_bits, shift = 0;
+  for (uint32_t i = 0; i < pl.n_passes; ++i) {
+    const uint32_t b = (left + (pl.n_passes - i) - 1) / (pl.n_passes - i);  // spread evenly, <= 8
+    pl.shift[i] = shift;
+    pl.bits[i] = b;
+    shift += b;
+    left -= b;
+  }
+  return pl;
+}
+
+template <typename KeyT>
+int sort_and_index(nc_context* c, const PassPlan& plan) {
+  using Smem = OnesweepSmem<KeyT, kSortThreads, kSortItems>;
+  const uint32_t n = (uint32_t)c->n_conns;
+  const uint32_t N = c->n_nodes;
+  const uint64_t n_tiles = ((uint64_t)n + Smem::kTile - 1) / Smem::kTile;
+  const BlockMap map = make_map(c);
+
+  KeyT* keys[2] = {(KeyT*)dev_alloc(c, (size_t)n * sizeof(KeyT)),
+                   plan.n_passes > 1 ? (KeyT*)dev_alloc(c, (size_t)n * sizeof(KeyT)) : nullptr};
+  uint32_t* vals[2] = {(uint32_t*)dev_alloc(c, (size_t)n * 4),
+                       plan.n_passes > 1 ? (uint32_t*)dev_alloc(c, (size_t)n * 4) : nullptr};
+  uint32_t* ghist = (uint32_t*)dev_alloc(c, kMaxPasses * kRadix * 4);
+  uint32_t* bin_start = (uint32_t*)dev_alloc(c, kMaxPasses * kRadix * 4);
+  uint64_t* status = (uint64_t*)dev_alloc(c, n_tiles * kRadix * 8);
+  uint32_t* tickets = (uint32_t*)dev_alloc(c, (kMaxPasses + 1) * 4);  // + the look-back error flag
+  c->s_src = (uint32_t*)dev_alloc(c, (size_t)n * 4);
+  c->s_tgt = (uint32_t*)dev_alloc(c, (size_t)n * 4);
+  c->s_w = (float*)dev_alloc(c, (size_t)n * 4);
+  c->s_d = (uint16_t*)dev_alloc(c, (size_t)n * 2);
+  const uint64_t head_tiles = ((uint64_t)n + kHeadTile - 1) / kHeadTile;
+  const uint64_t head_chunks = (head_tiles + kScanChunk - 1) / kScanChunk;
+  uint32_t* tile_heads = (uint32_t*)dev_alloc(c, head_tiles * 4);
+  uint32_t* tile_head_off = (uint32_t*)dev_alloc(c, head_tiles * 4);
+  uint32_t* head_partial = (uint32_t*)dev_alloc(c, head_chunks * 4);
+  uint64_t* d_total_groups = (uint64_t*)dev_alloc(c, 8);
+  bool ok = keys[0] && vals[0] && ghist && bin_start && status && tickets && c->s_src && c->s_tgt && c->s_w &&
+            c->s_d && tile_heads && tile_head_off && head_partial && d_total_groups;
+  if (plan.n_passes > 1) ok = ok && keys[1] && vals[1];
+  auto drop_scratch = [&](int final_buf) {
+    for (int i = 0; i < 2; ++i) {
+      dev_free_later(c, keys[i]);
+      if (i != final_buf) dev_free_later(c, vals[i]);
+    }
+    dev_free_later(c, ghist); dev_free_later(c, bin_start); dev_free_later(c, status); dev_free_later(c, tickets);
+    dev_free_later(c, tile_heads); dev_free_later(c, tile_head_off); dev_free_later(c, head_partial);
+    dev_free_later(c, d_total_groups);
+  };
+  if (!ok) {
+    drop_scratch(-1);
+    return fail(c, NC_ERR_OOM, "out of device memory in nc_finalize");
+  }
+
+  // ---- a9: digit histograms of all passes + their exclusive scans ----
+  {
+    Scope sc(c, NC_PHASE_HISTOGRAM);
+    NC_CUDA(c, cudaMemsetAsync(ghist, 0, kMaxPasses * kRadix * 4, c->stream));
+    NC_CUDA(c, cudaMemsetAsync(tickets, 0, (kMaxPasses + 1) * 4, c->stream));
+    NC_CUDA(c, cudaMemsetAsync(status, 0, n_tiles * kRadix * 8, c->stream));
+    const unsigned grid = (unsigned)(((uint64_t)n + kHistThreads * kHistItems - 1) / (kHistThreads * kHistItems));
+    histogram_kernel<KeyT><<<grid, kHistThreads, 0, c->stream>>>(map, n, c->delay_bits, plan, ghist);
+    NC_LAUNCH_CHECK(c, "histogram");
+    bin_scan_kernel<<<plan.n_passes, kRadix, 0, c->stream>>>(ghist, bin_start);
+    NC_LAUNCH_CHECK(c, "bin_scan");
+  }
+
+  // ---- a10: onesweep passes, ping-pong between the two buffers ----
+  const size_t smem = sizeof(Smem);
+  NC_CUDA(c, cudaFuncSetAttribute(onesweep_kernel<KeyT, true, kSortThreads, kSortItems>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  NC_CUDA(c, cudaFuncSetAttribute(onesweep_kernel<KeyT, false, kSortThreads, kSortItems>,
+                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int cur = 0;
+  {
+    Scope sc(c, NC_PHASE_SORT);
+    for (uint32_t ps = 0; ps < plan.n_passes; ++ps) {
+      Scope pass_sc(c, NC_PHASE_SORT, true);
+      SortPassParams<KeyT> sp{};
+      sp.map = map;
+      sp.delay_bits = c->delay_bits;
+      sp.n = n;
+      const int dst = ps == 0 ? 0 : 1 - cur;
+      sp.keys_in = ps == 0 ? nullptr : keys[cur];
+      sp.vals_in = ps == 0 ? nullptr : vals[cur];
+      sp.keys_out = keys[dst];
+      sp.vals_out = vals[dst];
+      sp.shift = plan.shift[ps];
+      sp.bits = plan.bits[ps];
+      sp.bin_start = bin_start + ps * kRadix;
+      sp.status = status;
+      sp.ticket = tickets + ps;
+      sp.error_flag = tickets + kMaxPasses;
+      sp.epoch = (uint64_t)(ps + 1) << 42;
+      if (ps == 0) {
+        onesweep_kernel<KeyT, true, kSortThreads, kSortItems><<<(unsigned)n_tiles, kSortThreads, smem, c->stream>>>(sp);
+      } else {
+        onesweep_kernel<KeyT, false, kSortThreads, kSortItems><<<(unsigned)n_tiles, kSortThreads, smem, c->stream>>>(sp);
+      }
+      NC_LAUNCH_CHECK(c, "onesweep");
+      cur = dst;
+    }
+  }
+  c->perm = vals[cur];
+
+  // ---- a11: permutation apply ----
+  {
+    Scope sc(c, NC_PHASE_PERMUTE);
+    const unsigned grid = (unsigned)(((uint64_t)n + kPermThreads - 1) / kPermThreads);
+    permute_kernel<KeyT><<<grid, kPermThreads, 0, c->stream>>>(map, n, c->delay_bits, keys[cur], c->perm, c->s_src,
+                                                              c->s_tgt, c->s_w, c->s_d);
+    NC_LAUNCH_CHECK(c, "permute");
+  }
+
+  // ---- a12-a14: heads, scan, compaction, per-source offsets ----
+  uint64_t total_groups = 0;
+  uint32_t lookback_error = 0;
+  {
+    Scope sc(c, NC_PHASE_INDEX);
+    head_count_kernel<KeyT><<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(keys[cur], n, tile_heads);
+    NC_LAUNCH_CHECK(c, "head_count");
+    int rc = device_scan(c, tile_heads, tile_head_off, head_tiles, head_partial, d_total_groups);
+    if (rc != NC_OK) return rc;
+    NC_CUDA(c, cudaMemcpyAsync(&total_groups, d_total_groups, 8, cudaMemcpyDeviceToHost, c->stream));
+    NC_CUDA(c, cudaMemcpyAsync(&lookback_error, tickets + kMaxPasses, 4, cudaMemcpyDeviceToHost, c->stream));
+  }
+  NC_CUDA(c, cudaStreamSynchronize(c->stream));  // total_groups sizes the group arrays
+  if (lookback_error) {
+    drop_scratch(cur);
+    return fail(c, NC_ERR_CUDA, "onesweep look-back timed out");
+  }
+  c->total_groups = (uint32_t)total_groups;
+  c->group_start = (uint32_t*)dev_alloc(c, (size_t)total_groups * 4);
+  c->group_delay = (uint16_t*)dev_alloc(c, (size_t)total_groups * 2);
+  if (!c->group_start || !c->group_delay) {
+    drop_scratch(cur);
+    return fail(c, NC_ERR_OOM, "out of device memory for the group arrays");
+  }
+  {
+    Scope sc(c, NC_PHASE_INDEX);
+    IndexOut io{c->src_offsets, c->group_ptr, c->group_start, c->group_delay, N};
+    index_scatter_kernel<KeyT><<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(keys[cur], n, c->delay_bits,
+                                                                                    tile_head_off, d_total_groups, io);
+    NC_LAUNCH_CHECK(c, "index_scatter");
+    index_finish_kernel<<<(N + 255) / 256, 256, 0, c->stream>>>(c->src_offsets, c->group_ptr, N, c->out_degree,
+                                                               c->group_count, c->d_max + 1);
+    NC_LAUNCH_CHECK(c, "index_finish");
+  }
+  drop_scratch(cur);
+  return NC_OK;
+}
+
+int collect_timings(nc_context* c) {
+  int rc = sync_stream(c);
+  if (rc != NC_OK) return rc;
+  for (Span& s : c->spans) {
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, s.a, s.b);
+    if (s.is_pass) {
+      c->acc.sort_pass_ms += ms;
+      c->acc.sort_passes += 1;
+    } else {
+      c->acc.ms[s.phase] += ms;
+    }
+    cudaEventDestroy(s.a);
+    cudaEventDestroy(s.b);
+  }
+  c->spans.clear();
+  return NC_OK;
+}
+
+// ---- self-test kernels ----
+__global__ void selftest_philox_kernel(uint32_t n, const uint32_t* ctr, const uint32_t* key, uint32_t* out) {
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const Philox4 r = philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], key[2 * i], key[2 * i + 1]);
+  out[4 * i] = r.x;
+  out[4 * i + 1] = r.y;
+  out[4 * i + 2] = r.z;
+  out[4 * i + 3] = r.w;
+}
+
+__device__ void atomic_max_double(double* addr, double v) {  // v >= 0: bit patterns order like the values
+  atomicMax(reinterpret_cast<unsigned long long*>(addr), (unsigned long long)__double_as_longlong(v));
+}
+
+__global__ void selftest_fastpath_kernel(double* out /* [3] */) {
+  const uint32_t v = blockIdx.x * blockDim.x + threadIdx.x;  // 0 .. 2^24-1
+  const uint32_t word = v << 8;
+  const float r32 = fast_radius(word);
+  const double u1 = (double)(v + 1u) * (1.0 / 16777216.0);
+  const double r64 = sqrt(-2.0 * log(u1));
+  double er = r64 > 0.0 ? fabs((double)r32 - r64) / r64 : fabs((double)r32);
+  float sn, cs;
+  fast_sincos(word, sn, cs);
+  const double th = 6.283185307179586 * ((double)v * (1.0 / 16777216.0));
+  double es = fabs((double)sn - sin(th)), ec = fabs((double)cs - cos(th));
+  for (int d = 16; d > 0; d >>= 1) {
+    er = fmax(er, __shfl_xor_sync(0xffffffffu, er, d));
+    es = fmax(es, __shfl_xor_sync(0xffffffffu, es, d));
+    ec = fmax(ec, __shfl_xor_sync(0xffffffffu, ec, d));
+  }
+  if ((threadIdx.x & 31) == 0) {
+    atomic_max_double(out + 0, er);
+    atomic_max_double(out + 1, es);
+    atomic_max_double(out + 2, ec);
+  }
+}
+
+}  // namespace
+
+// =================================================================================================
+// C ABI
+// =================================================================================================
+extern "C" {
+
+int nc_create(const nc_config* cfg, nc_context** out) {
+  if (!cfg || !out) return NC_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!(cfg->dt_ms > 0.0) || std::isinf(cfg->dt_ms)) return NC_ERR_INVALID_ARG;
+  if ((cfg->mem.alloc == nullptr) != (cfg->mem.free == nullptr)) return NC_ERR_INVALID_ARG;
+  int count = 0;
+  if (cudaGetDeviceCount(&count) != cudaSuccess || count == 0) {
+    cudaGetLastError();
+    return NC_ERR_CUDA;  // no CPU fallback
+  }
+  int dev = cfg->device;
+  if (dev < 0) {
+    if (cudaGetDevice(&dev) != cudaSuccess) return NC_ERR_CUDA;
+  } else {
+    if (dev >= count || cudaSetDevice(dev) != cudaSuccess) return NC_ERR_CUDA;
+  }
+  nc_context* c = new (std::nothrow) nc_context();
+  if (!c) return NC_ERR_OOM;
+  c->cfg = *cfg;
+  c->device = dev;
+  c->stream = (cudaStream_t)cfg->cuda_stream;
+  c->B = cfg->block_size ? cfg->block_size : (1ull << 24);  // Q10
+  c->dt = cfg->dt_ms;
+  c->inv_dt = 1.0 / cfg->dt_ms;  // Q5: computed once
+  c->off_tgt = align_up(c->B * 4, 256);
+  c->off_w = c->off_tgt + align_up(c->B * 4, 256);
+  c->off_d = c->off_w + align_up(c->B * 4, 256);
+  c->block_bytes = c->off_d + align_up(c->B * 2, 256);
+  c->d_max = (uint32_t*)dev_alloc(c, 8);
+  if (!c->d_max) {
+    delete c;
+    return NC_ERR_OOM;
+  }
+  if (cudaMemsetAsync(c->d_max, 0, 8, c->stream) != cudaSuccess) {
+    dev_free(c, c->d_max);
+    delete c;
+    return NC_ERR_CUDA;
+  }
+  *out = c;
+  return NC_OK;
+}
+
+int nc_destroy(nc_context* c) {
+  if (!c) return NC_OK;
+  cudaStreamSynchronize(c->stream);
+  for (Span& s : c->spans) {
+    cudaEventDestroy(s.a);
+    cudaEventDestroy(s.b);
+  }
+  release_deferred(c);
+  std::vector<void*> all;
+  for (auto& kv : c->live) all.push_back(kv.first);
+  for (void* p : all) dev_free(c, p);
+  delete c;
+  return NC_OK;
+}
+
+const char* nc_last_error(nc_context* c) { return c ? c->err.c_str() : "null context"; }
+
+int nc_synchronize(nc_context* c) {
+  if (!c) return NC_ERR_INVALID_ARG;
+  return sync_stream(c);
+}
+
+int nc_create_population(nc_context* c, uint32_t n, uint32_t* first_id) {
+  if (!c || !first_id || n == 0) return fail(c, NC_ERR_INVALID_ARG, "nc_create_population: bad argument");
+  if (c->finalized) return fail(c, NC_ERR_STATE, "nc_create_population after nc_finalize");
+  if ((uint64_t)c->n_nodes + n > 0xffffffffull) return fail(c, NC_ERR_CAPACITY, "more than 2^32-1 nodes");
+  *first_id = c->n_nodes;  // D1
+  c->n_nodes += n;
+  return NC_OK;
+}
+
+int nc_connect(nc_context* c, nc_range src, nc_range tgt, nc_rule rule, const nc_rule_params* params,
+               const nc_syn_spec* syn, uint64_t seed) {
+  if (!c) return NC_ERR_INVALID_ARG;
+  if (c->finalized) return fail(c, NC_ERR_STATE, "nc_connect after nc_finalize");
+  if (!params || !syn) return fail(c, NC_ERR_INVALID_ARG, "nc_connect: null params");
+  if (src.count == 0 || tgt.count == 0) return fail(c, NC_ERR_INVALID_ARG, "nc_connect: empty node range");
+  if ((uint64_t)src.first + src.count > c->n_nodes || (uint64_t)tgt.first + tgt.count > c->n_nodes)
+    return fail(c, NC_ERR_INVALID_ARG, "nc_connect: node range outside the created nodes");
+  if (!dist_ok(syn->weight) || !dist_ok(syn->delay_ms))
+    return fail(c, NC_ERR_INVALID_ARG, "nc_connect: bad distribution (sd < 0, lo > hi or NaN)");
+  const uint64_t K = params->degree_or_total;
+  uint64_t n_new = 0;
+  switch (rule) {
+    case NC_ONE_TO_ONE:
+      if (src.count != tgt.count) return fail(c, NC_ERR_INVALID_ARG, "one_to_one needs N_sources == N_targets");
+      n_new = src.count;
+      break;
+    case NC_ALL_TO_ALL:
+      n_new = (uint64_t)src.count * tgt.count;
+      break;
+    case NC_FIXED_OUTDEGREE:
+      if (K > kMaxConns) return fail(c, NC_ERR_CAPACITY, "out-degree too large");
+      n_new = (uint64_t)src.count * K;
+      break;
+    case NC_FIXED_INDEGREE:
+      if (K > kMaxConns) return fail(c, NC_ERR_CAPACITY, "in-degree too large");
+      n_new = (uint64_t)tgt.count * K;
+      break;
+    case NC_FIXED_TOTAL_NUMBER:
+      n_new = K;
+      break;
+    case NC_PAIRWISE_BERNOULLI:
+      if (!(params->p >= 0.0 && params->p <= 1.0)) return fail(c, NC_ERR_INVALID_ARG, "p outside [0, 1]");
+      break;
+    default:
+      return fail(c, NC_ERR_INVALID_ARG, "unknown rule");
+  }
+  if (rule != NC_PAIRWISE_BERNOULLI && n_new > kMaxConns) return fail(c, NC_ERR_CAPACITY, "more than 2^32-1 connections");
+  const double bound = delay_bound_steps(syn->delay_ms, c->inv_dt);
+  if (bound > 65535.0) return fail(c, NC_ERR_CAPACITY, "delay can exceed 65535 steps");
+  if (rule != NC_PAIRWISE_BERNOULLI && c->n_conns + n_new > kMaxConns)
+    return fail(c, NC_ERR_CAPACITY, "more than 2^32-1 connections");
+
+  GenParams gp{};
+  gp.pos0 = c->n_conns;
+  gp.n = n_new;
+  gp.s0 = src.first;
+  gp.n_src = src.count;
+  gp.t0 = tgt.first;
+  gp.n_tgt = tgt.count;
+  gp.K = (uint32_t)K;
+  gp.seed_lo = (uint32_t)(seed & 0xffffffffull);
+  gp.seed_hi = (uint32_t)(seed >> 32);
+  gp.projection_id = c->n_proj;
+  gp.syn = make_syn(c, *syn);
+
+  if (rule == NC_PAIRWISE_BERNOULLI) {
+    int rc = connect_bernoulli(c, gp, params->p);
+    if (rc != NC_OK) return rc;
+  } else if (n_new > 0) {
+    int rc = reserve_blocks(c, n_new);
+    if (rc != NC_OK) return rc;
+    gp.map = make_map(c);
+    const bool vec = (c->B % 4) == 0;
+    {
+      Scope sc(c, NC_PHASE_GENERATE);
+      switch (rule) {
+        case NC_ONE_TO_ONE: launch_generate<kOneToOne>(c, gp, vec); break;
+        case NC_ALL_TO_ALL: launch_generate<kAllToAll>(c, gp, vec); break;
+        case NC_FIXED_INDEGREE: launch_generate<kFixedIndegree>(c, gp, vec); break;
+        case NC_FIXED_OUTDEGREE: launch_generate<kFixedOutdegree>(c, gp, vec); break;
+        default: launch_generate<kFixedTotalNumber>(c, gp, vec); break;
+      }
+      NC_LAUNCH_CHECK(c, "generate");
+    }
+    c->n_conns += n_new;
+  }
+  c->n_proj += 1;
+  if (bound > (double)c->max_delay_steps) c->max_delay_steps = (uint32_t)bound;
+  c->have_in = c->have_out = false;
+  return NC_OK;
+}
+
+int nc_finalize(nc_context* c) {
+  if (!c) return NC_ERR_INVALID_ARG;
+  if (c->finalized) return fail(c, NC_ERR_STATE, "nc_finalize called twice");
+  const uint32_t N = c->n_nodes;
+  c->src_offsets = (uint32_t*)dev_alloc(c, ((size_t)N + 1) * 4);
+  c->group_ptr = (uint32_t*)dev_alloc(c, ((size_t)N + 1) * 4);
+  c->group_count = (uint32_t*)dev_alloc(c, (size_t)N * 4);
+  if (!c->out_degree) c->out_degree = (uint32_t*)dev_alloc(c, (size_t)N * 4);
+  if (!c->src_offsets || !c->group_ptr || !c->group_count || !c->out_degree)
+    return fail(c, NC_ERR_OOM, "out of device memory for the index");
+  NC_CUDA(c, cudaMemsetAsync(c->d_max + 1, 0, 4, c->stream));
+
+  // key-width plan: source bits from the node count, delay bits from the analytic bound (Q6)
+  c->delay_bits = std::max(1u, bit_width_u64(c->max_delay_steps));
+  const uint32_t src_bits = std::max(1u, bit_width_u64(N > 0 ? (uint64_t)N - 1 : 0));
+  c->key_bits = src_bits + c->delay_bits;
+  const PassPlan plan = plan_passes(c->key_bits);
+  c->sort_passes = plan.n_passes;
+
+  if (c->n_conns == 0) {
+    NC_CUDA(c, cudaMemsetAsync(c->src_offsets, 0, ((size_t)N + 1) * 4, c->stream));
+    NC_CUDA(c, cudaMemsetAsync(c->group_ptr, 0, ((size_t)N + 1) * 4, c->stream));
+    if (N) {
+      NC_CUDA(c, cudaMemsetAsync(c->group_count, 0, (size_t)N * 4, c->stream));
+      NC_CUDA(c, cudaMemsetAsync(c->out_degree, 0, (size_t)N * 4, c->stream));
+    }
+    c->total_groups = 0;
+    c->sort_passes = 0;
+  } else {
+    int rc = c->key_bits <= 32 ? sort_and_index<uint32_t>(c, plan) : sort_and_index<uint64_t>(c, plan);
+    if (rc != NC_OK) return rc;
+  }
+  c->finalized = true;
+  c->have_out = true;
+  return NC_OK;
+}
+
+int nc_num_connections(nc_context* c, uint64_t* n) {
+  if (!c || !n) return NC_ERR_INVALID_ARG;
+  *n = c->n_conns;  // pairwise_bernoulli already waited for its count inside nc_connect
+  return NC_OK;
+}
+
+int nc_num_nodes(nc_context* c, uint32_t* n) {
+  if (!c || !n) return NC_ERR_INVALID_ARG;
+  *n = c->n_nodes;
+  return NC_OK;
+}
+
+int nc_get_connections(nc_context* c, int sorted, nc_connections_view* out) {
+  if (!c || !out) return NC_ERR_INVALID_ARG;
+  std::memset(out, 0, sizeof(*out));
+  out->n = c->n_conns;
+  out->block_size = c->B;
+  if (sorted) {
+    if (!c->finalized) return fail(c, NC_ERR_STATE, "sorted view before nc_finalize");
+    out->source = c->s_src;
+    out->target = c->s_tgt;
+    out->weight = c->s_w;
+    out->delay = c->s_d;
+    out->perm = c->perm;
+    return NC_OK;
+  }
+  out->n_blocks = c->blocks.size();
+  out->blocks = c->blocks.data();
+  out->off_source = 0;
+  out->off_target = c->off_tgt;
+  out->off_weight = c->off_w;
+  out->off_delay = c->off_d;
+  if (c->blocks.size() == 1) {
+    char* b = (char*)c->blocks[0];
+    out->source = (const uint32_t*)b;
+    out->target = (const uint32_t*)(b + c->off_tgt);
+    out->weight = (const float*)(b + c->off_w);
+    out->delay = (const uint16_t*)(b + c->off_d);
+  }
+  return NC_OK;
+}
+
+int nc_get_index(nc_context* c, nc_index_view* out) {
+  if (!c || !out) return NC_ERR_INVALID_ARG;
+  if (!c->finalized) return fail(c, NC_ERR_STATE, "index before nc_finalize");
+  out->src_offsets = c->src_offsets;
+  out->group_count = c->group_count;
+  out->group_ptr = c->group_ptr;
+  out->group_start = c->group_start;
+  out->group_delay = c->group_delay;
+  out->n_nodes = c->n_nodes;
+  out->total_groups = c->total_groups;
+  return NC_OK;
+}
+
+int nc_degree_histogram(nc_context* c, int kind, const uint32_t** per_node_degree, uint32_t* max_degree) {
+  if (!c || (kind != 0 && kind != 1)) return fail(c, NC_ERR_INVALID_ARG, "nc_degree_histogram: bad argument");
+  const uint32_t N = c->n_nodes;
+  bool& have = kind == 0 ? c->have_in : c->have_out;
+  uint32_t*& deg = kind == 0 ? c->in_degree : c->out_degree;
+  if (!have) {
+    if (!deg) {
+      deg = (uint32_t*)dev_alloc(c, (size_t)N * 4);
+      if (!deg) return fail(c, NC_ERR_OOM, "out of device memory for the degree histogram");
+    }
+    Scope sc(c, NC_PHASE_DEGREE);
+    if (N) NC_CUDA(c, cudaMemsetAsync(deg, 0, (size_t)N * 4, c->stream));
+    NC_CUDA(c, cudaMemsetAsync(c->d_max + kind, 0, 4, c->stream));
+    if (c->n_conns && N) {
+      const unsigned grid = (unsigned)std::min<uint64_t>((c->n_conns + 255) / 256, 148ull * 32);
+      degree_count_kernel<<<grid, 256, 0, c->stream>>>(make_map(c), c->n_conns, kind, deg);
+      NC_LAUNCH_CHECK(c, "degree_count");
+      max_u32_kernel<<<std::min<unsigned>((N + 255) / 256, 1024u), 256, 0, c->stream>>>(deg, N, c->d_max + kind);
+      NC_LAUNCH_CHECK(c, "max_u32");
+    }
+    have = true;
+  }
+  if (per_node_degree) *per_node_degree = deg;
+  if (max_degree) {
+    NC_CUDA(c, cudaMemcpyAsync(max_degree, c->d_max + kind, 4, cudaMemcpyDeviceToHost, c->stream));
+    int rc = sync_stream(c);
+    if (rc != NC_OK) return rc;
+  }
+  return NC_OK;
+}
+
+int nc_get_stats(nc_context* c, nc_stats* out) {
+  if (!c || !out) return NC_ERR_INVALID_ARG;
+  out->kernel_launches = c->launches;
+  out->bytes_in_use = c->bytes_in_use;
+  out->bytes_peak = c->bytes_peak;
+  out->n_blocks = c->blocks.size();
+  out->n_projections = c->n_proj;
+  out->key_bits = c->key_bits;
+  out->sort_passes = c->sort_passes;
+  out->delay_bits = c->delay_bits;
+  return NC_OK;
+}
+
+int nc_get_timings(nc_context* c, nc_timings* out) {
+  if (!c || !out) return NC_ERR_INVALID_ARG;
+  if (!(c->cfg.flags & NC_FLAG_TIMING)) return fail(c, NC_ERR_STATE, "context was created without NC_FLAG_TIMING");
+  int rc = collect_timings(c);
+  if (rc != NC_OK) return rc;
+  *out = c->acc;
+  return NC_OK;
+}
+
+int nc_read_connections(nc_context* c, int sorted, uint64_t first, uint64_t count, uint32_t* source, uint32_t* target,
+                        float* weight, uint16_t* delay, uint32_t* perm) {
+  if (!c) return NC_ERR_INVALID_ARG;
+  if (first + count > c->n_conns) return fail(c, NC_ERR_INVALID_ARG, "nc_read_connections: range outside the connections");
+  if (sorted && !c->finalized) return fail(c, NC_ERR_STATE, "sorted view before nc_finalize");
+  if (count == 0) return NC_OK;
+  const cudaMemcpyKind k = cudaMemcpyDeviceToHost;
+  if (sorted) {
+    if (source) NC_CUDA(c, cudaMemcpyAsync(source, c->s_src + first, count * 4, k, c->stream));
+    if (target) NC_CUDA(c, cudaMemcpyAsync(target, c->s_tgt + first, count * 4, k, c->stream));
+    if (weight) NC_CUDA(c, cudaMemcpyAsync(weight, c->s_w + first, count * 4, k, c->stream));
+    if (delay) NC_CUDA(c, cudaMemcpyAsync(delay, c->s_d + first, count * 2, k, c->stream));
+    if (perm) NC_CUDA(c, cudaMemcpyAsync(perm, c->perm + first, count * 4, k, c->stream));
+  } else {
+    uint64_t pos = first, done = 0;
+    while (done < count) {
+      const uint64_t blk = pos / c->B, slot = pos % c->B;
+      const uint64_t m = std::min(count - done, c->B - slot);
+      char* b = (char*)c->blocks[blk];
+      if (source) NC_CUDA(c, cudaMemcpyAsync(source + done, (uint32_t*)b + slot, m * 4, k, c->stream));
+      if (target) NC_CUDA(c, cudaMemcpyAsync(target + done, (uint32_t*)(b + c->off_tgt) + slot, m * 4, k, c->stream));
+      if (weight) NC_CUDA(c, cudaMemcpyAsync(weight + done, (float*)(b + c->off_w) + slot, m * 4, k, c->stream));
+      if (delay) NC_CUDA(c, cudaMemcpyAsync(delay + done, (uint16_t*)(b + c->off_d) + slot, m * 2, k, c->stream));
+      pos += m;
+      done += m;
+    }
+  }
+  return sync_stream(c);
+}
+
+int nc_read_index(nc_context* c, uint32_t* src_offsets, uint32_t* group_count, uint32_t* group_ptr, uint32_t* group_start,
+                  uint16_t* group_delay) {
+  if (!c) return NC_ERR_INVALID_ARG;
+  if (!c->finalized) return fail(c, NC_ERR_STATE, "index before nc_finalize");
+  const cudaMemcpyKind k = cudaMemcpyDeviceToHost;
+  const size_t N = c->n_nodes, G = c->total_groups;
+  if (src_offsets) NC_CUDA(c, cudaMemcpyAsync(src_offsets, c->src_offsets, (N + 1) * 4, k, c->stream));
+  if (group_ptr) NC_CUDA(c, cudaMemcpyAsync(group_ptr, c->group_ptr, (N + 1) * 4, k, c->stream));
+  if (group_count && N) NC_CUDA(c, cudaMemcpyAsync(group_count, c->group_count, N * 4, k, c->stream));
+  if (group_start && G) NC_CUDA(c, cudaMemcpyAsync(group_start, c->group_start, G * 4, k, c->stream));
+  if (group_delay && G) NC_CUDA(c, cudaMemcpyAsync(group_delay, c->group_delay, G * 2, k, c->stream));
+  return sync_stream(c);
+}
+
+int nc_read_degree_histogram(nc_context* c, int kind, uint32_t* per_node_degree, uint32_t* max_degree) {
+  const uint32_t* dev = nullptr;
+  int rc = nc_degree_histogram(c, kind, &dev, max_degree);
+  if (rc != NC_OK) return rc;
+  if (per_node_degree && c->n_nodes)
+    NC_CUDA(c, cudaMemcpyAsync(per_node_degree, dev, (size_t)c->n_nodes * 4, cudaMemcpyDeviceToHost, c->stream));
+  return sync_stream(c);
+}
+
+int nc_selftest_philox(nc_context* c, uint32_t n, const uint32_t* ctr, const uint32_t* key, uint32_t* out) {
+  if (!c || !ctr || !key || !out) return NC_ERR_INVALID_ARG;
+  if (n == 0) return NC_OK;
+  uint32_t* d_ctr = (uint32_t*)dev_alloc(c, (size_t)n * 16);
+  uint32_t* d_key = (uint32_t*)dev_alloc(c, (size_t)n * 8);
+  uint32_t* d_out = (uint32_t*)dev_alloc(c, (size_t)n * 16);
+  if (!d_ctr || !d_key || !d_out) return fail(c, NC_ERR_OOM, "selftest: out of device memory");
+  NC_CUDA(c, cudaMemcpyAsync(d_ctr, ctr, (size_t)n * 16, cudaMemcpyHostToDevice, c->stream));
+  NC_CUDA(c, cudaMemcpyAsync(d_key, key, (size_t)n * 8, cudaMemcpyHostToDevice, c->stream));
+  selftest_philox_kernel<<<(n + 127) / 128, 128, 0, c->stream>>>(n, d_ctr, d_key, d_out);
+  NC_LAUNCH_CHECK(c, "selftest_philox");
+  NC_CUDA(c, cudaMemcpyAsync(out, d_out, (size_t)n * 16, cudaMemcpyDeviceToHost, c->stream));
+  int rc = sync_stream(c);
+  dev_free(c, d_ctr);
+  dev_free(c, d_key);
+  dev_free(c, d_out);
+  return rc;
+}
+
+int nc_selftest_fastpath(nc_context* c, double* max_rel_err_r, double* max_abs_err_sin, double* max_abs_err_cos) {
+  if (!c) return NC_ERR_INVALID_ARG;
+  double* d = (double*)dev_alloc(c, 24);
+  if (!d) return fail(c, NC_ERR_OOM, "selftest: out of device memory");
+  NC_CUDA(c, cudaMemsetAsync(d, 0, 24, c->stream));
+  selftest_fastpath_kernel<<<(1u << 24) / 256, 256, 0, c->stream>>>(d);
+  NC_LAUNCH_CHECK(c, "selftest_fastpath");
+  double h[3] = {0, 0, 0};
+  NC_CUDA(c, cudaMemcpyAsync(h, d, 24, cudaMemcpyDeviceToHost, c->stream));
+  int rc = sync_stream(c);
+  dev_free(c, d);
+  if (max_rel_err_r) *max_rel_err_r = h[0];
+  if (max_abs_err_sin) *max_abs_err_sin = h[1];
+  if (max_abs_err_cos) *max_abs_err_cos = h[2];
+  return rc;
+}
+
+}  // extern "C"

@@ -1,0 +1,243 @@
+// nc_index.cuh -- index construction over the sorted keys (steps a12-a15 of DESIGN.md):
+// group heads (source or delay differs from the previous connection), their device-wide exclusive scan,
+// compaction into group_start / group_delay, per-source offsets src_offsets and p_i of Eq. 14, G_i and
+// the degree histograms.  Also a generic device-wide exclusive scan used by pairwise_bernoulli.
+#pragma once
+
+#include "nc_common.cuh"
+
+namespace nc {
+
+// ---------------------------------------------------------------------------------------------
+// Device-wide exclusive scan of a u32 array (reduce -> scan of partials -> downsweep).
+// ---------------------------------------------------------------------------------------------
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 16;
+constexpr int kScanChunk = kScanThreads * kScanItems;
+
+__device__ __forceinline__ uint32_t block_exclusive_scan_256(uint32_t v, uint32_t* warp_tmp /*[8]*/, uint32_t& total) {
+  uint32_t inc = v;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d);
+    if (lane_id() >= (uint32_t)d) inc += t;
+  }
+  __syncthreads();  // protect warp_tmp against a previous use
+  if (lane_id() == 31) warp_tmp[threadIdx.x >> 5] = inc;
+  __syncthreads();
+  uint32_t base = 0, tot = 0;
+#pragma unroll
+  for (uint32_t w = 0; w < kScanThreads / 32; ++w) {
+    const uint32_t t = warp_tmp[w];
+    if (w < (threadIdx.x >> 5)) base += t;
+    tot += t;
+  }
+  total = tot;
+  return base + inc - v;
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_reduce_kernel(const uint32_t* __restrict__ in, uint64_t n,
+                                                                  uint32_t* __restrict__ partial) {
+  __shared__ uint32_t warp_tmp[kScanThreads / 32];
+  const uint64_t base = (uint64_t)blockIdx.x * kScanChunk;
+  uint32_t s = 0;
+#pragma unroll
+  for (int i = 0; i < kScanItems; ++i) {
+    const uint64_t idx = base + (uint64_t)i * kScanThreads + threadIdx.x;
+    if (idx < n) s += in[idx];
+  }
+  s = __reduce_add_sync(0xffffffffu, s);
+  if (lane_id() == 0) warp_tmp[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t t = 0;
+#pragma unroll
+    for (int w = 0; w < kScanThreads / 32; ++w) t += warp_tmp[w];
+    partial[blockIdx.x] = t;
+  }
+}
+
+// single CTA: exclusive scan of the partials in place, grand total (64-bit) to *total
+__global__ void __launch_bounds__(kScanThreads) scan_partials_kernel(uint32_t* __restrict__ partial, uint64_t n_partial,
+                                                                    uint64_t* __restrict__ total) {
+  __shared__ uint32_t warp_tmp[kScanThreads / 32];
+  uint64_t run = 0;
+  for (uint64_t base = 0; base < n_partial; base += kScanThreads) {
+    const uint64_t idx = base + threadIdx.x;
+    const uint32_t v = idx < n_partial ? partial[idx] : 0u;
+    uint32_t tot;
+    const uint32_t ex = block_exclusive_scan_256(v, warp_tmp, tot);
+    if (idx < n_partial) partial[idx] = (uint32_t)run + ex;
+    run += tot;
+  }
+  if (threadIdx.x == 0) *total = run;
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_downsweep_kernel(const uint32_t* __restrict__ in, uint64_t n,
+                                                                     const uint32_t* __restrict__ partial,
+                                                                     uint32_t* __restrict__ out) {
+  __shared__ uint32_t warp_tmp[kScanThreads / 32];
+  const uint64_t base = (uint64_t)blockIdx.x * kScanChunk + (uint64_t)threadIdx.x * kScanItems;
+  uint32_t v[kScanItems];
+  uint32_t s = 0;
+#pragma unroll
+  for (int i = 0; i < kScanItems; ++i) {
+    v[i] = (base + i < n) ? in[base + i] : 0u;
+    s += v[i];
+  }
+  uint32_t tot;
+  uint32_t ex = block_exclusive_scan_256(s, warp_tmp, tot) + partial[blockIdx.x];
+#pragma unroll
+  for (int i = 0; i < kScanItems; ++i) {
+    if (base + i < n) out[base + i] = ex;
+    ex += v[i];
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Group heads.  Position j is a head iff j == 0 or key[j] != key[j-1] (the key packs source and delay).
+// ---------------------------------------------------------------------------------------------
+constexpr int kHeadThreads = 256;
+constexpr int kHeadItems = 8;
+constexpr int kHeadTile = kHeadThreads * kHeadItems;
+
+template <typename KeyT>
+__global__ void __launch_bounds__(kHeadThreads) head_count_kernel(const KeyT* __restrict__ keys, uint32_t n,
+                                                                 uint32_t* __restrict__ tile_heads) {
+  __shared__ uint32_t warp_tmp[kHeadThreads / 32];
+  const uint64_t base = (uint64_t)blockIdx.x * kHeadTile + (uint64_t)threadIdx.x * kHeadItems;
+  uint32_t c = 0;
+  if (base < n) {
+    KeyT prev = base > 0 ? keys[base - 1] : (KeyT)0;
+#pragma unroll
+    for (int i = 0; i < kHeadItems; ++i) {
+      const uint64_t j = base + i;
+      if (j < n) {
+        const KeyT k = keys[j];
+        c += (j == 0 || k != prev) ? 1u : 0u;
+        prev = k;
+      }
+    }
+  }
+  c = __reduce_add_sync(0xffffffffu, c);
+  if (lane_id() == 0) warp_tmp[threadIdx.x >> 5] = c;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t t = 0;
+#pragma unroll
+    for (int w = 0; w < kHeadThreads / 32; ++w) t += warp_tmp[w];
+    tile_heads[blockIdx.x] = t;
+  }
+}
+
+struct IndexOut {
+  uint32_t* src_offsets;  // [n_nodes + 1]
+  uint32_t* group_ptr;    // [n_nodes + 1]
+  uint32_t* group_start;  // [total_groups]
+  uint16_t* group_delay;  // [total_groups]
+  uint32_t n_nodes;
+};
+
+// One thread per kHeadItems consecutive sorted positions.  A head at position j gets group number
+// g = (heads before j); if it is also the first connection of its source s, then for every node s' in
+// (previous source, s] (the ones in between have no outgoing connection, Q9):
+//   src_offsets[s'] = j  and  group_ptr[s'] = g   -- exactly exclusive_scan(out_degree) and Eq. 14.
+template <typename KeyT>
+__global__ void __launch_bounds__(kHeadThreads) index_scatter_kernel(const KeyT* __restrict__ keys, uint32_t n,
+                                                                    uint32_t delay_bits,
+                                                                    const uint32_t* __restrict__ tile_head_off,
+                                                                    const uint64_t* __restrict__ total_groups,
+                                                                    const __grid_constant__ IndexOut out) {
+  __shared__ uint32_t warp_tmp[kHeadThreads / 32];
+  const uint64_t base = (uint64_t)blockIdx.x * kHeadTile + (uint64_t)threadIdx.x * kHeadItems;
+  KeyT k[kHeadItems];
+  KeyT prev0 = 0;
+  uint32_t flags = 0, c = 0;
+  if (base < n) {
+    prev0 = base > 0 ? keys[base - 1] : (KeyT)0;
+    KeyT prev = prev0;
+#pragma unroll
+    for (int i = 0; i < kHeadItems; ++i) {
+      const uint64_t j = base + i;
+      k[i] = j < n ? keys[j] : (KeyT)0;
+      if (j < n && (j == 0 || k[i] != prev)) {
+        flags |= 1u << i;
+        ++c;
+      }
+      prev = k[i];
+    }
+  }
+  uint32_t tot;
+  uint32_t g = block_exclusive_scan_256(c, warp_tmp, tot) + tile_head_off[blockIdx.x];
+  if (base >= n) return;
+  const uint32_t dmask = (1u << delay_bits) - 1u;
+  KeyT prev = prev0;
+#pragma unroll
+  for (int i = 0; i < kHeadItems; ++i) {
+    const uint64_t j = base + i;
+    if (j < n) {
+      if (flags & (1u << i)) {
+        const uint32_t s = (uint32_t)(k[i] >> delay_bits);
+        out.group_start[g] = (uint32_t)j;
+        out.group_delay[g] = (uint16_t)((uint32_t)k[i] & dmask);
+        const bool first_of_source = (j == 0) || (uint32_t)(prev >> delay_bits) != s;
+        if (first_of_source) {
+          const uint32_t lo = (j == 0) ? 0u : (uint32_t)(prev >> delay_bits) + 1u;
+          for (uint32_t node = lo; node <= s; ++node) {
+            out.src_offsets[node] = (uint32_t)j;
+            out.group_ptr[node] = g;
+          }
+        }
+        ++g;
+      }
+      if (j == (uint64_t)n - 1) {  // nodes after the last source, and the closing entries
+        const uint32_t s = (uint32_t)(k[i] >> delay_bits);
+        const uint32_t tg = (uint32_t)(*total_groups);
+        for (uint64_t node = (uint64_t)s + 1; node <= out.n_nodes; ++node) {
+          out.src_offsets[node] = n;
+          out.group_ptr[node] = tg;
+        }
+      }
+      prev = k[i];
+    }
+  }
+}
+
+// G_i = p_{i+1} - p_i and out_degree_i = src_offsets_{i+1} - src_offsets_i, plus the maximum out-degree.
+__global__ void __launch_bounds__(256) index_finish_kernel(const uint32_t* __restrict__ src_offsets,
+                                                          const uint32_t* __restrict__ group_ptr, uint32_t n_nodes,
+                                                          uint32_t* __restrict__ out_degree,
+                                                          uint32_t* __restrict__ group_count,
+                                                          uint32_t* __restrict__ max_out_degree) {
+  const uint32_t s = blockIdx.x * 256u + threadIdx.x;
+  uint32_t deg = 0;
+  if (s < n_nodes) {
+    deg = src_offsets[s + 1] - src_offsets[s];
+    out_degree[s] = deg;
+    group_count[s] = group_ptr[s + 1] - group_ptr[s];
+  }
+  deg = __reduce_max_sync(0xffffffffu, deg);
+  if (lane_id() == 0 && deg) atomicMax(max_out_degree, deg);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Degree histograms over the storage blocks (creation order; usable before nc_finalize).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) degree_count_kernel(const __grid_constant__ BlockMap map, uint64_t n, int kind,
+                                                          uint32_t* __restrict__ degree) {
+  const uint64_t stride = (uint64_t)gridDim.x * 256u;
+  for (uint64_t pos = (uint64_t)blockIdx.x * 256u + threadIdx.x; pos < n; pos += stride) {
+    const BlockAddr a = locate(map, pos);
+    const uint32_t node = kind == 0 ? *tgt_ptr(map, a) : *src_ptr(map, a);
+    atomicAdd(degree + node, 1u);
+  }
+}
+
+__global__ void __launch_bounds__(256) max_u32_kernel(const uint32_t* __restrict__ v, uint32_t n, uint32_t* __restrict__ out) {
+  uint32_t m = 0;
+  for (uint64_t i = (uint64_t)blockIdx.x * 256u + threadIdx.x; i < n; i += (uint64_t)gridDim.x * 256u) m = max(m, v[i]);
+  m = __reduce_max_sync(0xffffffffu, m);
+  if (lane_id() == 0 && m) atomicMax(out, m);
+}
+
+}  // namespace nc

@@ -1,0 +1,298 @@
+// nc_sort.cuh -- stable LSD radix sort of all connections by the packed (source, delay) key
+// (steps a9-a11 of DESIGN.md; "hierarchically using two sorting keys: the index of the
+// source node as the first key and the delay as the second"; reading D10: ties keep creation order).
+//
+//   key  = (source << delay_bits) | delay          payload = creation position (u32)
+//   histogram_kernel : one read of (source, delay) from the storage blocks -> P digit histograms
+//   onesweep_kernel  : one pass per digit: a tile is ranked in shared memory (warp match), its digit
+//                      counts are chained to the previous tiles by decoupled look-back (Merrill & Garland
+//                      style single-pass scan, one 64-bit status word per (tile, digit)), and keys +
+//                      payload are written out as per-digit runs staged through shared memory
+//   permute_kernel   : sorted target/weight gathered by the permutation; source/delay unpacked from the key
+#pragma once
+
+#include "nc_common.cuh"
+
+namespace nc {
+
+constexpr int kRadixBits = 8;
+constexpr int kRadix = 1 << kRadixBits;
+constexpr int kMaxPasses = 6;  // 48-bit keys: 32-bit source + 16-bit delay
+
+struct PassPlan {
+  uint32_t n_passes;
+  uint32_t shift[kMaxPasses];
+  uint32_t bits[kMaxPasses];
+};
+
+template <typename KeyT>
+__device__ __forceinline__ uint32_t digit_of(KeyT key, uint32_t shift, uint32_t mask) {
+  return (uint32_t)(key >> shift) & mask;
+}
+
+template <typename KeyT>
+__device__ __forceinline__ KeyT load_key_from_storage(const BlockMap& map, uint64_t pos, uint32_t delay_bits) {
+  const BlockAddr a = locate(map, pos);
+  const uint32_t s = *src_ptr(map, a);
+  const uint32_t d = *d_ptr(map, a);
+  return ((KeyT)s << delay_bits) | (KeyT)d;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Digit histograms of all passes in one read of the keys.
+// ---------------------------------------------------------------------------------------------
+constexpr int kHistThreads = 512;
+constexpr int kHistItems = 16;
+
+template <typename KeyT>
+__global__ void __launch_bounds__(kHistThreads) histogram_kernel(const __grid_constant__ BlockMap map, uint32_t n,
+                                                                uint32_t delay_bits,
+                                                                const __grid_constant__ PassPlan plan,
+                                                                uint32_t* __restrict__ ghist /* [P][256] */) {
+  __shared__ uint32_t hist[kMaxPasses][kRadix];
+  for (int i = threadIdx.x; i < kMaxPasses * kRadix; i += kHistThreads) (&hist[0][0])[i] = 0;
+  __syncthreads();
+  const uint64_t tile0 = (uint64_t)blockIdx.x * (kHistThreads * kHistItems);
+#pragma unroll 4
+  for (int i = 0; i < kHistItems; ++i) {
+    const uint64_t pos = tile0 + (uint64_t)i * kHistThreads + threadIdx.x;
+    if (pos < n) {
+      const KeyT key = load_key_from_storage<KeyT>(map, pos, delay_bits);
+      for (uint32_t ps = 0; ps < plan.n_passes; ++ps) {
+        const uint32_t d = digit_of(key, plan.shift[ps], (1u << plan.bits[ps]) - 1u);
+        atomicAdd(&hist[ps][d], 1u);
+      }
+    }
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < (int)plan.n_passes * kRadix; i += kHistThreads) {
+    const uint32_t v = (&hist[0][0])[i];
+    if (v) atomicAdd(ghist + i, v);
+  }
+}
+
+// exclusive scan of each pass's 256 bins -> first output position of every digit
+__global__ void __launch_bounds__(kRadix) bin_scan_kernel(const uint32_t* __restrict__ ghist,
+                                                         uint32_t* __restrict__ bin_start) {
+  __shared__ uint32_t warp_tot[kRadix / 32];
+  const uint32_t ps = blockIdx.x;
+  const uint32_t v = ghist[ps * kRadix + threadIdx.x];
+  uint32_t inc = v;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d);
+    if (lane_id() >= (uint32_t)d) inc += t;
+  }
+  if (lane_id() == 31) warp_tot[threadIdx.x >> 5] = inc;
+  __syncthreads();
+  uint32_t base = 0;
+  for (uint32_t w = 0; w < (threadIdx.x >> 5); ++w) base += warp_tot[w];
+  bin_start[ps * kRadix + threadIdx.x] = base + inc - v;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Onesweep digit pass.
+// Look-back status word (one per tile and digit, never re-zeroed: the epoch tag tells passes apart):
+//   bits  0..39 count | bits 40..41 flag (1 = tile aggregate, 2 = inclusive prefix) | bits 42..63 epoch
+// ---------------------------------------------------------------------------------------------
+constexpr uint64_t kFlagAggregate = 1ull << 40;
+constexpr uint64_t kFlagInclusive = 2ull << 40;
+constexpr uint64_t kCountMask = (1ull << 40) - 1;
+
+template <typename KeyT>
+struct SortPassParams {
+  BlockMap map;  // FIRST pass: keys are built from the storage blocks and the payload is the position
+  uint32_t delay_bits;
+  uint32_t n;
+  const KeyT* keys_in;
+  const uint32_t* vals_in;
+  KeyT* keys_out;
+  uint32_t* vals_out;
+  uint32_t shift, bits;
+  const uint32_t* bin_start;  // [256]
+  uint64_t* status;           // [n_tiles][256]
+  uint32_t* ticket;
+  uint32_t* error_flag;       // set to 1 if a look-back ever gives up (never expected; avoids a device hang)
+  uint64_t epoch;             // already shifted to bits 42..63
+};
+
+template <typename KeyT, int THREADS, int ITEMS>
+struct OnesweepSmem {
+  static constexpr int kTile = THREADS * ITEMS;
+  static constexpr int kWarps = THREADS / 32;
+  KeyT keys[kTile];
+  uint32_t vals[kTile];
+  uint32_t warp_hist[kWarps][kRadix];
+  uint32_t tile_excl[kRadix];   // exclusive scan of the tile's digit counts
+  uint32_t global_off[kRadix];  // (global first position of the digit for this tile) - tile_excl[d]
+  uint32_t scan_tmp[kRadix / 32];
+  uint32_t tile_id;
+};
+
+template <typename KeyT, bool FIRST, int THREADS, int ITEMS>
+__global__ void __launch_bounds__(THREADS) onesweep_kernel(const __grid_constant__ SortPassParams<KeyT> p) {
+  using Smem = OnesweepSmem<KeyT, THREADS, ITEMS>;
+  constexpr int kTile = Smem::kTile;
+  constexpr int kWarps = Smem::kWarps;
+  static_assert(THREADS >= kRadix, "one thread per digit is needed for the look-back");
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
+
+  const uint32_t warp = threadIdx.x >> 5, lane = lane_id();
+  // tiles are handed out in launch order so that a tile only ever waits on tiles that already run
+  if (threadIdx.x == 0) sm.tile_id = atomicAdd(p.ticket, 1u);
+  for (int i = threadIdx.x; i < kWarps * kRadix; i += THREADS) (&sm.warp_hist[0][0])[i] = 0;
+  __syncthreads();
+  const uint32_t tile = sm.tile_id;
+  const uint64_t tile0 = (uint64_t)tile * kTile;
+  const uint32_t valid = (uint32_t)min((uint64_t)kTile, (uint64_t)p.n - tile0);
+  const uint32_t mask = (1u << p.bits) - 1u;
+
+  // ---- load keys, warp-striped: element (warp, i, lane) is tile position warp*ITEMS*32 + i*32 + lane ----
+  KeyT key[ITEMS];
+  const uint32_t wbase = warp * (ITEMS * 32) + lane;
+#pragma unroll
+  for (int i = 0; i < ITEMS; ++i) {
+    const uint32_t e = wbase + i * 32;
+    if (e < valid) {
+      if (FIRST) {
+        key[i] = load_key_from_storage<KeyT>(p.map, tile0 + e, p.delay_bits);
+      } else {
+        key[i] = p.keys_in[tile0 + e];
+      }
+    } else {
+      key[i] = ~(KeyT)0;  // sorts behind every real key of the tile and is never written out
+    }
+  }
+
+  // ---- stable rank inside the warp: peers with the same digit, counted in position order ----
+  uint32_t rank[ITEMS];
+  uint32_t* my_hist = sm.warp_hist[warp];
+#pragma unroll
+  for (int i = 0; i < ITEMS; ++i) {
+    const uint32_t d = digit_of(key[i], p.shift, mask);
+    const uint32_t peers = __match_any_sync(0xffffffffu, d);
+    const uint32_t below = __popc(peers & lanemask_lt());
+    uint32_t pre = 0;
+    if (below == 0) {  // lowest lane of the peer group owns the counter update
+      pre = my_hist[d];
+      my_hist[d] = pre + __popc(peers);
+    }
+    __syncwarp();
+    pre = __shfl_sync(0xffffffffu, pre, __ffs(peers) - 1);
+    rank[i] = pre + below;
+  }
+  __syncthreads();
+
+  // ---- per digit: exclusive scan over the warps, tile count, look-back, global offset ----
+  uint32_t tile_count = 0;
+  if (threadIdx.x < kRadix) {
+    const uint32_t d = threadIdx.x;
+    uint32_t run = 0;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) {
+      const uint32_t c = sm.warp_hist[w][d];
+      sm.warp_hist[w][d] = run;
+      run += c;
+    }
+    tile_count = run;
+    // padding keys of a ragged last tile all carry the largest digit; they are not part of the data
+    const uint32_t real = (d == mask) ? run - (kTile - valid) : run;
+    uint64_t* my_status = p.status + (uint64_t)tile * kRadix + d;
+    uint64_t excl = 0;
+    if (tile == 0) {
+      st_relaxed_u64(my_status, p.epoch | kFlagInclusive | real);
+    } else {
+      st_relaxed_u64(my_status, p.epoch | kFlagAggregate | real);
+      const uint64_t* look = my_status - kRadix;
+      uint32_t spins = 0;
+      while (true) {
+        const uint64_t w = ld_relaxed_u64(look);
+        if ((w & ~(kCountMask | kFlagAggregate | kFlagInclusive)) != p.epoch || (w & (kFlagAggregate | kFlagInclusive)) == 0) {
+          if (++spins > (1u << 24)) {  // seconds: a predecessor is lost -> report instead of hanging the GPU
+            *p.error_flag = 1u;
+            break;
+          }
+          __nanosleep(20);
+          continue;  // predecessor has not published yet
+        }
+        excl += w & kCountMask;
+        if (w & kFlagInclusive) break;
+        look -= kRadix;
+      }
+      st_relaxed_u64(my_status, p.epoch | kFlagInclusive | (excl + real));
+    }
+    // exclusive scan of tile_count across the 256 digits
+    uint32_t inc = tile_count;
+#pragma unroll
+    for (int s = 1; s < 32; s <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, s);
+      if (lane >= (uint32_t)s) inc += t;
+    }
+    if (lane == 31) sm.scan_tmp[warp] = inc;
+    // (the sync below is only among the kRadix/32 warps that hold digits)
+    asm volatile("bar.sync 1, %0;" ::"n"(kRadix));
+    uint32_t base = 0;
+    for (uint32_t w = 0; w < warp; ++w) base += sm.scan_tmp[w];
+    const uint32_t te = base + inc - tile_count;
+    sm.tile_excl[d] = te;
+    sm.global_off[d] = p.bin_start[d] + (uint32_t)excl - te;
+  }
+  __syncthreads();
+
+  // ---- scatter into shared memory in tile-sorted order ----
+#pragma unroll
+  for (int i = 0; i < ITEMS; ++i) {
+    const uint32_t d = digit_of(key[i], p.shift, mask);
+    const uint32_t pos = sm.tile_excl[d] + my_hist[d] + rank[i];
+    rank[i] = pos;
+    sm.keys[pos] = key[i];
+  }
+#pragma unroll
+  for (int i = 0; i < ITEMS; ++i) {
+    const uint32_t e = wbase + i * 32;
+    uint32_t v = 0;
+    if (e < valid) v = FIRST ? (uint32_t)(tile0 + e) : p.vals_in[tile0 + e];
+    sm.vals[rank[i]] = v;
+  }
+  __syncthreads();
+
+  // ---- write out: consecutive threads write consecutive elements of a digit run ----
+#pragma unroll
+  for (int i = 0; i < ITEMS; ++i) {
+    const uint32_t j = i * THREADS + threadIdx.x;
+    if (j < valid) {
+      const KeyT k = sm.keys[j];
+      const uint32_t g = sm.global_off[digit_of(k, p.shift, mask)] + j;
+      p.keys_out[g] = k;
+      p.vals_out[g] = sm.vals[j];
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Permutation apply (step a11): sorted_target[j] = target[perm[j]], sorted_weight[j] = weight[perm[j]];
+// source and delay are unpacked from the sorted key.
+// ---------------------------------------------------------------------------------------------
+constexpr int kPermThreads = 256;
+
+template <typename KeyT>
+__global__ void __launch_bounds__(kPermThreads) permute_kernel(const __grid_constant__ BlockMap map, uint32_t n,
+                                                              uint32_t delay_bits, const KeyT* __restrict__ keys,
+                                                              const uint32_t* __restrict__ perm,
+                                                              uint32_t* __restrict__ out_src,
+                                                              uint32_t* __restrict__ out_tgt,
+                                                              float* __restrict__ out_w,
+                                                              uint16_t* __restrict__ out_d) {
+  const uint64_t j = (uint64_t)blockIdx.x * kPermThreads + threadIdx.x;
+  if (j >= n) return;
+  const KeyT k = keys[j];
+  const uint32_t pos = perm[j];
+  const BlockAddr a = locate(map, pos);
+  out_src[j] = (uint32_t)(k >> delay_bits);
+  out_d[j] = (uint16_t)((uint32_t)k & ((1u << delay_bits) - 1u));
+  out_tgt[j] = *tgt_ptr(map, a);
+  out_w[j] = *w_ptr(map, a);
+}
+
+}  // namespace nc

@@ -1,0 +1,72 @@
+"""The C-ABI library builds for sm_100a on a machine without a GPU, loads, exports every symbol that
+include/nc.h declares, and refuses to run without a device (no CPU fallback).  CPU only."""
+import ctypes
+import re
+from pathlib import Path
+
+import pytest
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2306_09855_b200 import build
+    return ctypes.CDLL(str(build.build()))
+
+
+def declared_symbols():
+    text = (ROOT / "include" / "nc.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(nc_[a-z_0-9]+)\s*\(", text)))
+
+
+def test_header_symbols_exported(lib):
+    from paper_2306_09855_b200 import binding
+    names = declared_symbols()
+    assert len(names) >= 19
+    for n in names:
+        assert hasattr(lib, n), f"libnc.so does not export {n}"
+    assert sorted(binding.SYMBOLS) == names, "binding.SYMBOLS out of step with include/nc.h"
+
+
+def test_struct_layouts_match_header():
+    """sizeof of the ctypes mirrors = what a C compiler gives for include/nc.h (gcc, x86-64)."""
+    import subprocess
+    import tempfile
+    from paper_2306_09855_b200 import binding as b
+    src = '#include "nc.h"\n#include <stdio.h>\nint main(){printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\\n",' \
+          'sizeof(nc_config),sizeof(nc_rule_params),sizeof(nc_dist),sizeof(nc_syn_spec),sizeof(nc_range),' \
+          'sizeof(nc_connections_view),sizeof(nc_index_view),sizeof(nc_timings),sizeof(nc_stats),sizeof(nc_allocator));return 0;}'
+    with tempfile.TemporaryDirectory() as d:
+        (Path(d) / "t.c").write_text(src)
+        subprocess.run(["gcc", "-I", str(ROOT / "include"), "-o", f"{d}/t", f"{d}/t.c"], check=True)
+        out = subprocess.run([f"{d}/t"], check=True, capture_output=True, text=True).stdout.split()
+    want = [ctypes.sizeof(x) for x in (b.Config, b.RuleParams, b.Dist, b.SynSpec, b.Range, b.ConnectionsView,
+                                       b.IndexView, b.Timings, b.Stats, b.Allocator)]
+    assert [int(v) for v in out] == want
+
+
+def test_no_cpu_fallback_without_gpu(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from paper_2306_09855_b200 import binding as b
+    cfg = b.Config()
+    cfg.dt_ms = 0.1
+    cfg.device = -1
+    h = ctypes.c_void_p()
+    L = b.load_library()
+    assert L.nc_create(ctypes.byref(cfg), ctypes.byref(h)) == b.ERR_CUDA and not h.value
+    with pytest.raises(RuntimeError):
+        b.NC()
+
+
+def test_invalid_config_rejected(lib):
+    from paper_2306_09855_b200 import binding as b
+    L = b.load_library()
+    cfg = b.Config()
+    cfg.dt_ms = 0.0
+    h = ctypes.c_void_p()
+    assert L.nc_create(ctypes.byref(cfg), ctypes.byref(h)) == b.ERR_INVALID_ARG
+    assert L.nc_create(None, ctypes.byref(h)) == b.ERR_INVALID_ARG

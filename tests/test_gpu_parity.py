@@ -1,0 +1,182 @@
+"""GPU parity tests proper: the CUDA path, called through the C ABI, against the CPU oracle on the same
+seeded recipes -- element by element at sizes the oracle finishes in seconds (several sort tiles plus a
+ragged tail), edge cases, and device self-tests of the RNG and of the fp32 fast path."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2306_09855_b200 import workloads as WL
+from tests import parity_util as PU
+
+pytestmark = pytest.mark.gpu
+INF = math.inf
+W = (20.0, 2.0, 0.0, INF)
+D = (1.5, 0.75, 0.1, INF)
+
+
+@pytest.fixture(scope="module")
+def nc_mod():
+    from paper_2306_09855_b200 import binding, build
+    build.build()
+    return binding
+
+
+def test_device_philox_matches_known_answers_and_oracle(nc_mod, oracle_mod):
+    g = nc_mod.NC()
+    ctr = np.array([[0, 0, 0, 0], [0xffffffff] * 4, [0x243f6a88, 0x85a308d3, 0x13198a2e, 0x03707344]], dtype=np.uint32)
+    key = np.array([[0, 0], [0xffffffff] * 2, [0xa4093822, 0x299f31d0]], dtype=np.uint32)
+    out = g.selftest_philox(ctr, key)
+    want = np.array([[0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8], [0x408f276d, 0x41c83b0e, 0xa20bc7c6, 0x6d5451fd],
+                     [0xd16cfe09, 0x94fdcceb, 0x5001e420, 0x24126ea1]], dtype=np.uint32)
+    assert np.array_equal(out, want)
+    rng = np.random.default_rng(1)
+    ctr = rng.integers(0, 2**32, size=(2000, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2**32, size=(2000, 2), dtype=np.uint64).astype(np.uint32)
+    out = g.selftest_philox(ctr, key)
+    ref = np.array([oracle_mod.philox4x32_10(c.tolist(), k.tolist()) for c, k in zip(ctr, key)], dtype=np.uint32)
+    assert np.array_equal(out, ref)
+    g.close()
+
+
+def test_fastpath_error_is_inside_the_guard_band(nc_mod):
+    """Exhaustive over all 2^24 u1 and all 2^24 u2 on the device: the fp32 radius and sin/cos stay within
+    the error the guard band assumes (|dz1| <= 5.77 (er + es) must be far
+    below 5.769 * 32 ulp = 1.1e-5)."""
+    g = nc_mod.NC()
+    er, es, ec = g.selftest_fastpath()
+    g.close()
+    print(f"fast path: max rel err r {er:.3e}, max abs err sin {es:.3e}, cos {ec:.3e}")
+    assert er < 4 * 2.0**-24 and es < 4 * 2.0**-24 and ec < 4 * 2.0**-24
+    assert 5.7681 * (er + es) < 0.25 * 5.769 * 32 * 2.0**-24
+
+
+@pytest.mark.parametrize("B", [0, 10, 64, 1000])
+def test_config0_tiny_full_parity(nc_mod, oracle_mod, B):
+    rep, rep_s = PU.full_parity(WL.config0_tiny(), oracle_mod, nc_mod, B=B)
+    assert rep["n"] == 1000 and rep["delay_mismatches"] == 0
+
+
+@pytest.mark.parametrize("rule,scale", [("one_to_one", 1.0), ("all_to_all", 0.15), ("fixed_indegree", 0.3),
+                                        ("fixed_outdegree", 0.25), ("fixed_total_number", 0.3),
+                                        ("pairwise_bernoulli", 0.4)])
+def test_config1_rule_sweep_parity(nc_mod, oracle_mod, rule, scale):
+    net = WL.config1_rule(rule, scale=scale)
+    rep, _ = PU.full_parity(net, oracle_mod, nc_mod)
+    print(net.name, rep)
+    assert rep["n"] > 5000
+
+
+def test_config1_exact_fp64_flag_gives_same_delays(nc_mod, oracle_mod):
+    net = WL.config1_rule("fixed_total_number", scale=0.2)
+    rep, _ = PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_EXACT_FP64)
+    assert rep["delay_mismatches"] == 0
+
+
+def test_microcircuit_scaled_parity(nc_mod, oracle_mod):
+    """configs[2] at 10 % of the populations (same probabilities): 55 projections, ~3e6 synapses, I and E delays."""
+    net = WL.config2_microcircuit(scale=0.1)
+    rep, _ = PU.full_parity(net, oracle_mod, nc_mod)
+    print(net.name, rep)
+    assert len(net.projections) >= 50 and rep["n"] > 2_000_000
+
+
+def test_block_sizes_paper_default_and_odd(nc_mod, oracle_mod):
+    """B = 10^7 (the paper's default, not a power of two -> magic division) and an odd B (scalar stores)."""
+    net = WL.config3_large_indegree(scale=0.02)  # 1600+400 nodes, K = 160 / 40 -> 400k synapses
+    for B in (10_000_000, 100_003, 4096):
+        rep, _ = PU.full_parity(net, oracle_mod, nc_mod, B=B)
+        assert rep["n"] == 2000 * 200
+
+
+def test_bernoulli_and_outdegree_mix_scaled_c4(nc_mod, oracle_mod):
+    net = WL.config4_large_bernoulli(scale=0.01)  # 1600 + 400 nodes: 4e6 trials, ~1e5 accepted, + K = 5 out-degree
+    rep, _ = PU.full_parity(net, oracle_mod, nc_mod)
+    assert rep["n"] > 90_000
+
+
+def test_edge_cases(nc_mod, oracle_mod):
+    # empty network
+    g = nc_mod.NC()
+    g.create_population(5)
+    g.finalize()
+    idx = g.read_index()
+    assert idx["total_groups"] == 0 and idx["src_offsets"].tolist() == [0] * 6 and idx["group_ptr"].tolist() == [0] * 6
+    assert g.read_connections(sorted=True)["n"] == 0
+    g.close()
+    # sources with no outgoing connection at both ends and in the middle; constant weight/delay; p = 0 and 1
+    net = WL.Network("edges", [7, 50, 9, 30, 11])
+    net.projections = [
+        WL.Projection(1, 3, "pairwise_bernoulli", p=1.0, weight=W, delay_ms=D, seed=3),
+        WL.Projection(3, 1, "pairwise_bernoulli", p=0.0, weight=W, delay_ms=D, seed=3),
+        WL.Projection(3, 3, "one_to_one", weight=(2.5, 0.0, -INF, INF), delay_ms=(0.25, 0.0, -INF, INF), seed=3),
+        WL.Projection(3, 0, "fixed_indegree", degree_or_total=0, weight=W, delay_ms=D, seed=3),
+        WL.Projection(1, 1, "fixed_total_number", degree_or_total=1, weight=W, delay_ms=D, seed=3),
+        WL.Projection(1, 3, "all_to_all", weight=(-1.0, 3.0, -2.0, 0.0), delay_ms=(1.0, 5.0, 0.1, 3.0), seed=4),
+    ]
+    rep, _ = PU.full_parity(net, oracle_mod, nc_mod, B=64)
+    assert rep["n"] == 50 * 30 + 30 + 1 + 50 * 30
+    # a single source with every connection (one huge group run) and delay bound at the u16 limit
+    net2 = WL.Network("one_source", [1, 20000])
+    net2.projections = [WL.Projection(0, 1, "all_to_all", weight=W, delay_ms=(6553.5, 0.0, -INF, INF), seed=1),
+                        WL.Projection(0, 1, "fixed_outdegree", degree_or_total=30000, weight=W, delay_ms=D, seed=1)]
+    rep2, _ = PU.full_parity(net2, oracle_mod, nc_mod)
+    assert rep2["n"] == 50000
+
+
+def test_wide_key_uses_64_bit_sort(nc_mod, oracle_mod):
+    """2^17 nodes and delays up to 65535 steps -> 17 + 16 = 33 key bits -> the u64 instantiation."""
+    net = WL.Network("wide", [131072])
+    net.projections = [WL.Projection(0, 0, "fixed_total_number", degree_or_total=300_000, weight=W,
+                                     delay_ms=(3000.0, 1500.0, 0.1, 6553.5), seed=8)]
+    o, g = PU.build_both(net, oracle_mod, nc_mod)
+    assert g.stats()["key_bits"] == 33 and g.stats()["sort_passes"] == 5
+    PU.compare_connections(g.read_connections(sorted=True), o.connections(sorted=True), PU.weight_scale(net), "wide")
+    PU.compare_index(g.read_index(), o.index(), "wide")
+    g.close()
+
+
+def test_error_codes_match_oracle(nc_mod, oracle_mod):
+    g = nc_mod.NC()
+    o = oracle_mod.Oracle(dt_ms=0.1)
+    for b in (g, o):
+        b.create_population(10)
+        b.create_population(20)
+    ok = dict(weight=W, delay_ms=D, seed=1)
+    cases = [
+        ((0, 10), (10, 20), 0, {}),                            # one_to_one size mismatch
+        ((25, 10), (10, 20), 1, {}),                           # outside created nodes
+        ((0, 0), (10, 20), 1, {}),                             # empty range
+        ((0, 10), (10, 20), 5, dict(p=1.5)),
+        ((0, 10), (10, 20), 9, {}),
+        ((0, 10), (10, 20), 4, dict(degree_or_total=2**32)),
+        ((0, 10), (10, 20), 2, dict(degree_or_total=2**31)),
+    ]
+    for src, tgt, rule, extra in cases:
+        assert g.connect_rc(src, tgt, rule, **extra, **ok) == o.connect_rc(src, tgt, rule, **extra, **ok) != 0
+    bad_w = dict(weight=(1, -1, -INF, INF), delay_ms=D, seed=1)
+    assert g.connect_rc((0, 10), (10, 20), 1, **bad_w) == o.connect_rc((0, 10), (10, 20), 1, **bad_w) == nc_mod.ERR_INVALID_ARG
+    big_d = dict(weight=W, delay_ms=(7000.0, 0.0, -INF, INF), seed=1)
+    assert g.connect_rc((0, 10), (10, 20), 1, **big_d) == o.connect_rc((0, 10), (10, 20), 1, **big_d) == nc_mod.ERR_CAPACITY
+    assert g.num_connections() == 0
+    g.connect((0, 10), (10, 20), 4, degree_or_total=5, **ok)  # projection id 0: failures consumed none
+    o.connect((0, 10), (10, 20), 4, degree_or_total=5, **ok)
+    assert np.array_equal(g.read_connections()["source"], o.connections()["source"])
+    with pytest.raises(nc_mod.NCError):
+        g.read_connections(sorted=True)
+    g.finalize()
+    assert g.connect_rc((0, 10), (10, 20), 1, **ok) == nc_mod.ERR_STATE
+    with pytest.raises(nc_mod.NCError):
+        g.finalize()
+    g.close()
+
+
+def test_default_cuda_allocator_path(nc_mod, oracle_mod):
+    """mem.alloc == NULL -> cudaMalloc/cudaFree inside the library."""
+    net = WL.config0_tiny()
+    o = oracle_mod.Oracle(dt_ms=0.1)
+    WL.run(net, o)
+    g = nc_mod.NC(use_torch_allocator=False)
+    WL.run(net, g)
+    PU.compare_connections(g.read_connections(sorted=True), o.connections(sorted=True), PU.weight_scale(net), "cudaMalloc")
+    g.close()
