@@ -1,0 +1,287 @@
+#!/usr/bin/env python
+"""bench.py -- synapses constructed per second (generate + sort + index), device-timed, on the
+cortical-microcircuit-shaped workload (BASELINE.json configs[2]: 77,169 neurons, 298,880,970 synapses).
+
+    python bench.py --gpus N --steps K --warmup W            # the CUDA path (one replica per GPU)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle on a bounded sample
+
+One "step" = one pass of the whole hot path: create the populations, issue all 55 nc_connect calls (rule
+expansion + draws + append into block storage), nc_finalize (histogram, onesweep passes, permute, index).
+Prints ONE JSON line on rank 0.  See DESIGN.md "Measurement" for how every field is obtained.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "synapses constructed/s (generate+sort+index, device-timed)"
+UNIT = "synapses/s"
+# algorithmic bytes per synapse
+BYTES = {"generate": 14, "histogram": 6, "sort_pass": 16, "permute": 26, "index": 4}
+
+
+def workload(name: str):
+    from paper_2306_09855_b200 import workloads as WL
+    if name == "c2":
+        return WL.config2_microcircuit()
+    if name.startswith("c2x"):
+        return WL.config2_microcircuit(scale=float(name[3:]))
+    if name == "c3":
+        return WL.config3_large_indegree()
+    if name == "c4":
+        return WL.config4_large_bernoulli()
+    if name.startswith("c1:"):
+        return WL.config1_rule(name[3:])
+    if name == "c0":
+        return WL.config0_tiny()
+    raise SystemExit(f"unknown workload {name}")
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz, self._halt = index, [], set(), None, threading.Event()
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {
+                nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+            }
+            while not self._halt.is_set():
+                self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+                time.sleep(0.02)
+        except Exception as e:  # NVML missing: report that instead of failing the bench
+            self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+
+    def stop(self):
+        self._halt.set()
+        self.join(timeout=2)
+        return {"sm_mhz": statistics.median(self.samples) if self.samples else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def one_step(binding, WL, net, flags):
+    """The public API call sequence a user makes.  Returns the (still open) context."""
+    g = binding.NC(dt_ms=net.dt_ms, flags=flags)
+    WL.run(net, g)
+    return g
+
+
+def cpu_oracle_sample(sample_scale: float, steps: int = 1):
+    """The oracle as it stands, one thread, on a bounded sample of the same workload."""
+    import oracle
+    from paper_2306_09855_b200 import workloads as WL
+    net = WL.config2_microcircuit(scale=sample_scale)
+    oracle.build()
+    times, n = [], 0
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        o = oracle.Oracle(dt_ms=net.dt_ms)
+        WL.run(net, o)
+        n = o.num_connections()
+        times.append(time.perf_counter() - t0)
+        o.close()
+    return net, n, times
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    scale = args.sample_scale if args.sample_scale else 0.1
+    for _ in range(args.warmup):
+        cpu_oracle_sample(min(scale, 0.03))
+    net, n, times = cpu_oracle_sample(scale, steps=args.steps)
+    value = n * len(times) / sum(times)
+    sample = f"configs[2] with populations scaled x{scale:g} ({net.n_nodes} nodes, {n} synapses, 55 projections) per step"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "configs[2] cortical-microcircuit-shaped, fixed_total_number, seed 7 (bounded sample)",
+                   "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="nc", choices=["nc", "reference"])
+    ap.add_argument("--workload", default="c2")
+    ap.add_argument("--sample-scale", type=float, default=0.0, help="cpu baseline sample: population scale of configs[2]")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--flags", type=int, default=0, help="extra NC_FLAG_* bits (e.g. 4 = sort (key, position) pairs + gather)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2306_09855_b200 import binding, build, workloads as WL
+    build.build()
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    net = workload(args.workload)
+    stream = torch.cuda.current_stream()
+    flags = binding.FLAG_TIMING | args.flags
+
+    # ---- warm-up (also warms torch's caching allocator: the timed steps allocate from its cache) ----
+    n_syn = 0
+    for _ in range(max(args.warmup, 0)):
+        g = one_step(binding, WL, net, flags)
+        n_syn = g.num_connections()
+        g.close()
+    barrier()
+
+    # ---- timed region: K steps, CUDA events on the stream the kernels are launched on ----
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    phase_acc, launches, stats = {}, 0, {}
+    barrier()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        g = one_step(binding, WL, net, flags)
+        n_syn = g.num_connections()
+        t = g.timings()  # synchronises this context's stream; the events were recorded on the device
+        stats = g.stats()
+        launches += stats["kernel_launches"]
+        for k, v in t.items():
+            phase_acc[k] = phase_acc.get(k, 0.0) + v
+        g.close()
+    ev1.record(stream)
+    barrier()
+    total_ms = ev0.elapsed_time(ev1)
+    clocks = sampler.stop()
+    if dist is not None:
+        tt = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms = float(tt.item())
+    ms_per_step = total_ms / args.steps
+    value = world * n_syn * args.steps / (total_ms * 1e-3)
+
+    # ---- end to end through the public API with host buffers: context creation, host descriptors in,
+    #      index arrays read back into host memory, wall clock ----
+    e2e_times, d2h = [], 0
+    for _ in range(max(2, min(args.steps, 5))):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        g = one_step(binding, WL, net, args.flags)
+        idx = g.read_index()
+        cnt = g.num_connections()
+        g.synchronize()
+        e2e_times.append(time.perf_counter() - t0)
+        d2h = sum(v.nbytes for v in idx.values() if hasattr(v, "nbytes")) + 8 + 4
+        nblocks = g.stats()["n_blocks"]
+        g.close()
+    h2d = len(net.projections) * (8 + 8 + 16 + 64 + 8) + 8 * nblocks  # per nc_connect: ranges, rule params, syn spec, seed; block table
+    if dist is not None:
+        tt = torch.tensor([max(e2e_times)], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        e2e_t = float(tt.item())
+    else:
+        e2e_t = statistics.median(e2e_times)
+    e2e_value = world * cnt / e2e_t
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    peak = float(peaks.get("hbm_gbs", 6650.0))
+    peak_kind = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6.65 TB/s"
+    K = args.steps
+    per = {k: v / K for k, v in phase_acc.items()}
+    passes = max(1, int(round(per.get("sort_passes", 0))))
+    pass_ms = per["sort_pass_ms"] / passes if per.get("sort_pass_ms") else None
+    roof = None
+    if pass_ms:
+        ach = BYTES["sort_pass"] * n_syn / (pass_ms * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": "onesweep_kernel (one digit pass: 8 B read + 8 B written per synapse)",
+                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None, "peak_kind": peak_kind,
+                "launch_ms": pass_ms, "launches_per_step": passes}
+    phases = {}
+    for name, b in (("generate", BYTES["generate"]), ("histogram", BYTES["histogram"]), ("sort", BYTES["sort_pass"] * passes),
+                    ("permute", BYTES["permute"]), ("index", BYTES["index"])):
+        ms = per.get(f"{name}_ms", 0.0)
+        if ms > 0:
+            gbs = b * n_syn / (ms * 1e-3) / 1e9
+            phases[name] = {"ms": round(ms, 4), "alg_bytes_per_synapse": b, "GBps": round(gbs, 1),
+                            "frac_of_measured_peak": round(gbs / peak, 4), "frac_of_8TBps": round(gbs / 8000.0, 4)}
+
+    cpu = None
+    if not args.no_cpu_baseline and args.workload.startswith("c2"):
+        scale = args.sample_scale if args.sample_scale else 0.25
+        snet, sn, st = cpu_oracle_sample(scale)
+        cpu = {"value": sn / st[0], "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"configs[2] with populations scaled x{scale:g}: {snet.n_nodes} nodes, {sn} synapses, generate+sort+index, {st[0]:.1f} s",
+               "host_cpus": os.cpu_count()}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32+f32",
+        "data": "synthetic",
+        "config": {"workload": f"{net.name}: BASELINE.json configs[2] cortical-microcircuit-shaped network, "
+                               f"{net.n_nodes} nodes, {len(net.projections)} fixed_total_number projections, seed 7"
+                   if args.workload == "c2" else net.name,
+                   "synapses_per_step": n_syn, "parallelism": "replicas only (one independent network per GPU)",
+                   "l2": "every step regenerates and re-sorts its own 4.2 GB of connections (>> 126 MB L2); no input is reused",
+                   "key_bits": stats.get("key_bits"), "sort_passes": stats.get("sort_passes"), "flags": flags},
+        "clocks": clocks, "gpu_launches": launches,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "what": "wall clock of nc_create + populations + all nc_connect + nc_finalize + nc_read_index into host buffers"},
+        "roofline": roof, "phases": phases, "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -70,8 +70,9 @@ typedef struct {
 enum {
   NC_FLAG_TIMING = 1u << 0,     /* record CUDA events around every phase (nc_get_timings) */
   NC_FLAG_EXACT_FP64 = 1u << 1, /* debug: draw every delay on the fp64 path (no fp32 fast path) */
-  NC_FLAG_CARRY_PAYLOAD = 1u << 2 /* sort carries (target, weight) through the passes instead of
-                                     gathering them by the permutation afterwards */
+  NC_FLAG_SORT_PAIRS = 1u << 2  /* sort (key, position) pairs and gather target/weight by the permutation
+                                   afterwards, instead of carrying the whole connection through the digit
+                                   passes (the default for keys of <= 32 bits; wider keys always use pairs) */
 };
 
 typedef struct {

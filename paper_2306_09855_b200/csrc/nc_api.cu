@@ -481,7 +481,7 @@ int sort_and_index(nc_context* c, const PassPlan& plan) {
   uint32_t lookback_error = 0;
   {
     Scope sc(c, NC_PHASE_INDEX);
-    head_count_kernel<KeyT><<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(keys[cur], n, tile_heads);
+    head_count_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(PackedKeys<KeyT>{keys[cur], c->delay_bits}, n, tile_heads);
     NC_LAUNCH_CHECK(c, "head_count");
     int rc = device_scan(c, tile_heads, tile_head_off, head_tiles, head_partial, d_total_groups);
     if (rc != NC_OK) return rc;
@@ -503,14 +503,165 @@ int sort_and_index(nc_context* c, const PassPlan& plan) {
   {
     Scope sc(c, NC_PHASE_INDEX);
     IndexOut io{c->src_offsets, c->group_ptr, c->group_start, c->group_delay, N};
-    index_scatter_kernel<KeyT><<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(keys[cur], n, c->delay_bits,
-                                                                                    tile_head_off, d_total_groups, io);
+    index_scatter_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(PackedKeys<KeyT>{keys[cur], c->delay_bits}, n,
+                                                                              tile_head_off, d_total_groups, io);
     NC_LAUNCH_CHECK(c, "index_scatter");
     index_finish_kernel<<<(N + 255) / 256, 256, 0, c->stream>>>(c->src_offsets, c->group_ptr, N, c->out_degree,
                                                                c->group_count, c->d_max + 1);
     NC_LAUNCH_CHECK(c, "index_finish");
   }
   drop_scratch(cur);
+  return NC_OK;
+}
+
+// Record-carrying organisation step (keys of <= 32 bits): histogram, P onesweep passes that move whole
+// connections, final pass writes the sorted SoA arrays; then the index over (source, delay).
+constexpr int kRecThreads = 512;
+constexpr int kRecItems = 8;
+constexpr int kRecMinCtas = 2;
+
+template <bool FIRST, bool LAST>
+int launch_rec_pass(nc_context* c, const SortRecParams& sp, uint64_t n_tiles) {
+  using Smem = OnesweepRecSmem<kRecThreads, kRecItems>;
+  auto kern = onesweep_rec_kernel<FIRST, LAST, kRecThreads, kRecItems, kRecMinCtas>;
+  NC_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem)));
+  kern<<<(unsigned)n_tiles, kRecThreads, sizeof(Smem), c->stream>>>(sp);
+  NC_LAUNCH_CHECK(c, "onesweep_rec");
+  return NC_OK;
+}
+
+int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag);
+
+int sort_carry_and_index(nc_context* c, const PassPlan& plan) {
+  using Smem = OnesweepRecSmem<kRecThreads, kRecItems>;
+  const uint32_t n = (uint32_t)c->n_conns;
+  const uint64_t n_tiles = ((uint64_t)n + Smem::kTile - 1) / Smem::kTile;
+  const BlockMap map = make_map(c);
+  const uint32_t P = plan.n_passes;
+
+  uint4* recs[2] = {P > 1 ? (uint4*)dev_alloc(c, (size_t)n * 16) : nullptr,
+                    P > 2 ? (uint4*)dev_alloc(c, (size_t)n * 16) : nullptr};
+  uint32_t* ghist = (uint32_t*)dev_alloc(c, kMaxPasses * kRadix * 4);
+  uint32_t* bin_start = (uint32_t*)dev_alloc(c, kMaxPasses * kRadix * 4);
+  uint64_t* status = (uint64_t*)dev_alloc(c, n_tiles * kRadix * 8);
+  uint32_t* tickets = (uint32_t*)dev_alloc(c, (kMaxPasses + 1) * 4);
+  c->s_src = (uint32_t*)dev_alloc(c, (size_t)n * 4);
+  c->s_tgt = (uint32_t*)dev_alloc(c, (size_t)n * 4);
+  c->s_w = (float*)dev_alloc(c, (size_t)n * 4);
+  c->s_d = (uint16_t*)dev_alloc(c, (size_t)n * 2);
+  c->perm = (uint32_t*)dev_alloc(c, (size_t)n * 4);
+  bool ok = ghist && bin_start && status && tickets && c->s_src && c->s_tgt && c->s_w && c->s_d && c->perm;
+  if (P > 1) ok = ok && recs[0];
+  if (P > 2) ok = ok && recs[1];
+  auto drop_scratch = [&]() {
+    dev_free_later(c, recs[0]); dev_free_later(c, recs[1]);
+    dev_free_later(c, ghist); dev_free_later(c, bin_start); dev_free_later(c, status); dev_free_later(c, tickets);
+  };
+  if (!ok) {
+    drop_scratch();
+    return fail(c, NC_ERR_OOM, "out of device memory in nc_finalize");
+  }
+  {
+    Scope sc(c, NC_PHASE_HISTOGRAM);
+    NC_CUDA(c, cudaMemsetAsync(ghist, 0, kMaxPasses * kRadix * 4, c->stream));
+    NC_CUDA(c, cudaMemsetAsync(tickets, 0, (kMaxPasses + 1) * 4, c->stream));
+    NC_CUDA(c, cudaMemsetAsync(status, 0, n_tiles * kRadix * 8, c->stream));
+    const unsigned grid = (unsigned)(((uint64_t)n + kHistThreads * kHistItems - 1) / (kHistThreads * kHistItems));
+    histogram_kernel<uint32_t><<<grid, kHistThreads, 0, c->stream>>>(map, n, c->delay_bits, plan, ghist);
+    NC_LAUNCH_CHECK(c, "histogram");
+    bin_scan_kernel<<<P, kRadix, 0, c->stream>>>(ghist, bin_start);
+    NC_LAUNCH_CHECK(c, "bin_scan");
+  }
+  {
+    Scope sc(c, NC_PHASE_SORT);
+    int cur = -1;
+    for (uint32_t ps = 0; ps < P; ++ps) {
+      Scope pass_sc(c, NC_PHASE_SORT, true);
+      const bool first = ps == 0, last = ps + 1 == P;
+      SortRecParams sp{};
+      sp.map = map;
+      sp.delay_bits = c->delay_bits;
+      sp.n = n;
+      const int dst = cur < 0 ? 0 : 1 - cur;
+      sp.recs_in = first ? nullptr : recs[cur];
+      sp.recs_out = last ? nullptr : recs[dst];
+      sp.out_src = c->s_src;
+      sp.out_tgt = c->s_tgt;
+      sp.out_w = c->s_w;
+      sp.out_d = c->s_d;
+      sp.out_perm = c->perm;
+      sp.shift = plan.shift[ps];
+      sp.bits = plan.bits[ps];
+      sp.bin_start = bin_start + ps * kRadix;
+      sp.status = status;
+      sp.ticket = tickets + ps;
+      sp.error_flag = tickets + kMaxPasses;
+      sp.epoch = (uint64_t)(ps + 1) << 42;
+      int rc;
+      if (first && last) rc = launch_rec_pass<true, true>(c, sp, n_tiles);
+      else if (first) rc = launch_rec_pass<true, false>(c, sp, n_tiles);
+      else if (last) rc = launch_rec_pass<false, true>(c, sp, n_tiles);
+      else rc = launch_rec_pass<false, false>(c, sp, n_tiles);
+      if (rc != NC_OK) return rc;
+      cur = dst;
+    }
+  }
+  int rc = build_index_from_sorted(c, n, tickets + kMaxPasses);
+  drop_scratch();
+  return rc;
+}
+
+// a12-a14 over the final source / delay arrays.
+int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) {
+  const uint32_t N = c->n_nodes;
+  const uint64_t head_tiles = ((uint64_t)n + kHeadTile - 1) / kHeadTile;
+  const uint64_t head_chunks = (head_tiles + kScanChunk - 1) / kScanChunk;
+  uint32_t* tile_heads = (uint32_t*)dev_alloc(c, head_tiles * 4);
+  uint32_t* tile_head_off = (uint32_t*)dev_alloc(c, head_tiles * 4);
+  uint32_t* head_partial = (uint32_t*)dev_alloc(c, head_chunks * 4);
+  uint64_t* d_total_groups = (uint64_t*)dev_alloc(c, 8);
+  auto drop = [&]() {
+    dev_free_later(c, tile_heads); dev_free_later(c, tile_head_off); dev_free_later(c, head_partial);
+    dev_free_later(c, d_total_groups);
+  };
+  if (!tile_heads || !tile_head_off || !head_partial || !d_total_groups) {
+    drop();
+    return fail(c, NC_ERR_OOM, "out of device memory for the index scratch");
+  }
+  const SoAKeys keys{c->s_src, c->s_d, 16u};
+  uint64_t total_groups = 0;
+  uint32_t lookback_error = 0;
+  {
+    Scope sc(c, NC_PHASE_INDEX);
+    head_count_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(keys, n, tile_heads);
+    NC_LAUNCH_CHECK(c, "head_count");
+    int rc = device_scan(c, tile_heads, tile_head_off, head_tiles, head_partial, d_total_groups);
+    if (rc != NC_OK) return rc;
+    NC_CUDA(c, cudaMemcpyAsync(&total_groups, d_total_groups, 8, cudaMemcpyDeviceToHost, c->stream));
+    NC_CUDA(c, cudaMemcpyAsync(&lookback_error, lookback_flag, 4, cudaMemcpyDeviceToHost, c->stream));
+  }
+  NC_CUDA(c, cudaStreamSynchronize(c->stream));  // total_groups sizes the group arrays
+  if (lookback_error) {
+    drop();
+    return fail(c, NC_ERR_CUDA, "onesweep look-back timed out");
+  }
+  c->total_groups = (uint32_t)total_groups;
+  c->group_start = (uint32_t*)dev_alloc(c, (size_t)total_groups * 4);
+  c->group_delay = (uint16_t*)dev_alloc(c, (size_t)total_groups * 2);
+  if (!c->group_start || !c->group_delay) {
+    drop();
+    return fail(c, NC_ERR_OOM, "out of device memory for the group arrays");
+  }
+  {
+    Scope sc(c, NC_PHASE_INDEX);
+    IndexOut io{c->src_offsets, c->group_ptr, c->group_start, c->group_delay, N};
+    index_scatter_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(keys, n, tile_head_off, d_total_groups, io);
+    NC_LAUNCH_CHECK(c, "index_scatter");
+    index_finish_kernel<<<(N + 255) / 256, 256, 0, c->stream>>>(c->src_offsets, c->group_ptr, N, c->out_degree,
+                                                               c->group_count, c->d_max + 1);
+    NC_LAUNCH_CHECK(c, "index_finish");
+  }
+  drop();
   return NC_OK;
 }
 
@@ -763,7 +914,10 @@ int nc_finalize(nc_context* c) {
     c->total_groups = 0;
     c->sort_passes = 0;
   } else {
-    int rc = c->key_bits <= 32 ? sort_and_index<uint32_t>(c, plan) : sort_and_index<uint64_t>(c, plan);
+    int rc;
+    if (c->key_bits > 32) rc = sort_and_index<uint64_t>(c, plan);
+    else if (c->cfg.flags & NC_FLAG_SORT_PAIRS) rc = sort_and_index<uint32_t>(c, plan);
+    else rc = sort_carry_and_index(c, plan);
     if (rc != NC_OK) return rc;
   }
   c->finalized = true;

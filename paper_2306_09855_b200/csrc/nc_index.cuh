@@ -101,9 +101,27 @@ constexpr int kHeadThreads = 256;
 constexpr int kHeadItems = 8;
 constexpr int kHeadTile = kHeadThreads * kHeadItems;
 
-template <typename KeyT>
-__global__ void __launch_bounds__(kHeadThreads) head_count_kernel(const KeyT* __restrict__ keys, uint32_t n,
+// Where the sorted (source, delay) keys come from: the packed key array of the pairs sort, or the final
+// source / delay arrays written by the record-carrying sort (packed here with a fixed 16-bit delay field).
+template <typename K>
+struct PackedKeys {
+  using KeyT = K;
+  const K* k;
+  uint32_t delay_bits;
+  __device__ __forceinline__ K operator[](uint64_t j) const { return k[j]; }
+};
+struct SoAKeys {
+  using KeyT = uint64_t;
+  const uint32_t* src;
+  const uint16_t* dly;
+  uint32_t delay_bits;  // always 16
+  __device__ __forceinline__ uint64_t operator[](uint64_t j) const { return ((uint64_t)src[j] << 16) | dly[j]; }
+};
+
+template <typename Keys>
+__global__ void __launch_bounds__(kHeadThreads) head_count_kernel(const Keys keys, uint32_t n,
                                                                  uint32_t* __restrict__ tile_heads) {
+  using KeyT = typename Keys::KeyT;
   __shared__ uint32_t warp_tmp[kHeadThreads / 32];
   const uint64_t base = (uint64_t)blockIdx.x * kHeadTile + (uint64_t)threadIdx.x * kHeadItems;
   uint32_t c = 0;
@@ -142,12 +160,13 @@ struct IndexOut {
 // g = (heads before j); if it is also the first connection of its source s, then for every node s' in
 // (previous source, s] (the ones in between have no outgoing connection, Q9):
 //   src_offsets[s'] = j  and  group_ptr[s'] = g   -- exactly exclusive_scan(out_degree) and Eq. 14.
-template <typename KeyT>
-__global__ void __launch_bounds__(kHeadThreads) index_scatter_kernel(const KeyT* __restrict__ keys, uint32_t n,
-                                                                    uint32_t delay_bits,
+template <typename Keys>
+__global__ void __launch_bounds__(kHeadThreads) index_scatter_kernel(const Keys keys, uint32_t n,
                                                                     const uint32_t* __restrict__ tile_head_off,
                                                                     const uint64_t* __restrict__ total_groups,
                                                                     const __grid_constant__ IndexOut out) {
+  using KeyT = typename Keys::KeyT;
+  const uint32_t delay_bits = keys.delay_bits;
   __shared__ uint32_t warp_tmp[kHeadThreads / 32];
   const uint64_t base = (uint64_t)blockIdx.x * kHeadTile + (uint64_t)threadIdx.x * kHeadItems;
   KeyT k[kHeadItems];

@@ -271,6 +271,189 @@ __global__ void __launch_bounds__(THREADS) onesweep_kernel(const __grid_constant
 }
 
 // ---------------------------------------------------------------------------------------------
+// Onesweep digit pass that carries the whole connection (32-bit keys only).
+//
+// Record = (key, creation position, target, weight) = one uint4.  The first pass builds records from the
+// storage blocks, middle passes move AoS records (128-bit loads and stores, digit runs of ~16 records =
+// 256 contiguous bytes), and the last pass writes the final SoA arrays (source and delay unpacked from the
+// key, target, weight, permutation) directly -- so there is no gather by the permutation at all: every byte
+// the organisation step moves is streamed.  Same ranking, look-back and status words as onesweep_kernel.
+// ---------------------------------------------------------------------------------------------
+struct SortRecParams {
+  BlockMap map;  // FIRST
+  uint32_t delay_bits;
+  uint32_t n;
+  const uint4* recs_in;
+  uint4* recs_out;
+  // LAST: final arrays
+  uint32_t* out_src;
+  uint32_t* out_tgt;
+  float* out_w;
+  uint16_t* out_d;
+  uint32_t* out_perm;
+  uint32_t shift, bits;
+  const uint32_t* bin_start;
+  uint64_t* status;
+  uint32_t* ticket;
+  uint32_t* error_flag;
+  uint64_t epoch;
+};
+
+template <int THREADS, int ITEMS>
+struct OnesweepRecSmem {
+  static constexpr int kTile = THREADS * ITEMS;
+  static constexpr int kWarps = THREADS / 32;
+  uint4 recs[kTile];
+  uint32_t warp_hist[kWarps][kRadix];
+  uint32_t tile_excl[kRadix];
+  uint32_t global_off[kRadix];
+  uint32_t scan_tmp[kRadix / 32];
+  uint32_t tile_id;
+};
+
+template <bool FIRST, bool LAST, int THREADS, int ITEMS, int MIN_CTAS>
+__global__ void __launch_bounds__(THREADS, MIN_CTAS) onesweep_rec_kernel(const __grid_constant__ SortRecParams p) {
+  using Smem = OnesweepRecSmem<THREADS, ITEMS>;
+  constexpr int kTile = Smem::kTile;
+  constexpr int kWarps = Smem::kWarps;
+  static_assert(THREADS >= kRadix, "one thread per digit is needed for the look-back");
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
+
+  const uint32_t warp = threadIdx.x >> 5, lane = lane_id();
+  if (threadIdx.x == 0) sm.tile_id = atomicAdd(p.ticket, 1u);
+  for (int i = threadIdx.x; i < kWarps * kRadix; i += THREADS) (&sm.warp_hist[0][0])[i] = 0;
+  __syncthreads();
+  const uint32_t tile = sm.tile_id;
+  const uint64_t tile0 = (uint64_t)tile * kTile;
+  const uint32_t valid = (uint32_t)min((uint64_t)kTile, (uint64_t)p.n - tile0);
+  const uint32_t mask = (1u << p.bits) - 1u;
+
+  // ---- load records, warp-striped ----
+  uint4 rec[ITEMS];
+  const uint32_t wbase = warp * (ITEMS * 32) + lane;
+#pragma unroll
+  for (int i = 0; i < ITEMS; ++i) {
+    const uint32_t e = wbase + i * 32;
+    if (e < valid) {
+      if (FIRST) {
+        const uint64_t pos = tile0 + e;
+        const BlockAddr a = locate(p.map, pos);
+        const uint32_t s = *src_ptr(p.map, a);
+        const uint32_t d = *d_ptr(p.map, a);
+        rec[i].x = (s << p.delay_bits) | d;
+        rec[i].y = (uint32_t)pos;
+        rec[i].z = *tgt_ptr(p.map, a);
+        rec[i].w = __float_as_uint(*w_ptr(p.map, a));
+      } else {
+        rec[i] = p.recs_in[tile0 + e];
+      }
+    } else {
+      rec[i] = make_uint4(0xffffffffu, 0u, 0u, 0u);
+    }
+  }
+
+  // ---- stable rank inside the warp ----
+  uint32_t rank[ITEMS];
+  uint32_t* my_hist = sm.warp_hist[warp];
+#pragma unroll
+  for (int i = 0; i < ITEMS; ++i) {
+    const uint32_t d = (rec[i].x >> p.shift) & mask;
+    const uint32_t peers = __match_any_sync(0xffffffffu, d);
+    const uint32_t below = __popc(peers & lanemask_lt());
+    uint32_t pre = 0;
+    if (below == 0) {
+      pre = my_hist[d];
+      my_hist[d] = pre + __popc(peers);
+    }
+    __syncwarp();
+    pre = __shfl_sync(0xffffffffu, pre, __ffs(peers) - 1);
+    rank[i] = pre + below;
+  }
+  __syncthreads();
+
+  // ---- per digit: scan over warps, tile count, look-back, global offset ----
+  if (threadIdx.x < kRadix) {
+    const uint32_t d = threadIdx.x;
+    uint32_t run = 0;
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) {
+      const uint32_t c = sm.warp_hist[w][d];
+      sm.warp_hist[w][d] = run;
+      run += c;
+    }
+    const uint32_t tile_count = run;
+    const uint32_t real = (d == mask) ? run - (kTile - valid) : run;
+    uint64_t* my_status = p.status + (uint64_t)tile * kRadix + d;
+    uint64_t excl = 0;
+    if (tile == 0) {
+      st_relaxed_u64(my_status, p.epoch | kFlagInclusive | real);
+    } else {
+      st_relaxed_u64(my_status, p.epoch | kFlagAggregate | real);
+      const uint64_t* look = my_status - kRadix;
+      uint32_t spins = 0;
+      while (true) {
+        const uint64_t w = ld_relaxed_u64(look);
+        if ((w & ~(kCountMask | kFlagAggregate | kFlagInclusive)) != p.epoch || (w & (kFlagAggregate | kFlagInclusive)) == 0) {
+          if (++spins > (1u << 24)) {
+            *p.error_flag = 1u;
+            break;
+          }
+          __nanosleep(20);
+          continue;
+        }
+        excl += w & kCountMask;
+        if (w & kFlagInclusive) break;
+        look -= kRadix;
+      }
+      st_relaxed_u64(my_status, p.epoch | kFlagInclusive | (excl + real));
+    }
+    uint32_t inc = tile_count;
+#pragma unroll
+    for (int s = 1; s < 32; s <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, s);
+      if (lane >= (uint32_t)s) inc += t;
+    }
+    if (lane == 31) sm.scan_tmp[warp] = inc;
+    asm volatile("bar.sync 1, %0;" ::"n"(kRadix));
+    uint32_t base = 0;
+    for (uint32_t w = 0; w < warp; ++w) base += sm.scan_tmp[w];
+    const uint32_t te = base + inc - tile_count;
+    sm.tile_excl[d] = te;
+    sm.global_off[d] = p.bin_start[d] + (uint32_t)excl - te;
+  }
+  __syncthreads();
+
+  // ---- scatter records into shared memory in tile-sorted order ----
+#pragma unroll
+  for (int i = 0; i < ITEMS; ++i) {
+    const uint32_t d = (rec[i].x >> p.shift) & mask;
+    sm.recs[sm.tile_excl[d] + my_hist[d] + rank[i]] = rec[i];
+  }
+  __syncthreads();
+
+  // ---- write out ----
+  const uint32_t dmask = (1u << p.delay_bits) - 1u;
+#pragma unroll
+  for (int i = 0; i < ITEMS; ++i) {
+    const uint32_t j = i * THREADS + threadIdx.x;
+    if (j < valid) {
+      const uint4 r = sm.recs[j];
+      const uint32_t g = sm.global_off[(r.x >> p.shift) & mask] + j;
+      if (LAST) {
+        p.out_src[g] = r.x >> p.delay_bits;
+        p.out_d[g] = (uint16_t)(r.x & dmask);
+        p.out_tgt[g] = r.z;
+        p.out_w[g] = __uint_as_float(r.w);
+        p.out_perm[g] = r.y;
+      } else {
+        p.recs_out[g] = r;
+      }
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
 // Permutation apply (step a11): sorted_target[j] = target[perm[j]], sorted_weight[j] = weight[perm[j]];
 // source and delay are unpacked from the sorted key.
 // ---------------------------------------------------------------------------------------------

@@ -81,6 +81,25 @@ def test_microcircuit_scaled_parity(nc_mod, oracle_mod):
     assert len(net.projections) >= 50 and rep["n"] > 2_000_000
 
 
+def test_sort_pairs_variant_parity(nc_mod, oracle_mod):
+    """NC_FLAG_SORT_PAIRS: (key, position) pairs + gather by the permutation instead of carrying the connection."""
+    for net in (WL.config2_microcircuit(scale=0.06), WL.config1_rule("fixed_indegree", scale=0.2)):
+        rep, _ = PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_PAIRS)
+        assert rep["n"] > 300_000
+
+
+def test_single_pass_key(nc_mod, oracle_mod):
+    """<= 8 key bits: one digit pass that is both the first and the last (storage blocks -> final arrays)."""
+    net = WL.Network("narrow", [16])
+    net.projections = [WL.Projection(0, 0, "fixed_total_number", degree_or_total=100_000, weight=W,
+                                     delay_ms=(0.5, 0.3, 0.1, 1.5), seed=8)]
+    o, g = PU.build_both(net, oracle_mod, nc_mod)
+    assert g.stats()["sort_passes"] == 1
+    g.close()
+    PU.full_parity(net, oracle_mod, nc_mod)
+    PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_PAIRS)
+
+
 def test_block_sizes_paper_default_and_odd(nc_mod, oracle_mod):
     """B = 10^7 (the paper's default, not a power of two -> magic division) and an odd B (scalar stores)."""
     net = WL.config3_large_indegree(scale=0.02)  # 1600+400 nodes, K = 160 / 40 -> 400k synapses
