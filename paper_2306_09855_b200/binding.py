@@ -90,10 +90,12 @@ def load_library():
     global _lib
     if _lib is not None:
         return _lib
-    if not LIB_PATH.exists():
-        raise RuntimeError(f"{LIB_PATH} is not built: run `python -m paper_2306_09855_b200.build` "
+    import os
+    path = Path(os.environ.get("NC_LIB_PATH", str(LIB_PATH)))  # development override: another build of the same ABI
+    if not path.exists():
+        raise RuntimeError(f"{path} is not built: run `python -m paper_2306_09855_b200.build` "
                            "(there is no CPU fallback)")
-    L = C.CDLL(str(LIB_PATH))
+    L = C.CDLL(str(path))
     P, vp = C.POINTER, C.c_void_p
     L.nc_create.argtypes = [P(Config), P(vp)]
     L.nc_destroy.argtypes = [vp]
@@ -114,7 +116,7 @@ def load_library():
     L.nc_read_index.argtypes = [vp, vp, vp, vp, vp, vp]
     L.nc_read_degree_histogram.argtypes = [vp, C.c_int, vp, P(C.c_uint32)]
     L.nc_selftest_philox.argtypes = [vp, C.c_uint32, vp, vp, vp]
-    L.nc_selftest_fastpath.argtypes = [vp, P(C.c_double), P(C.c_double), P(C.c_double)]
+    L.nc_selftest_fastpath.argtypes = [vp, P(C.c_double)]
     for name in SYMBOLS:
         if name != "nc_last_error":
             getattr(L, name).restype = C.c_int
@@ -301,6 +303,6 @@ class NC:
         return out
 
     def selftest_fastpath(self):
-        a, b, c = C.c_double(), C.c_double(), C.c_double()
-        self._check(self._L.nc_selftest_fastpath(self._h, C.byref(a), C.byref(b), C.byref(c)))
-        return a.value, b.value, c.value
+        out = (C.c_double * 4)()
+        self._check(self._L.nc_selftest_fastpath(self._h, out))
+        return tuple(out)

@@ -7,6 +7,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <unordered_map>
@@ -218,11 +219,12 @@ SynConst make_syn(const nc_context* c, const nc_syn_spec& s) {
   k.d_lo = (float)s.delay_ms.lo;
   k.d_hi = (float)s.delay_ms.hi;
   k.inv_dt = (float)c->inv_dt;
-  // Guard band: 32 fp32 ulps of the largest |sd z1| / dt term, 32 relative
-  // ulps of x itself (covers the fp32 roundings of mean, sd, bounds, 1/dt and of the products), and a floor.
-  const double ulp32 = 1.0 / 16777216.0 * 32.0;
-  k.eps_abs = (float)(std::fabs(s.delay_ms.sd) * c->inv_dt * kZMax * ulp32 + 1e-6);
-  k.eps_rel = (float)ulp32;
+  // Guard band: the error of z1 (bounded in the kernel from r) enters x scaled
+  // by sd / dt; 32 relative fp32 ulps of x cover the fp32 roundings of mean, sd, the bounds, 1/dt and of the
+  // products; plus a small floor.
+  k.eps_scale = (float)(std::fabs(s.delay_ms.sd) * c->inv_dt);
+  k.eps_rel = (float)(32.0 / 16777216.0);
+  k.eps_abs = 1e-6f;
   k.exact = (c->cfg.flags & NC_FLAG_EXACT_FP64) ? 1 : 0;
   k.dd_mean = s.delay_ms.mean;
   k.dd_sd = s.delay_ms.sd;
@@ -423,7 +425,8 @@ int sort_and_index(nc_context* c, const PassPlan& plan) {
     NC_CUDA(c, cudaMemsetAsync(tickets, 0, (kMaxPasses + 1) * 4, c->stream));
     NC_CUDA(c, cudaMemsetAsync(status, 0, n_tiles * kRadix * 8, c->stream));
     const unsigned grid = (unsigned)(((uint64_t)n + kHistThreads * kHistItems - 1) / (kHistThreads * kHistItems));
-    histogram_kernel<KeyT><<<grid, kHistThreads, 0, c->stream>>>(map, n, c->delay_bits, plan, ghist);
+    if (c->B % 4 == 0) histogram_kernel<KeyT, true><<<grid, kHistThreads, 0, c->stream>>>(map, n, c->delay_bits, plan, ghist);
+    else histogram_kernel<KeyT, false><<<grid, kHistThreads, 0, c->stream>>>(map, n, c->delay_bits, plan, ghist);
     NC_LAUNCH_CHECK(c, "histogram");
     bin_scan_kernel<<<plan.n_passes, kRadix, 0, c->stream>>>(ghist, bin_start);
     NC_LAUNCH_CHECK(c, "bin_scan");
@@ -516,26 +519,51 @@ int sort_and_index(nc_context* c, const PassPlan& plan) {
 
 // Record-carrying organisation step (keys of <= 32 bits): histogram, P onesweep passes that move whole
 // connections, final pass writes the sorted SoA arrays; then the index over (source, delay).
-constexpr int kRecThreads = 512;
-constexpr int kRecItems = 8;
-constexpr int kRecMinCtas = 2;
+// Launch shapes of the record pass (threads, records per thread, CTAs per SM the registers are budgeted for).
+// Variant 0 is the default; NC_SORT_VARIANT selects another one for tuning runs.
+struct RecShape {
+  int threads, items;
+};
+constexpr RecShape kRecShapes[] = {{384, 8}, {256, 8}, {512, 8}, {512, 8}, {512, 8}, {256, 16}, {384, 8}, {320, 8}};
 
-template <bool FIRST, bool LAST>
-int launch_rec_pass(nc_context* c, const SortRecParams& sp, uint64_t n_tiles) {
-  using Smem = OnesweepRecSmem<kRecThreads, kRecItems>;
-  auto kern = onesweep_rec_kernel<FIRST, LAST, kRecThreads, kRecItems, kRecMinCtas>;
+int rec_variant() {
+  const char* e = getenv("NC_SORT_VARIANT");
+  const int v = e ? atoi(e) : 0;
+  return (v >= 0 && v < (int)(sizeof(kRecShapes) / sizeof(kRecShapes[0]))) ? v : 0;
+}
+
+template <bool FIRST, bool LAST, int THREADS, int ITEMS, int MIN_CTAS, int MATCH>
+int launch_rec_pass_shape(nc_context* c, const SortRecParams& sp) {
+  using Smem = OnesweepRecSmem<THREADS, ITEMS>;
+  auto kern = onesweep_rec_kernel<FIRST, LAST, THREADS, ITEMS, MIN_CTAS, MATCH>;
+  const uint64_t n_tiles = ((uint64_t)sp.n + Smem::kTile - 1) / Smem::kTile;
   NC_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem)));
-  kern<<<(unsigned)n_tiles, kRecThreads, sizeof(Smem), c->stream>>>(sp);
+  kern<<<(unsigned)n_tiles, THREADS, sizeof(Smem), c->stream>>>(sp);
   NC_LAUNCH_CHECK(c, "onesweep_rec");
   return NC_OK;
+}
+
+template <bool FIRST, bool LAST>
+int launch_rec_pass(nc_context* c, const SortRecParams& sp, int variant) {
+  switch (variant) {
+    case 1: return launch_rec_pass_shape<FIRST, LAST, 256, 8, 4, kMatchSmem>(c, sp);
+    case 2: return launch_rec_pass_shape<FIRST, LAST, 512, 8, 2, kMatchSmem>(c, sp);
+    case 3: return launch_rec_pass_shape<FIRST, LAST, 512, 8, 2, kMatchAny>(c, sp);
+    case 4: return launch_rec_pass_shape<FIRST, LAST, 512, 8, 2, kMatchBallot>(c, sp);
+    case 5: return launch_rec_pass_shape<FIRST, LAST, 256, 16, 2, kMatchSmem>(c, sp);
+    case 6: return launch_rec_pass_shape<FIRST, LAST, 384, 8, 3, kMatchBallot>(c, sp);
+    case 7: return launch_rec_pass_shape<FIRST, LAST, 320, 8, 3, kMatchSmem>(c, sp);
+    default: return launch_rec_pass_shape<FIRST, LAST, 384, 8, 3, kMatchSmem>(c, sp);
+  }
 }
 
 int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag);
 
 int sort_carry_and_index(nc_context* c, const PassPlan& plan) {
-  using Smem = OnesweepRecSmem<kRecThreads, kRecItems>;
   const uint32_t n = (uint32_t)c->n_conns;
-  const uint64_t n_tiles = ((uint64_t)n + Smem::kTile - 1) / Smem::kTile;
+  const int variant = rec_variant();
+  const uint64_t tile = (uint64_t)kRecShapes[variant].threads * kRecShapes[variant].items;
+  const uint64_t n_tiles = ((uint64_t)n + tile - 1) / tile;
   const BlockMap map = make_map(c);
   const uint32_t P = plan.n_passes;
 
@@ -567,7 +595,8 @@ int sort_carry_and_index(nc_context* c, const PassPlan& plan) {
     NC_CUDA(c, cudaMemsetAsync(tickets, 0, (kMaxPasses + 1) * 4, c->stream));
     NC_CUDA(c, cudaMemsetAsync(status, 0, n_tiles * kRadix * 8, c->stream));
     const unsigned grid = (unsigned)(((uint64_t)n + kHistThreads * kHistItems - 1) / (kHistThreads * kHistItems));
-    histogram_kernel<uint32_t><<<grid, kHistThreads, 0, c->stream>>>(map, n, c->delay_bits, plan, ghist);
+    if (c->B % 4 == 0) histogram_kernel<uint32_t, true><<<grid, kHistThreads, 0, c->stream>>>(map, n, c->delay_bits, plan, ghist);
+    else histogram_kernel<uint32_t, false><<<grid, kHistThreads, 0, c->stream>>>(map, n, c->delay_bits, plan, ghist);
     NC_LAUNCH_CHECK(c, "histogram");
     bin_scan_kernel<<<P, kRadix, 0, c->stream>>>(ghist, bin_start);
     NC_LAUNCH_CHECK(c, "bin_scan");
@@ -598,10 +627,10 @@ int sort_carry_and_index(nc_context* c, const PassPlan& plan) {
       sp.error_flag = tickets + kMaxPasses;
       sp.epoch = (uint64_t)(ps + 1) << 42;
       int rc;
-      if (first && last) rc = launch_rec_pass<true, true>(c, sp, n_tiles);
-      else if (first) rc = launch_rec_pass<true, false>(c, sp, n_tiles);
-      else if (last) rc = launch_rec_pass<false, true>(c, sp, n_tiles);
-      else rc = launch_rec_pass<false, false>(c, sp, n_tiles);
+      if (first && last) rc = launch_rec_pass<true, true>(c, sp, variant);
+      else if (first) rc = launch_rec_pass<true, false>(c, sp, variant);
+      else if (last) rc = launch_rec_pass<false, true>(c, sp, variant);
+      else rc = launch_rec_pass<false, false>(c, sp, variant);
       if (rc != NC_OK) return rc;
       cur = dst;
     }
@@ -699,26 +728,33 @@ __device__ void atomic_max_double(double* addr, double v) {  // v >= 0: bit patt
   atomicMax(reinterpret_cast<unsigned long long*>(addr), (unsigned long long)__double_as_longlong(v));
 }
 
-__global__ void selftest_fastpath_kernel(double* out /* [3] */) {
+__global__ void selftest_fastpath_kernel(double* out /* [4] */) {
   const uint32_t v = blockIdx.x * blockDim.x + threadIdx.x;  // 0 .. 2^24-1
   const uint32_t word = v << 8;
-  const float r32 = fast_radius(word);
+  float inv_r;
+  const float r32 = fast_radius(word, inv_r);
   const double u1 = (double)(v + 1u) * (1.0 / 16777216.0);
   const double r64 = sqrt(-2.0 * log(u1));
-  double er = r64 > 0.0 ? fabs((double)r32 - r64) / r64 : fabs((double)r32);
+  const double dr = fabs((double)r32 - r64);
+  // ratio of the actual error of r to the bound the guard band assumes, evaluated with the kernel's own r, 1/r
+  const double bound = (double)kErrRa * (double)inv_r + (double)kErrRb * (double)r32;
+  double e0 = r64 > 0.0 ? dr / bound : (dr == 0.0 ? 0.0 : 1e30);
+  double e3 = r64 > 0.0 ? dr / r64 : 0.0;
   float sn, cs;
   fast_sincos(word, sn, cs);
   const double th = 6.283185307179586 * ((double)v * (1.0 / 16777216.0));
-  double es = fabs((double)sn - sin(th)), ec = fabs((double)cs - cos(th));
+  double e1 = fabs((double)sn - sin(th)) / (double)kErrTrig, e2 = fabs((double)cs - cos(th)) / (double)kErrTrig;
   for (int d = 16; d > 0; d >>= 1) {
-    er = fmax(er, __shfl_xor_sync(0xffffffffu, er, d));
-    es = fmax(es, __shfl_xor_sync(0xffffffffu, es, d));
-    ec = fmax(ec, __shfl_xor_sync(0xffffffffu, ec, d));
+    e0 = fmax(e0, __shfl_xor_sync(0xffffffffu, e0, d));
+    e1 = fmax(e1, __shfl_xor_sync(0xffffffffu, e1, d));
+    e2 = fmax(e2, __shfl_xor_sync(0xffffffffu, e2, d));
+    e3 = fmax(e3, __shfl_xor_sync(0xffffffffu, e3, d));
   }
   if ((threadIdx.x & 31) == 0) {
-    atomic_max_double(out + 0, er);
-    atomic_max_double(out + 1, es);
-    atomic_max_double(out + 2, ec);
+    atomic_max_double(out + 0, e0);
+    atomic_max_double(out + 1, e1);
+    atomic_max_double(out + 2, e2);
+    atomic_max_double(out + 3, e3);
   }
 }
 
@@ -1105,20 +1141,16 @@ int nc_selftest_philox(nc_context* c, uint32_t n, const uint32_t* ctr, const uin
   return rc;
 }
 
-int nc_selftest_fastpath(nc_context* c, double* max_rel_err_r, double* max_abs_err_sin, double* max_abs_err_cos) {
-  if (!c) return NC_ERR_INVALID_ARG;
-  double* d = (double*)dev_alloc(c, 24);
+int nc_selftest_fastpath(nc_context* c, double out[4]) {
+  if (!c || !out) return NC_ERR_INVALID_ARG;
+  double* d = (double*)dev_alloc(c, 32);
   if (!d) return fail(c, NC_ERR_OOM, "selftest: out of device memory");
-  NC_CUDA(c, cudaMemsetAsync(d, 0, 24, c->stream));
+  NC_CUDA(c, cudaMemsetAsync(d, 0, 32, c->stream));
   selftest_fastpath_kernel<<<(1u << 24) / 256, 256, 0, c->stream>>>(d);
   NC_LAUNCH_CHECK(c, "selftest_fastpath");
-  double h[3] = {0, 0, 0};
-  NC_CUDA(c, cudaMemcpyAsync(h, d, 24, cudaMemcpyDeviceToHost, c->stream));
+  NC_CUDA(c, cudaMemcpyAsync(out, d, 32, cudaMemcpyDeviceToHost, c->stream));
   int rc = sync_stream(c);
   dev_free(c, d);
-  if (max_rel_err_r) *max_rel_err_r = h[0];
-  if (max_abs_err_sin) *max_abs_err_sin = h[1];
-  if (max_abs_err_cos) *max_abs_err_cos = h[2];
   return rc;
 }
 

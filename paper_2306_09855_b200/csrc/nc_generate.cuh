@@ -25,7 +25,9 @@ struct SynConst {
   // fp32 fast path
   float w_mean, w_sd, w_lo, w_hi;
   float d_mean, d_sd, d_lo, d_hi, inv_dt;
-  float eps_abs, eps_rel;  // guard band around a rounding boundary inside which the delay is redone in fp64
+  // guard band around a rounding boundary inside which the delay is redone in fp64:
+  //   eps = eps_scale * (bound on |z1_32 - z1|) + eps_rel * |x| + eps_abs
+  float eps_scale, eps_rel, eps_abs;
   int exact;               // NC_FLAG_EXACT_FP64: always take the fp64 path
   // fp64 path (same operations, in the order reading D8 writes them)
   double dd_mean, dd_sd, dd_lo, dd_hi, dinv_dt;
@@ -57,41 +59,58 @@ __device__ __noinline__ uint32_t delay_steps_fp64(uint32_t w2, uint32_t w3, cons
   return (uint32_t)st;
 }
 
-// fp32 fast path of D5/D6.  The 24-bit uniforms are exact in fp32; r = sqrt(-2 ln u1); (sin, cos)(2 pi u2)
-// go through sincospi(2 u2), whose argument is exact.  nc_selftest_fastpath measures these two functions
-// exhaustively (2^24 inputs each) against fp64 on the device; DESIGN.md derives the guard band from that.
-__device__ __forceinline__ float fast_radius(uint32_t w2) {
-  const float u1 = (float)((w2 >> 8) + 1u) * (1.0f / 16777216.0f);
-  return sqrtf(-2.0f * logf(u1));
+// ---------------------------------------------------------------------------------------------
+// fp32 fast path of D5/D6 on the special-function unit.
+//   r^2 = -2 ln u1 : lg2.approx away from u1 = 1; for t = 1 - u1 < 2^-5 (exact in fp32) the series
+//         2t(1 + t/2 + t^2/3 + t^3/4 + t^4/5), because the absolute error of lg2.approx would otherwise
+//         dominate a small r.  r = r^2 * rsqrt.approx(r^2).
+//   (sin, cos)(2 pi u2) : sin.approx / cos.approx.
+// Error model the guard band relies on (nc_selftest_fastpath checks it exhaustively, all 2^24 u1 and all
+// 2^24 u2, against fp64 on the device, and the GPU tests require a 4x margin):
+//   |r32 - r| <= kErrRa / r + kErrRb * r        |sin32 - sin|, |cos32 - cos| <= kErrTrig
+// ---------------------------------------------------------------------------------------------
+constexpr float kErrRa = 8.0e-7f;
+constexpr float kErrRb = 1.0e-6f;
+constexpr float kErrTrig = 4.0e-6f;
+
+__device__ __forceinline__ float fast_radius(uint32_t w2, float& inv_r) {
+  const float u1 = (float)((w2 >> 8) + 1u) * (1.0f / 16777216.0f);  // D5: exact in fp32
+  const float t = 1.0f - u1;                                        // exact
+  const float series = 2.0f * t * fmaf(t, fmaf(t, fmaf(t, fmaf(t, 0.2f, 0.25f), 0.33333334f), 0.5f), 1.0f);
+  const float r2 = t < 0.03125f ? series : -1.3862943611198906f * __log2f(u1);
+  inv_r = rsqrtf(r2);  // +inf when u1 == 1
+  return r2 > 0.0f ? r2 * inv_r : 0.0f;
 }
 __device__ __forceinline__ void fast_sincos(uint32_t w3, float& sn, float& cs) {
-  const float u2x2 = (float)(w3 >> 8) * (1.0f / 8388608.0f);  // 2 u2, exact
-  sincospif(u2x2, &sn, &cs);
+  const float theta = (float)(w3 >> 8) * (6.283185307179586f / 16777216.0f);
+  sn = __sinf(theta);
+  cs = __cosf(theta);
 }
 
 // Weight (fp32) and delay (steps) of one synapse from Philox words 2 and 3.
 __device__ __forceinline__ void draw_weight_delay(uint32_t w2, uint32_t w3, const SynConst& c, float& weight,
                                                   uint32_t& steps) {
-  const float r = fast_radius(w2);
+  float inv_r;
+  const float r = fast_radius(w2, inv_r);
   float sn, cs;
   fast_sincos(w3, sn, cs);
   const float z0 = r * cs, z1 = r * sn;
   // D7
   weight = fminf(fmaxf(fmaf(c.w_sd, z0, c.w_mean), c.w_lo), c.w_hi);
-  // D8 on the fast path, with a guard band: |x32 - x| is far below eps,
-  // so outside the band floor(x + 0.5) is the same integer in fp32 and fp64.
+  // D8 on the fast path.  y = x + 0.5; m = nearest integer to y (magic-number rounding, exact for
+  // |y| < 2^22); |y - m| is the distance of x to the nearest rounding boundary.  Outside the guard band
+  // floor(y) is the same integer in fp32 and in the oracle's fp64; inside it the delay is redone in fp64.
   const float d = fminf(fmaxf(fmaf(c.d_sd, z1, c.d_mean), c.d_lo), c.d_hi);
-  const float x = d * c.inv_dt;
-  const float fl = floorf(x);
-  const float frac = x - fl;
-  const float eps = fmaf(c.eps_rel, fabsf(x), c.eps_abs);
-  const bool near = fabsf(frac - 0.5f) < eps;
-  if (near || c.exact || !(fabsf(x) < 1.0e6f)) {
+  const float y = fmaf(d, c.inv_dt, 0.5f);
+  const float m = (y + 12582912.0f) - 12582912.0f;
+  const float err_z = fmaf(kErrRa, inv_r, (kErrRb + kErrTrig) * r);      // bound on |z1_32 - z1| (x 1/4 margin)
+  const float eps = fmaf(c.eps_scale, err_z, fmaf(c.eps_rel, fabsf(y), c.eps_abs));
+  const bool near = !(fabsf(y - m) >= eps);  // also true for NaN / inf
+  if (near || c.exact || !(fabsf(y) < 4.0e6f)) {
     steps = delay_steps_fp64(w2, w3, c);
   } else {
-    float st = fl + (frac >= 0.5f ? 1.0f : 0.0f);
-    st = fminf(fmaxf(st, 1.0f), 65535.0f);
-    steps = (uint32_t)st;
+    const float fl = m > y ? m - 1.0f : m;  // floor(y)
+    steps = (uint32_t)(int)fminf(fmaxf(fl, 1.0f), 65535.0f);
   }
 }
 

@@ -44,7 +44,7 @@ __device__ __forceinline__ KeyT load_key_from_storage(const BlockMap& map, uint6
 constexpr int kHistThreads = 512;
 constexpr int kHistItems = 16;
 
-template <typename KeyT>
+template <typename KeyT, bool VEC>
 __global__ void __launch_bounds__(kHistThreads) histogram_kernel(const __grid_constant__ BlockMap map, uint32_t n,
                                                                 uint32_t delay_bits,
                                                                 const __grid_constant__ PassPlan plan,
@@ -52,20 +52,46 @@ __global__ void __launch_bounds__(kHistThreads) histogram_kernel(const __grid_co
   __shared__ uint32_t hist[kMaxPasses][kRadix];
   for (int i = threadIdx.x; i < kMaxPasses * kRadix; i += kHistThreads) (&hist[0][0])[i] = 0;
   __syncthreads();
+  uint32_t shift[kMaxPasses], dmask[kMaxPasses];
+#pragma unroll
+  for (int ps = 0; ps < kMaxPasses; ++ps) {
+    shift[ps] = plan.shift[ps];
+    dmask[ps] = (1u << plan.bits[ps]) - 1u;
+  }
+  const uint32_t n_passes = plan.n_passes;
+  auto count = [&](KeyT key) {
+#pragma unroll
+    for (int ps = 0; ps < kMaxPasses; ++ps) {
+      if ((uint32_t)ps < n_passes) atomicAdd(&hist[ps][digit_of(key, shift[ps], dmask[ps])], 1u);
+    }
+  };
   const uint64_t tile0 = (uint64_t)blockIdx.x * (kHistThreads * kHistItems);
-#pragma unroll 4
-  for (int i = 0; i < kHistItems; ++i) {
-    const uint64_t pos = tile0 + (uint64_t)i * kHistThreads + threadIdx.x;
-    if (pos < n) {
-      const KeyT key = load_key_from_storage<KeyT>(map, pos, delay_bits);
-      for (uint32_t ps = 0; ps < plan.n_passes; ++ps) {
-        const uint32_t d = digit_of(key, plan.shift[ps], (1u << plan.bits[ps]) - 1u);
-        atomicAdd(&hist[ps][d], 1u);
+  if (VEC) {
+    // B % 4 == 0: a 4-aligned group of positions sits in one block, 16-byte aligned -> 128/64-bit loads
+#pragma unroll
+    for (int g = 0; g < kHistItems / 4; ++g) {
+      const uint64_t pos = tile0 + ((uint64_t)g * kHistThreads + threadIdx.x) * 4;
+      if (pos + 3 < n) {
+        const BlockAddr a = locate(map, pos);
+        const uint4 s4 = *reinterpret_cast<const uint4*>(src_ptr(map, a));
+        const uint2 d2 = *reinterpret_cast<const uint2*>(d_ptr(map, a));
+        count(((KeyT)s4.x << delay_bits) | (KeyT)(d2.x & 0xffffu));
+        count(((KeyT)s4.y << delay_bits) | (KeyT)(d2.x >> 16));
+        count(((KeyT)s4.z << delay_bits) | (KeyT)(d2.y & 0xffffu));
+        count(((KeyT)s4.w << delay_bits) | (KeyT)(d2.y >> 16));
+      } else {
+        for (uint64_t q = pos; q < n; ++q) count(load_key_from_storage<KeyT>(map, q, delay_bits));
       }
+    }
+  } else {
+#pragma unroll 4
+    for (int i = 0; i < kHistItems; ++i) {
+      const uint64_t pos = tile0 + (uint64_t)i * kHistThreads + threadIdx.x;
+      if (pos < n) count(load_key_from_storage<KeyT>(map, pos, delay_bits));
     }
   }
   __syncthreads();
-  for (int i = threadIdx.x; i < (int)plan.n_passes * kRadix; i += kHistThreads) {
+  for (int i = threadIdx.x; i < (int)n_passes * kRadix; i += kHistThreads) {
     const uint32_t v = (&hist[0][0])[i];
     if (v) atomicAdd(ghist + i, v);
   }
@@ -98,6 +124,84 @@ __global__ void __launch_bounds__(kRadix) bin_scan_kernel(const uint32_t* __rest
 constexpr uint64_t kFlagAggregate = 1ull << 40;
 constexpr uint64_t kFlagInclusive = 2ull << 40;
 constexpr uint64_t kCountMask = (1ull << 40) - 1;
+
+// Lanes of the warp whose digit equals mine, three ways (measured on B200, cycles per warp-wide call per SM at
+// full occupancy: match.any 61.5, eight ballots 25.3, shared-memory atomicOr 7.3 -- profiles/README.md):
+//   kMatchAny   : one MATCH.ANY
+//   kMatchBallot: one VOTE per digit bit
+//   kMatchSmem  : every lane ORs its lane bit into a per-(warp, digit) mask word in shared memory, the warp
+//                 reads the word back, the lowest peer clears it for the next item
+enum MatchMode : int { kMatchAny = 0, kMatchBallot = 1, kMatchSmem = 2 };
+
+template <int MODE>
+__device__ __forceinline__ uint32_t peers_of(uint32_t d, uint32_t* warp_masks /* [256], all zero between calls */) {
+  if (MODE == kMatchAny) return __match_any_sync(0xffffffffu, d);
+  if (MODE == kMatchBallot) {
+    uint32_t peers = 0xffffffffu;
+#pragma unroll
+    for (int b = 0; b < kRadixBits; ++b) {
+      const bool bit = (d >> b) & 1u;
+      const uint32_t vote = __ballot_sync(0xffffffffu, bit);
+      peers &= bit ? vote : ~vote;
+    }
+    return peers;
+  }
+  uint32_t* m = warp_masks + d;
+  atomicOr(m, 1u << lane_id());
+  __syncwarp();
+  const uint32_t peers = *m;
+  __syncwarp();
+  if ((peers & lanemask_lt()) == 0) *m = 0u;
+  __syncwarp();
+  return peers;
+}
+
+// Decoupled look-back for one digit of one tile: sum the counts of the preceding tiles, walking backwards
+// until a tile that already knows its inclusive prefix.  The status words of kLookBatch predecessors are
+// fetched with independent loads (they are L2 hits a few hundred cycles away; issuing them one at a time
+// made the walk, not the data movement, the critical path of a pass), then consumed in order.
+constexpr int kLookBatch = 8;
+
+__device__ __forceinline__ bool status_ready(uint64_t w, uint64_t epoch) {
+  return (w & ~(kCountMask | kFlagAggregate | kFlagInclusive)) == epoch && (w & (kFlagAggregate | kFlagInclusive)) != 0;
+}
+
+__device__ __forceinline__ uint64_t look_back(const uint64_t* status, uint32_t tile, uint32_t d, uint64_t epoch,
+                                              uint32_t* error_flag) {
+  uint64_t excl = 0;
+  int64_t t = (int64_t)tile - 1;
+  uint32_t spins = 0;
+  while (t >= 0) {
+    uint64_t w[kLookBatch];
+#pragma unroll
+    for (int k = 0; k < kLookBatch; ++k) {
+      const int64_t tk = t - k;
+      w[k] = tk >= 0 ? ld_relaxed_u64(status + (uint64_t)tk * kRadix + d) : (epoch | kFlagInclusive);
+    }
+    bool done = false;
+    int used = 0;
+#pragma unroll
+    for (int k = 0; k < kLookBatch; ++k) {
+      if (!done && used == k) {
+        if (status_ready(w[k], epoch)) {
+          excl += w[k] & kCountMask;
+          used = k + 1;
+          if (w[k] & kFlagInclusive) done = true;
+        }
+      }
+    }
+    if (done) break;
+    t -= used;
+    if (used == 0) {
+      if (++spins > (1u << 22)) {  // seconds: a predecessor is lost -> report instead of hanging the GPU
+        *error_flag = 1u;
+        break;
+      }
+      __nanosleep(32);
+    }
+  }
+  return excl;
+}
 
 template <typename KeyT>
 struct SortPassParams {
@@ -204,22 +308,7 @@ __global__ void __launch_bounds__(THREADS) onesweep_kernel(const __grid_constant
       st_relaxed_u64(my_status, p.epoch | kFlagInclusive | real);
     } else {
       st_relaxed_u64(my_status, p.epoch | kFlagAggregate | real);
-      const uint64_t* look = my_status - kRadix;
-      uint32_t spins = 0;
-      while (true) {
-        const uint64_t w = ld_relaxed_u64(look);
-        if ((w & ~(kCountMask | kFlagAggregate | kFlagInclusive)) != p.epoch || (w & (kFlagAggregate | kFlagInclusive)) == 0) {
-          if (++spins > (1u << 24)) {  // seconds: a predecessor is lost -> report instead of hanging the GPU
-            *p.error_flag = 1u;
-            break;
-          }
-          __nanosleep(20);
-          continue;  // predecessor has not published yet
-        }
-        excl += w & kCountMask;
-        if (w & kFlagInclusive) break;
-        look -= kRadix;
-      }
+      excl = look_back(p.status, tile, d, p.epoch, p.error_flag);
       st_relaxed_u64(my_status, p.epoch | kFlagInclusive | (excl + real));
     }
     // exclusive scan of tile_count across the 256 digits
@@ -304,14 +393,15 @@ struct OnesweepRecSmem {
   static constexpr int kTile = THREADS * ITEMS;
   static constexpr int kWarps = THREADS / 32;
   uint4 recs[kTile];
-  uint32_t warp_hist[kWarps][kRadix];
+  uint32_t warp_hist[kWarps][kRadix];   // per-warp digit counts, then the warp's running offset per digit
+  uint32_t warp_masks[kWarps][kRadix];  // kMatchSmem: peer-mask words (zero between uses)
   uint32_t tile_excl[kRadix];
   uint32_t global_off[kRadix];
   uint32_t scan_tmp[kRadix / 32];
   uint32_t tile_id;
 };
 
-template <bool FIRST, bool LAST, int THREADS, int ITEMS, int MIN_CTAS>
+template <bool FIRST, bool LAST, int THREADS, int ITEMS, int MIN_CTAS, int MATCH>
 __global__ void __launch_bounds__(THREADS, MIN_CTAS) onesweep_rec_kernel(const __grid_constant__ SortRecParams p) {
   using Smem = OnesweepRecSmem<THREADS, ITEMS>;
   constexpr int kTile = Smem::kTile;
@@ -321,93 +411,79 @@ __global__ void __launch_bounds__(THREADS, MIN_CTAS) onesweep_rec_kernel(const _
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
 
   const uint32_t warp = threadIdx.x >> 5, lane = lane_id();
+  // tiles are handed out in launch order so that a tile only ever waits on tiles that already run
   if (threadIdx.x == 0) sm.tile_id = atomicAdd(p.ticket, 1u);
-  for (int i = threadIdx.x; i < kWarps * kRadix; i += THREADS) (&sm.warp_hist[0][0])[i] = 0;
+  for (int i = threadIdx.x; i < 2 * kWarps * kRadix; i += THREADS) (&sm.warp_hist[0][0])[i] = 0;  // + warp_masks
   __syncthreads();
   const uint32_t tile = sm.tile_id;
   const uint64_t tile0 = (uint64_t)tile * kTile;
   const uint32_t valid = (uint32_t)min((uint64_t)kTile, (uint64_t)p.n - tile0);
   const uint32_t mask = (1u << p.bits) - 1u;
 
-  // ---- load records, warp-striped ----
+  // ---- load records, warp-striped: element (warp, i, lane) is tile position warp*ITEMS*32 + i*32 + lane ----
   uint4 rec[ITEMS];
   const uint32_t wbase = warp * (ITEMS * 32) + lane;
+  if (FIRST) {
+    // records are built from the SoA storage blocks; when the whole tile sits in one block (the common case)
+    // the block is located once per tile instead of once per record
+    const BlockAddr a0 = locate(p.map, tile0);
+    const bool one_block = a0.slot + kTile <= p.map.B;
+    const uint32_t* sp = reinterpret_cast<const uint32_t*>(a0.base) + a0.slot;
+    const uint32_t* tp = reinterpret_cast<const uint32_t*>(a0.base + p.map.off_tgt) + a0.slot;
+    const uint32_t* wp = reinterpret_cast<const uint32_t*>(a0.base + p.map.off_w) + a0.slot;
+    const uint16_t* dp = reinterpret_cast<const uint16_t*>(a0.base + p.map.off_d) + a0.slot;
 #pragma unroll
-  for (int i = 0; i < ITEMS; ++i) {
-    const uint32_t e = wbase + i * 32;
-    if (e < valid) {
-      if (FIRST) {
-        const uint64_t pos = tile0 + e;
-        const BlockAddr a = locate(p.map, pos);
-        const uint32_t s = *src_ptr(p.map, a);
-        const uint32_t d = *d_ptr(p.map, a);
-        rec[i].x = (s << p.delay_bits) | d;
-        rec[i].y = (uint32_t)pos;
-        rec[i].z = *tgt_ptr(p.map, a);
-        rec[i].w = __float_as_uint(*w_ptr(p.map, a));
+    for (int i = 0; i < ITEMS; ++i) {
+      const uint32_t e = wbase + i * 32;
+      if (e < valid) {
+        uint32_t s, d, t, w;
+        if (one_block) {
+          s = sp[e]; d = dp[e]; t = tp[e]; w = wp[e];
+        } else {
+          const BlockAddr a = locate(p.map, tile0 + e);
+          s = *src_ptr(p.map, a);
+          d = *d_ptr(p.map, a);
+          t = *tgt_ptr(p.map, a);
+          w = __float_as_uint(*w_ptr(p.map, a));
+        }
+        rec[i] = make_uint4((s << p.delay_bits) | d, (uint32_t)(tile0 + e), t, w);
       } else {
-        rec[i] = p.recs_in[tile0 + e];
+        rec[i] = make_uint4(0xffffffffu, 0u, 0u, 0u);
       }
-    } else {
-      rec[i] = make_uint4(0xffffffffu, 0u, 0u, 0u);
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < ITEMS; ++i) {
+      const uint32_t e = wbase + i * 32;
+      // padding sorts behind every real record of the tile and is never written out
+      rec[i] = e < valid ? p.recs_in[tile0 + e] : make_uint4(0xffffffffu, 0u, 0u, 0u);
     }
   }
 
-  // ---- stable rank inside the warp ----
-  uint32_t rank[ITEMS];
+  // ---- early counts: per-warp digit histogram with fire-and-forget shared-memory atomics ----
   uint32_t* my_hist = sm.warp_hist[warp];
 #pragma unroll
-  for (int i = 0; i < ITEMS; ++i) {
-    const uint32_t d = (rec[i].x >> p.shift) & mask;
-    const uint32_t peers = __match_any_sync(0xffffffffu, d);
-    const uint32_t below = __popc(peers & lanemask_lt());
-    uint32_t pre = 0;
-    if (below == 0) {
-      pre = my_hist[d];
-      my_hist[d] = pre + __popc(peers);
-    }
-    __syncwarp();
-    pre = __shfl_sync(0xffffffffu, pre, __ffs(peers) - 1);
-    rank[i] = pre + below;
-  }
+  for (int i = 0; i < ITEMS; ++i) atomicAdd(&my_hist[(rec[i].x >> p.shift) & mask], 1u);
   __syncthreads();
 
-  // ---- per digit: scan over warps, tile count, look-back, global offset ----
+  // ---- per digit: exclusive scan over the warps, tile count -> publish the tile aggregate right away;
+  //      exclusive scan over the digits -> where each digit's run starts inside the tile ----
+  uint32_t real = 0, my_excl = 0;
   if (threadIdx.x < kRadix) {
     const uint32_t d = threadIdx.x;
+    uint32_t cnt[kWarps];
+#pragma unroll
+    for (int w = 0; w < kWarps; ++w) cnt[w] = sm.warp_hist[w][d];
     uint32_t run = 0;
 #pragma unroll
     for (int w = 0; w < kWarps; ++w) {
-      const uint32_t c = sm.warp_hist[w][d];
       sm.warp_hist[w][d] = run;
-      run += c;
+      run += cnt[w];
     }
     const uint32_t tile_count = run;
-    const uint32_t real = (d == mask) ? run - (kTile - valid) : run;
-    uint64_t* my_status = p.status + (uint64_t)tile * kRadix + d;
-    uint64_t excl = 0;
-    if (tile == 0) {
-      st_relaxed_u64(my_status, p.epoch | kFlagInclusive | real);
-    } else {
-      st_relaxed_u64(my_status, p.epoch | kFlagAggregate | real);
-      const uint64_t* look = my_status - kRadix;
-      uint32_t spins = 0;
-      while (true) {
-        const uint64_t w = ld_relaxed_u64(look);
-        if ((w & ~(kCountMask | kFlagAggregate | kFlagInclusive)) != p.epoch || (w & (kFlagAggregate | kFlagInclusive)) == 0) {
-          if (++spins > (1u << 24)) {
-            *p.error_flag = 1u;
-            break;
-          }
-          __nanosleep(20);
-          continue;
-        }
-        excl += w & kCountMask;
-        if (w & kFlagInclusive) break;
-        look -= kRadix;
-      }
-      st_relaxed_u64(my_status, p.epoch | kFlagInclusive | (excl + real));
-    }
+    // padding records of a ragged last tile all carry the largest digit; they are not part of the data
+    real = (d == mask) ? run - (kTile - valid) : run;
+    st_relaxed_u64(p.status + (uint64_t)tile * kRadix + d, p.epoch | (tile == 0 ? kFlagInclusive : kFlagAggregate) | real);
     uint32_t inc = tile_count;
 #pragma unroll
     for (int s = 1; s < 32; s <<= 1) {
@@ -418,21 +494,38 @@ __global__ void __launch_bounds__(THREADS, MIN_CTAS) onesweep_rec_kernel(const _
     asm volatile("bar.sync 1, %0;" ::"n"(kRadix));
     uint32_t base = 0;
     for (uint32_t w = 0; w < warp; ++w) base += sm.scan_tmp[w];
-    const uint32_t te = base + inc - tile_count;
-    sm.tile_excl[d] = te;
-    sm.global_off[d] = p.bin_start[d] + (uint32_t)excl - te;
+    my_excl = base + inc - tile_count;
+    sm.tile_excl[d] = my_excl;
   }
   __syncthreads();
 
-  // ---- scatter records into shared memory in tile-sorted order ----
+  // ---- stable rank + scatter into shared memory in one go: the lowest lane of each group of equal digits
+  //      bumps the warp's running offset for that digit (atomics of one warp to one address retire in
+  //      program order, so items keep their position order) and the group shares the old value ----
 #pragma unroll
   for (int i = 0; i < ITEMS; ++i) {
     const uint32_t d = (rec[i].x >> p.shift) & mask;
-    sm.recs[sm.tile_excl[d] + my_hist[d] + rank[i]] = rec[i];
+    const uint32_t peers = peers_of<MATCH>(d, sm.warp_masks[warp]);
+    const uint32_t below = __popc(peers & lanemask_lt());
+    uint32_t old = 0;
+    if (below == 0) old = atomicAdd(&my_hist[d], (uint32_t)__popc(peers));
+    old = __shfl_sync(0xffffffffu, old, __ffs(peers) - 1);
+    sm.recs[sm.tile_excl[d] + old + below] = rec[i];
+  }
+
+  // ---- look-back: where this tile's run of each digit starts in the output ----
+  if (threadIdx.x < kRadix) {
+    const uint32_t d = threadIdx.x;
+    uint64_t excl = 0;
+    if (tile != 0) {
+      excl = look_back(p.status, tile, d, p.epoch, p.error_flag);
+      st_relaxed_u64(p.status + (uint64_t)tile * kRadix + d, p.epoch | kFlagInclusive | (excl + real));
+    }
+    sm.global_off[d] = p.bin_start[d] + (uint32_t)excl - my_excl;
   }
   __syncthreads();
 
-  // ---- write out ----
+  // ---- write out: consecutive threads write consecutive records of a digit run ----
   const uint32_t dmask = (1u << p.delay_bits) - 1u;
 #pragma unroll
   for (int i = 0; i < ITEMS; ++i) {

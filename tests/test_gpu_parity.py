@@ -40,15 +40,15 @@ def test_device_philox_matches_known_answers_and_oracle(nc_mod, oracle_mod):
 
 
 def test_fastpath_error_is_inside_the_guard_band(nc_mod):
-    """Exhaustive over all 2^24 u1 and all 2^24 u2 on the device: the fp32 radius and sin/cos stay within
-    the error the guard band assumes (|dz1| <= 5.77 (er + es) must be far
-    below 5.769 * 32 ulp = 1.1e-5)."""
+    """Exhaustive over all 2^24 u1 and all 2^24 u2 on the device: the special-function fast path of the
+    radius and of sin/cos stays within a quarter of the error bound the delay guard band assumes (DESIGN.md
+    'delay fast path'), and the radius is relatively accurate enough for the 1e-5 weight tolerance."""
     g = nc_mod.NC()
-    er, es, ec = g.selftest_fastpath()
+    ratio_r, ratio_sin, ratio_cos, rel_r = g.selftest_fastpath()
     g.close()
-    print(f"fast path: max rel err r {er:.3e}, max abs err sin {es:.3e}, cos {ec:.3e}")
-    assert er < 4 * 2.0**-24 and es < 4 * 2.0**-24 and ec < 4 * 2.0**-24
-    assert 5.7681 * (er + es) < 0.25 * 5.769 * 32 * 2.0**-24
+    print(f"fast path: worst error/bound: r {ratio_r:.3f}, sin {ratio_sin:.3f}, cos {ratio_cos:.3f}; max rel err r {rel_r:.3e}")
+    assert ratio_r < 0.25 and ratio_sin < 0.25 and ratio_cos < 0.25
+    assert rel_r < 2e-5
 
 
 @pytest.mark.parametrize("B", [0, 10, 64, 1000])
