@@ -70,9 +70,13 @@ typedef struct {
 enum {
   NC_FLAG_TIMING = 1u << 0,     /* record CUDA events around every phase (nc_get_timings) */
   NC_FLAG_EXACT_FP64 = 1u << 1, /* debug: draw every delay on the fp64 path (no fp32 fast path) */
-  NC_FLAG_SORT_PAIRS = 1u << 2  /* sort (key, position) pairs and gather target/weight by the permutation
-                                   afterwards, instead of carrying the whole connection through the digit
-                                   passes (the default for keys of <= 32 bits; wider keys always use pairs) */
+  NC_FLAG_SORT_PAIRS = 1u << 2, /* sort (key, position) pairs with single-pass digit sweeps (decoupled look-back)
+                                   and gather target/weight by the permutation afterwards, instead of carrying
+                                   the whole connection through the digit passes; keys wider than 32 bits always
+                                   take this path */
+  NC_FLAG_SORT_ONESWEEP = 1u << 3 /* carry the whole connection, but chain the tiles of a digit pass inside the
+                                   pass (decoupled look-back) instead of the default count / scan / scatter
+                                   kernels per pass */
 };
 
 typedef struct {

@@ -17,6 +17,7 @@
 #include "nc_generate.cuh"
 #include "nc_index.cuh"
 #include "nc_sort.cuh"
+#include "nc_sort_split.cuh"
 
 using namespace nc;
 
@@ -640,6 +641,110 @@ int sort_carry_and_index(nc_context* c, const PassPlan& plan) {
   return rc;
 }
 
+// Default organisation step for keys of <= 32 bits (nc_sort_split.cuh): per digit pass, per-tile digit counts ->
+// scan -> scatter of whole connections; the last pass writes the sorted SoA arrays; then the index.
+constexpr int kSplitWarps = 8;
+constexpr int kSplitItems = 16;
+constexpr int kSplitTile = kSplitWarps * 32 * kSplitItems;
+
+template <bool FIRST, bool LAST>
+int launch_scatter_pass(nc_context* c, const ScatterParams& sp, uint32_t n_tiles) {
+  using Smem = ScatterSmem<kSplitWarps, kSplitItems, false>;
+  auto kern = scatter_pass_kernel<FIRST, LAST, kSplitWarps, kSplitItems, 2, kMatchBallot>;
+  NC_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem)));
+  kern<<<n_tiles, kSplitWarps * 32, sizeof(Smem), c->stream>>>(sp);
+  NC_LAUNCH_CHECK(c, "scatter_pass");
+  return NC_OK;
+}
+
+int sort_split_and_index(nc_context* c, const PassPlan& plan) {
+  const uint32_t n = (uint32_t)c->n_conns;
+  const uint32_t n_tiles = (uint32_t)(((uint64_t)n + kSplitTile - 1) / kSplitTile);
+  const uint32_t n_chunks = (n_tiles + kScanChunkTiles - 1) / kScanChunkTiles;
+  const BlockMap map = make_map(c);
+  const uint32_t P = plan.n_passes;
+
+  uint4* recs[2] = {P > 1 ? (uint4*)dev_alloc(c, (size_t)n * 16) : nullptr,
+                    P > 2 ? (uint4*)dev_alloc(c, (size_t)n * 16) : nullptr};
+  uint8_t* dig = P > 1 ? (uint8_t*)dev_alloc(c, (size_t)n) : nullptr;
+  uint16_t* counts = (uint16_t*)dev_alloc(c, (size_t)n_tiles * kRadix * 2);
+  uint32_t* offs = (uint32_t*)dev_alloc(c, (size_t)n_tiles * kRadix * 4);
+  uint32_t* chunk = (uint32_t*)dev_alloc(c, (size_t)n_chunks * kRadix * 4);
+  c->s_src = (uint32_t*)dev_alloc(c, (size_t)n * 4);
+  c->s_tgt = (uint32_t*)dev_alloc(c, (size_t)n * 4);
+  c->s_w = (float*)dev_alloc(c, (size_t)n * 4);
+  c->s_d = (uint16_t*)dev_alloc(c, (size_t)n * 2);
+  c->perm = (uint32_t*)dev_alloc(c, (size_t)n * 4);
+  bool ok = counts && offs && chunk && c->s_src && c->s_tgt && c->s_w && c->s_d && c->perm;
+  if (P > 1) ok = ok && recs[0] && dig;
+  if (P > 2) ok = ok && recs[1];
+  auto drop_scratch = [&]() {
+    dev_free_later(c, recs[0]); dev_free_later(c, recs[1]); dev_free_later(c, dig);
+    dev_free_later(c, counts); dev_free_later(c, offs); dev_free_later(c, chunk);
+  };
+  if (!ok) {
+    drop_scratch();
+    return fail(c, NC_ERR_OOM, "out of device memory in nc_finalize");
+  }
+  int cur = -1;
+  for (uint32_t ps = 0; ps < P; ++ps) {
+    const bool first = ps == 0, last = ps + 1 == P;
+    {
+      Scope sc(c, NC_PHASE_HISTOGRAM);
+      if (first) {
+        if (c->B % 4 == 0)
+          tile_count_first_kernel<true><<<n_tiles, kCountThreads, 0, c->stream>>>(map, n, kSplitTile, c->delay_bits,
+                                                                                plan.shift[0], plan.bits[0], counts);
+        else
+          tile_count_first_kernel<false><<<n_tiles, kCountThreads, 0, c->stream>>>(map, n, kSplitTile, c->delay_bits,
+                                                                                 plan.shift[0], plan.bits[0], counts);
+      } else {
+        tile_count_bytes_kernel<<<(n_tiles + kCountTilesPerCta - 1) / kCountTilesPerCta, kCountThreads, 0, c->stream>>>(
+            dig, n, kSplitTile, n_tiles, counts);
+      }
+      NC_LAUNCH_CHECK(c, "tile_count");
+      chunk_total_kernel<<<n_chunks, kRadix, 0, c->stream>>>(counts, n_tiles, chunk);
+      NC_LAUNCH_CHECK(c, "chunk_total");
+      chunk_scan_kernel<<<1, kRadix, 0, c->stream>>>(chunk, n_chunks);
+      NC_LAUNCH_CHECK(c, "chunk_scan");
+      tile_offsets_kernel<<<n_chunks, kRadix, 0, c->stream>>>(counts, n_tiles, chunk, offs);
+      NC_LAUNCH_CHECK(c, "tile_offsets");
+    }
+    {
+      Scope sc(c, NC_PHASE_SORT);
+      Scope pass_sc(c, NC_PHASE_SORT, true);
+      ScatterParams sp{};
+      sp.map = map;
+      sp.delay_bits = c->delay_bits;
+      sp.n = n;
+      const int dst = cur < 0 ? 0 : 1 - cur;
+      sp.recs_in = first ? nullptr : recs[cur];
+      sp.recs_out = last ? nullptr : recs[dst];
+      sp.dig_out = dig;
+      sp.out_src = c->s_src;
+      sp.out_tgt = c->s_tgt;
+      sp.out_w = c->s_w;
+      sp.out_d = c->s_d;
+      sp.out_perm = c->perm;
+      sp.shift = plan.shift[ps];
+      sp.bits = plan.bits[ps];
+      sp.next_shift = last ? 0 : plan.shift[ps + 1];
+      sp.next_bits = last ? 0 : plan.bits[ps + 1];
+      sp.offs = offs;
+      int rc;
+      if (first && last) rc = launch_scatter_pass<true, true>(c, sp, n_tiles);
+      else if (first) rc = launch_scatter_pass<true, false>(c, sp, n_tiles);
+      else if (last) rc = launch_scatter_pass<false, true>(c, sp, n_tiles);
+      else rc = launch_scatter_pass<false, false>(c, sp, n_tiles);
+      if (rc != NC_OK) return rc;
+      cur = dst;
+    }
+  }
+  int rc = build_index_from_sorted(c, n, nullptr);
+  drop_scratch();
+  return rc;
+}
+
 // a12-a14 over the final source / delay arrays.
 int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) {
   const uint32_t N = c->n_nodes;
@@ -667,7 +772,7 @@ int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) 
     int rc = device_scan(c, tile_heads, tile_head_off, head_tiles, head_partial, d_total_groups);
     if (rc != NC_OK) return rc;
     NC_CUDA(c, cudaMemcpyAsync(&total_groups, d_total_groups, 8, cudaMemcpyDeviceToHost, c->stream));
-    NC_CUDA(c, cudaMemcpyAsync(&lookback_error, lookback_flag, 4, cudaMemcpyDeviceToHost, c->stream));
+    if (lookback_flag) NC_CUDA(c, cudaMemcpyAsync(&lookback_error, lookback_flag, 4, cudaMemcpyDeviceToHost, c->stream));
   }
   NC_CUDA(c, cudaStreamSynchronize(c->stream));  // total_groups sizes the group arrays
   if (lookback_error) {
@@ -953,7 +1058,8 @@ int nc_finalize(nc_context* c) {
     int rc;
     if (c->key_bits > 32) rc = sort_and_index<uint64_t>(c, plan);
     else if (c->cfg.flags & NC_FLAG_SORT_PAIRS) rc = sort_and_index<uint32_t>(c, plan);
-    else rc = sort_carry_and_index(c, plan);
+    else if (c->cfg.flags & NC_FLAG_SORT_ONESWEEP) rc = sort_carry_and_index(c, plan);
+    else rc = sort_split_and_index(c, plan);
     if (rc != NC_OK) return rc;
   }
   c->finalized = true;

@@ -1,0 +1,352 @@
+// nc_sort_split.cuh -- stable LSD radix sort that carries the whole connection, digit passes WITHOUT any
+// communication between the CTAs of a pass (steps a9-a11 of DESIGN.md; the default organisation path for keys
+// of <= 32 bits).
+//
+// connections are sorted "using two sorting keys: the index of the source node as the first key
+// and the delay as the second"; reading D10: ties keep creation order, so every step here is stable.
+//
+// Per digit pass (reduce - scan - scatter):
+//   tile_count_*   : digit histogram of every tile of kTile consecutive records       -> counts[tile][256] (u16)
+//                    first pass : digits come from (source, delay) in the storage blocks (6 B / connection)
+//                    later      : digits come from the 1-byte-per-record side array the previous scatter wrote
+//   chunk_total / chunk_scan / tile_offsets : exclusive scan of the counts in (digit, tile) order
+//                                                                                     -> offs[tile][256]  (u32)
+//   scatter_pass   : a tile is ranked in shared memory (per-warp digit counters + warp match), its records are
+//                    staged in shared memory in tile-sorted order and written out as per-digit runs of
+//                    consecutive 16-byte records, starting at offs[tile][digit]; it also writes the next
+//                    pass's digit of every record to the side array.
+// Record = (key, creation position, target, weight) = one uint4, key = (source << delay_bits) | delay.  The
+// first pass builds records from the SoA storage blocks, the last pass writes the final SoA arrays (source and
+// delay unpacked from the key, target, weight, permutation): there is no gather by the permutation, every byte
+// the organisation step moves is streamed.
+//
+// Why not the single-pass ("onesweep") chaining of nc_sort.cuh: measured on B200 (profiles/README.md), the
+// scatter kernel alone moves a 2.99e8-record pass in 2.0 ms; every variant that chains tile prefixes inside the
+// pass (decoupled look-back by 256 threads, by a dedicated warp, or by scanner CTAs) cost 2.6 - 2.9 ms because
+// ~450 tiles are in flight and each needs the counts of all tiles before it within a few L2 round trips.  The
+// count + scan kernels cost 0.1 ms per pass and read 1 extra byte per record.
+#pragma once
+
+#include "nc_common.cuh"
+#include "nc_sort.cuh"
+
+namespace nc {
+
+// ---------------------------------------------------------------------------------------------
+// Per-tile digit counts.
+// ---------------------------------------------------------------------------------------------
+constexpr int kCountThreads = 256;
+
+// First pass: digits of key = (source << delay_bits) | delay straight from the storage blocks.
+template <bool VEC>
+__global__ void __launch_bounds__(kCountThreads) tile_count_first_kernel(const __grid_constant__ BlockMap map, uint32_t n,
+                                                                        uint32_t tile_size, uint32_t delay_bits,
+                                                                        uint32_t shift, uint32_t bits,
+                                                                        uint16_t* __restrict__ counts) {
+  __shared__ uint32_t hist[kRadix];
+  hist[threadIdx.x] = 0;
+  __syncthreads();
+  const uint32_t mask = (1u << bits) - 1u;
+  const uint64_t tile0 = (uint64_t)blockIdx.x * tile_size;
+  const uint32_t valid = (uint32_t)min((uint64_t)tile_size, (uint64_t)n - tile0);
+  if (VEC) {
+    // B % 4 == 0 and tile_size % 4 == 0: a 4-aligned group of positions sits in one block, 16-byte aligned
+    for (uint32_t e = threadIdx.x * 4; e < valid; e += kCountThreads * 4) {
+      const uint64_t pos = tile0 + e;
+      if (e + 3 < valid) {
+        const BlockAddr a = locate(map, pos);
+        const uint4 s4 = *reinterpret_cast<const uint4*>(src_ptr(map, a));
+        const uint2 d2 = *reinterpret_cast<const uint2*>(d_ptr(map, a));
+        atomicAdd(&hist[(((s4.x << delay_bits) | (d2.x & 0xffffu)) >> shift) & mask], 1u);
+        atomicAdd(&hist[(((s4.y << delay_bits) | (d2.x >> 16)) >> shift) & mask], 1u);
+        atomicAdd(&hist[(((s4.z << delay_bits) | (d2.y & 0xffffu)) >> shift) & mask], 1u);
+        atomicAdd(&hist[(((s4.w << delay_bits) | (d2.y >> 16)) >> shift) & mask], 1u);
+      } else {
+        for (uint32_t q = e; q < valid; ++q)
+          atomicAdd(&hist[(load_key_from_storage<uint32_t>(map, tile0 + q, delay_bits) >> shift) & mask], 1u);
+      }
+    }
+  } else {
+    for (uint32_t e = threadIdx.x; e < valid; e += kCountThreads)
+      atomicAdd(&hist[(load_key_from_storage<uint32_t>(map, tile0 + e, delay_bits) >> shift) & mask], 1u);
+  }
+  __syncthreads();
+  counts[(uint64_t)blockIdx.x * kRadix + threadIdx.x] = (uint16_t)hist[threadIdx.x];
+}
+
+// Later passes: digits come from the side array (one byte per record) written by the previous scatter.
+// One CTA counts kCountTilesPerCta consecutive tiles (tile_size % 16 == 0; the arrays are 256-byte aligned).
+constexpr int kCountTilesPerCta = 8;
+
+__global__ void __launch_bounds__(kCountThreads) tile_count_bytes_kernel(const uint8_t* __restrict__ dig, uint32_t n,
+                                                                        uint32_t tile_size, uint32_t n_tiles,
+                                                                        uint16_t* __restrict__ counts) {
+  __shared__ uint32_t hist[kRadix];
+  hist[threadIdx.x] = 0;
+  __syncthreads();
+  for (uint32_t k = 0; k < (uint32_t)kCountTilesPerCta; ++k) {
+    const uint32_t tile = blockIdx.x * kCountTilesPerCta + k;
+    if (tile >= n_tiles) break;
+    const uint64_t tile0 = (uint64_t)tile * tile_size;
+    const uint32_t valid = (uint32_t)min((uint64_t)tile_size, (uint64_t)n - tile0);
+    for (uint32_t e = threadIdx.x * 16; e < valid; e += kCountThreads * 16) {
+      if (e + 15 < valid) {
+        const uint4 v = *reinterpret_cast<const uint4*>(dig + tile0 + e);
+        const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          atomicAdd(&hist[w[j] & 0xffu], 1u);
+          atomicAdd(&hist[(w[j] >> 8) & 0xffu], 1u);
+          atomicAdd(&hist[(w[j] >> 16) & 0xffu], 1u);
+          atomicAdd(&hist[w[j] >> 24], 1u);
+        }
+      } else {
+        for (uint32_t q = e; q < valid; ++q) atomicAdd(&hist[dig[tile0 + q]], 1u);
+      }
+    }
+    __syncthreads();
+    counts[(uint64_t)tile * kRadix + threadIdx.x] = (uint16_t)hist[threadIdx.x];
+    hist[threadIdx.x] = 0;
+    __syncthreads();
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Exclusive scan of counts[tile][digit] in (digit, tile) order -> offs[tile][digit] = first output position
+// of the tile's run of that digit.  Tiles are grouped into chunks of kScanChunkTiles; thread = digit.
+// ---------------------------------------------------------------------------------------------
+constexpr int kScanChunkTiles = 128;
+
+__global__ void __launch_bounds__(kRadix) chunk_total_kernel(const uint16_t* __restrict__ counts, uint32_t n_tiles,
+                                                            uint32_t* __restrict__ chunk_tot) {
+  const uint32_t t0 = blockIdx.x * kScanChunkTiles;
+  const uint32_t t1 = min(t0 + (uint32_t)kScanChunkTiles, n_tiles);
+  uint32_t s = 0;
+#pragma unroll 8
+  for (uint32_t t = t0; t < t1; ++t) s += counts[(uint64_t)t * kRadix + threadIdx.x];
+  chunk_tot[(uint64_t)blockIdx.x * kRadix + threadIdx.x] = s;
+}
+
+// one CTA: digit totals -> exclusive scan over the digits (first output position of each digit), then the
+// running start of every chunk, in place (chunk_tot becomes chunk_base).
+__global__ void __launch_bounds__(kRadix) chunk_scan_kernel(uint32_t* __restrict__ chunk_tot, uint32_t n_chunks) {
+  __shared__ uint32_t warp_tot[kRadix / 32];
+  const uint32_t d = threadIdx.x;
+  uint32_t total = 0;
+#pragma unroll 8
+  for (uint32_t c = 0; c < n_chunks; ++c) total += chunk_tot[(uint64_t)c * kRadix + d];
+  uint32_t inc = total;
+#pragma unroll
+  for (int s = 1; s < 32; s <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xffffffffu, inc, s);
+    if (lane_id() >= (uint32_t)s) inc += t;
+  }
+  if (lane_id() == 31) warp_tot[d >> 5] = inc;
+  __syncthreads();
+  uint32_t run = inc - total;
+  for (uint32_t w = 0; w < (d >> 5); ++w) run += warp_tot[w];
+#pragma unroll 8
+  for (uint32_t c = 0; c < n_chunks; ++c) {
+    const uint32_t v = chunk_tot[(uint64_t)c * kRadix + d];
+    chunk_tot[(uint64_t)c * kRadix + d] = run;
+    run += v;
+  }
+}
+
+__global__ void __launch_bounds__(kRadix) tile_offsets_kernel(const uint16_t* __restrict__ counts, uint32_t n_tiles,
+                                                             const uint32_t* __restrict__ chunk_base,
+                                                             uint32_t* __restrict__ offs) {
+  const uint32_t t0 = blockIdx.x * kScanChunkTiles;
+  const uint32_t t1 = min(t0 + (uint32_t)kScanChunkTiles, n_tiles);
+  uint32_t run = chunk_base[(uint64_t)blockIdx.x * kRadix + threadIdx.x];
+#pragma unroll 8
+  for (uint32_t t = t0; t < t1; ++t) {
+    const uint32_t c = counts[(uint64_t)t * kRadix + threadIdx.x];
+    offs[(uint64_t)t * kRadix + threadIdx.x] = run;
+    run += c;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Scatter pass.
+// ---------------------------------------------------------------------------------------------
+struct ScatterParams {
+  BlockMap map;  // FIRST: records are built from the storage blocks
+  uint32_t delay_bits;
+  uint32_t n;
+  const uint4* recs_in;
+  uint4* recs_out;
+  uint8_t* dig_out;  // !LAST: digit of the NEXT pass for every record written
+  uint32_t* out_src;  // LAST: final arrays
+  uint32_t* out_tgt;
+  float* out_w;
+  uint16_t* out_d;
+  uint32_t* out_perm;
+  uint32_t shift, bits;            // this pass's digit
+  uint32_t next_shift, next_bits;  // the next pass's digit
+  const uint32_t* offs;            // [n_tiles][256]
+};
+
+template <int WARPS, int ITEMS, bool SMEM_MATCH>
+struct ScatterSmem {
+  static constexpr int kTile = WARPS * 32 * ITEMS;
+  uint4 recs[kTile];
+  uint32_t warp_hist[WARPS][kRadix];  // per-warp digit counts, then the warp's running tile position per digit
+  uint32_t warp_masks[SMEM_MATCH ? WARPS : 1][kRadix];  // kMatchSmem: peer-mask words (zero between uses)
+  uint32_t global_off[kRadix];  // (first output position of the tile's run of the digit) - (its start in the tile)
+  uint32_t scan_tmp[kRadix / 32];
+};
+
+template <bool FIRST, bool LAST, int WARPS, int ITEMS, int MIN_CTAS, int MATCH>
+__global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(const __grid_constant__ ScatterParams p) {
+  using Smem = ScatterSmem<WARPS, ITEMS, MATCH == kMatchSmem>;
+  constexpr int kThreads = WARPS * 32;
+  constexpr int kTile = Smem::kTile;
+  static_assert(kThreads >= kRadix, "one thread per digit is needed for the in-tile scan");
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
+
+  const uint32_t warp = threadIdx.x >> 5, lane = lane_id();
+  {
+    constexpr int kZero = (MATCH == kMatchSmem ? 2 : 1) * WARPS * kRadix / 4;  // warp_hist (+ warp_masks)
+    uint4* z = reinterpret_cast<uint4*>(&sm.warp_hist[0][0]);
+    for (int i = threadIdx.x; i < kZero; i += kThreads) z[i] = make_uint4(0u, 0u, 0u, 0u);
+  }
+  const uint32_t tile = blockIdx.x;
+  const uint64_t tile0 = (uint64_t)tile * kTile;
+  const uint32_t valid = (uint32_t)min((uint64_t)kTile, (uint64_t)p.n - tile0);
+  const uint32_t mask = (1u << p.bits) - 1u;
+
+  // ---- load records, warp-striped: element (warp, i, lane) is tile position warp*ITEMS*32 + i*32 + lane ----
+  uint4 rec[ITEMS];
+  const uint32_t wbase = warp * (ITEMS * 32) + lane;
+  uint32_t* my_hist = sm.warp_hist[warp];
+  if (FIRST) {
+    // records are built from the SoA storage blocks; when the whole tile sits in one block (the common case)
+    // the block is located once per tile instead of once per record
+    const BlockAddr a0 = locate(p.map, tile0);
+    const bool one_block = a0.slot + kTile <= p.map.B;
+    if (one_block && valid == kTile) {
+      const uint32_t* sp = reinterpret_cast<const uint32_t*>(a0.base) + a0.slot + wbase;
+      const uint32_t* tp = reinterpret_cast<const uint32_t*>(a0.base + p.map.off_tgt) + a0.slot + wbase;
+      const uint32_t* wp = reinterpret_cast<const uint32_t*>(a0.base + p.map.off_w) + a0.slot + wbase;
+      const uint16_t* dp = reinterpret_cast<const uint16_t*>(a0.base + p.map.off_d) + a0.slot + wbase;
+      uint32_t s[ITEMS], d[ITEMS];
+#pragma unroll
+      for (int i = 0; i < ITEMS; ++i) {
+        s[i] = sp[i * 32];
+        d[i] = dp[i * 32];
+        rec[i].z = tp[i * 32];
+        rec[i].w = wp[i * 32];
+      }
+#pragma unroll
+      for (int i = 0; i < ITEMS; ++i) {
+        rec[i].x = (s[i] << p.delay_bits) | d[i];
+        rec[i].y = (uint32_t)(tile0 + wbase + i * 32);
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < ITEMS; ++i) {
+        const uint32_t e = wbase + i * 32;
+        if (e < valid) {
+          const BlockAddr a = locate(p.map, tile0 + e);
+          const uint32_t s = *src_ptr(p.map, a);
+          const uint32_t d = *d_ptr(p.map, a);
+          rec[i] = make_uint4((s << p.delay_bits) | d, (uint32_t)(tile0 + e), *tgt_ptr(p.map, a),
+                              __float_as_uint(*w_ptr(p.map, a)));
+        } else {
+          rec[i] = make_uint4(0xffffffffu, 0u, 0u, 0u);
+        }
+      }
+    }
+  } else {
+    const uint4* in = p.recs_in + tile0 + wbase;
+    if (valid == kTile) {
+#pragma unroll
+      for (int i = 0; i < ITEMS; ++i) rec[i] = in[i * 32];
+    } else {
+#pragma unroll
+      for (int i = 0; i < ITEMS; ++i) {
+        // padding sorts behind every real record of the tile and is never written out
+        rec[i] = wbase + i * 32 < valid ? in[i * 32] : make_uint4(0xffffffffu, 0u, 0u, 0u);
+      }
+    }
+  }
+  __syncthreads();  // the counters are zero
+  // ---- per-warp digit histogram with fire-and-forget shared-memory atomics ----
+#pragma unroll
+  for (int i = 0; i < ITEMS; ++i) atomicAdd(&my_hist[(rec[i].x >> p.shift) & mask], 1u);
+  __syncthreads();
+
+  // ---- per digit: exclusive scan over the warps; exclusive scan over the digits -> where each digit's run
+  //      starts inside the tile; where it starts in the output comes from the scan kernels ----
+  if (threadIdx.x < kRadix) {
+    const uint32_t d = threadIdx.x;
+    const uint32_t out0 = p.offs[(uint64_t)tile * kRadix + d];
+    uint32_t cnt[WARPS];
+#pragma unroll
+    for (int w = 0; w < WARPS; ++w) cnt[w] = sm.warp_hist[w][d];
+    uint32_t run = 0;
+#pragma unroll
+    for (int w = 0; w < WARPS; ++w) {
+      const uint32_t c = cnt[w];
+      cnt[w] = run;
+      run += c;
+    }
+    uint32_t inc = run;
+#pragma unroll
+    for (int s = 1; s < 32; s <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, s);
+      if (lane >= (uint32_t)s) inc += t;
+    }
+    if (lane == 31) sm.scan_tmp[warp] = inc;
+    asm volatile("bar.sync 1, %0;" ::"n"(kRadix));
+    uint32_t base = 0;
+#pragma unroll
+    for (uint32_t w = 0; w < kRadix / 32; ++w) base += w < warp ? sm.scan_tmp[w] : 0u;
+    const uint32_t my_excl = base + inc - run;
+    sm.global_off[d] = out0 - my_excl;
+#pragma unroll
+    for (int w = 0; w < WARPS; ++w) sm.warp_hist[w][d] = my_excl + cnt[w];  // tile position of the warp's first
+  }
+  __syncthreads();
+
+  // ---- stable rank + scatter into shared memory in one go: the lowest lane of each group of equal digits
+  //      bumps the warp's running offset for that digit (atomics of one warp to one address retire in
+  //      program order, so items keep their position order) and the group shares the old value ----
+#pragma unroll
+  for (int i = 0; i < ITEMS; ++i) {
+    const uint32_t d = (rec[i].x >> p.shift) & mask;
+    const uint32_t peers = peers_of<MATCH>(d, sm.warp_masks[MATCH == kMatchSmem ? warp : 0]);
+    const uint32_t below = __popc(peers & lanemask_lt());
+    uint32_t old = 0;
+    if (below == 0) old = atomicAdd(&my_hist[d], (uint32_t)__popc(peers));
+    old = __shfl_sync(0xffffffffu, old, __ffs(peers) - 1);
+    sm.recs[old + below] = rec[i];
+  }
+  __syncthreads();
+
+  // ---- write out: consecutive threads write consecutive records of a digit run ----
+  const uint32_t dmask = (1u << p.delay_bits) - 1u;
+  const uint32_t next_mask = (1u << p.next_bits) - 1u;
+#pragma unroll
+  for (int i = 0; i < ITEMS; ++i) {
+    const uint32_t j = i * kThreads + threadIdx.x;
+    if (j < valid) {
+      const uint4 r = sm.recs[j];
+      const uint32_t g = sm.global_off[(r.x >> p.shift) & mask] + j;
+      if (LAST) {
+        p.out_src[g] = r.x >> p.delay_bits;
+        p.out_d[g] = (uint16_t)(r.x & dmask);
+        p.out_tgt[g] = r.z;
+        p.out_w[g] = __uint_as_float(r.w);
+        p.out_perm[g] = r.y;
+      } else {
+        p.recs_out[g] = r;
+        p.dig_out[g] = (uint8_t)((r.x >> p.next_shift) & next_mask);
+      }
+    }
+  }
+}
+
+}  // namespace nc

@@ -88,6 +88,14 @@ def test_sort_pairs_variant_parity(nc_mod, oracle_mod):
         assert rep["n"] > 300_000
 
 
+def test_onesweep_lookback_variant_parity(nc_mod, oracle_mod):
+    """NC_FLAG_SORT_ONESWEEP: whole connections carried through single-pass digit sweeps chained by decoupled
+    look-back (the alternative to the default count / scan / scatter kernels per pass)."""
+    for net in (WL.config2_microcircuit(scale=0.06), WL.config1_rule("fixed_indegree", scale=0.2)):
+        rep, _ = PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_ONESWEEP)
+        assert rep["n"] > 300_000
+
+
 def test_single_pass_key(nc_mod, oracle_mod):
     """<= 8 key bits: one digit pass that is both the first and the last (storage blocks -> final arrays)."""
     net = WL.Network("narrow", [16])
@@ -98,6 +106,7 @@ def test_single_pass_key(nc_mod, oracle_mod):
     g.close()
     PU.full_parity(net, oracle_mod, nc_mod)
     PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_PAIRS)
+    PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_ONESWEEP)
 
 
 def test_block_sizes_paper_default_and_odd(nc_mod, oracle_mod):
