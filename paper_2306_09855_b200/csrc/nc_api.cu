@@ -643,22 +643,43 @@ int sort_carry_and_index(nc_context* c, const PassPlan& plan) {
 
 // Default organisation step for keys of <= 32 bits (nc_sort_split.cuh): per digit pass, per-tile digit counts ->
 // scan -> scatter of whole connections; the last pass writes the sorted SoA arrays; then the index.
-constexpr int kSplitWarps = 8;
-constexpr int kSplitItems = 16;
-constexpr int kSplitTile = kSplitWarps * 32 * kSplitItems;
+struct SplitShape {
+  int warps, items;
+};
+constexpr SplitShape kSplitShapes[] = {{8, 16}, {16, 8}, {12, 8}, {8, 8}, {16, 4}, {24, 4}};
 
-template <bool FIRST, bool LAST>
-int launch_scatter_pass(nc_context* c, const ScatterParams& sp, uint32_t n_tiles) {
-  using Smem = ScatterSmem<kSplitWarps, kSplitItems, false>;
-  auto kern = scatter_pass_kernel<FIRST, LAST, kSplitWarps, kSplitItems, 2, kMatchBallot>;
+int split_variant() {
+  const char* e = getenv("NC_SPLIT_VARIANT");
+  const int v = e ? atoi(e) : 0;
+  return (v >= 0 && v < (int)(sizeof(kSplitShapes) / sizeof(kSplitShapes[0]))) ? v : 0;
+}
+
+template <bool FIRST, bool LAST, int WARPS, int ITEMS, int MIN_CTAS>
+int launch_scatter_shape(nc_context* c, const ScatterParams& sp, uint32_t n_tiles) {
+  using Smem = ScatterSmem<WARPS, ITEMS, false>;
+  auto kern = scatter_pass_kernel<FIRST, LAST, WARPS, ITEMS, MIN_CTAS, kMatchBallot>;
   NC_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem)));
-  kern<<<n_tiles, kSplitWarps * 32, sizeof(Smem), c->stream>>>(sp);
+  kern<<<n_tiles, WARPS * 32, sizeof(Smem), c->stream>>>(sp);
   NC_LAUNCH_CHECK(c, "scatter_pass");
   return NC_OK;
 }
 
+template <bool FIRST, bool LAST>
+int launch_scatter_pass(nc_context* c, const ScatterParams& sp, uint32_t n_tiles, int variant) {
+  switch (variant) {
+    case 1: return launch_scatter_shape<FIRST, LAST, 16, 8, 2>(c, sp, n_tiles);
+    case 2: return launch_scatter_shape<FIRST, LAST, 12, 8, 3>(c, sp, n_tiles);
+    case 3: return launch_scatter_shape<FIRST, LAST, 8, 8, 4>(c, sp, n_tiles);
+    case 4: return launch_scatter_shape<FIRST, LAST, 16, 4, 4>(c, sp, n_tiles);
+    case 5: return launch_scatter_shape<FIRST, LAST, 24, 4, 2>(c, sp, n_tiles);
+    default: return launch_scatter_shape<FIRST, LAST, 8, 16, 2>(c, sp, n_tiles);
+  }
+}
+
 int sort_split_and_index(nc_context* c, const PassPlan& plan) {
   const uint32_t n = (uint32_t)c->n_conns;
+  const int variant = split_variant();
+  const uint32_t kSplitTile = (uint32_t)kSplitShapes[variant].warps * 32u * (uint32_t)kSplitShapes[variant].items;
   const uint32_t n_tiles = (uint32_t)(((uint64_t)n + kSplitTile - 1) / kSplitTile);
   const uint32_t n_chunks = (n_tiles + kScanChunkTiles - 1) / kScanChunkTiles;
   const BlockMap map = make_map(c);
@@ -732,10 +753,10 @@ int sort_split_and_index(nc_context* c, const PassPlan& plan) {
       sp.next_bits = last ? 0 : plan.bits[ps + 1];
       sp.offs = offs;
       int rc;
-      if (first && last) rc = launch_scatter_pass<true, true>(c, sp, n_tiles);
-      else if (first) rc = launch_scatter_pass<true, false>(c, sp, n_tiles);
-      else if (last) rc = launch_scatter_pass<false, true>(c, sp, n_tiles);
-      else rc = launch_scatter_pass<false, false>(c, sp, n_tiles);
+      if (first && last) rc = launch_scatter_pass<true, true>(c, sp, n_tiles, variant);
+      else if (first) rc = launch_scatter_pass<true, false>(c, sp, n_tiles, variant);
+      else if (last) rc = launch_scatter_pass<false, true>(c, sp, n_tiles, variant);
+      else rc = launch_scatter_pass<false, false>(c, sp, n_tiles, variant);
       if (rc != NC_OK) return rc;
       cur = dst;
     }
