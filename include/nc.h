@@ -221,8 +221,9 @@ int nc_read_degree_histogram(nc_context* ctx, int kind, uint32_t* per_node_degre
  * nc_selftest_philox: out[4*k..4*k+3] = Philox4x32-10(ctr[4*k..], key[2*k..]) computed on the device (D2).
  * nc_selftest_fastpath: exhaustive check of the fp32 Box-Muller fast path against fp64 on the device over all
  *   2^24 values of u1 and of u2 (D5, D6).  out[0] = max |r32 - r64| / (bound on it that the delay guard band
- *   assumes), out[1], out[2] = the same ratio for sin and cos, out[3] = max |r32 - r64| / r64.  The guard band
- *   is sound iff out[0..2] < 1; the GPU tests require < 0.25. */
+ *   assumes), out[1], out[2] = the same ratio for sin and cos, out[3] = max |r32 - r64| (the fp32 weight is off by
+ *   at most sd_w (out[3] + r |cos32 - cos|)).  The guard band is sound iff out[0..2] < 1; the GPU tests require
+ *   < 0.25 and out[3] < 4e-6. */
 int nc_selftest_philox(nc_context* ctx, uint32_t n, const uint32_t* ctr, const uint32_t* key, uint32_t* out);
 int nc_selftest_fastpath(nc_context* ctx, double out[4]);
 

@@ -86,6 +86,8 @@ struct nc_context {
   uint64_t launches = 0;
   uint32_t key_bits = 0, delay_bits = 0, sort_passes = 0;
   std::vector<Span> spans;
+  bool gen_open = false;  // a span over consecutive generate launches is open (no events in between: they may overlap)
+  cudaEvent_t gen_a = nullptr;
   nc_timings acc{};
 };
 
@@ -159,12 +161,15 @@ int sync_stream(nc_context* c) {
   return NC_OK;
 }
 
+void gen_span_end(nc_context* c);
+
 struct Scope {  // CUDA-event span around a phase (NC_FLAG_TIMING)
   nc_context* c;
   Span s{};
   bool on;
   Scope(nc_context* c_, int phase, bool is_pass = false) : c(c_), on((c_->cfg.flags & NC_FLAG_TIMING) != 0) {
     if (!on) return;
+    gen_span_end(c);
     s.phase = phase;
     s.is_pass = is_pass;
     cudaEventCreate(&s.a);
@@ -177,6 +182,26 @@ struct Scope {  // CUDA-event span around a phase (NC_FLAG_TIMING)
     c->spans.push_back(s);
   }
 };
+
+// Consecutive generate launches are timed as ONE span (first launch .. close), because an event between two of
+// them would serialise kernels that are allowed to overlap (programmatic dependent launch).
+void gen_span_begin(nc_context* c) {
+  if (!(c->cfg.flags & NC_FLAG_TIMING) || c->gen_open) return;
+  cudaEventCreate(&c->gen_a);
+  cudaEventRecord(c->gen_a, c->stream);
+  c->gen_open = true;
+}
+void gen_span_end(nc_context* c) {
+  if (!c->gen_open) return;
+  Span s{};
+  s.phase = NC_PHASE_GENERATE;
+  s.is_pass = false;
+  s.a = c->gen_a;
+  cudaEventCreate(&s.b);
+  cudaEventRecord(s.b, c->stream);
+  c->spans.push_back(s);
+  c->gen_open = false;
+}
 
 BlockMap make_map(const nc_context* c) {
   BlockMap m{};
@@ -223,15 +248,20 @@ SynConst make_syn(const nc_context* c, const nc_syn_spec& s) {
   // Guard band: the error of z1 (bounded in the kernel from r) enters x scaled
   // by sd / dt; 32 relative fp32 ulps of x cover the fp32 roundings of mean, sd, the bounds, 1/dt and of the
   // products; plus a small floor.
-  k.eps_scale = (float)(std::fabs(s.delay_ms.sd) * c->inv_dt);
+  const double scale = std::fabs(s.delay_ms.sd) * c->inv_dt;
+  k.eps_a = (float)(scale * (double)kErrRa);
+  k.eps_b = (float)(scale * ((double)kErrRb + (double)kErrTrig));
   k.eps_rel = (float)(32.0 / 16777216.0);
-  k.eps_abs = 1e-6f;
-  k.exact = (c->cfg.flags & NC_FLAG_EXACT_FP64) ? 1 : 0;
+  k.eps_abs = (c->cfg.flags & NC_FLAG_EXACT_FP64) ? INFINITY : 1e-6f;
   k.dd_mean = s.delay_ms.mean;
   k.dd_sd = s.delay_ms.sd;
   k.dd_lo = s.delay_ms.lo;
   k.dd_hi = s.delay_ms.hi;
   k.dinv_dt = c->inv_dt;
+  k.dw_mean = s.weight.mean;
+  k.dw_sd = s.weight.sd;
+  k.dw_lo = s.weight.lo;
+  k.dw_hi = s.weight.hi;
   return k;
 }
 
@@ -271,18 +301,32 @@ int reserve_blocks(nc_context* c, uint64_t n_new) {
   return NC_OK;
 }
 
+// Generation kernels write disjoint ranges, so consecutive launches may overlap: programmatic dependent launch
+// lets the next kernel of the stream start while the previous one drains (each kernel waits for its predecessor
+// before it exits, so completion stays in stream order).  NC_NO_PDL=1 in the environment disables it.
+bool use_pdl() {
+  static const bool on = [] {
+    const char* e = getenv("NC_NO_PDL");
+    return !(e && atoi(e) != 0);
+  }();
+  return on;
+}
+
 template <int RULE>
-void launch_generate(nc_context* c, const GenParams& p, bool vec) {
-  const uint64_t first_group = p.pos0 >> 2;
-  const uint64_t last_group = (p.pos0 + p.n + 3) >> 2;
-  const uint64_t groups = last_group - first_group;
-  const uint64_t per_cta = (uint64_t)kGenThreads * kGenGroups;
-  const unsigned grid = (unsigned)((groups + per_cta - 1) / per_cta);
-  if (vec) {
-    generate_kernel<RULE, true><<<grid, kGenThreads, 0, c->stream>>>(p);
-  } else {
-    generate_kernel<RULE, false><<<grid, kGenThreads, 0, c->stream>>>(p);
-  }
+cudaError_t launch_generate(nc_context* c, const GenParams& p) {
+  const uint64_t first_tile = p.pos0 / kGenTile;
+  const uint64_t last_tile = (p.pos0 + p.n - 1) / kGenTile;
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3((unsigned)(last_tile - first_tile + 1));
+  cfg.blockDim = dim3(kGenThreads);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = c->stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = use_pdl() ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, generate_kernel<RULE>, p);
 }
 
 int device_scan(nc_context* c, const uint32_t* in, uint32_t* out, uint64_t n, uint32_t* partial, uint64_t* total) {
@@ -296,7 +340,7 @@ int device_scan(nc_context* c, const uint32_t* in, uint32_t* out, uint64_t n, ui
   return NC_OK;
 }
 
-int connect_bernoulli(nc_context* c, GenParams gp, double p) {
+int connect_bernoulli(nc_context* c, GenParams gp, double p, uint32_t seed_lo, uint32_t seed_hi) {
   const uint64_t n_pairs = (uint64_t)gp.n_src * gp.n_tgt;
   const uint64_t T = (uint64_t)std::floor(std::ldexp(p, 32));  // Q14
   if (T == 0) return NC_OK;                                    // realised probability 0: nothing to create
@@ -318,14 +362,13 @@ int connect_bernoulli(nc_context* c, GenParams gp, double p) {
     return fail(c, NC_ERR_OOM, "out of device memory for pairwise_bernoulli scratch");
   }
   uint64_t total = 0;
+  gen_span_end(c);
   {
     Scope sc(c, NC_PHASE_GENERATE);
     BernParams bp{};
     bp.n_pairs = n_pairs;
     bp.threshold = T;
-    bp.seed_lo = gp.seed_lo;
-    bp.seed_hi = gp.seed_hi;
-    bp.projection_id = gp.projection_id;
+    bp.rng = make_philox_stream(seed_lo, seed_hi, c->n_proj, 1u);
     bp.mask = mask;
     bp.tile_count = tile_count;
     bernoulli_trials_kernel<<<(unsigned)n_tiles, kBernThreads, 0, c->stream>>>(bp);
@@ -821,6 +864,7 @@ int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) 
 }
 
 int collect_timings(nc_context* c) {
+  gen_span_end(c);
   int rc = sync_stream(c);
   if (rc != NC_OK) return rc;
   for (Span& s : c->spans) {
@@ -857,17 +901,20 @@ __device__ void atomic_max_double(double* addr, double v) {  // v >= 0: bit patt
 __global__ void selftest_fastpath_kernel(double* out /* [4] */) {
   const uint32_t v = blockIdx.x * blockDim.x + threadIdx.x;  // 0 .. 2^24-1
   const uint32_t word = v << 8;
-  float inv_r;
-  const float r32 = fast_radius(word, inv_r);
+  const float r2c = fmaxf(fast_r2(word), 1e-30f);
+  const float inv_r = rsqrt_approx(r2c);
+  const float r32 = r2c * inv_r;
   const double u1 = (double)(v + 1u) * (1.0 / 16777216.0);
   const double r64 = sqrt(-2.0 * log(u1));
   const double dr = fabs((double)r32 - r64);
   // ratio of the actual error of r to the bound the guard band assumes, evaluated with the kernel's own r, 1/r
   const double bound = (double)kErrRa * (double)inv_r + (double)kErrRb * (double)r32;
-  double e0 = r64 > 0.0 ? dr / bound : (dr == 0.0 ? 0.0 : 1e30);
-  double e3 = r64 > 0.0 ? dr / r64 : 0.0;
+  double e0 = dr / bound;  // u1 = 1: r32 = 1e-15 instead of 0, far inside the (then infinite) bound
+  double e3 = dr;  // absolute error of r: the weight error is sd_w * (dr + r * dcos)
   float sn, cs;
-  fast_sincos(word, sn, cs);
+  fast_sincos_shifted(word, sn, cs);  // sin, cos of (theta - pi) = -sin, -cos of theta
+  sn = -sn;
+  cs = -cs;
   const double th = 6.283185307179586 * ((double)v * (1.0 / 16777216.0));
   double e1 = fabs((double)sn - sin(th)) / (double)kErrTrig, e2 = fabs((double)cs - cos(th)) / (double)kErrTrig;
   for (int d = 16; d > 0; d >>= 1) {
@@ -935,6 +982,7 @@ int nc_create(const nc_config* cfg, nc_context** out) {
 
 int nc_destroy(nc_context* c) {
   if (!c) return NC_OK;
+  gen_span_end(c);
   cudaStreamSynchronize(c->stream);
   for (Span& s : c->spans) {
     cudaEventDestroy(s.a);
@@ -1015,28 +1063,30 @@ int nc_connect(nc_context* c, nc_range src, nc_range tgt, nc_rule rule, const nc
   gp.t0 = tgt.first;
   gp.n_tgt = tgt.count;
   gp.K = (uint32_t)K;
-  gp.seed_lo = (uint32_t)(seed & 0xffffffffull);
-  gp.seed_hi = (uint32_t)(seed >> 32);
-  gp.projection_id = c->n_proj;
+  gp.div = rule == NC_ALL_TO_ALL ? tgt.count : (rule == NC_FIXED_INDEGREE || rule == NC_FIXED_OUTDEGREE) ? (uint32_t)K : 1u;
+  gp.div_magic = make_div_magic(gp.div);
+  const uint32_t seed_lo = (uint32_t)(seed & 0xffffffffull), seed_hi = (uint32_t)(seed >> 32);
+  gp.rng = make_philox_stream(seed_lo, seed_hi, c->n_proj, 0u);  // D2: synapse stream
   gp.syn = make_syn(c, *syn);
 
   if (rule == NC_PAIRWISE_BERNOULLI) {
-    int rc = connect_bernoulli(c, gp, params->p);
+    int rc = connect_bernoulli(c, gp, params->p, seed_lo, seed_hi);
     if (rc != NC_OK) return rc;
   } else if (n_new > 0) {
     int rc = reserve_blocks(c, n_new);
     if (rc != NC_OK) return rc;
     gp.map = make_map(c);
-    const bool vec = (c->B % 4) == 0;
     {
-      Scope sc(c, NC_PHASE_GENERATE);
+      gen_span_begin(c);
+      cudaError_t e;
       switch (rule) {
-        case NC_ONE_TO_ONE: launch_generate<kOneToOne>(c, gp, vec); break;
-        case NC_ALL_TO_ALL: launch_generate<kAllToAll>(c, gp, vec); break;
-        case NC_FIXED_INDEGREE: launch_generate<kFixedIndegree>(c, gp, vec); break;
-        case NC_FIXED_OUTDEGREE: launch_generate<kFixedOutdegree>(c, gp, vec); break;
-        default: launch_generate<kFixedTotalNumber>(c, gp, vec); break;
+        case NC_ONE_TO_ONE: e = launch_generate<kOneToOne>(c, gp); break;
+        case NC_ALL_TO_ALL: e = launch_generate<kAllToAll>(c, gp); break;
+        case NC_FIXED_INDEGREE: e = launch_generate<kFixedIndegree>(c, gp); break;
+        case NC_FIXED_OUTDEGREE: e = launch_generate<kFixedOutdegree>(c, gp); break;
+        default: e = launch_generate<kFixedTotalNumber>(c, gp); break;
       }
+      if (e != cudaSuccess) return fail(c, NC_ERR_CUDA, std::string("launch generate: ") + cudaGetErrorString(e));
       NC_LAUNCH_CHECK(c, "generate");
     }
     c->n_conns += n_new;
@@ -1050,6 +1100,7 @@ int nc_connect(nc_context* c, nc_range src, nc_range tgt, nc_rule rule, const nc
 int nc_finalize(nc_context* c) {
   if (!c) return NC_ERR_INVALID_ARG;
   if (c->finalized) return fail(c, NC_ERR_STATE, "nc_finalize called twice");
+  gen_span_end(c);
   const uint32_t N = c->n_nodes;
   c->src_offsets = (uint32_t*)dev_alloc(c, ((size_t)N + 1) * 4);
   c->group_ptr = (uint32_t*)dev_alloc(c, ((size_t)N + 1) * 4);

@@ -84,8 +84,96 @@ __device__ __forceinline__ Philox4 philox4x32_10(uint32_t c0, uint32_t c1, uint3
   return Philox4{c0, c1, c2, c3};
 }
 
+// ---------------------------------------------------------------------------------------------
+// Philox4x32-10 specialised for one stream of counters (x, y, projection_id, stream) under one key
+// (reading D2).  Everything that does not depend on (x, y) is evaluated once on the host
+// (make_philox_stream) and reaches the kernel as launch constants: the ten round keys, the product
+// M1 * projection_id of the first round and, when y == 0 (every rule with N_newconns < 2^32), the
+// uniform halves of rounds two and three.  Per call: 18 IMAD.WIDE + 19 LOP3 (Y0) or 19 + 20 (general),
+// no key-schedule additions.
+// ---------------------------------------------------------------------------------------------
+constexpr uint32_t kPhiloxM0 = 0xD2511F53u, kPhiloxM1 = 0xCD9E8D57u;
+constexpr uint32_t kPhiloxW0 = 0x9E3779B9u, kPhiloxW1 = 0xBB67AE85u;
+
+struct PhiloxStream {
+  uint32_t k0[10], k1[10];  // round keys: k0[r] = seed_lo + r W0, k1[r] = seed_hi + r W1
+  uint32_t u0;              // hi(M1 projection) ^ k0[0]      after round 1: c0 = u0 ^ y
+  uint32_t l1;              // lo(M1 projection)                             c1 = l1
+  uint32_t a;               // stream ^ k1[0]                                c2 = hi(M0 x) ^ a,  c3 = lo(M0 x)
+  uint32_t b;               // y == 0: l1 ^ k0[1]             after round 2: c0 = hi(M1 c2) ^ b, c1 = lo(M1 c2)
+  uint32_t c;               // y == 0: hi(M0 u0) ^ k1[1]                     c2 = lo(M0 x) ^ c,  c3 = lo(M0 u0)
+  uint32_t d;               // y == 0: lo(M0 u0) ^ k1[2]      after round 3: c2 = hi(M0 c0) ^ d
+};
+
+inline PhiloxStream make_philox_stream(uint32_t seed_lo, uint32_t seed_hi, uint32_t projection_id, uint32_t stream) {
+  PhiloxStream s{};
+  for (int r = 0; r < 10; ++r) {
+    s.k0[r] = seed_lo + (uint32_t)r * kPhiloxW0;
+    s.k1[r] = seed_hi + (uint32_t)r * kPhiloxW1;
+  }
+  const uint64_t p1 = (uint64_t)kPhiloxM1 * projection_id;
+  s.u0 = (uint32_t)(p1 >> 32) ^ s.k0[0];
+  s.l1 = (uint32_t)p1;
+  s.a = stream ^ s.k1[0];
+  const uint64_t q0 = (uint64_t)kPhiloxM0 * s.u0;
+  s.b = s.l1 ^ s.k0[1];
+  s.c = (uint32_t)(q0 >> 32) ^ s.k1[1];
+  s.d = (uint32_t)q0 ^ s.k1[2];
+  return s;
+}
+
+template <bool Y0>
+__device__ __forceinline__ Philox4 philox_stream(uint32_t x, uint32_t y, const PhiloxStream& s) {
+  uint32_t c0, c1, c2, c3;
+  const uint64_t px = (uint64_t)kPhiloxM0 * (uint64_t)x;
+  int first;
+  if (Y0) {
+    const uint32_t e2 = (uint32_t)(px >> 32) ^ s.a;             // round 1, lane-dependent half
+    const uint64_t p1 = (uint64_t)kPhiloxM1 * (uint64_t)e2;     // round 2
+    const uint32_t f0 = (uint32_t)(p1 >> 32) ^ s.b;
+    const uint32_t f2 = (uint32_t)px ^ s.c;
+    const uint64_t q0 = (uint64_t)kPhiloxM0 * (uint64_t)f0;     // round 3
+    const uint64_t q1 = (uint64_t)kPhiloxM1 * (uint64_t)f2;
+    c0 = (uint32_t)(q1 >> 32) ^ (uint32_t)p1 ^ s.k0[2];
+    c1 = (uint32_t)q1;
+    c2 = (uint32_t)(q0 >> 32) ^ s.d;
+    c3 = (uint32_t)q0;
+    first = 3;
+  } else {
+    c0 = s.u0 ^ y;
+    c1 = s.l1;
+    c2 = (uint32_t)(px >> 32) ^ s.a;
+    c3 = (uint32_t)px;
+    first = 1;
+  }
+#pragma unroll
+  for (int r = 1; r < 10; ++r) {
+    if (r < first) continue;
+    const uint64_t p0 = (uint64_t)kPhiloxM0 * (uint64_t)c0;
+    const uint64_t p1 = (uint64_t)kPhiloxM1 * (uint64_t)c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ s.k0[r];
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ s.k1[r];
+    c1 = (uint32_t)p1;
+    c3 = (uint32_t)p0;
+    c0 = n0;
+    c2 = n2;
+  }
+  return Philox4{c0, c1, c2, c3};
+}
+
 // rand(N) of PAPER.md:95 as a multiply-high (reading D3): floor(word * N / 2^32), no rejection.
 __device__ __forceinline__ uint32_t bounded(uint32_t word, uint32_t n) { return __umulhi(word, n); }
+
+// i / d and i % d for 32-bit i with a host-computed reciprocal m = floor(2^64 / d) + 1 (exact for i < 2^32).
+__device__ __forceinline__ uint32_t div_magic(uint32_t i, uint64_t m) { return (uint32_t)__umul64hi((uint64_t)i, m); }
+inline uint64_t make_div_magic(uint32_t d) {
+  return d <= 1 ? 0ull : (uint64_t)(((unsigned __int128)1 << 64) / d) + 1ull;  // d == 1 is handled by the caller
+}
+
+// Programmatic dependent launch (sm_90+): lets the next kernel of the stream start while this one drains,
+// and (at the end of a kernel) waits for the previous one, so completion stays in stream order.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait_prior() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 // ---------------------------------------------------------------------------------------------
 // Global-memory accesses with explicit ordering (decoupled look-back status words).
