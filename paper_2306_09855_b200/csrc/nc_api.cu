@@ -78,6 +78,8 @@ struct nc_context {
   uint32_t *src_offsets = nullptr, *group_count = nullptr, *group_ptr = nullptr, *group_start = nullptr;
   uint16_t* group_delay = nullptr;
   uint32_t total_groups = 0;
+  uint64_t* d_total_groups = nullptr;  // device scalar; total_groups is fetched on first use (no sync in nc_finalize)
+  bool total_groups_pending = false;
   uint32_t *out_degree = nullptr, *in_degree = nullptr, *d_max = nullptr;  // d_max: [2] device scalars
   bool have_in = false, have_out = false;
   uint32_t max_in = 0, max_out = 0;
@@ -769,7 +771,7 @@ int sort_split_and_index(nc_context* c, const PassPlan& plan) {
       NC_LAUNCH_CHECK(c, "tile_count");
       chunk_total_kernel<<<n_chunks, kRadix, 0, c->stream>>>(counts, n_tiles, chunk);
       NC_LAUNCH_CHECK(c, "chunk_total");
-      chunk_scan_kernel<<<1, kRadix, 0, c->stream>>>(chunk, n_chunks);
+      chunk_scan_kernel<<<1, kRadix * kChunkScanSegs, 0, c->stream>>>(chunk, n_chunks);
       NC_LAUNCH_CHECK(c, "chunk_scan");
       tile_offsets_kernel<<<n_chunks, kRadix, 0, c->stream>>>(counts, n_tiles, chunk, offs);
       NC_LAUNCH_CHECK(c, "tile_offsets");
@@ -817,35 +819,45 @@ int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) 
   uint32_t* tile_heads = (uint32_t*)dev_alloc(c, head_tiles * 4);
   uint32_t* tile_head_off = (uint32_t*)dev_alloc(c, head_tiles * 4);
   uint32_t* head_partial = (uint32_t*)dev_alloc(c, head_chunks * 4);
-  uint64_t* d_total_groups = (uint64_t*)dev_alloc(c, 8);
+  if (!c->d_total_groups) c->d_total_groups = (uint64_t*)dev_alloc(c, 8);
   auto drop = [&]() {
     dev_free_later(c, tile_heads); dev_free_later(c, tile_head_off); dev_free_later(c, head_partial);
-    dev_free_later(c, d_total_groups);
   };
-  if (!tile_heads || !tile_head_off || !head_partial || !d_total_groups) {
+  if (!tile_heads || !tile_head_off || !head_partial || !c->d_total_groups) {
     drop();
     return fail(c, NC_ERR_OOM, "out of device memory for the index scratch");
   }
+  // A group is a distinct (source, delay) pair, so total_groups <= min(n, N_nodes * max delay).  When that bound
+  // is small next to the connections themselves the group arrays are sized by it and nc_finalize never waits for
+  // the device; otherwise the exact count is read back first.
+  const uint64_t bound = std::min<uint64_t>(n, (uint64_t)N * c->max_delay_steps);
+  const bool presize = !lookback_flag && bound * 6 <= std::max<uint64_t>((uint64_t)n * 2, 1u << 20);
   const SoAKeys keys{c->s_src, c->s_d, 16u};
-  uint64_t total_groups = 0;
-  uint32_t lookback_error = 0;
   {
     Scope sc(c, NC_PHASE_INDEX);
     head_count_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(keys, n, tile_heads);
     NC_LAUNCH_CHECK(c, "head_count");
-    int rc = device_scan(c, tile_heads, tile_head_off, head_tiles, head_partial, d_total_groups);
+    int rc = device_scan(c, tile_heads, tile_head_off, head_tiles, head_partial, c->d_total_groups);
     if (rc != NC_OK) return rc;
-    NC_CUDA(c, cudaMemcpyAsync(&total_groups, d_total_groups, 8, cudaMemcpyDeviceToHost, c->stream));
+  }
+  uint64_t cap = bound;
+  if (!presize) {
+    uint64_t total_groups = 0;
+    uint32_t lookback_error = 0;
+    NC_CUDA(c, cudaMemcpyAsync(&total_groups, c->d_total_groups, 8, cudaMemcpyDeviceToHost, c->stream));
     if (lookback_flag) NC_CUDA(c, cudaMemcpyAsync(&lookback_error, lookback_flag, 4, cudaMemcpyDeviceToHost, c->stream));
+    NC_CUDA(c, cudaStreamSynchronize(c->stream));  // total_groups sizes the group arrays
+    if (lookback_error) {
+      drop();
+      return fail(c, NC_ERR_CUDA, "onesweep look-back timed out");
+    }
+    c->total_groups = (uint32_t)total_groups;
+    cap = total_groups;
+  } else {
+    c->total_groups_pending = true;
   }
-  NC_CUDA(c, cudaStreamSynchronize(c->stream));  // total_groups sizes the group arrays
-  if (lookback_error) {
-    drop();
-    return fail(c, NC_ERR_CUDA, "onesweep look-back timed out");
-  }
-  c->total_groups = (uint32_t)total_groups;
-  c->group_start = (uint32_t*)dev_alloc(c, (size_t)total_groups * 4);
-  c->group_delay = (uint16_t*)dev_alloc(c, (size_t)total_groups * 2);
+  c->group_start = (uint32_t*)dev_alloc(c, (size_t)cap * 4);
+  c->group_delay = (uint16_t*)dev_alloc(c, (size_t)cap * 2);
   if (!c->group_start || !c->group_delay) {
     drop();
     return fail(c, NC_ERR_OOM, "out of device memory for the group arrays");
@@ -853,13 +865,25 @@ int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) 
   {
     Scope sc(c, NC_PHASE_INDEX);
     IndexOut io{c->src_offsets, c->group_ptr, c->group_start, c->group_delay, N};
-    index_scatter_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(keys, n, tile_head_off, d_total_groups, io);
+    index_scatter_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(keys, n, tile_head_off, c->d_total_groups, io);
     NC_LAUNCH_CHECK(c, "index_scatter");
     index_finish_kernel<<<(N + 255) / 256, 256, 0, c->stream>>>(c->src_offsets, c->group_ptr, N, c->out_degree,
                                                                c->group_count, c->d_max + 1);
     NC_LAUNCH_CHECK(c, "index_finish");
   }
   drop();
+  return NC_OK;
+}
+
+// total_groups when nc_finalize did not wait for it.
+int ensure_total_groups(nc_context* c) {
+  if (!c->total_groups_pending) return NC_OK;
+  uint64_t total_groups = 0;
+  NC_CUDA(c, cudaMemcpyAsync(&total_groups, c->d_total_groups, 8, cudaMemcpyDeviceToHost, c->stream));
+  int rc = sync_stream(c);
+  if (rc != NC_OK) return rc;
+  c->total_groups = (uint32_t)total_groups;
+  c->total_groups_pending = false;
   return NC_OK;
 }
 
@@ -1184,6 +1208,8 @@ int nc_get_connections(nc_context* c, int sorted, nc_connections_view* out) {
 int nc_get_index(nc_context* c, nc_index_view* out) {
   if (!c || !out) return NC_ERR_INVALID_ARG;
   if (!c->finalized) return fail(c, NC_ERR_STATE, "index before nc_finalize");
+  int rc = ensure_total_groups(c);
+  if (rc != NC_OK) return rc;
   out->src_offsets = c->src_offsets;
   out->group_count = c->group_count;
   out->group_ptr = c->group_ptr;
@@ -1281,6 +1307,8 @@ int nc_read_index(nc_context* c, uint32_t* src_offsets, uint32_t* group_count, u
                   uint16_t* group_delay) {
   if (!c) return NC_ERR_INVALID_ARG;
   if (!c->finalized) return fail(c, NC_ERR_STATE, "index before nc_finalize");
+  int rc0 = ensure_total_groups(c);
+  if (rc0 != NC_OK) return rc0;
   const cudaMemcpyKind k = cudaMemcpyDeviceToHost;
   const size_t N = c->n_nodes, G = c->total_groups;
   if (src_offsets) NC_CUDA(c, cudaMemcpyAsync(src_offsets, c->src_offsets, (N + 1) * 4, k, c->stream));

@@ -109,14 +109,52 @@ struct PackedKeys {
   const K* k;
   uint32_t delay_bits;
   __device__ __forceinline__ K operator[](uint64_t j) const { return k[j]; }
+  // keys of positions base .. base+7 (0 beyond n)
+  __device__ __forceinline__ void load8(uint64_t base, uint32_t n, K (&out)[8]) const {
+#pragma unroll
+    for (int i = 0; i < 8; ++i) out[i] = base + i < n ? k[base + i] : (K)0;
+  }
 };
 struct SoAKeys {
   using KeyT = uint64_t;
-  const uint32_t* src;
+  const uint32_t* src;  // 256-byte aligned arrays
   const uint16_t* dly;
   uint32_t delay_bits;  // always 16
   __device__ __forceinline__ uint64_t operator[](uint64_t j) const { return ((uint64_t)src[j] << 16) | dly[j]; }
+  // base % 8 == 0: two 128-bit loads of sources and one of delays
+  __device__ __forceinline__ void load8(uint64_t base, uint32_t n, uint64_t (&out)[8]) const {
+    if (base + 8 <= n) {
+      const uint4 s0 = *reinterpret_cast<const uint4*>(src + base);
+      const uint4 s1 = *reinterpret_cast<const uint4*>(src + base + 4);
+      const uint4 d = *reinterpret_cast<const uint4*>(dly + base);
+      out[0] = ((uint64_t)s0.x << 16) | (d.x & 0xffffu);
+      out[1] = ((uint64_t)s0.y << 16) | (d.x >> 16);
+      out[2] = ((uint64_t)s0.z << 16) | (d.y & 0xffffu);
+      out[3] = ((uint64_t)s0.w << 16) | (d.y >> 16);
+      out[4] = ((uint64_t)s1.x << 16) | (d.z & 0xffffu);
+      out[5] = ((uint64_t)s1.y << 16) | (d.z >> 16);
+      out[6] = ((uint64_t)s1.z << 16) | (d.w & 0xffffu);
+      out[7] = ((uint64_t)s1.w << 16) | (d.w >> 16);
+    } else {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) out[i] = base + i < n ? (*this)[base + i] : 0ull;
+    }
+  }
 };
+
+// The 8 keys of a thread plus the key just before them: from the lane below, or (lane 0) from memory.
+template <typename Keys>
+__device__ __forceinline__ void load_keys_and_prev(const Keys& keys, uint64_t base, uint32_t n,
+                                                   typename Keys::KeyT (&k)[8], typename Keys::KeyT& prev) {
+  using KeyT = typename Keys::KeyT;
+  static_assert(kHeadItems == 8, "load8 handles 8 positions");
+#pragma unroll
+  for (int i = 0; i < 8; ++i) k[i] = (KeyT)0;
+  if (base < n) keys.load8(base, n, k);
+  const KeyT up = __shfl_up_sync(0xffffffffu, k[7], 1);
+  prev = up;
+  if (lane_id() == 0) prev = (base > 0 && base < n) ? keys[base - 1] : (KeyT)0;
+}
 
 template <typename Keys>
 __global__ void __launch_bounds__(kHeadThreads) head_count_kernel(const Keys keys, uint32_t n,
@@ -124,18 +162,14 @@ __global__ void __launch_bounds__(kHeadThreads) head_count_kernel(const Keys key
   using KeyT = typename Keys::KeyT;
   __shared__ uint32_t warp_tmp[kHeadThreads / 32];
   const uint64_t base = (uint64_t)blockIdx.x * kHeadTile + (uint64_t)threadIdx.x * kHeadItems;
+  KeyT k[kHeadItems], prev;
+  load_keys_and_prev(keys, base, n, k, prev);
   uint32_t c = 0;
-  if (base < n) {
-    KeyT prev = base > 0 ? keys[base - 1] : (KeyT)0;
 #pragma unroll
-    for (int i = 0; i < kHeadItems; ++i) {
-      const uint64_t j = base + i;
-      if (j < n) {
-        const KeyT k = keys[j];
-        c += (j == 0 || k != prev) ? 1u : 0u;
-        prev = k;
-      }
-    }
+  for (int i = 0; i < kHeadItems; ++i) {
+    const uint64_t j = base + i;
+    if (j < n) c += (j == 0 || k[i] != prev) ? 1u : 0u;
+    prev = k[i];
   }
   c = __reduce_add_sync(0xffffffffu, c);
   if (lane_id() == 0) warp_tmp[threadIdx.x >> 5] = c;
@@ -170,15 +204,14 @@ __global__ void __launch_bounds__(kHeadThreads) index_scatter_kernel(const Keys 
   __shared__ uint32_t warp_tmp[kHeadThreads / 32];
   const uint64_t base = (uint64_t)blockIdx.x * kHeadTile + (uint64_t)threadIdx.x * kHeadItems;
   KeyT k[kHeadItems];
-  KeyT prev0 = 0;
+  KeyT prev0;
   uint32_t flags = 0, c = 0;
-  if (base < n) {
-    prev0 = base > 0 ? keys[base - 1] : (KeyT)0;
+  load_keys_and_prev(keys, base, n, k, prev0);
+  {
     KeyT prev = prev0;
 #pragma unroll
     for (int i = 0; i < kHeadItems; ++i) {
       const uint64_t j = base + i;
-      k[i] = j < n ? keys[j] : (KeyT)0;
       if (j < n && (j == 0 || k[i] != prev)) {
         flags |= 1u << i;
         ++c;

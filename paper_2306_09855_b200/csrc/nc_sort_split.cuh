@@ -127,26 +127,42 @@ __global__ void __launch_bounds__(kRadix) chunk_total_kernel(const uint16_t* __r
   chunk_tot[(uint64_t)blockIdx.x * kRadix + threadIdx.x] = s;
 }
 
-// one CTA: digit totals -> exclusive scan over the digits (first output position of each digit), then the
-// running start of every chunk, in place (chunk_tot becomes chunk_base).
-__global__ void __launch_bounds__(kRadix) chunk_scan_kernel(uint32_t* __restrict__ chunk_tot, uint32_t n_chunks) {
+// one CTA of kChunkScanSegs x 256 threads: thread (seg, digit) owns a contiguous segment of the chunks.  Digit
+// totals -> exclusive scan over the digits (first output position of each digit), then the running start of
+// every chunk, in place (chunk_tot becomes chunk_base).
+constexpr int kChunkScanSegs = 4;
+
+__global__ void __launch_bounds__(kRadix * kChunkScanSegs) chunk_scan_kernel(uint32_t* __restrict__ chunk_tot,
+                                                                             uint32_t n_chunks) {
+  __shared__ uint32_t seg_tot[kChunkScanSegs][kRadix];
   __shared__ uint32_t warp_tot[kRadix / 32];
-  const uint32_t d = threadIdx.x;
+  const uint32_t d = threadIdx.x & (kRadix - 1), seg = threadIdx.x / kRadix;
+  const uint32_t per_seg = (n_chunks + kChunkScanSegs - 1) / kChunkScanSegs;
+  const uint32_t c0 = min(seg * per_seg, n_chunks), c1 = min(c0 + per_seg, n_chunks);
   uint32_t total = 0;
 #pragma unroll 8
-  for (uint32_t c = 0; c < n_chunks; ++c) total += chunk_tot[(uint64_t)c * kRadix + d];
-  uint32_t inc = total;
+  for (uint32_t c = c0; c < c1; ++c) total += chunk_tot[(uint64_t)c * kRadix + d];
+  seg_tot[seg][d] = total;
+  __syncthreads();
+  uint32_t digit_total = 0, before = 0;  // over all segments / over the segments below mine
+#pragma unroll
+  for (int g = 0; g < kChunkScanSegs; ++g) {
+    const uint32_t v = seg_tot[g][d];
+    digit_total += v;
+    if ((uint32_t)g < seg) before += v;
+  }
+  uint32_t inc = digit_total;
 #pragma unroll
   for (int s = 1; s < 32; s <<= 1) {
     const uint32_t t = __shfl_up_sync(0xffffffffu, inc, s);
     if (lane_id() >= (uint32_t)s) inc += t;
   }
-  if (lane_id() == 31) warp_tot[d >> 5] = inc;
+  if (seg == 0 && lane_id() == 31) warp_tot[d >> 5] = inc;
   __syncthreads();
-  uint32_t run = inc - total;
+  uint32_t run = inc - digit_total + before;
   for (uint32_t w = 0; w < (d >> 5); ++w) run += warp_tot[w];
 #pragma unroll 8
-  for (uint32_t c = 0; c < n_chunks; ++c) {
+  for (uint32_t c = c0; c < c1; ++c) {
     const uint32_t v = chunk_tot[(uint64_t)c * kRadix + d];
     chunk_tot[(uint64_t)c * kRadix + d] = run;
     run += v;
