@@ -409,7 +409,9 @@ int connect_bernoulli(nc_context* c, GenParams gp, double p, uint32_t seed_lo, u
 
 PassPlan plan_passes(uint32_t key_bits) {
   PassPlan pl{};
-  pl.n_passes = (key_bits + kRadixBits - 1) / kRadixBits;
+  int digit_bits = kRadixBits;
+  if (const char* e = getenv("NC_EXP_DIGIT_BITS")) digit_bits = std::max(1, std::min((int)kRadixBits, atoi(e)));  // timing experiments
+  pl.n_passes = (key_bits + digit_bits - 1) / digit_bits;
   uint32_t left = key_bits, shift = 0;
   for (uint32_t i = 0; i < pl.n_passes; ++i) {
     const uint32_t b = (left + (pl.n_passes - i) - 1) / (pl.n_passes - i);  // spread evenly, <= 8
@@ -699,14 +701,29 @@ int split_variant() {
   return (v >= 0 && v < (int)(sizeof(kSplitShapes) / sizeof(kSplitShapes[0]))) ? v : 0;
 }
 
-template <bool FIRST, bool LAST, int WARPS, int ITEMS, int MIN_CTAS>
-int launch_scatter_shape(nc_context* c, const ScatterParams& sp, uint32_t n_tiles) {
-  using Smem = ScatterSmem<WARPS, ITEMS, false>;
-  auto kern = scatter_pass_kernel<FIRST, LAST, WARPS, ITEMS, MIN_CTAS, kMatchBallot>;
+int split_match() {  // NC_SPLIT_MATCH=2: shared-memory peer masks instead of eight ballots (experiment)
+  static const int m = [] {
+    const char* e = getenv("NC_SPLIT_MATCH");
+    return e && atoi(e) == 2 ? (int)kMatchSmem : (int)kMatchBallot;
+  }();
+  return m;
+}
+
+template <bool FIRST, bool LAST, int WARPS, int ITEMS, int MIN_CTAS, int MATCH>
+int launch_scatter_match(nc_context* c, const ScatterParams& sp, uint32_t n_tiles) {
+  using Smem = ScatterSmem<WARPS, ITEMS, MATCH == kMatchSmem>;
+  auto kern = scatter_pass_kernel<FIRST, LAST, WARPS, ITEMS, MIN_CTAS, MATCH>;
   NC_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem)));
   kern<<<n_tiles, WARPS * 32, sizeof(Smem), c->stream>>>(sp);
   NC_LAUNCH_CHECK(c, "scatter_pass");
   return NC_OK;
+}
+
+template <bool FIRST, bool LAST, int WARPS, int ITEMS, int MIN_CTAS>
+int launch_scatter_shape(nc_context* c, const ScatterParams& sp, uint32_t n_tiles) {
+  if (WARPS == 8 && ITEMS == 16 && split_match() == kMatchSmem)
+    return launch_scatter_match<FIRST, LAST, WARPS, ITEMS, MIN_CTAS, kMatchSmem>(c, sp, n_tiles);
+  return launch_scatter_match<FIRST, LAST, WARPS, ITEMS, MIN_CTAS, kMatchBallot>(c, sp, n_tiles);
 }
 
 template <bool FIRST, bool LAST>

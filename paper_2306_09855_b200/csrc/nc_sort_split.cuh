@@ -232,6 +232,8 @@ __global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(cons
   const uint64_t tile0 = (uint64_t)tile * kTile;
   const uint32_t valid = (uint32_t)min((uint64_t)kTile, (uint64_t)p.n - tile0);
   const uint32_t mask = (1u << p.bits) - 1u;
+  // first output position of this tile's run of digit threadIdx.x: fetched now, needed after the histogram
+  const uint32_t out0 = threadIdx.x < kRadix ? __ldg(p.offs + (uint64_t)tile * kRadix + threadIdx.x) : 0u;
 
   // ---- load records, warp-striped: element (warp, i, lane) is tile position warp*ITEMS*32 + i*32 + lane ----
   uint4 rec[ITEMS];
@@ -298,7 +300,6 @@ __global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(cons
   //      starts inside the tile; where it starts in the output comes from the scan kernels ----
   if (threadIdx.x < kRadix) {
     const uint32_t d = threadIdx.x;
-    const uint32_t out0 = p.offs[(uint64_t)tile * kRadix + d];
     uint32_t cnt[WARPS];
 #pragma unroll
     for (int w = 0; w < WARPS; ++w) cnt[w] = sm.warp_hist[w][d];
@@ -340,24 +341,35 @@ __global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(cons
     old = __shfl_sync(0xffffffffu, old, __ffs(peers) - 1);
     sm.recs[old + below] = rec[i];
   }
-  __syncthreads();
 
-  // ---- write out: consecutive threads write consecutive records of a digit run ----
-  const uint32_t dmask = (1u << p.delay_bits) - 1u;
-  const uint32_t next_mask = (1u << p.next_bits) - 1u;
+  if (LAST) {
+    __syncthreads();
+    // ---- final arrays: consecutive threads write consecutive records of a digit run ----
+    const uint32_t dmask = (1u << p.delay_bits) - 1u;
 #pragma unroll
-  for (int i = 0; i < ITEMS; ++i) {
-    const uint32_t j = i * kThreads + threadIdx.x;
-    if (j < valid) {
-      const uint4 r = sm.recs[j];
-      const uint32_t g = sm.global_off[(r.x >> p.shift) & mask] + j;
-      if (LAST) {
+    for (int i = 0; i < ITEMS; ++i) {
+      const uint32_t j = i * kThreads + threadIdx.x;
+      if (j < valid) {
+        const uint4 r = sm.recs[j];
+        const uint32_t g = sm.global_off[(r.x >> p.shift) & mask] + j;
         p.out_src[g] = r.x >> p.delay_bits;
         p.out_d[g] = (uint16_t)(r.x & dmask);
         p.out_tgt[g] = r.z;
         p.out_w[g] = __uint_as_float(r.w);
         p.out_perm[g] = r.y;
-      } else {
+      }
+    }
+  } else {
+    __syncthreads();
+    // ---- records and the next pass's digit of each: consecutive threads write consecutive records of a run.
+    //      (One TMA bulk copy per run was measured slower: the 32 copies a warp issues are serialised.) ----
+    const uint32_t next_mask = (1u << p.next_bits) - 1u;
+#pragma unroll
+    for (int i = 0; i < ITEMS; ++i) {
+      const uint32_t j = i * kThreads + threadIdx.x;
+      if (j < valid) {
+        const uint4 r = sm.recs[j];
+        const uint32_t g = sm.global_off[(r.x >> p.shift) & mask] + j;
         p.recs_out[g] = r;
         p.dig_out[g] = (uint8_t)((r.x >> p.next_shift) & next_mask);
       }
