@@ -26,7 +26,20 @@ if ROOT not in sys.path:
 METRIC = "synapses constructed/s (generate+sort+index, device-timed)"
 UNIT = "synapses/s"
 # algorithmic bytes per synapse
-BYTES = {"generate": 14, "histogram": 6, "sort_pass": 16, "permute": 26, "index": 4}
+# sort_pass: the record-carrying digit pass reads 16 B and writes 16 B per synapse (SURVEY 8(d) "carry (tgt, w) as extra
+# payload -> P x 32 B, permute vanishes"); histogram: 6 B (first pass) + 1 B per later pass; index: 6 B read twice.
+BYTES = {"generate": 14, "histogram": 8, "sort_pass": 32, "permute": 26, "index": 12}
+
+
+def ncu_traffic_per_launch():
+    """dram__bytes_read.sum + dram__bytes_write.sum of one scatter pass, from the committed ncu --set full capture."""
+    try:
+        for line in open(os.path.join(ROOT, "profiles", "r01_scatter_traffic.txt")):
+            if line.startswith("traffic_bytes_per_launch"):
+                return float(line.split("=")[1])
+    except Exception:
+        pass
+    return None
 
 
 def workload(name: str):
@@ -243,8 +256,11 @@ def main():
     roof = None
     if pass_ms:
         ach = BYTES["sort_pass"] * n_syn / (pass_ms * 1e-3) / 1e9
-        roof = {"bound": "hbm", "kernel": "onesweep_kernel (one digit pass: 8 B read + 8 B written per synapse)",
-                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None, "peak_kind": peak_kind,
+        roof = {"bound": "hbm", "kernel": "scatter_pass_kernel (one digit pass carrying the whole connection: 16 B read + "
+                                          "16 B written per synapse)",
+                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": ncu_traffic_per_launch() if args.workload == "c2" and not args.flags else None,
+                "peak_kind": peak_kind,
                 "launch_ms": pass_ms, "launches_per_step": passes}
     phases = {}
     for name, b in (("generate", BYTES["generate"]), ("histogram", BYTES["histogram"]), ("sort", BYTES["sort_pass"] * passes),

@@ -33,7 +33,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         if LIB.stat().st_mtime >= newest:
             return LIB
     tmp = LIB.with_suffix(f".so.tmp{os.getpid()}")
-    cmd = [NVCC, *NVCC_FLAGS, "-o", str(tmp), *map(str, cus)]
+    cmd = [NVCC, *NVCC_FLAGS, *os.environ.get("NC_NVCC_EXTRA", "").split(), "-o", str(tmp), *map(str, cus)]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)
