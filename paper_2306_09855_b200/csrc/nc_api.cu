@@ -882,7 +882,8 @@ int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) 
   {
     Scope sc(c, NC_PHASE_INDEX);
     IndexOut io{c->src_offsets, c->group_ptr, c->group_start, c->group_delay, N};
-    index_scatter_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(keys, n, tile_head_off, c->d_total_groups, io);
+    index_scatter_soa_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(c->s_src, c->s_d, n, tile_head_off,
+                                                                                    c->d_total_groups, io);
     NC_LAUNCH_CHECK(c, "index_scatter");
     index_finish_kernel<<<(N + 255) / 256, 256, 0, c->stream>>>(c->src_offsets, c->group_ptr, N, c->out_degree,
                                                                c->group_count, c->d_max + 1);

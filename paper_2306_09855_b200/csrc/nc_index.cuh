@@ -255,6 +255,101 @@ __global__ void __launch_bounds__(kHeadThreads) index_scatter_kernel(const Keys 
   }
 }
 
+// The same step over the final source / delay arrays of the record-carrying sort, written for the common case:
+// 128-bit loads, 32-bit compares, and all per-head work behind a find-first-set loop over the (sparse) head mask --
+// heads are a few percent of the connections, so the kernel is a streaming read.
+__global__ void __launch_bounds__(kHeadThreads) index_scatter_soa_kernel(const uint32_t* __restrict__ src,
+                                                                        const uint16_t* __restrict__ dly, uint32_t n,
+                                                                        const uint32_t* __restrict__ tile_head_off,
+                                                                        const uint64_t* __restrict__ total_groups,
+                                                                        const __grid_constant__ IndexOut out) {
+  __shared__ uint32_t warp_tmp[kHeadThreads / 32];
+  const uint32_t base = blockIdx.x * (uint32_t)kHeadTile + threadIdx.x * 8u;  // n < 2^32 and tiles are 2048 wide
+  const bool in_range = base < n && (uint64_t)blockIdx.x * kHeadTile + threadIdx.x * 8u < n;
+  uint32_t s[9], d[9];  // [0] = the connection just before this thread's eight
+#pragma unroll
+  for (int i = 0; i < 9; ++i) s[i] = d[i] = 0;
+  uint32_t cnt = 0;  // how many of the eight exist
+  if (in_range) {
+    if (n - base >= 8u) {
+      const uint4 s0 = *reinterpret_cast<const uint4*>(src + base);
+      const uint4 s1 = *reinterpret_cast<const uint4*>(src + base + 4);
+      const uint4 dd = *reinterpret_cast<const uint4*>(dly + base);
+      s[1] = s0.x; s[2] = s0.y; s[3] = s0.z; s[4] = s0.w; s[5] = s1.x; s[6] = s1.y; s[7] = s1.z; s[8] = s1.w;
+      d[1] = dd.x & 0xffffu; d[2] = dd.x >> 16; d[3] = dd.y & 0xffffu; d[4] = dd.y >> 16;
+      d[5] = dd.z & 0xffffu; d[6] = dd.z >> 16; d[7] = dd.w & 0xffffu; d[8] = dd.w >> 16;
+      cnt = 8;
+    } else {
+      cnt = n - base;
+#pragma unroll
+      for (int i = 0; i < 8; ++i)
+        if ((uint32_t)i < cnt) {
+          s[i + 1] = src[base + i];
+          d[i + 1] = dly[base + i];
+        }
+    }
+  }
+  // the predecessor: last element of the lane below, or (lane 0) from memory
+  const uint32_t up_s = __shfl_up_sync(0xffffffffu, s[8], 1), up_d = __shfl_up_sync(0xffffffffu, d[8], 1);
+  s[0] = up_s;
+  d[0] = up_d;
+  if (lane_id() == 0 && in_range && base > 0) {
+    s[0] = src[base - 1];
+    d[0] = dly[base - 1];
+  }
+  uint32_t heads = 0, first_of_source = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) {
+    const bool new_s = s[i + 1] != s[i];
+    if (new_s | (d[i + 1] != d[i])) heads |= 1u << i;
+    if (new_s) first_of_source |= 1u << i;
+  }
+  if (base == 0) {  // position 0 is a head and the first connection of its source
+    heads |= 1u;
+    first_of_source |= 1u;
+  }
+  const uint32_t live = cnt >= 8 ? 0xffu : ((1u << cnt) - 1u);
+  heads &= live;
+  first_of_source &= live;
+  uint32_t tot;
+  uint32_t g = block_exclusive_scan_256(__popc(heads), warp_tmp, tot) + tile_head_off[blockIdx.x];
+  uint32_t m = heads;
+  while (m) {
+    const int i = __ffs(m) - 1;
+    m &= m - 1;
+    const uint32_t j = base + i;
+    uint32_t si = s[1], di = d[1], sp = s[0];
+#pragma unroll
+    for (int q = 1; q < 8; ++q)
+      if (i == q) {
+        si = s[q + 1];
+        di = d[q + 1];
+        sp = s[q];
+      }
+    out.group_start[g] = j;
+    out.group_delay[g] = (uint16_t)di;
+    if (first_of_source & (1u << i)) {
+      const uint32_t lo = j == 0 ? 0u : sp + 1u;  // nodes in between have no outgoing connection (Q9)
+      for (uint32_t node = lo; node <= si; ++node) {
+        out.src_offsets[node] = j;
+        out.group_ptr[node] = g;
+      }
+    }
+    ++g;
+  }
+  if (cnt > 0 && base + cnt == n) {  // nodes after the last source, and the closing entries
+    uint32_t sl = s[1];
+#pragma unroll
+    for (int q = 1; q < 8; ++q)
+      if (cnt == (uint32_t)q + 1) sl = s[q + 1];
+    const uint32_t tg = (uint32_t)(*total_groups);
+    for (uint64_t node = (uint64_t)sl + 1; node <= out.n_nodes; ++node) {
+      out.src_offsets[node] = n;
+      out.group_ptr[node] = tg;
+    }
+  }
+}
+
 // G_i = p_{i+1} - p_i and out_degree_i = src_offsets_{i+1} - src_offsets_i, plus the maximum out-degree.
 __global__ void __launch_bounds__(256) index_finish_kernel(const uint32_t* __restrict__ src_offsets,
                                                           const uint32_t* __restrict__ group_ptr, uint32_t n_nodes,
