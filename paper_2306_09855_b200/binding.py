@@ -134,6 +134,20 @@ def _ptr(a):
     return None if a is None else a.ctypes.data_as(C.c_void_p)
 
 
+def _host_buffer(n, dtype):
+    """Host array for a device -> host read: page-locked (torch's caching host allocator), so the copy runs at PCIe
+    speed instead of being staged through a bounce buffer; plain numpy memory if pinning is not possible."""
+    dtype = np.dtype(dtype)
+    if int(n) * dtype.itemsize > (256 << 20):  # do not page-lock gigabytes
+        return np.empty(int(n), dtype=dtype)
+    try:
+        import torch
+        t = torch.empty(int(n) * dtype.itemsize, dtype=torch.uint8, pin_memory=True)
+        return t.numpy().view(dtype)  # the view keeps the tensor alive
+    except Exception:
+        return np.empty(int(n), dtype=dtype)
+
+
 class TorchAllocator:
     """nc_allocator backed by torch's caching allocator on the current device/stream."""
 
@@ -269,7 +283,7 @@ class NC:
             count = n - first
         out = {"n": int(count)}
         bufs = {"source": np.uint32, "target": np.uint32, "weight": np.float32, "delay": np.uint16, "perm": np.uint32}
-        arr = {k: (np.empty(count, dtype=dt) if (k in fields and (k != "perm" or sorted)) else None)
+        arr = {k: (_host_buffer(count, dt) if (k in fields and (k != "perm" or sorted)) else None)
                for k, dt in bufs.items()}
         self._check(self._L.nc_read_connections(self._h, 1 if sorted else 0, int(first), int(count), _ptr(arr["source"]),
                                                 _ptr(arr["target"]), _ptr(arr["weight"]), _ptr(arr["delay"]),
@@ -280,9 +294,9 @@ class NC:
     def read_index(self) -> dict:
         v = self.get_index()
         N, G = v.n_nodes, v.total_groups
-        a = {"src_offsets": np.empty(N + 1, np.uint32), "group_count": np.empty(N, np.uint32),
-             "group_ptr": np.empty(N + 1, np.uint32), "group_start": np.empty(G, np.uint32),
-             "group_delay": np.empty(G, np.uint16)}
+        a = {"src_offsets": _host_buffer(N + 1, np.uint32), "group_count": _host_buffer(N, np.uint32),
+             "group_ptr": _host_buffer(N + 1, np.uint32), "group_start": _host_buffer(G, np.uint32),
+             "group_delay": _host_buffer(G, np.uint16)}
         self._check(self._L.nc_read_index(self._h, _ptr(a["src_offsets"]), _ptr(a["group_count"]), _ptr(a["group_ptr"]),
                                           _ptr(a["group_start"]), _ptr(a["group_delay"])))
         a["n_nodes"], a["total_groups"] = int(N), int(G)
