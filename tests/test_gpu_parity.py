@@ -209,3 +209,76 @@ def test_default_cuda_allocator_path(nc_mod, oracle_mod):
     WL.run(net, g)
     PU.compare_connections(g.read_connections(sorted=True), o.connections(sorted=True), PU.weight_scale(net), "cudaMalloc")
     g.close()
+
+
+def test_full_size_microcircuit_in_bench_configuration(nc_mod, oracle_mod):
+    """configs[2] at FULL size (77,169 nodes, 298,880,970 connections), built exactly as bench.py builds it.
+    The oracle cannot hold this network in seconds, so: (1) sampled creation positions are compared one by one
+    with the oracle's per-synapse function; (2) the organised arrays are checked against the plain definitions
+    (reading D10, D11) evaluated with numpy on the GPU's own creation-order arrays: permutation, sortedness,
+    stability, gathered fields, offsets, group heads."""
+    net = WL.config2_microcircuit()
+    g = nc_mod.NC(dt_ms=net.dt_ms)
+    firsts = WL.run(net, g)
+    n = g.num_connections()
+    assert n == 298_880_970 and g.num_nodes() == 77_169
+    st = g.stats()
+    assert st["key_bits"] == 23 and st["sort_passes"] == 3
+
+    # (1) sampled synapses against the oracle, one by one
+    sizes = np.array([p.degree_or_total for p in net.projections], dtype=np.int64)
+    starts = np.concatenate([[0], np.cumsum(sizes)])
+    rng = np.random.default_rng(2306)
+    chunk_starts = np.concatenate([rng.integers(0, n - 64, size=300), starts[:-1], starts[1:] - 64, [n - 64]])
+    scale = PU.weight_scale(net)
+    checked = mism = 0
+    for c0 in chunk_starts:
+        c0 = int(max(0, c0))
+        got = g.read_connections(sorted=False, first=c0, count=64)
+        for k in range(0, 64, 3):
+            pos = c0 + k
+            pj = int(np.searchsorted(starts, pos, side="right") - 1)
+            pr = net.projections[pj]
+            o = oracle_mod.eval_synapse((firsts[pr.src_pop], net.populations[pr.src_pop]),
+                                        (firsts[pr.tgt_pop], net.populations[pr.tgt_pop]), WL.RULE_IDS[pr.rule],
+                                        pr.degree_or_total, pr.p, pr.weight, pr.delay_ms, pr.seed, pj, net.dt_ms,
+                                        pos - int(starts[pj]))
+            assert got["source"][k] == o["source"] and got["target"][k] == o["target"], (pos, pj)
+            assert abs(float(got["weight"][k]) - o["weight"]) <= PU.WEIGHT_RTOL * max(abs(o["weight"]), scale)
+            if got["delay"][k] != o["delay"]:
+                assert o["boundary"] and abs(int(got["delay"][k]) - o["delay"]) == 1
+                mism += 1
+            checked += 1
+    assert checked > 8000 and mism <= 1
+
+    # (2) the organisation step against its definition
+    u = g.read_connections(sorted=False, fields=("source", "delay"))
+    s = g.read_connections(sorted=True, fields=("source", "delay", "perm"))
+    perm = s["perm"]
+    seen = np.zeros(n, dtype=bool)
+    seen[perm] = True
+    assert seen.all(), "perm is not a permutation"
+    del seen
+    key = (s["source"].astype(np.uint64) << np.uint64(16)) | s["delay"].astype(np.uint64)
+    dk = key[1:] != key[:-1]
+    assert np.all(key[1:] >= key[:-1]), "not sorted by (source, delay)"
+    assert np.all(dk | (perm[1:] > perm[:-1])), "ties are not in creation order"
+    assert np.array_equal(u["source"][perm], s["source"]) and np.array_equal(u["delay"][perm], s["delay"])
+    idx = g.read_index()
+    out_deg = np.bincount(s["source"], minlength=net.n_nodes)
+    assert np.array_equal(idx["src_offsets"], np.concatenate([[0], np.cumsum(out_deg)]).astype(np.uint32))
+    heads = np.concatenate([[0], np.flatnonzero(dk) + 1]).astype(np.uint32)
+    assert idx["total_groups"] == heads.size
+    assert np.array_equal(idx["group_start"], heads)
+    assert np.array_equal(idx["group_delay"], s["delay"][heads])
+    gcount = np.bincount(s["source"][heads], minlength=net.n_nodes).astype(np.uint32)
+    assert np.array_equal(idx["group_count"], gcount)
+    assert np.array_equal(idx["group_ptr"], np.concatenate([[0], np.cumsum(gcount)]).astype(np.uint32))
+    del u, key, dk
+    # target and weight travel with the record: check them on a slice of the sorted order
+    j0 = n // 2
+    ss = g.read_connections(sorted=True, first=j0, count=200_000, fields=("target", "weight", "perm"))
+    for k in range(0, 200_000, 997):
+        one = g.read_connections(sorted=False, first=int(ss["perm"][k]), count=1, fields=("target", "weight"))
+        assert one["target"][0] == ss["target"][k] and one["weight"][0] == ss["weight"][k]
+    g.close()
