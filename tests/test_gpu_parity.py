@@ -282,3 +282,145 @@ def test_full_size_microcircuit_in_bench_configuration(nc_mod, oracle_mod):
         one = g.read_connections(sorted=False, first=int(ss["perm"][k]), count=1, fields=("target", "weight"))
         assert one["target"][0] == ss["target"][k] and one["weight"][0] == ss["weight"][k]
     g.close()
+
+
+def _check_organised_chunked(g, n, n_nodes, chunk=40_000_000):
+    """Readings D10/D11 checked on the device's own arrays at any size, a chunk of the sorted order at a time:
+    perm is a permutation, keys ascend, ties keep creation order, source and delay are the gathered creation-order
+    values, and every index array equals its definition."""
+    u = g.read_connections(sorted=False, fields=("source", "delay"))
+    seen = np.zeros(n, dtype=bool)
+    out_deg = np.zeros(n_nodes, dtype=np.int64)
+    gcount = np.zeros(n_nodes, dtype=np.int64)
+    heads, head_delay = [], []
+    prev_key, prev_perm = None, None
+    for j0 in range(0, n, chunk):
+        c = min(chunk, n - j0)
+        s = g.read_connections(sorted=True, first=j0, count=c, fields=("source", "delay", "perm"))
+        perm = s["perm"]
+        assert not seen[perm].any(), "perm repeats a position"
+        seen[perm] = True
+        assert np.array_equal(u["source"][perm], s["source"]) and np.array_equal(u["delay"][perm], s["delay"])
+        key = (s["source"].astype(np.uint64) << np.uint64(16)) | s["delay"].astype(np.uint64)
+        if prev_key is not None:
+            key = np.concatenate([[prev_key], key])
+            perm = np.concatenate([[prev_perm], perm])
+        dk = key[1:] != key[:-1]
+        assert np.all(key[1:] >= key[:-1]), "not sorted by (source, delay)"
+        assert np.all(dk | (perm[1:] > perm[:-1])), "ties are not in creation order"
+        h = np.flatnonzero(dk) + (j0 if prev_key is not None else j0 + 1)
+        if prev_key is None:
+            h = np.concatenate([[0], h])
+        heads.append(h.astype(np.uint32))
+        head_delay.append(s["delay"][h - j0])
+        out_deg += np.bincount(s["source"], minlength=n_nodes)
+        gcount += np.bincount(s["source"][h - j0], minlength=n_nodes)
+        prev_key, prev_perm = key[-1], perm[-1]
+    assert seen.all(), "perm is not a permutation"
+    idx = g.read_index()
+    heads = np.concatenate(heads)
+    assert idx["total_groups"] == heads.size
+    assert np.array_equal(idx["group_start"], heads) and np.array_equal(idx["group_delay"], np.concatenate(head_delay))
+    assert np.array_equal(idx["src_offsets"], np.concatenate([[0], np.cumsum(out_deg)]).astype(np.uint32))
+    assert np.array_equal(idx["group_count"], gcount.astype(np.uint32))
+    assert np.array_equal(idx["group_ptr"], np.concatenate([[0], np.cumsum(gcount)]).astype(np.uint32))
+
+
+def _check_sampled_synapses(g, net, firsts, oracle_mod, starts, n_chunks=150):
+    """Creation positions sampled in every projection against the oracle's per-synapse function (rules whose
+    i_newconns is the position inside the projection)."""
+    scale = PU.weight_scale(net)
+    rng = np.random.default_rng(99)
+    n = int(starts[-1])
+    chunk_starts = np.concatenate([rng.integers(0, n - 64, size=n_chunks), starts[:-1], starts[1:] - 64])
+    checked = mism = 0
+    for c0 in chunk_starts:
+        c0 = int(min(max(0, c0), n - 64))
+        got = g.read_connections(sorted=False, first=c0, count=64)
+        for k in range(0, 64, 5):
+            pos = c0 + k
+            pj = int(np.searchsorted(starts, pos, side="right") - 1)
+            pr = net.projections[pj]
+            if pr.rule == "pairwise_bernoulli":
+                continue
+            o = oracle_mod.eval_synapse((firsts[pr.src_pop], net.populations[pr.src_pop]),
+                                        (firsts[pr.tgt_pop], net.populations[pr.tgt_pop]), WL.RULE_IDS[pr.rule],
+                                        pr.degree_or_total, pr.p, pr.weight, pr.delay_ms, pr.seed, pj, net.dt_ms,
+                                        pos - int(starts[pj]))
+            assert got["source"][k] == o["source"] and got["target"][k] == o["target"], (pos, pj)
+            assert abs(float(got["weight"][k]) - o["weight"]) <= PU.WEIGHT_RTOL * max(abs(o["weight"]), scale)
+            if got["delay"][k] != o["delay"]:
+                assert o["boundary"] and abs(int(got["delay"][k]) - o["delay"]) == 1
+                mism += 1
+            checked += 1
+    assert mism <= 1
+    return checked
+
+
+def test_full_size_config3_large_indegree(nc_mod, oracle_mod):
+    """configs[3]: 100,000 nodes, 10^9 connections (fixed_indegree 8000 / 2000)."""
+    net = WL.config3_large_indegree()
+    g = nc_mod.NC(dt_ms=net.dt_ms)
+    firsts = WL.run(net, g)
+    n = g.num_connections()
+    assert n == 1_000_000_000
+    sizes = np.array([net.populations[p.tgt_pop] * p.degree_or_total for p in net.projections], dtype=np.int64)
+    starts = np.concatenate([[0], np.cumsum(sizes)])
+    assert _check_sampled_synapses(g, net, firsts, oracle_mod, starts) > 1500
+    deg, mx = g.read_degree_histogram(0)
+    assert np.all(deg == 10_000) and mx == 10_000  # exact in-degree K_E + K_I per target (Eq. 11)
+    _check_organised_chunked(g, n, net.n_nodes)
+    g.close()
+
+
+def test_full_size_config4_large_bernoulli(nc_mod, oracle_mod):
+    """configs[4]: 200,000 nodes, 4 x pairwise_bernoulli p = 0.025 over 4e10 pairs + fixed_outdegree K = 500.
+    Bernoulli projections: the count is within 5 sigma of the binomial, pairs ascend in q (D4), every sampled pair
+    is one the oracle's trial stream accepts and carries the oracle's weight and delay for that q, and the accepted
+    set of the first 200,000 pairs of every projection is exactly the oracle's."""
+    net = WL.config4_large_bernoulli()
+    g = nc_mod.NC(dt_ms=net.dt_ms)
+    firsts = [g.create_population(p) for p in net.populations]
+    counts = []
+    for pr in net.projections:
+        before = g.num_connections()
+        g.connect((firsts[pr.src_pop], net.populations[pr.src_pop]), (firsts[pr.tgt_pop], net.populations[pr.tgt_pop]),
+                  WL.RULE_IDS[pr.rule], degree_or_total=pr.degree_or_total, p=pr.p, weight=pr.weight,
+                  delay_ms=pr.delay_ms, seed=pr.seed)
+        counts.append(g.num_connections() - before)
+    g.finalize()
+    n = g.num_connections()
+    starts = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
+    scale = PU.weight_scale(net)
+    rng = np.random.default_rng(4)
+    for pj, pr in enumerate(net.projections):
+        ns, nt = net.populations[pr.src_pop], net.populations[pr.tgt_pop]
+        s0, t0 = firsts[pr.src_pop], firsts[pr.tgt_pop]
+        if pr.rule != "pairwise_bernoulli":
+            assert counts[pj] == ns * pr.degree_or_total
+            continue
+        T = oracle_mod.bernoulli_threshold(pr.p)
+        pt = T / 2.0**32
+        mean, sd = ns * nt * pt, math.sqrt(ns * nt * pt * (1 - pt))
+        assert abs(counts[pj] - mean) < 5 * sd, (pj, counts[pj], mean, sd)
+        # the head of the projection: exactly the oracle's accepted pairs among q < 200,000
+        head = g.read_connections(sorted=False, first=int(starts[pj]), count=min(8000, counts[pj]))
+        q = (head["source"].astype(np.int64) - s0) * nt + (head["target"].astype(np.int64) - t0)
+        assert np.all(np.diff(q) > 0)
+        want = [qq for qq in range(200_000) if oracle_mod.bernoulli_trial_word(pr.seed, pj, qq) < T]
+        assert np.array_equal(q[q < 200_000], np.array(want, dtype=np.int64))
+        # sampled pairs anywhere in the projection
+        for c0 in rng.integers(int(starts[pj]), int(starts[pj + 1]) - 32, size=40):
+            got = g.read_connections(sorted=False, first=int(c0), count=32)
+            q = (got["source"].astype(np.int64) - s0) * nt + (got["target"].astype(np.int64) - t0)
+            assert np.all(np.diff(q) > 0) and q[0] >= 0 and q[-1] < ns * nt
+            for k in range(0, 32, 4):
+                assert oracle_mod.bernoulli_trial_word(pr.seed, pj, int(q[k])) < T
+                o = oracle_mod.eval_synapse((s0, ns), (t0, nt), WL.RULE_IDS[pr.rule], 0, pr.p, pr.weight, pr.delay_ms,
+                                            pr.seed, pj, net.dt_ms, int(q[k]))
+                assert o["accepted"] and o["source"] == got["source"][k] and o["target"] == got["target"][k]
+                assert abs(float(got["weight"][k]) - o["weight"]) <= PU.WEIGHT_RTOL * max(abs(o["weight"]), scale)
+                assert got["delay"][k] == o["delay"] or (o["boundary"] and abs(int(got["delay"][k]) - o["delay"]) == 1)
+    assert _check_sampled_synapses(g, net, firsts, oracle_mod, starts) > 50  # the fixed_outdegree projection
+    _check_organised_chunked(g, n, net.n_nodes)
+    g.close()
