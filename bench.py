@@ -157,23 +157,16 @@ def main():
         return run_reference(args)
 
     import torch
-    from paper_2306_09855_b200 import binding, build, workloads as WL
+    from paper_2306_09855_b200 import binding, build, replicas, workloads as WL
     build.build()
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world, rank, local = replicas.env_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (the path has no CPU fallback)")
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dist = replicas.init("nccl", torch.device("cuda", local))
 
     def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
+        replicas.barrier(dist, torch.cuda.synchronize)
 
     net = workload(args.workload)
     stream = torch.cuda.current_stream()
@@ -207,12 +200,9 @@ def main():
     barrier()
     total_ms = ev0.elapsed_time(ev1)
     clocks = sampler.stop()
-    if dist is not None:
-        tt = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
+    total_ms = replicas.max_over_ranks(dist, total_ms, "cuda")
     ms_per_step = total_ms / args.steps
-    value = world * n_syn * args.steps / (total_ms * 1e-3)
+    value = replicas.whole_job_rate(n_syn, args.steps, world, total_ms)
 
     # ---- end to end through the public API with host buffers: context creation, host descriptors in,
     #      index arrays read back into host memory, wall clock ----
@@ -229,13 +219,8 @@ def main():
         nblocks = g.stats()["n_blocks"]
         g.close()
     h2d = len(net.projections) * (8 + 8 + 16 + 64 + 8) + 8 * nblocks  # per nc_connect: ranges, rule params, syn spec, seed; block table
-    if dist is not None:
-        tt = torch.tensor([max(e2e_times)], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        e2e_t = float(tt.item())
-    else:
-        e2e_t = statistics.median(e2e_times)
-    e2e_value = world * cnt / e2e_t
+    e2e_t = replicas.max_over_ranks(dist, statistics.median(e2e_times), "cuda")
+    e2e_value = replicas.whole_job_rate(cnt, 1, world, e2e_t * 1e3)
 
     if rank != 0:
         if dist is not None:
