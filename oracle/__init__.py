@@ -33,13 +33,13 @@ OK, ERR_INVALID_ARG, ERR_STATE, ERR_CAPACITY, ERR_OOM = 0, -1, -2, -3, -4
 
 
 def build(force: bool = False) -> Path:
-    """Compile oracle.cpp -> liboracle.so (g++ -O2 -ffp-contract=off, one translation unit)."""
-    srcs = [_HERE / "oracle.cpp", _HERE / "oracle.h"]
+    """Compile oracle.cpp + delivery.cpp -> liboracle.so (g++ -O2 -ffp-contract=off)."""
+    srcs = [_HERE / "oracle.cpp", _HERE / "oracle.h", _HERE / "delivery.cpp", _HERE / "delivery.h"]
     if not force and _LIB_PATH.exists() and all(_LIB_PATH.stat().st_mtime >= s.stat().st_mtime for s in srcs):
         return _LIB_PATH
     tmp = _LIB_PATH.with_suffix(f".so.tmp{os.getpid()}")
     cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-Wall", "-Wextra",
-           "-o", str(tmp), str(_HERE / "oracle.cpp")]
+           "-o", str(tmp), str(_HERE / "oracle.cpp"), str(_HERE / "delivery.cpp")]
     subprocess.run(cmd, check=True)
     os.replace(tmp, _LIB_PATH)
     return _LIB_PATH
@@ -277,3 +277,54 @@ class Oracle:
         if rc != 0:
             raise OracleError(rc)
         return _np(p, self.num_nodes(), np.uint32).copy(), mx.value
+
+
+class Delivery:
+    """Spike delivery over a finalized Oracle (delivery.h).  `input` is an fp64 array of n_nodes that
+    every step accumulates into."""
+
+    def __init__(self, oracle: "Oracle"):
+        L = lib()
+        L.oc_delivery_create.argtypes = [C.c_void_p, C.POINTER(C.c_void_p)]
+        L.oc_delivery_destroy.argtypes = [C.c_void_p]
+        L.oc_delivery_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
+        L.oc_delivery_spike_array.argtypes = [C.c_void_p, C.POINTER(C.POINTER(C.c_uint32)),
+                                              C.POINTER(C.POINTER(C.c_uint32)), C.POINTER(C.c_uint32)]
+        L.oc_delivery_counts.argtypes = [C.c_void_p, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+        self._L, self._oracle = L, oracle  # the oracle context must outlive this object
+        self._h = C.c_void_p()
+        rc = L.oc_delivery_create(oracle._h, C.byref(self._h))
+        if rc != 0:
+            raise OracleError(rc)
+        self.n_nodes = oracle.num_nodes()
+
+    def step(self, nodes, mult, input_f64):
+        nodes = np.ascontiguousarray(nodes, dtype=np.uint32)
+        m = None if mult is None else np.ascontiguousarray(mult, dtype=np.uint32)
+        assert input_f64.dtype == np.float64 and input_f64.size == self.n_nodes and input_f64.flags.c_contiguous
+        rc = self._L.oc_delivery_step(self._h, nodes.ctypes.data_as(C.c_void_p),
+                                      None if m is None else m.ctypes.data_as(C.c_void_p), nodes.size,
+                                      input_f64.ctypes.data_as(C.c_void_p))
+        if rc != 0:
+            raise OracleError(rc)
+
+    def spike_array(self):
+        g, m, n = C.POINTER(C.c_uint32)(), C.POINTER(C.c_uint32)(), C.c_uint32()
+        self._L.oc_delivery_spike_array(self._h, C.byref(g), C.byref(m), C.byref(n))
+        return _np(g, n.value, np.uint32).copy(), _np(m, n.value, np.uint32).copy()
+
+    def counts(self):
+        b, e = C.c_uint64(), C.c_uint64()
+        self._L.oc_delivery_counts(self._h, C.byref(b), C.byref(e))
+        return b.value, e.value
+
+    def close(self):
+        if self._h:
+            self._L.oc_delivery_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
