@@ -27,6 +27,9 @@ SYMBOLS = (
     "nc_finalize", "nc_num_connections", "nc_num_nodes", "nc_get_connections", "nc_get_index",
     "nc_degree_histogram", "nc_get_stats", "nc_get_timings", "nc_read_connections", "nc_read_index",
     "nc_read_degree_histogram", "nc_selftest_philox", "nc_selftest_fastpath",
+    # include/nc_delivery.h
+    "nc_delivery_create", "nc_delivery_destroy", "nc_delivery_step", "nc_delivery_read_spike_array",
+    "nc_delivery_counts",
 )
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_void_p, C.c_size_t)
@@ -117,6 +120,11 @@ def load_library():
     L.nc_read_degree_histogram.argtypes = [vp, C.c_int, vp, P(C.c_uint32)]
     L.nc_selftest_philox.argtypes = [vp, C.c_uint32, vp, vp, vp]
     L.nc_selftest_fastpath.argtypes = [vp, P(C.c_double)]
+    L.nc_delivery_create.argtypes = [vp, C.c_uint32, P(vp)]
+    L.nc_delivery_destroy.argtypes = [vp]
+    L.nc_delivery_step.argtypes = [vp, vp, vp, C.c_uint32, vp]
+    L.nc_delivery_read_spike_array.argtypes = [vp, vp, vp, C.c_uint32, P(C.c_uint32)]
+    L.nc_delivery_counts.argtypes = [vp, P(C.c_uint64), P(C.c_uint64), P(C.c_uint64), P(C.c_uint64)]
     for name in SYMBOLS:
         if name != "nc_last_error":
             getattr(L, name).restype = C.c_int
@@ -320,3 +328,45 @@ class NC:
         out = (C.c_double * 4)()
         self._check(self._L.nc_selftest_fastpath(self._h, out))
         return tuple(out)
+
+
+class Delivery:
+    """Spike delivery over a finalized NC context (include/nc_delivery.h).  Arguments of step() are
+    torch CUDA tensors (uint32 / int32 node ids and multiplicities, float32 input): device memory only, every step
+    of the path runs in the library's kernels."""
+
+    def __init__(self, nc: NC, capacity: int):
+        self._nc, self._L = nc, nc._L  # the context must outlive this object
+        self._h = C.c_void_p()
+        nc._check(self._L.nc_delivery_create(nc._h, int(capacity), C.byref(self._h)))
+        self.capacity = int(capacity)
+
+    def step(self, nodes, mult, input_f32, n_new=None):
+        n = int(nodes.numel()) if n_new is None else int(n_new)
+        assert input_f32.is_cuda and input_f32.element_size() == 4 and input_f32.numel() == self._nc.num_nodes()
+        assert nodes.is_cuda and nodes.element_size() == 4 and (mult is None or (mult.is_cuda and mult.element_size() == 4))
+        self._nc._check(self._L.nc_delivery_step(self._h, nodes.data_ptr() if n else None,
+                                                 mult.data_ptr() if (mult is not None and n) else None, n,
+                                                 input_f32.data_ptr()))
+
+    def read_spike_array(self):
+        n = C.c_uint32()
+        g, m = _host_buffer(self.capacity, np.uint32), _host_buffer(self.capacity, np.uint32)
+        self._nc._check(self._L.nc_delivery_read_spike_array(self._h, _ptr(g), _ptr(m), self.capacity, C.byref(n)))
+        return g[:n.value].copy(), m[:n.value].copy()
+
+    def counts(self) -> dict:
+        v = [C.c_uint64() for _ in range(4)]
+        self._nc._check(self._L.nc_delivery_counts(self._h, *[C.byref(x) for x in v]))
+        return dict(zip(("buffered", "events", "dropped", "bad_nodes"), (x.value for x in v)))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.nc_delivery_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -14,6 +14,7 @@
 #include <vector>
 
 #include "nc_common.cuh"
+#include "nc_internal.h"
 #include "nc_generate.cuh"
 #include "nc_index.cuh"
 #include "nc_sort.cuh"
@@ -1379,3 +1380,24 @@ int nc_selftest_fastpath(nc_context* c, double out[4]) {
 }
 
 }  // extern "C"
+
+// ---- nc_internal.h ----
+int nc_internal_organised_view(nc_context* c, nc_organised_view* out) {
+  if (!c || !out) return NC_ERR_INVALID_ARG;
+  if (!c->finalized) return fail(c, NC_ERR_STATE, "the connections are not organised yet (nc_finalize)");
+  int rc = ensure_total_groups(c);
+  if (rc != NC_OK) return rc;
+  out->target = c->s_tgt;
+  out->weight = c->s_w;
+  out->group_ptr = c->group_ptr;
+  out->group_start = c->group_start;
+  out->group_delay = c->group_delay;
+  out->n_nodes = c->n_nodes;
+  out->total_groups = c->total_groups;
+  out->n = c->n_conns;
+  out->stream = c->stream;
+  return NC_OK;
+}
+void* nc_internal_alloc(nc_context* c, size_t bytes) { return dev_alloc(c, bytes); }
+void nc_internal_free(nc_context* c, void* p) { dev_free(c, p); }
+int nc_internal_fail(nc_context* c, int code, const char* msg) { return fail(c, code, msg); }

@@ -1,0 +1,260 @@
+// nc_delivery.cu -- spike delivery over the organised connections (include/nc_delivery.h).
+//
+// The paper keeps one queue per neuron and, every step, increments the time index of every buffered spike.  Here
+// the buffered spikes of ALL neurons live in one flat device list of 16-byte entries (source, emission step, next
+// group, multiplicity): the time index is `now - emission step`, so nothing is incremented, and one step is
+//   advance_insert_kernel : one thread per buffered spike -- matured spikes append (group, multiplicity) to the
+//                           spike array, spikes with groups left are re-appended to the other list (ping-pong),
+//                           and the spikes emitted in this step are appended behind them (warp-aggregated atomics);
+//   deliver_kernel        : one warp per spike-array entry, lanes over the connections of the group (coalesced
+//                           reads of target and weight, one float atomic add per connection).
+// Counts stay on the device: the host never waits inside a step.
+#include "../../include/nc_delivery.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <new>
+
+#include "nc_common.cuh"
+#include "nc_internal.h"
+
+using namespace nc;
+
+namespace {
+
+struct Counters {
+  uint32_t n_live_a;   // entries of live list A
+  uint32_t n_arr;      // entries of the spike array
+  uint32_t n_live_b;   // entries of live list B
+  uint32_t pad_;
+  unsigned long long events, dropped, bad_nodes;
+};
+
+struct StepParams {
+  nc_organised_view v;
+  const uint4* live_in;   // (source, emission step, next global group, multiplicity)
+  uint4* live_out;
+  const uint32_t* n_live_in;
+  uint32_t* n_live_out;
+  uint32_t* n_arr;
+  uint2* arr;             // (global group, multiplicity)
+  Counters* ctr;
+  const uint32_t* new_nodes;
+  const uint32_t* new_mult;
+  uint32_t n_new, capacity, now;
+};
+
+// append `item` for the lanes with `want` set; returns false for the lanes that did not fit
+__device__ __forceinline__ uint32_t warp_reserve(uint32_t* counter, bool want) {
+  const uint32_t m = __ballot_sync(0xffffffffu, want);
+  uint32_t base = 0;
+  if (m && lane_id() == (uint32_t)(__ffs(m) - 1)) base = atomicAdd(counter, (uint32_t)__popc(m));
+  base = __shfl_sync(0xffffffffu, base, m ? __ffs(m) - 1 : 0);
+  return base + __popc(m & lanemask_lt());
+}
+
+constexpr int kStepThreads = 256;
+
+__global__ void __launch_bounds__(kStepThreads) advance_insert_kernel(const __grid_constant__ StepParams p) {
+  const uint32_t n_live = min(*p.n_live_in, p.capacity);
+  const uint32_t total = n_live + p.n_new;
+  const uint32_t rounds = (total + gridDim.x * kStepThreads - 1) / (gridDim.x * kStepThreads);
+  for (uint32_t r = 0; r < rounds; ++r) {  // whole warps stay in the loop: the ballots below need all lanes
+    const uint32_t i = (r * gridDim.x + blockIdx.x) * kStepThreads + threadIdx.x;
+    bool keep = false, mature = false, bad = false;
+    uint4 sp = make_uint4(0u, 0u, 0u, 0u);
+    uint32_t g_mature = 0;
+    if (i < n_live) {
+      sp = p.live_in[i];
+      const uint32_t end = p.v.group_ptr[sp.x + 1];
+      // time index = steps since emission ("the time indexes of all the spikes are increased by one")
+      if (p.v.group_delay[sp.z] == p.now - sp.y) {
+        mature = true;
+        g_mature = sp.z;
+        sp.z += 1;  // "its connection group index is incremented by one unit"
+      }
+      keep = sp.z < end;
+    } else if (i < total) {
+      const uint32_t k = i - n_live;
+      const uint32_t s = p.new_nodes[k], m = p.new_mult ? p.new_mult[k] : 1u;
+      if (s >= p.v.n_nodes) {
+        bad = true;
+      } else {
+        const uint32_t g0 = p.v.group_ptr[s], g1 = p.v.group_ptr[s + 1];
+        keep = m != 0 && g0 < g1;  // a node without outgoing connections buffers nothing
+        sp = make_uint4(s, p.now, g0, m);
+      }
+    }
+    const uint32_t a = warp_reserve(p.n_arr, mature);
+    if (mature) p.arr[a] = make_uint2(g_mature, sp.w);  // one entry per buffered spike at most: always fits
+    const uint32_t o = warp_reserve(p.n_live_out, keep);
+    if (keep) {
+      if (o < p.capacity) p.live_out[o] = sp;
+      else atomicAdd(&p.ctr->dropped, 1ull);
+    }
+    if (bad) atomicAdd(&p.ctr->bad_nodes, 1ull);
+  }
+}
+
+struct DeliverParams {
+  nc_organised_view v;
+  const uint32_t* n_arr;
+  const uint2* arr;
+  Counters* ctr;
+  float* input;
+  uint32_t capacity;
+};
+
+__global__ void __launch_bounds__(256) deliver_kernel(const __grid_constant__ DeliverParams p) {
+  const uint32_t n_arr = min(*p.n_arr, p.capacity);
+  const uint32_t warps = gridDim.x * (256 / 32);
+  unsigned long long ev = 0;
+  for (uint32_t e = blockIdx.x * (256 / 32) + (threadIdx.x >> 5); e < n_arr; e += warps) {
+    const uint2 ent = p.arr[e];
+    const uint32_t c0 = p.v.group_start[ent.x];
+    const uint32_t c1 = ent.x + 1 < p.v.total_groups ? p.v.group_start[ent.x + 1] : (uint32_t)p.v.n;
+    const float m = (float)ent.y;
+    for (uint32_t c = c0 + lane_id(); c < c1; c += 32) atomicAdd(p.input + p.v.target[c], p.v.weight[c] * m);
+    ev += c1 - c0;
+  }
+  if (lane_id() == 0 && ev) atomicAdd(&p.ctr->events, ev);
+}
+
+}  // namespace
+
+struct nc_delivery {
+  nc_context* ctx = nullptr;
+  nc_organised_view v{};
+  uint32_t capacity = 0, now = 0;
+  int cur = 0;  // which live list is the input of the next step
+  uint4* live[2] = {nullptr, nullptr};
+  uint2* arr = nullptr;
+  Counters* ctr = nullptr;
+  int sms = 148;
+};
+
+extern "C" {
+
+int nc_delivery_create(nc_context* ctx, uint32_t capacity, nc_delivery** out) {
+  if (!ctx || !out || capacity == 0) return NC_ERR_INVALID_ARG;
+  *out = nullptr;
+  nc_organised_view v{};
+  int rc = nc_internal_organised_view(ctx, &v);
+  if (rc != NC_OK) return rc;
+  nc_delivery* d = new (std::nothrow) nc_delivery();
+  if (!d) return NC_ERR_OOM;
+  d->ctx = ctx;
+  d->v = v;
+  d->capacity = capacity;
+  d->live[0] = (uint4*)nc_internal_alloc(ctx, (size_t)capacity * 16);
+  d->live[1] = (uint4*)nc_internal_alloc(ctx, (size_t)capacity * 16);
+  d->arr = (uint2*)nc_internal_alloc(ctx, (size_t)capacity * 8);
+  d->ctr = (Counters*)nc_internal_alloc(ctx, sizeof(Counters));
+  if (!d->live[0] || !d->live[1] || !d->arr || !d->ctr) {
+    nc_delivery_destroy(d);
+    return nc_internal_fail(ctx, NC_ERR_OOM, "out of device memory for the spike buffers");
+  }
+  if (cudaMemsetAsync(d->ctr, 0, sizeof(Counters), v.stream) != cudaSuccess) {
+    nc_delivery_destroy(d);
+    return nc_internal_fail(ctx, NC_ERR_CUDA, "cudaMemsetAsync failed");
+  }
+  int dev = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&d->sms, cudaDevAttrMultiProcessorCount, dev);
+  *out = d;
+  return NC_OK;
+}
+
+int nc_delivery_destroy(nc_delivery* d) {
+  if (!d) return NC_OK;
+  cudaStreamSynchronize(d->v.stream);
+  nc_internal_free(d->ctx, d->live[0]);
+  nc_internal_free(d->ctx, d->live[1]);
+  nc_internal_free(d->ctx, d->arr);
+  nc_internal_free(d->ctx, d->ctr);
+  delete d;
+  return NC_OK;
+}
+
+int nc_delivery_step(nc_delivery* d, const uint32_t* d_nodes, const uint32_t* d_mult, uint32_t n_new, float* d_input) {
+  if (!d || !d_input || (n_new && !d_nodes)) return NC_ERR_INVALID_ARG;
+  cudaStream_t st = d->v.stream;
+  // the spike array and the list that is written in this step start empty; they sit next to each other in Counters
+  uint32_t* n_live_in = d->cur == 0 ? &d->ctr->n_live_a : &d->ctr->n_live_b;
+  uint32_t* n_live_out = d->cur == 0 ? &d->ctr->n_live_b : &d->ctr->n_live_a;
+  uint32_t* reset_from = d->cur == 0 ? &d->ctr->n_arr : &d->ctr->n_live_a;  // {n_arr, n_live_b} or {n_live_a, n_arr}
+  if (cudaMemsetAsync(reset_from, 0, 8, st) != cudaSuccess) return nc_internal_fail(d->ctx, NC_ERR_CUDA, "cudaMemsetAsync failed");
+  d->now += 1;
+  StepParams sp{};
+  sp.v = d->v;
+  sp.live_in = d->live[d->cur];
+  sp.live_out = d->live[1 - d->cur];
+  sp.n_live_in = n_live_in;
+  sp.n_live_out = n_live_out;
+  sp.n_arr = &d->ctr->n_arr;
+  sp.arr = d->arr;
+  sp.ctr = d->ctr;
+  sp.new_nodes = d_nodes;
+  sp.new_mult = d_mult;
+  sp.n_new = n_new;
+  sp.capacity = d->capacity;
+  sp.now = d->now;
+  // the number of buffered spikes is only known on the device: a fixed grid strides over them
+  const uint64_t most = (uint64_t)d->capacity + n_new;
+  const unsigned grid = (unsigned)std::max<uint64_t>(1, std::min<uint64_t>((most + kStepThreads - 1) / kStepThreads, (uint64_t)d->sms * 8));
+  advance_insert_kernel<<<grid, kStepThreads, 0, st>>>(sp);
+  DeliverParams dp{};
+  dp.v = d->v;
+  dp.n_arr = &d->ctr->n_arr;
+  dp.arr = d->arr;
+  dp.ctr = d->ctr;
+  dp.input = d_input;
+  dp.capacity = d->capacity;
+  const unsigned dgrid = (unsigned)std::max<uint64_t>(1, std::min<uint64_t>(((uint64_t)d->capacity + 7) / 8, (uint64_t)d->sms * 8));
+  deliver_kernel<<<dgrid, 256, 0, st>>>(dp);
+  d->cur = 1 - d->cur;
+  if (cudaPeekAtLastError() != cudaSuccess)
+    return nc_internal_fail(d->ctx, NC_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));
+  return NC_OK;
+}
+
+int nc_delivery_read_spike_array(nc_delivery* d, uint32_t* group, uint32_t* mult, uint32_t cap, uint32_t* n) {
+  if (!d || !n) return NC_ERR_INVALID_ARG;
+  cudaStream_t st = d->v.stream;
+  uint32_t cnt = 0;
+  if (cudaMemcpyAsync(&cnt, &d->ctr->n_arr, 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+      cudaStreamSynchronize(st) != cudaSuccess)
+    return nc_internal_fail(d->ctx, NC_ERR_CUDA, "reading the spike array failed");
+  *n = cnt;
+  const uint32_t take = cnt < cap ? cnt : cap;
+  if (take && group && mult) {
+    uint2* tmp = new (std::nothrow) uint2[take];
+    if (!tmp) return NC_ERR_OOM;
+    cudaError_t e = cudaMemcpyAsync(tmp, d->arr, (size_t)take * 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    for (uint32_t i = 0; i < take && e == cudaSuccess; ++i) {
+      group[i] = tmp[i].x;
+      mult[i] = tmp[i].y;
+    }
+    delete[] tmp;
+    if (e != cudaSuccess) return nc_internal_fail(d->ctx, NC_ERR_CUDA, cudaGetErrorString(e));
+  }
+  return NC_OK;
+}
+
+int nc_delivery_counts(nc_delivery* d, uint64_t* buffered, uint64_t* events, uint64_t* dropped, uint64_t* bad_nodes) {
+  if (!d) return NC_ERR_INVALID_ARG;
+  Counters h{};
+  cudaStream_t st = d->v.stream;
+  if (cudaMemcpyAsync(&h, d->ctr, sizeof(Counters), cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+      cudaStreamSynchronize(st) != cudaSuccess)
+    return nc_internal_fail(d->ctx, NC_ERR_CUDA, "reading the delivery counters failed");
+  const uint32_t live = d->cur == 0 ? h.n_live_a : h.n_live_b;
+  if (buffered) *buffered = live < d->capacity ? live : d->capacity;
+  if (events) *events = h.events;
+  if (dropped) *dropped = h.dropped;
+  if (bad_nodes) *bad_nodes = h.bad_nodes;
+  return NC_OK;
+}
+
+}  // extern "C"

@@ -1,5 +1,5 @@
 """The C-ABI library builds for sm_100a on a machine without a GPU, loads, exports every symbol that
-include/nc.h declares, and refuses to run without a device (no CPU fallback).  CPU only."""
+include/*.h declare, and refuses to run without a device (no CPU fallback).  CPU only."""
 import ctypes
 import re
 from pathlib import Path
@@ -16,9 +16,12 @@ def lib():
 
 
 def declared_symbols():
-    text = (ROOT / "include" / "nc.h").read_text()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(nc_[a-z_0-9]+)\s*\(", text)))
+    """every function any header under include/ declares"""
+    names = set()
+    for h in sorted((ROOT / "include").glob("*.h")):
+        text = re.sub(r"/\*.*?\*/", "", h.read_text(), flags=re.S)
+        names |= set(re.findall(r"\b(nc_[a-z_0-9]+)\s*\(", text))
+    return sorted(names)
 
 
 def test_header_symbols_exported(lib):
@@ -27,7 +30,7 @@ def test_header_symbols_exported(lib):
     assert len(names) >= 19
     for n in names:
         assert hasattr(lib, n), f"libnc.so does not export {n}"
-    assert sorted(binding.SYMBOLS) == names, "binding.SYMBOLS out of step with include/nc.h"
+    assert sorted(binding.SYMBOLS) == names, "binding.SYMBOLS out of step with include/*.h"
 
 
 def test_struct_layouts_match_header():

@@ -1,0 +1,106 @@
+"""GPU parity of spike delivery (include/nc_delivery.h) against oracle/delivery.cpp on the same seeded spike
+rasters: per step the spike array (as a multiset: its order on the device is arbitrary) must be identical, and the
+input of every node must match the oracle's fp64 sum within the fp32 accumulation tolerance
+|err| <= 1e-5 * max(1, max |input|) (sums of at most a few hundred terms of magnitude <= 400, fp32 atomics in arbitrary
+order: relative error ~ sqrt(terms) * 6e-8)."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2306_09855_b200 import workloads as WL
+
+pytestmark = pytest.mark.gpu
+INF = math.inf
+
+
+@pytest.fixture(scope="module")
+def nc_mod():
+    from paper_2306_09855_b200 import binding, build
+    build.build()
+    return binding
+
+
+def _raster(rng, n_nodes, steps, rate, max_mult):
+    out = []
+    for _ in range(steps):
+        k = int(rng.binomial(n_nodes, rate))
+        nodes = rng.choice(n_nodes, size=k, replace=False).astype(np.uint32)
+        out.append((nodes, rng.integers(1, max_mult + 1, size=k).astype(np.uint32)))
+    return out
+
+
+def _run_both(nc_mod, oracle_mod, net, steps, tail, rate, capacity, max_mult=3, use_mult=True, seed=11):
+    import torch
+    o = oracle_mod.Oracle(dt_ms=net.dt_ms)
+    WL.run(net, o)
+    g = nc_mod.NC(dt_ms=net.dt_ms)
+    WL.run(net, g)
+    od, gd = oracle_mod.Delivery(o), nc_mod.Delivery(g, capacity)
+    rng = np.random.default_rng(seed)
+    raster = _raster(rng, net.n_nodes, steps, rate, max_mult)
+    inp = torch.zeros(net.n_nodes, dtype=torch.float32, device="cuda")
+    worst = 0.0
+    for k in range(steps + tail):
+        nodes, mult = raster[k] if k < steps else (np.zeros(0, np.uint32), np.zeros(0, np.uint32))
+        want = np.zeros(net.n_nodes)
+        od.step(nodes, mult if use_mult else None, want)
+        inp.zero_()
+        tn = torch.from_numpy(nodes.astype(np.int32)).cuda()
+        tm = torch.from_numpy(mult.astype(np.int32)).cuda() if use_mult else None
+        gd.step(tn, tm, inp)
+        got = inp.cpu().numpy().astype(np.float64)
+        tol = 1e-5 * max(1.0, float(np.abs(want).max()))
+        err = float(np.abs(got - want).max())
+        assert err <= tol, f"step {k}: input error {err} > {tol}"
+        worst = max(worst, err / tol)
+        og, om = od.spike_array()
+        gg, gm = gd.read_spike_array()
+        assert np.array_equal(np.sort(og.astype(np.uint64) << np.uint64(32) | om), np.sort(gg.astype(np.uint64) << np.uint64(32) | gm)), f"step {k}: spike array"
+    ob, oe = od.counts()
+    c = gd.counts()
+    assert c["buffered"] == ob and c["events"] == oe and c["dropped"] == 0 and c["bad_nodes"] == 0
+    gd.close(); od.close(); g.close(); o.close()
+    return worst, oe
+
+
+def test_delivery_tiny_network_every_step(nc_mod, oracle_mod):
+    worst, events = _run_both(nc_mod, oracle_mod, WL.config0_tiny(), steps=80, tail=70, rate=0.05, capacity=4096)
+    assert events > 1000
+
+
+def test_delivery_without_multiplicities(nc_mod, oracle_mod):
+    _run_both(nc_mod, oracle_mod, WL.config0_tiny(), steps=40, tail=70, rate=0.1, capacity=4096, use_mult=False)
+
+
+def test_delivery_microcircuit_scaled(nc_mod, oracle_mod):
+    """configs[2] at 5 % of the populations (3,858 nodes, 7.5e5 connections, E and I delays): many groups per source,
+    several warps' worth of connections per group, a few hundred spikes in flight."""
+    worst, events = _run_both(nc_mod, oracle_mod, WL.config2_microcircuit(scale=0.05), steps=50, tail=65, rate=0.01,
+                              capacity=1 << 16, seed=3)
+    assert events > 3e5
+
+
+def test_delivery_edge_cases(nc_mod, oracle_mod):
+    import torch
+    net = WL.config0_tiny()
+    g = nc_mod.NC(dt_ms=net.dt_ms)
+    firsts = WL.run(net, g, finalize=False)
+    with pytest.raises(nc_mod.NCError) as e:  # before nc_finalize
+        nc_mod.Delivery(g, 16)
+    assert e.value.code == nc_mod.ERR_STATE
+    g.finalize()
+    with pytest.raises(nc_mod.NCError):
+        nc_mod.Delivery(g, 0)
+    d = nc_mod.Delivery(g, 4)  # room for four buffered spikes only
+    inp = torch.zeros(net.n_nodes, dtype=torch.float32, device="cuda")
+    d.step(torch.zeros(0, dtype=torch.int32, device="cuda"), None, inp)  # an empty step
+    nodes = torch.tensor([0, 1, 2, 3, 4, 5, 1000], dtype=torch.int32, device="cuda")  # one id outside the network
+    d.step(nodes, None, inp)
+    c = d.counts()
+    assert c["buffered"] == 4 and c["dropped"] == 2 and c["bad_nodes"] == 1
+    mult0 = torch.zeros(3, dtype=torch.int32, device="cuda")
+    d2 = nc_mod.Delivery(g, 64)
+    d2.step(torch.tensor([7, 8, 9], dtype=torch.int32, device="cuda"), mult0, inp)  # multiplicity 0 = no spike
+    assert d2.counts()["buffered"] == 0
+    d.close(); d2.close(); g.close()
