@@ -568,18 +568,14 @@ int sort_and_index(nc_context* c, const PassPlan& plan) {
 
 // Record-carrying organisation step (keys of <= 32 bits): histogram, P onesweep passes that move whole
 // connections, final pass writes the sorted SoA arrays; then the index over (source, delay).
-// Launch shapes of the record pass (threads, records per thread, CTAs per SM the registers are budgeted for).
-// Variant 0 is the default; NC_SORT_VARIANT selects another one for tuning runs.
+// Launch shape of the record pass: 384 threads x 8 records, registers budgeted for 3 CTAs per SM, shared-memory
+// peer masks (the best of the eight shapes tried on B200, profiles/r01_baseline.md).
 struct RecShape {
   int threads, items;
 };
-constexpr RecShape kRecShapes[] = {{384, 8}, {256, 8}, {512, 8}, {512, 8}, {512, 8}, {256, 16}, {384, 8}, {320, 8}};
+constexpr RecShape kRecShapes[] = {{384, 8}};
 
-int rec_variant() {
-  const char* e = getenv("NC_SORT_VARIANT");
-  const int v = e ? atoi(e) : 0;
-  return (v >= 0 && v < (int)(sizeof(kRecShapes) / sizeof(kRecShapes[0]))) ? v : 0;
-}
+int rec_variant() { return 0; }
 
 template <bool FIRST, bool LAST, int THREADS, int ITEMS, int MIN_CTAS, int MATCH>
 int launch_rec_pass_shape(nc_context* c, const SortRecParams& sp) {
@@ -593,17 +589,8 @@ int launch_rec_pass_shape(nc_context* c, const SortRecParams& sp) {
 }
 
 template <bool FIRST, bool LAST>
-int launch_rec_pass(nc_context* c, const SortRecParams& sp, int variant) {
-  switch (variant) {
-    case 1: return launch_rec_pass_shape<FIRST, LAST, 256, 8, 4, kMatchSmem>(c, sp);
-    case 2: return launch_rec_pass_shape<FIRST, LAST, 512, 8, 2, kMatchSmem>(c, sp);
-    case 3: return launch_rec_pass_shape<FIRST, LAST, 512, 8, 2, kMatchAny>(c, sp);
-    case 4: return launch_rec_pass_shape<FIRST, LAST, 512, 8, 2, kMatchBallot>(c, sp);
-    case 5: return launch_rec_pass_shape<FIRST, LAST, 256, 16, 2, kMatchSmem>(c, sp);
-    case 6: return launch_rec_pass_shape<FIRST, LAST, 384, 8, 3, kMatchBallot>(c, sp);
-    case 7: return launch_rec_pass_shape<FIRST, LAST, 320, 8, 3, kMatchSmem>(c, sp);
-    default: return launch_rec_pass_shape<FIRST, LAST, 384, 8, 3, kMatchSmem>(c, sp);
-  }
+int launch_rec_pass(nc_context* c, const SortRecParams& sp, int /*variant*/) {
+  return launch_rec_pass_shape<FIRST, LAST, 384, 8, 3, kMatchSmem>(c, sp);
 }
 
 int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag);
@@ -694,20 +681,12 @@ int sort_carry_and_index(nc_context* c, const PassPlan& plan) {
 struct SplitShape {
   int warps, items;
 };
-constexpr SplitShape kSplitShapes[] = {{8, 16}, {16, 8}, {12, 8}, {8, 8}, {16, 4}, {24, 4}};
+constexpr SplitShape kSplitShapes[] = {{8, 16}, {12, 8}};
 
 int split_variant() {
   const char* e = getenv("NC_SPLIT_VARIANT");
   const int v = e ? atoi(e) : 0;
   return (v >= 0 && v < (int)(sizeof(kSplitShapes) / sizeof(kSplitShapes[0]))) ? v : 0;
-}
-
-int split_match() {  // NC_SPLIT_MATCH=2: shared-memory peer masks instead of eight ballots (experiment)
-  static const int m = [] {
-    const char* e = getenv("NC_SPLIT_MATCH");
-    return e && atoi(e) == 2 ? (int)kMatchSmem : (int)kMatchBallot;
-  }();
-  return m;
 }
 
 template <bool FIRST, bool LAST, int WARPS, int ITEMS, int MIN_CTAS, int MATCH>
@@ -722,19 +701,13 @@ int launch_scatter_match(nc_context* c, const ScatterParams& sp, uint32_t n_tile
 
 template <bool FIRST, bool LAST, int WARPS, int ITEMS, int MIN_CTAS>
 int launch_scatter_shape(nc_context* c, const ScatterParams& sp, uint32_t n_tiles) {
-  if (WARPS == 8 && ITEMS == 16 && split_match() == kMatchSmem)
-    return launch_scatter_match<FIRST, LAST, WARPS, ITEMS, MIN_CTAS, kMatchSmem>(c, sp, n_tiles);
   return launch_scatter_match<FIRST, LAST, WARPS, ITEMS, MIN_CTAS, kMatchBallot>(c, sp, n_tiles);
 }
 
 template <bool FIRST, bool LAST>
 int launch_scatter_pass(nc_context* c, const ScatterParams& sp, uint32_t n_tiles, int variant) {
   switch (variant) {
-    case 1: return launch_scatter_shape<FIRST, LAST, 16, 8, 2>(c, sp, n_tiles);
-    case 2: return launch_scatter_shape<FIRST, LAST, 12, 8, 3>(c, sp, n_tiles);
-    case 3: return launch_scatter_shape<FIRST, LAST, 8, 8, 4>(c, sp, n_tiles);
-    case 4: return launch_scatter_shape<FIRST, LAST, 16, 4, 4>(c, sp, n_tiles);
-    case 5: return launch_scatter_shape<FIRST, LAST, 24, 4, 2>(c, sp, n_tiles);
+    case 1: return launch_scatter_shape<FIRST, LAST, 12, 8, 3>(c, sp, n_tiles);
     default: return launch_scatter_shape<FIRST, LAST, 8, 16, 2>(c, sp, n_tiles);
   }
 }
