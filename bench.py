@@ -65,6 +65,7 @@ class ClockSampler(threading.Thread):
     def __init__(self, index: int):
         super().__init__(daemon=True)
         self.index, self.samples, self.reasons, self.max_mhz, self._halt = index, [], set(), None, threading.Event()
+        self.ready = threading.Event()  # NVML is initialised: sampling has begun
 
     def run(self):
         try:
@@ -78,15 +79,17 @@ class ClockSampler(threading.Thread):
                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
                 nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
             }
+            self.ready.set()
             while not self._halt.is_set():
                 self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
                 r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
                 for bit, nm in names.items():
                     if r & bit:
                         self.reasons.add(nm)
-                time.sleep(0.02)
+                time.sleep(0.004)
         except Exception as e:  # NVML missing: report that instead of failing the bench
             self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+            self.ready.set()
 
     def stop(self):
         self._halt.set()
@@ -244,6 +247,7 @@ def main():
     # ---- timed region: K steps, CUDA events on the stream the kernels are launched on ----
     sampler = ClockSampler(local)
     sampler.start()
+    sampler.ready.wait(timeout=10)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     phase_acc, launches, stats = {}, 0, {}
     barrier()
@@ -319,7 +323,7 @@ def main():
 
     cpu = None
     if not args.no_cpu_baseline and args.workload.startswith("c2"):
-        scale = args.sample_scale if args.sample_scale else 0.25
+        scale = args.sample_scale if args.sample_scale else 0.5
         snet, sn, st = cpu_oracle_sample(scale)
         cpu = {"value": sn / st[0], "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"configs[2] with populations scaled x{scale:g}: {snet.n_nodes} nodes, {sn} synapses, generate+sort+index, {st[0]:.1f} s",
