@@ -193,6 +193,16 @@ int nc_create_population(nc_context* ctx, uint32_t n, uint32_t* first_id);
 int nc_connect(nc_context* ctx, nc_range src, nc_range tgt, nc_rule rule, const nc_rule_params* params,
                const nc_syn_spec* syn, uint64_t seed);
 
+/* The same with explicit node arrays ("If the indexes of source or target nodes are not consecutive but
+ * are explicitly given by an array, the above formulas are used to derive the indexes of the array elements from
+ * which to extract the node indexes").  src_nodes / tgt_nodes are HOST arrays of n_src / n_tgt node ids (copied
+ * during the call; ids may repeat and need not be sorted; every id must be a created node, else NC_ERR_INVALID_ARG);
+ * a NULL array means "use the range argument of that side".  Rule formulas and random draws are those of nc_connect
+ * with N_sources = n_src, N_targets = n_tgt and s0 = t0 = 0; the result indexes the arrays. ---- */
+int nc_connect_nodes(nc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, nc_range src,
+                     const uint32_t* tgt_nodes, uint32_t n_tgt, nc_range tgt, nc_rule rule,
+                     const nc_rule_params* params, const nc_syn_spec* syn, uint64_t seed);
+
 /* ---- calibration: stable sort by (source, delay), then the group index ---- */
 int nc_finalize(nc_context* ctx);
 

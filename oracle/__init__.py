@@ -202,8 +202,21 @@ class Oracle:
                    delay_ms=(1.0, 0.0, -math.inf, math.inf), seed=0) -> int:
         rp = _RuleParams(int(degree_or_total), float(p))
         sp = _syn(weight, delay_ms)
-        return int(lib().oc_connect(self._h, _Range(*src), _Range(*tgt), int(rule), C.byref(rp), C.byref(sp),
-                                    int(seed)))
+        if isinstance(src, tuple) and isinstance(tgt, tuple):
+            return int(lib().oc_connect(self._h, _Range(*src), _Range(*tgt), int(rule), C.byref(rp), C.byref(sp),
+                                        int(seed)))
+        # a side that is not a (first, count) tuple is an explicit array of node ids
+        sa = None if isinstance(src, tuple) else np.ascontiguousarray(src, dtype=np.uint32)
+        ta = None if isinstance(tgt, tuple) else np.ascontiguousarray(tgt, dtype=np.uint32)
+        L = lib()
+        L.oc_connect_nodes.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, _Range, C.c_void_p, C.c_uint32, _Range, C.c_int,
+                                       C.c_void_p, C.c_void_p, C.c_uint64]
+        L.oc_connect_nodes.restype = C.c_int
+        return int(L.oc_connect_nodes(self._h, None if sa is None else sa.ctypes.data_as(C.c_void_p),
+                                      0 if sa is None else sa.size, _Range(0, 0) if sa is not None else _Range(*src),
+                                      None if ta is None else ta.ctypes.data_as(C.c_void_p),
+                                      0 if ta is None else ta.size, _Range(0, 0) if ta is not None else _Range(*tgt),
+                                      int(rule), C.byref(rp), C.byref(sp), int(seed)))
 
     def connect(self, *a, **k):
         rc = self.connect_rc(*a, **k)

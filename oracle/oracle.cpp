@@ -244,12 +244,14 @@ int oc_create_population(oc_context* ctx, uint32_t n, uint32_t* first_id) {
   return OC_OK;
 }
 
-int oc_connect(oc_context* ctx, oc_range src, oc_range tgt, int rule, const oc_rule_params* params,
-               const oc_syn_spec* syn, uint64_t seed) {
+/* node_space: the size of the index space the two ranges must fit in (the node count, or -- for explicit node
+ * arrays, PAPER.md:117 -- the array lengths, because the formulas then produce array indexes). */
+static int connect_core(oc_context* ctx, uint64_t node_space, oc_range src, oc_range tgt, int rule,
+                        const oc_rule_params* params, const oc_syn_spec* syn, uint64_t seed) {
   if (!ctx) return OC_ERR_INVALID_ARG;
   if (ctx->finalized) return OC_ERR_STATE;
   uint64_t n_iter = 0;
-  int rc = validate(ctx->n_nodes, src, tgt, rule, params, syn, ctx->inv_dt, &n_iter);
+  int rc = validate((uint32_t)std::min<uint64_t>(node_space, 0xffffffffull), src, tgt, rule, params, syn, ctx->inv_dt, &n_iter);
   if (rc != OC_OK) return rc;
 
   Projection pr{src, tgt, rule, *params, *syn, seed, ctx->n_projections};
@@ -301,6 +303,40 @@ int oc_connect(oc_context* ctx, oc_range src, oc_range tgt, int rule, const oc_r
   ctx->n_blocks += n_newblocks;
   ctx->n_projections += 1;
   ctx->have_in = ctx->have_out = false;
+  return OC_OK;
+}
+
+int oc_connect(oc_context* ctx, oc_range src, oc_range tgt, int rule, const oc_rule_params* params,
+               const oc_syn_spec* syn, uint64_t seed) {
+  if (!ctx) return OC_ERR_INVALID_ARG;
+  return connect_core(ctx, ctx->n_nodes, src, tgt, rule, params, syn, seed);
+}
+
+/* "If the indexes of source or target nodes are not consecutive but are explicitly given by an array,
+ * the above formulas are used to derive the indexes of the array elements from which to extract the node indexes."
+ * So: run the rule over the index ranges 0..n_src-1 / 0..n_tgt-1 (s0 = t0 = 0), then look every result up. */
+int oc_connect_nodes(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, oc_range src,
+                     const uint32_t* tgt_nodes, uint32_t n_tgt, oc_range tgt, int rule, const oc_rule_params* params,
+                     const oc_syn_spec* syn, uint64_t seed) {
+  if (!ctx) return OC_ERR_INVALID_ARG;
+  if (ctx->finalized) return OC_ERR_STATE;
+  for (uint32_t k = 0; src_nodes && k < n_src; ++k)
+    if (src_nodes[k] >= ctx->n_nodes) return OC_ERR_INVALID_ARG;
+  for (uint32_t k = 0; tgt_nodes && k < n_tgt; ++k)
+    if (tgt_nodes[k] >= ctx->n_nodes) return OC_ERR_INVALID_ARG;
+  if (src_nodes) src = oc_range{0u, n_src};
+  if (tgt_nodes) tgt = oc_range{0u, n_tgt};
+  if ((!src_nodes && (uint64_t)src.first + src.count > ctx->n_nodes) ||
+      (!tgt_nodes && (uint64_t)tgt.first + tgt.count > ctx->n_nodes))
+    return OC_ERR_INVALID_ARG;
+  const uint64_t space = std::max<uint64_t>(ctx->n_nodes, std::max<uint64_t>(src_nodes ? n_src : 0, tgt_nodes ? n_tgt : 0));
+  const size_t before = ctx->src.size();
+  int rc = connect_core(ctx, space, src, tgt, rule, params, syn, seed);
+  if (rc != OC_OK) return rc;
+  for (size_t j = before; j < ctx->src.size(); ++j) {
+    if (src_nodes) ctx->src[j] = src_nodes[ctx->src[j]];
+    if (tgt_nodes) ctx->tgt[j] = tgt_nodes[ctx->tgt[j]];
+  }
   return OC_OK;
 }
 

@@ -97,6 +97,10 @@ int oc_destroy(oc_context* ctx);
 int oc_create_population(oc_context* ctx, uint32_t n, uint32_t* first_id);
 int oc_connect(oc_context* ctx, oc_range src, oc_range tgt, int rule, const oc_rule_params* params,
                const oc_syn_spec* syn, uint64_t seed);
+/* explicit node arrays: HOST arrays of n_src / n_tgt node ids; NULL = use the range of that side */
+int oc_connect_nodes(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, oc_range src,
+                     const uint32_t* tgt_nodes, uint32_t n_tgt, oc_range tgt, int rule, const oc_rule_params* params,
+                     const oc_syn_spec* syn, uint64_t seed);
 int oc_finalize(oc_context* ctx);
 int oc_num_connections(oc_context* ctx, uint64_t* n);
 int oc_num_nodes(oc_context* ctx, uint32_t* n);

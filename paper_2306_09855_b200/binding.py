@@ -27,6 +27,7 @@ SYMBOLS = (
     "nc_finalize", "nc_num_connections", "nc_num_nodes", "nc_get_connections", "nc_get_index",
     "nc_degree_histogram", "nc_get_stats", "nc_get_timings", "nc_read_connections", "nc_read_index",
     "nc_read_degree_histogram", "nc_selftest_philox", "nc_selftest_fastpath",
+    "nc_connect_nodes",
     # include/nc_delivery.h
     "nc_delivery_create", "nc_delivery_destroy", "nc_delivery_step", "nc_delivery_read_spike_array",
     "nc_delivery_counts",
@@ -120,6 +121,7 @@ def load_library():
     L.nc_read_degree_histogram.argtypes = [vp, C.c_int, vp, P(C.c_uint32)]
     L.nc_selftest_philox.argtypes = [vp, C.c_uint32, vp, vp, vp]
     L.nc_selftest_fastpath.argtypes = [vp, P(C.c_double)]
+    L.nc_connect_nodes.argtypes = [vp, vp, C.c_uint32, Range, vp, C.c_uint32, Range, C.c_int, vp, vp, C.c_uint64]
     L.nc_delivery_create.argtypes = [vp, C.c_uint32, P(vp)]
     L.nc_delivery_destroy.argtypes = [vp]
     L.nc_delivery_step.argtypes = [vp, vp, vp, C.c_uint32, vp]
@@ -242,7 +244,15 @@ class NC:
                    delay_ms=(1.0, 0.0, -math.inf, math.inf), seed=0) -> int:
         rp = RuleParams(int(degree_or_total), float(p))
         sp = SynSpec(Dist(*map(float, weight)), Dist(*map(float, delay_ms)))
-        return int(self._L.nc_connect(self._h, Range(*src), Range(*tgt), int(rule), C.byref(rp), C.byref(sp), int(seed)))
+        if isinstance(src, tuple) and isinstance(tgt, tuple):
+            return int(self._L.nc_connect(self._h, Range(*src), Range(*tgt), int(rule), C.byref(rp), C.byref(sp), int(seed)))
+        # a side that is not a (first, count) tuple is an explicit host array of node ids (nc_connect_nodes)
+        sa = None if isinstance(src, tuple) else np.ascontiguousarray(src, dtype=np.uint32)
+        ta = None if isinstance(tgt, tuple) else np.ascontiguousarray(tgt, dtype=np.uint32)
+        return int(self._L.nc_connect_nodes(self._h, _ptr(sa), 0 if sa is None else sa.size,
+                                            Range(0, 0) if sa is not None else Range(*src), _ptr(ta),
+                                            0 if ta is None else ta.size, Range(0, 0) if ta is not None else Range(*tgt),
+                                            int(rule), C.byref(rp), C.byref(sp), int(seed)))
 
     def connect(self, *a, **k):
         self._check(self.connect_rc(*a, **k))

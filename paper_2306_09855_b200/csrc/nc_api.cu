@@ -315,8 +315,8 @@ bool use_pdl() {
   return on;
 }
 
-template <int RULE>
-cudaError_t launch_generate(nc_context* c, const GenParams& p) {
+template <int RULE, bool ARR>
+cudaError_t launch_generate_as(nc_context* c, const GenParams& p) {
   const uint64_t first_tile = p.pos0 / kGenTile;
   const uint64_t last_tile = (p.pos0 + p.n - 1) / kGenTile;
   cudaLaunchConfig_t cfg{};
@@ -329,7 +329,12 @@ cudaError_t launch_generate(nc_context* c, const GenParams& p) {
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = use_pdl() ? 1 : 0;
-  return cudaLaunchKernelEx(&cfg, generate_kernel<RULE>, p);
+  return cudaLaunchKernelEx(&cfg, generate_kernel<RULE, ARR>, p);
+}
+
+template <int RULE>
+cudaError_t launch_generate(nc_context* c, const GenParams& p) {
+  return (p.src_nodes || p.tgt_nodes) ? launch_generate_as<RULE, true>(c, p) : launch_generate_as<RULE, false>(c, p);
 }
 
 int device_scan(nc_context* c, const uint32_t* in, uint32_t* out, uint64_t n, uint32_t* partial, uint64_t* total) {
@@ -410,9 +415,7 @@ int connect_bernoulli(nc_context* c, GenParams gp, double p, uint32_t seed_lo, u
 
 PassPlan plan_passes(uint32_t key_bits) {
   PassPlan pl{};
-  int digit_bits = kRadixBits;
-  if (const char* e = getenv("NC_EXP_DIGIT_BITS")) digit_bits = std::max(1, std::min((int)kRadixBits, atoi(e)));  // timing experiments
-  pl.n_passes = (key_bits + digit_bits - 1) / digit_bits;
+  pl.n_passes = (key_bits + kRadixBits - 1) / kRadixBits;
   uint32_t left = key_bits, shift = 0;
   for (uint32_t i = 0; i < pl.n_passes; ++i) {
     const uint32_t b = (left + (pl.n_passes - i) - 1) / (pl.n_passes - i);  // spread evenly, <= 8
@@ -1028,14 +1031,22 @@ int nc_create_population(nc_context* c, uint32_t n, uint32_t* first_id) {
   return NC_OK;
 }
 
-int nc_connect(nc_context* c, nc_range src, nc_range tgt, nc_rule rule, const nc_rule_params* params,
-               const nc_syn_spec* syn, uint64_t seed) {
+// src_nodes / tgt_nodes: HOST arrays of src.count / tgt.count node ids, or NULL for the consecutive range
+static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, const uint32_t* tgt_nodes, nc_range tgt,
+                        nc_rule rule, const nc_rule_params* params, const nc_syn_spec* syn, uint64_t seed) {
   if (!c) return NC_ERR_INVALID_ARG;
   if (c->finalized) return fail(c, NC_ERR_STATE, "nc_connect after nc_finalize");
   if (!params || !syn) return fail(c, NC_ERR_INVALID_ARG, "nc_connect: null params");
   if (src.count == 0 || tgt.count == 0) return fail(c, NC_ERR_INVALID_ARG, "nc_connect: empty node range");
-  if ((uint64_t)src.first + src.count > c->n_nodes || (uint64_t)tgt.first + tgt.count > c->n_nodes)
+  if (src_nodes) src.first = 0;
+  if (tgt_nodes) tgt.first = 0;
+  if ((!src_nodes && (uint64_t)src.first + src.count > c->n_nodes) ||
+      (!tgt_nodes && (uint64_t)tgt.first + tgt.count > c->n_nodes))
     return fail(c, NC_ERR_INVALID_ARG, "nc_connect: node range outside the created nodes");
+  for (uint32_t k = 0; src_nodes && k < src.count; ++k)
+    if (src_nodes[k] >= c->n_nodes) return fail(c, NC_ERR_INVALID_ARG, "nc_connect_nodes: source id outside the created nodes");
+  for (uint32_t k = 0; tgt_nodes && k < tgt.count; ++k)
+    if (tgt_nodes[k] >= c->n_nodes) return fail(c, NC_ERR_INVALID_ARG, "nc_connect_nodes: target id outside the created nodes");
   if (!dist_ok(syn->weight) || !dist_ok(syn->delay_ms))
     return fail(c, NC_ERR_INVALID_ARG, "nc_connect: bad distribution (sd < 0, lo > hi or NaN)");
   const uint64_t K = params->degree_or_total;
@@ -1084,6 +1095,17 @@ int nc_connect(nc_context* c, nc_range src, nc_range tgt, nc_rule rule, const nc
   const uint32_t seed_lo = (uint32_t)(seed & 0xffffffffull), seed_hi = (uint32_t)(seed >> 32);
   gp.rng = make_philox_stream(seed_lo, seed_hi, c->n_proj, 0u);  // D2: synapse stream
   gp.syn = make_syn(c, *syn);
+  // explicit node arrays: copied into library-owned device memory, released once the stream has been synchronised
+  for (int side = 0; side < 2; ++side) {
+    const uint32_t* host = side == 0 ? src_nodes : tgt_nodes;
+    if (!host) continue;
+    const size_t bytes = (size_t)(side == 0 ? src.count : tgt.count) * sizeof(uint32_t);
+    uint32_t* dev = (uint32_t*)dev_alloc(c, bytes);
+    if (!dev) return fail(c, NC_ERR_OOM, "out of device memory for a node array");
+    dev_free_later(c, dev);
+    NC_CUDA(c, cudaMemcpyAsync(dev, host, bytes, cudaMemcpyHostToDevice, c->stream));
+    (side == 0 ? gp.src_nodes : gp.tgt_nodes) = dev;
+  }
 
   if (rule == NC_PAIRWISE_BERNOULLI) {
     int rc = connect_bernoulli(c, gp, params->p, seed_lo, seed_hi);
@@ -1111,6 +1133,19 @@ int nc_connect(nc_context* c, nc_range src, nc_range tgt, nc_rule rule, const nc
   if (bound > (double)c->max_delay_steps) c->max_delay_steps = (uint32_t)bound;
   c->have_in = c->have_out = false;
   return NC_OK;
+}
+
+int nc_connect(nc_context* c, nc_range src, nc_range tgt, nc_rule rule, const nc_rule_params* params,
+               const nc_syn_spec* syn, uint64_t seed) {
+  return connect_impl(c, nullptr, src, nullptr, tgt, rule, params, syn, seed);
+}
+
+int nc_connect_nodes(nc_context* c, const uint32_t* src_nodes, uint32_t n_src, nc_range src, const uint32_t* tgt_nodes,
+                     uint32_t n_tgt, nc_range tgt, nc_rule rule, const nc_rule_params* params, const nc_syn_spec* syn,
+                     uint64_t seed) {
+  if (src_nodes) src = nc_range{0u, n_src};
+  if (tgt_nodes) tgt = nc_range{0u, n_tgt};
+  return connect_impl(c, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed);
 }
 
 int nc_finalize(nc_context* c) {

@@ -39,6 +39,10 @@ struct GenParams {
   uint64_t pos0;  // N_conns before this call: first creation position written
   uint64_t n;     // N_newconns (Eq. 2)
   uint32_t s0, n_src, t0, n_tgt;
+  // explicit node arrays ("the above formulas are used to derive the indexes of the array elements
+  // from which to extract the node indexes"): when set, s0 / t0 are 0 and the formula's result indexes the array
+  const uint32_t* src_nodes;
+  const uint32_t* tgt_nodes;
   uint32_t K;          // in/out-degree for the fixed-degree rules
   uint32_t div;        // divisor of the deterministic coordinate (N_tgt for all_to_all, K for fixed degree)
   uint64_t div_magic;  // floor(2^64 / div) + 1
@@ -208,7 +212,13 @@ __device__ __noinline__ void redo_fp64(const GenParams& p, uint32_t i, uint64_t 
   *d_ptr(p.map, a) = (uint16_t)st;
 }
 
-template <int RULE>
+__device__ __forceinline__ void map_nodes(const GenParams& p, uint32_t& s, uint32_t& t) {
+  if (p.src_nodes) s = __ldg(p.src_nodes + s);
+  if (p.tgt_nodes) t = __ldg(p.tgt_nodes + t);
+}
+
+// ARR: the projection names its sources and/or targets by explicit node arrays (kept out of the range kernels)
+template <int RULE, bool ARR>
 __global__ void __launch_bounds__(kGenThreads) generate_kernel(const __grid_constant__ GenParams p) {
   pdl_launch_dependents();
   const uint64_t end = p.pos0 + p.n;
@@ -236,6 +246,7 @@ __global__ void __launch_bounds__(kGenThreads) generate_kernel(const __grid_cons
       for (int e = 0; e < 4; ++e) {
         const Philox4 rnd = philox_stream<true>(i0 + e, 0u, p.rng);
         rule_coords<RULE>(p, i0 + e, quo, rem, rnd.x, rnd.y, src[e], tgt[e]);
+        if (ARR) map_nodes(p, src[e], tgt[e]);
         if (RULE == kAllToAll || RULE == kFixedIndegree || RULE == kFixedOutdegree) {
           if (++rem == p.div) {
             rem = 0;
@@ -276,6 +287,7 @@ __global__ void __launch_bounds__(kGenThreads) generate_kernel(const __grid_cons
       split_index<RULE>(p, i, quo, rem);
       const Philox4 rnd = philox_stream<true>(i, 0u, p.rng);
       rule_coords<RULE>(p, i, quo, rem, rnd.x, rnd.y, s, t);
+      if (ARR) map_nodes(p, s, t);
       draw_weight_delay(rnd.z, rnd.w, p.syn, wgt, dly);
       const BlockAddr a = locate(p.map, pos);
       *src_ptr(p.map, a) = s;
@@ -410,8 +422,10 @@ __global__ void __launch_bounds__(kBernThreads) bernoulli_write_kernel(const __g
     uint32_t dly;
     draw_weight_delay(rnd.z, rnd.w, p.g.syn, wgt, dly);
     const BlockAddr a = locate(p.g.map, out0 + k);
-    *src_ptr(p.g.map, a) = p.g.s0 + (uint32_t)row0 + dq;
-    *tgt_ptr(p.g.map, a) = p.g.t0 + col;
+    uint32_t s = p.g.s0 + (uint32_t)row0 + dq, t = p.g.t0 + col;
+    map_nodes(p.g, s, t);
+    *src_ptr(p.g.map, a) = s;
+    *tgt_ptr(p.g.map, a) = t;
     *w_ptr(p.g.map, a) = wgt;
     *d_ptr(p.g.map, a) = (uint16_t)dly;
   }

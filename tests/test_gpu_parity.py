@@ -424,3 +424,40 @@ def test_full_size_config4_large_bernoulli(nc_mod, oracle_mod):
     assert _check_sampled_synapses(g, net, firsts, oracle_mod, starts) > 50  # the fixed_outdegree projection
     _check_organised_chunked(g, n, net.n_nodes)
     g.close()
+
+
+def test_explicit_node_arrays_parity(nc_mod, oracle_mod):
+    """nc_connect_nodes: sources and/or targets given as arrays of node ids (unsorted, repeated ids,
+    longer than a tile), every rule, mixed with range projections -- bit-exact against the oracle including the
+    organised arrays and the index."""
+    rng = np.random.default_rng(17)
+    n_nodes = 3000
+    src_ids = rng.choice(n_nodes, size=700, replace=False).astype(np.uint32)
+    tgt_ids = rng.integers(0, n_nodes, size=900).astype(np.uint32)  # with repeats
+    calls = [
+        (src_ids, tgt_ids, "fixed_total_number", dict(degree_or_total=300_000)),
+        ((100, 500), tgt_ids, "fixed_indegree", dict(degree_or_total=37)),
+        (src_ids, (0, 3000), "fixed_outdegree", dict(degree_or_total=41)),
+        (src_ids[:300], tgt_ids[:300], "one_to_one", {}),
+        (src_ids[:64], tgt_ids[:100], "all_to_all", {}),
+        (src_ids, tgt_ids, "pairwise_bernoulli", dict(p=0.05)),
+        ((0, 3000), (0, 3000), "fixed_total_number", dict(degree_or_total=50_000)),
+    ]
+    o, g = oracle_mod.Oracle(dt_ms=0.1), nc_mod.NC(dt_ms=0.1)
+    for b in (o, g):
+        b.create_population(n_nodes)
+        for s, t, rule, kw in calls:
+            b.connect(s, t, WL.RULE_IDS[rule], weight=W, delay_ms=D, seed=23, **kw)
+        b.finalize()
+    rep = PU.compare_connections(g.read_connections(sorted=False), o.connections(sorted=False), 22.0, "node arrays, creation order")
+    assert rep["n"] > 400_000 and rep["delay_mismatches"] == 0
+    PU.compare_connections(g.read_connections(sorted=True), o.connections(sorted=True), 22.0, "node arrays, sorted")
+    PU.compare_index(g.read_index(), o.index(), "node arrays")
+    # bad ids are rejected with the oracle's code and leave the context usable
+    g2, o2 = nc_mod.NC(), oracle_mod.Oracle()
+    for b in (g2, o2):
+        b.create_population(10)
+        assert b.connect_rc(np.array([1, 10]), (0, 10), WL.RULE_IDS["all_to_all"]) == nc_mod.ERR_INVALID_ARG
+        assert b.connect_rc(np.array([1, 2, 3]), np.array([4, 5]), WL.RULE_IDS["one_to_one"]) == nc_mod.ERR_INVALID_ARG
+        assert b.num_connections() == 0
+    g.close(); o.close(); g2.close(); o2.close()
