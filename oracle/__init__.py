@@ -33,13 +33,14 @@ OK, ERR_INVALID_ARG, ERR_STATE, ERR_CAPACITY, ERR_OOM = 0, -1, -2, -3, -4
 
 
 def build(force: bool = False) -> Path:
-    """Compile oracle.cpp + delivery.cpp -> liboracle.so (g++ -O2 -ffp-contract=off)."""
-    srcs = [_HERE / "oracle.cpp", _HERE / "oracle.h", _HERE / "delivery.cpp", _HERE / "delivery.h"]
+    """Compile oracle.cpp + delivery.cpp + copass.cpp -> liboracle.so (g++ -O2 -ffp-contract=off)."""
+    srcs = [_HERE / "oracle.cpp", _HERE / "oracle.h", _HERE / "delivery.cpp", _HERE / "delivery.h",
+            _HERE / "copass.cpp", _HERE / "copass.h"]
     if not force and _LIB_PATH.exists() and all(_LIB_PATH.stat().st_mtime >= s.stat().st_mtime for s in srcs):
         return _LIB_PATH
     tmp = _LIB_PATH.with_suffix(f".so.tmp{os.getpid()}")
     cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-Wall", "-Wextra",
-           "-o", str(tmp), str(_HERE / "oracle.cpp"), str(_HERE / "delivery.cpp")]
+           "-o", str(tmp), str(_HERE / "oracle.cpp"), str(_HERE / "delivery.cpp"), str(_HERE / "copass.cpp")]
     subprocess.run(cmd, check=True)
     os.replace(tmp, _LIB_PATH)
     return _LIB_PATH
@@ -341,3 +342,56 @@ class Delivery:
             self.close()
         except Exception:
             pass
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# COPASS block-sort (copass.h)
+# ---------------------------------------------------------------------------------------------------------------
+class _CopassInfo(C.Structure):
+    _fields_ = [("t", C.c_int64), ("iterations", C.c_uint32), ("last_step", C.c_int32)]
+
+
+class _CopassStats(C.Structure):
+    _fields_ = [("aux_peak", C.c_uint64), ("moved", C.c_uint64), ("partitions", C.c_uint32),
+                ("iterations", C.c_uint32), ("last_step_1", C.c_uint32), ("last_step_2", C.c_uint32)]
+
+
+def copass_partition(keys, start, length, m):
+    """oc_copass_partition: keys int64 flat array, subarray i = keys[start[i] : start[i] + length[i]] ascending.
+    Returns (m_i uint64[k], t, iterations, last_step)."""
+    L = lib()
+    L.oc_copass_partition.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint64, C.c_void_p,
+                                      C.POINTER(_CopassInfo)]
+    keys = np.ascontiguousarray(keys, dtype=np.int64)
+    start = np.ascontiguousarray(start, dtype=np.uint64)
+    length = np.ascontiguousarray(length, dtype=np.uint64)
+    assert start.size == length.size
+    out = np.zeros(start.size, dtype=np.uint64)
+    info = _CopassInfo()
+    rc = L.oc_copass_partition(keys.ctypes.data_as(C.c_void_p), start.ctypes.data_as(C.c_void_p),
+                               length.ctypes.data_as(C.c_void_p), start.size, int(m),
+                               out.ctypes.data_as(C.c_void_p), C.byref(info))
+    if rc != 0:
+        raise OracleError(rc)
+    return out, info.t, info.iterations, info.last_step
+
+
+def copass_block_sort(keys, vals, sizes, max_extract=None):
+    """oc_copass_block_sort on copies of keys (int64) / vals (uint32); blocks of the given sizes lie one after the
+    other.  Returns (keys, vals, sub_start, sub_len, stats dict)."""
+    L = lib()
+    L.oc_copass_block_sort.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p,
+                                       C.c_void_p, C.POINTER(_CopassStats)]
+    keys = np.array(keys, dtype=np.int64)
+    vals = np.array(vals, dtype=np.uint32)
+    sizes = np.ascontiguousarray(sizes, dtype=np.uint64)
+    assert keys.size == vals.size == int(sizes.sum())
+    k = sizes.size
+    sub_start, sub_len = np.zeros(k, dtype=np.uint64), np.zeros(k, dtype=np.uint64)
+    st = _CopassStats()
+    rc = L.oc_copass_block_sort(keys.ctypes.data_as(C.c_void_p), vals.ctypes.data_as(C.c_void_p),
+                                sizes.ctypes.data_as(C.c_void_p), k, k if max_extract is None else int(max_extract),
+                                sub_start.ctypes.data_as(C.c_void_p), sub_len.ctypes.data_as(C.c_void_p), C.byref(st))
+    if rc != 0:
+        raise OracleError(rc)
+    return keys, vals, sub_start, sub_len, {f: getattr(st, f) for f, _ in _CopassStats._fields_}
