@@ -74,9 +74,15 @@ enum {
                                    and gather target/weight by the permutation afterwards, instead of carrying
                                    the whole connection through the digit passes; keys wider than 32 bits always
                                    take this path */
-  NC_FLAG_SORT_ONESWEEP = 1u << 3 /* carry the whole connection, but chain the tiles of a digit pass inside the
+  NC_FLAG_SORT_ONESWEEP = 1u << 3, /* carry the whole connection, but chain the tiles of a digit pass inside the
                                    pass (decoupled look-back) instead of the default count / scan / scatter
                                    kernels per pass */
+  NC_FLAG_ORGANISE_COPASS = 1u << 4 /* organise the connections INSIDE their storage blocks with the COPASS block-sort
+                                   of PAPER.md:426-642 (Appendix A): auxiliary memory of a few blocks instead of two
+                                   more copies of all connections.  The organised view then keeps the block structure
+                                   (see nc_connections_view) and the creation-order view is gone after nc_finalize.
+                                   Needs a (source, delay) key of <= 32 bits and <= 4096 blocks (NC_ERR_CAPACITY).
+                                   See include/nc_copass.h. */
 };
 
 typedef struct {
@@ -118,7 +124,11 @@ typedef struct {
  *              blocks is a HOST array of n_blocks device base pointers; inside a block the four arrays
  *              start at byte offsets off_source/off_target/off_weight/off_delay.  Creation position pos
  *              is entry pos % block_size of block pos / block_size (D9).  The flat pointers are NULL
- *              unless n_blocks == 1, in which case they point into that single block. */
+ *              unless n_blocks == 1, in which case they point into that single block.
+ *  sorted = 1 under NC_FLAG_ORGANISE_COPASS: the organised connections stay in the storage blocks: sorted position j
+ *              is entry j % block_size of block j / block_size, the view is filled as for sorted = 0 plus
+ *              off_perm (creation positions), and sorted = 0 is NC_ERR_STATE after nc_finalize (the blocks were
+ *              sorted in place). */
 typedef struct {
   const uint32_t* source;
   const uint32_t* target;
@@ -130,6 +140,7 @@ typedef struct {
   uint64_t n_blocks;
   void* const* blocks;
   uint64_t off_source, off_target, off_weight, off_delay;
+  uint64_t off_perm; /* only under NC_FLAG_ORGANISE_COPASS with sorted = 1, else 0 */
 } nc_connections_view;
 
 /* Index over the sorted connections (D11).  All device pointers.
@@ -155,7 +166,8 @@ typedef enum {
   NC_PHASE_PERMUTE = 3,  /* materialise sorted source/target/weight/delay */
   NC_PHASE_INDEX = 4,    /* head flags, scans, group compaction */
   NC_PHASE_DEGREE = 5,   /* nc_degree_histogram */
-  NC_PHASE_COUNT = 6
+  NC_PHASE_COPASS = 6,   /* COPASS organisation: partitions and the moves of Fig. 6 D-E */
+  NC_PHASE_COUNT = 7
 } nc_phase;
 
 typedef struct {

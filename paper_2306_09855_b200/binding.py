@@ -18,8 +18,8 @@ LIB_PATH = _HERE / "libnc.so"
 
 OK, ERR_INVALID_ARG, ERR_STATE, ERR_CAPACITY, ERR_OOM, ERR_CUDA = 0, -1, -2, -3, -4, -5
 ONE_TO_ONE, ALL_TO_ALL, FIXED_INDEGREE, FIXED_OUTDEGREE, FIXED_TOTAL_NUMBER, PAIRWISE_BERNOULLI = range(6)
-FLAG_TIMING, FLAG_EXACT_FP64, FLAG_SORT_PAIRS, FLAG_SORT_ONESWEEP = 1, 2, 4, 8
-PHASES = ("generate", "histogram", "sort", "permute", "index", "degree")
+FLAG_TIMING, FLAG_EXACT_FP64, FLAG_SORT_PAIRS, FLAG_SORT_ONESWEEP, FLAG_ORGANISE_COPASS = 1, 2, 4, 8, 16
+PHASES = ("generate", "histogram", "sort", "permute", "index", "degree", "copass")
 
 # every symbol include/nc.h declares (checked by tests/test_abi.py against the header and the library)
 SYMBOLS = (
@@ -31,6 +31,8 @@ SYMBOLS = (
     # include/nc_delivery.h
     "nc_delivery_create", "nc_delivery_destroy", "nc_delivery_step", "nc_delivery_read_spike_array",
     "nc_delivery_counts",
+    # include/nc_copass.h
+    "nc_copass_partition", "nc_get_copass_stats",
 )
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_void_p, C.c_size_t)
@@ -66,7 +68,7 @@ class ConnectionsView(C.Structure):
     _fields_ = [("source", C.c_void_p), ("target", C.c_void_p), ("weight", C.c_void_p), ("delay", C.c_void_p),
                 ("perm", C.c_void_p), ("n", C.c_uint64), ("block_size", C.c_uint64), ("n_blocks", C.c_uint64),
                 ("blocks", C.POINTER(C.c_void_p)), ("off_source", C.c_uint64), ("off_target", C.c_uint64),
-                ("off_weight", C.c_uint64), ("off_delay", C.c_uint64)]
+                ("off_weight", C.c_uint64), ("off_delay", C.c_uint64), ("off_perm", C.c_uint64)]
 
 
 class IndexView(C.Structure):
@@ -76,7 +78,7 @@ class IndexView(C.Structure):
 
 
 class Timings(C.Structure):
-    _fields_ = [("ms", C.c_double * 6), ("launches", C.c_uint32 * 6), ("sort_pass_ms", C.c_double),
+    _fields_ = [("ms", C.c_double * 7), ("launches", C.c_uint32 * 7), ("sort_pass_ms", C.c_double),
                 ("sort_passes", C.c_uint32)]
 
 
@@ -84,6 +86,15 @@ class Stats(C.Structure):
     _fields_ = [("kernel_launches", C.c_uint64), ("bytes_in_use", C.c_uint64), ("bytes_peak", C.c_uint64),
                 ("n_blocks", C.c_uint64), ("n_projections", C.c_uint32), ("key_bits", C.c_uint32),
                 ("sort_passes", C.c_uint32), ("delay_bits", C.c_uint32)]
+
+
+class CopassInfo(C.Structure):
+    _fields_ = [("t", C.c_uint32), ("iterations", C.c_uint32), ("last_step", C.c_int32)]
+
+
+class CopassStats(C.Structure):
+    _fields_ = [("partitions", C.c_uint32), ("iterations", C.c_uint32), ("last_step_1", C.c_uint32),
+                ("last_step_2", C.c_uint32), ("n_blocks", C.c_uint64), ("aux_bytes", C.c_uint64)]
 
 
 _lib = None
@@ -122,6 +133,8 @@ def load_library():
     L.nc_selftest_philox.argtypes = [vp, C.c_uint32, vp, vp, vp]
     L.nc_selftest_fastpath.argtypes = [vp, P(C.c_double)]
     L.nc_connect_nodes.argtypes = [vp, vp, C.c_uint32, Range, vp, C.c_uint32, Range, C.c_int, vp, vp, C.c_uint64]
+    L.nc_copass_partition.argtypes = [vp, vp, C.c_uint64, vp, vp, C.c_uint32, C.c_uint32, vp, P(CopassInfo)]
+    L.nc_get_copass_stats.argtypes = [vp, P(CopassStats)]
     L.nc_delivery_create.argtypes = [vp, C.c_uint32, P(vp)]
     L.nc_delivery_destroy.argtypes = [vp]
     L.nc_delivery_step.argtypes = [vp, vp, vp, C.c_uint32, vp]
@@ -325,6 +338,23 @@ class NC:
         mx = C.c_uint32()
         self._check(self._L.nc_read_degree_histogram(self._h, int(kind), _ptr(deg), C.byref(mx)))
         return deg, mx.value
+
+    # -- COPASS block-sort (include/nc_copass.h) --
+    def copass_partition(self, keys, start, length, m):
+        """nc_copass_partition on host arrays: returns (m_i uint32[k], t, iterations, last_step)."""
+        keys = np.ascontiguousarray(keys, dtype=np.uint32)
+        start = np.ascontiguousarray(start, dtype=np.uint32)
+        length = np.ascontiguousarray(length, dtype=np.uint32)
+        out = np.zeros(start.size, dtype=np.uint32)
+        info = CopassInfo()
+        self._check(self._L.nc_copass_partition(self._h, _ptr(keys), keys.size, _ptr(start), _ptr(length), start.size,
+                                                int(m), _ptr(out), C.byref(info)))
+        return out, info.t, info.iterations, info.last_step
+
+    def copass_stats(self) -> dict:
+        s = CopassStats()
+        self._check(self._L.nc_get_copass_stats(self._h, C.byref(s)))
+        return {f: getattr(s, f) for f, _ in CopassStats._fields_}
 
     # -- device self-tests --
     def selftest_philox(self, ctr: np.ndarray, key: np.ndarray) -> np.ndarray:

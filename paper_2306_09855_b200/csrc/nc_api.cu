@@ -19,6 +19,8 @@
 #include "nc_index.cuh"
 #include "nc_sort.cuh"
 #include "nc_sort_split.cuh"
+#include "nc_copass.cuh"
+#include "../../include/nc_copass.h"
 
 using namespace nc;
 
@@ -66,6 +68,10 @@ struct nc_context {
   uint64_t* d_table = nullptr;
   size_t table_cap = 0;
   uint64_t off_tgt = 0, off_w = 0, off_d = 0, block_bytes = 0;
+  uint64_t off_perm = 0;            // NC_FLAG_ORGANISE_COPASS: a fifth array per block (creation positions)
+  bool organised_in_blocks = false; // nc_finalize left the organised connections in the storage blocks
+  CopassTotals* d_copass_totals = nullptr;
+  uint64_t copass_aux_bytes = 0;
 
   // allocations
   std::unordered_map<void*, size_t> live;
@@ -805,6 +811,208 @@ int sort_split_and_index(nc_context* c, const PassPlan& plan) {
   return rc;
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// COPASS organisation (NC_FLAG_ORGANISE_COPASS; nc_copass.cuh): the connections are sorted inside
+// their storage blocks with auxiliary memory of a few blocks instead of two more copies of everything.
+// ---------------------------------------------------------------------------------------------------------------
+struct CopassScratch {
+  uint4* buf[2];   // intermediate records of the radix passes (one block each)
+  uint8_t* dig;    // next-pass digit per record
+  uint16_t* counts;
+  uint32_t* offs;
+  uint32_t* chunk;
+};
+
+// The underlying sort: stable radix passes over n <= B records.  Input: one storage block in its
+// creation-order layout (from_storage; map addresses it as block 0; pos_base = its first creation position) or an
+// array of records.  Output: n records at `out`.
+int copass_sort_records(nc_context* c, const PassPlan& plan, const CopassScratch& sc, bool from_storage,
+                        const BlockMap& map, uint32_t pos_base, const uint4* in, uint32_t n, uint4* out) {
+  const uint32_t kTile = (uint32_t)kSplitShapes[0].warps * 32u * (uint32_t)kSplitShapes[0].items;
+  const uint32_t n_tiles = (n + kTile - 1) / kTile;
+  const uint32_t n_chunks = (n_tiles + kScanChunkTiles - 1) / kScanChunkTiles;
+  const uint32_t P = plan.n_passes;
+  const uint4* cur_in = in;
+  for (uint32_t ps = 0; ps < P; ++ps) {
+    const bool storage = from_storage && ps == 0, last = ps + 1 == P;
+    {
+      Scope scp(c, NC_PHASE_HISTOGRAM);
+      if (storage) {
+        if (c->B % 4 == 0)
+          tile_count_first_kernel<true><<<n_tiles, kCountThreads, 0, c->stream>>>(map, n, kTile, c->delay_bits,
+                                                                                plan.shift[0], plan.bits[0], sc.counts);
+        else
+          tile_count_first_kernel<false><<<n_tiles, kCountThreads, 0, c->stream>>>(map, n, kTile, c->delay_bits,
+                                                                                 plan.shift[0], plan.bits[0], sc.counts);
+      } else if (ps == 0) {
+        tile_count_recs_kernel<<<n_tiles, kCountThreads, 0, c->stream>>>(in, n, kTile, plan.shift[0], plan.bits[0],
+                                                                        sc.counts);
+      } else {
+        tile_count_bytes_kernel<<<(n_tiles + kCountTilesPerCta - 1) / kCountTilesPerCta, kCountThreads, 0, c->stream>>>(
+            sc.dig, n, kTile, n_tiles, sc.counts);
+      }
+      NC_LAUNCH_CHECK(c, "tile_count");
+      chunk_total_kernel<<<n_chunks, kRadix, 0, c->stream>>>(sc.counts, n_tiles, sc.chunk);
+      NC_LAUNCH_CHECK(c, "chunk_total");
+      chunk_scan_kernel<<<1, kRadix * kChunkScanSegs, 0, c->stream>>>(sc.chunk, n_chunks);
+      NC_LAUNCH_CHECK(c, "chunk_scan");
+      tile_offsets_kernel<<<n_chunks, kRadix, 0, c->stream>>>(sc.counts, n_tiles, sc.chunk, sc.offs);
+      NC_LAUNCH_CHECK(c, "tile_offsets");
+    }
+    {
+      Scope scp(c, NC_PHASE_SORT);
+      Scope pass_sc(c, NC_PHASE_SORT, true);
+      ScatterParams sp{};
+      sp.map = map;
+      sp.delay_bits = c->delay_bits;
+      sp.n = n;
+      sp.pos_base = pos_base;
+      sp.recs_in = storage ? nullptr : cur_in;
+      sp.recs_out = last ? out : sc.buf[ps & 1];
+      sp.dig_out = sc.dig;
+      sp.shift = plan.shift[ps];
+      sp.bits = plan.bits[ps];
+      sp.next_shift = last ? 0 : plan.shift[ps + 1];
+      sp.next_bits = last ? 0 : plan.bits[ps + 1];
+      sp.offs = sc.offs;
+      const int rc = storage ? launch_scatter_pass<true, false>(c, sp, n_tiles, 0)
+                             : launch_scatter_pass<false, false>(c, sp, n_tiles, 0);
+      if (rc != NC_OK) return rc;
+      cur_in = sp.recs_out;
+    }
+  }
+  return NC_OK;
+}
+
+int organise_copass(nc_context* c, const PassPlan& plan) {
+  const uint32_t n = (uint32_t)c->n_conns;
+  const uint64_t B = c->B;
+  const uint32_t k = (uint32_t)c->blocks.size();
+  if (k > kCopassMaxBlocks)
+    return fail(c, NC_ERR_CAPACITY, "COPASS organisation handles at most 4096 storage blocks: raise block_size");
+  const uint32_t big = (uint32_t)std::min<uint64_t>(B, n);  // the largest block (Eq. A3)
+  const uint32_t kTile = (uint32_t)kSplitShapes[0].warps * 32u * (uint32_t)kSplitShapes[0].items;
+  const uint32_t max_tiles = (big + kTile - 1) / kTile;
+  const uint32_t max_chunks = (max_tiles + kScanChunkTiles - 1) / kScanChunkTiles;
+  auto block_n = [&](uint32_t b) { return (uint32_t)std::min<uint64_t>(B, (uint64_t)n - (uint64_t)b * B); };
+
+  const uint64_t bytes_before = c->bytes_in_use;
+  void* spare = dev_alloc(c, c->block_bytes);                       // the free block of Fig. 6E
+  uint4* aux = k > 1 ? (uint4*)dev_alloc(c, (size_t)big * 16) : nullptr;  // the auxiliary array (Eq. A3)
+  CopassScratch sc{};
+  sc.buf[0] = plan.n_passes > 1 ? (uint4*)dev_alloc(c, (size_t)big * 16) : nullptr;
+  sc.buf[1] = plan.n_passes > 2 ? (uint4*)dev_alloc(c, (size_t)big * 16) : nullptr;
+  sc.dig = (uint8_t*)dev_alloc(c, (size_t)big);
+  sc.counts = (uint16_t*)dev_alloc(c, (size_t)max_tiles * kRadix * 2);
+  sc.offs = (uint32_t*)dev_alloc(c, (size_t)max_tiles * kRadix * 4);
+  sc.chunk = (uint32_t*)dev_alloc(c, (size_t)max_chunks * kRadix * 4);
+  // partition state: two (start[k+1], len[k]) sets used in turn, m_i, left_prefix[k+1], right_src[k], what it did
+  const size_t k1 = (size_t)k + 1;
+  uint32_t* st = (uint32_t*)dev_alloc(c, (7 * k1) * 4 + sizeof(CopassInfo));
+  if (!c->d_copass_totals) c->d_copass_totals = (CopassTotals*)dev_alloc(c, sizeof(CopassTotals));
+  auto drop = [&]() {
+    dev_free_later(c, spare); dev_free_later(c, aux); dev_free_later(c, sc.buf[0]); dev_free_later(c, sc.buf[1]);
+    dev_free_later(c, sc.dig); dev_free_later(c, sc.counts); dev_free_later(c, sc.offs); dev_free_later(c, sc.chunk);
+    dev_free_later(c, st);
+  };
+  bool ok = spare && sc.dig && sc.counts && sc.offs && sc.chunk && st && c->d_copass_totals && (k == 1 || aux);
+  if (plan.n_passes > 1) ok = ok && sc.buf[0];
+  if (plan.n_passes > 2) ok = ok && sc.buf[1];
+  if (!ok) {
+    drop();
+    return fail(c, NC_ERR_OOM, "out of device memory in nc_finalize (COPASS organisation)");
+  }
+  c->copass_aux_bytes = c->bytes_in_use - bytes_before;
+  NC_CUDA(c, cudaMemsetAsync(c->d_copass_totals, 0, sizeof(CopassTotals), c->stream));
+  uint32_t* start[2] = {st, st + 2 * k1};
+  uint32_t* len[2] = {st + k1, st + 3 * k1};
+  uint32_t* m_out = st + 4 * k1;
+  uint32_t* left_prefix = st + 5 * k1;
+  uint32_t* right_src = st + 6 * k1;
+  CopassInfo* info = (CopassInfo*)(st + 7 * k1);
+
+  // block b takes the place of the spare block (whose memory the caller has just filled) and becomes the spare
+  auto swap_with_spare = [&](uint32_t b) -> int {
+    std::swap(c->blocks[b], spare);
+    copass_poke_kernel<<<1, 1, 0, c->stream>>>(c->d_table, b, (uint64_t)c->blocks[b], 0xffffffffu, 0);
+    NC_LAUNCH_CHECK(c, "copass_poke");
+    return NC_OK;
+  };
+  const BlockMap map = make_map(c);
+  int rc;
+
+  // Fig. 6B: every block sorted on its own, creation-order layout -> records
+  for (uint32_t b = 0; b < k; ++b) {
+    BlockMap one = map;
+    one.table = c->d_table + b;
+    rc = copass_sort_records(c, plan, sc, true, one, (uint32_t)((uint64_t)b * B), nullptr, block_n(b), (uint4*)spare);
+    if (rc != NC_OK) return rc;
+    if ((rc = swap_with_spare(b)) != NC_OK) return rc;
+  }
+  if (k > 1) {
+    {
+      Scope scp(c, NC_PHASE_COPASS);
+      copass_init_subarrays_kernel<<<(k + 255) / 256, 256, 0, c->stream>>>(start[0], len[0], k, (uint32_t)B, n);
+      NC_LAUNCH_CHECK(c, "copass_init_subarrays");
+    }
+    const size_t part_smem = 7 * k1 * 4, gather_smem = (2 * k1) * 4;
+    auto part = copass_partition_kernel<RecKeys>;
+    NC_CUDA(c, cudaFuncSetAttribute(part, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)part_smem));
+    NC_CUDA(c, cudaFuncSetAttribute(copass_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gather_smem));
+    const uint32_t per_cta = kGatherThreads * kGatherItems;
+    int cur = 0;
+    for (uint32_t b = 0; b + 1 < k; ++b) {
+      const uint32_t N_b = (uint32_t)B;  // every block but the last is full
+      const uint32_t new_base = (uint32_t)((uint64_t)(b + 1) * B);
+      {
+        Scope scp(c, NC_PHASE_COPASS);
+        // Fig. 6C
+        part<<<1, kCopassThreads, part_smem, c->stream>>>(RecKeys{map}, k, N_b, start[cur], len[cur], new_base, m_out,
+                                                         left_prefix, right_src, start[1 - cur], len[1 - cur], info,
+                                                         c->d_copass_totals);
+        NC_LAUNCH_CHECK(c, "copass_partition");
+        // Fig. 6D
+        copass_gather_kernel<<<(N_b + per_cta - 1) / per_cta, kGatherThreads, gather_smem, c->stream>>>(
+            map, k, left_prefix, start[cur], 0u, N_b, aux);
+        NC_LAUNCH_CHECK(c, "copass_gather_left");
+        // Fig. 6E, last destination block first: everything a block receives lies at or before it
+        for (uint32_t j = k - 1; j > b; --j) {
+          const uint32_t cnt = block_n(j);
+          copass_gather_kernel<<<(cnt + per_cta - 1) / per_cta, kGatherThreads, gather_smem, c->stream>>>(
+              map, k, start[1 - cur], right_src, (uint32_t)((uint64_t)j * B), cnt, (uint4*)spare);
+          NC_LAUNCH_CHECK(c, "copass_shift");
+          if ((rc = swap_with_spare(j)) != NC_OK) return rc;
+        }
+      }
+      // Fig. 6F: the auxiliary array, sorted, into block b (all of whose old content has moved)
+      rc = copass_sort_records(c, plan, sc, false, map, 0, aux, N_b, (uint4*)c->blocks[b]);
+      if (rc != NC_OK) return rc;
+      cur = 1 - cur;
+    }
+    // the last block: what is left is its content (reading C5); its k ascending pieces are merged by the sort
+    rc = copass_sort_records(c, plan, sc, false, map, 0, (const uint4*)c->blocks[k - 1], block_n(k - 1), (uint4*)spare);
+    if (rc != NC_OK) return rc;
+    if ((rc = swap_with_spare(k - 1)) != NC_OK) return rc;
+  }
+  // records -> source / target / weight / delay / creation position arrays of the block
+  {
+    Scope scp(c, NC_PHASE_PERMUTE);
+    for (uint32_t b = 0; b < k; ++b) {
+      char* o = (char*)spare;
+      const uint32_t cnt = block_n(b);
+      copass_unpack_kernel<<<std::min<uint32_t>((cnt + 255) / 256, 148 * 16), 256, 0, c->stream>>>(
+          (const uint4*)c->blocks[b], cnt, c->delay_bits, (uint32_t*)o, (uint32_t*)(o + c->off_tgt),
+          (float*)(o + c->off_w), (uint16_t*)(o + c->off_d), (uint32_t*)(o + c->off_perm));
+      NC_LAUNCH_CHECK(c, "copass_unpack");
+      if ((rc = swap_with_spare(b)) != NC_OK) return rc;
+    }
+  }
+  c->organised_in_blocks = true;
+  rc = build_index_from_sorted(c, n, nullptr);
+  drop();
+  return rc;
+}
+
 // a12-a14 over the final source / delay arrays.
 int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) {
   const uint32_t N = c->n_nodes;
@@ -827,9 +1035,13 @@ int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) 
   const uint64_t bound = std::min<uint64_t>(n, (uint64_t)N * c->max_delay_steps);
   const bool presize = !lookback_flag && bound * 6 <= std::max<uint64_t>((uint64_t)n * 2, 1u << 20);
   const SoAKeys keys{c->s_src, c->s_d, 16u};
+  const BlockKeys block_keys{make_map(c), 16u};
   {
     Scope sc(c, NC_PHASE_INDEX);
-    head_count_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(keys, n, tile_heads);
+    if (c->organised_in_blocks)
+      head_count_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(block_keys, n, tile_heads);
+    else
+      head_count_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(keys, n, tile_heads);
     NC_LAUNCH_CHECK(c, "head_count");
     int rc = device_scan(c, tile_heads, tile_head_off, head_tiles, head_partial, c->d_total_groups);
     if (rc != NC_OK) return rc;
@@ -859,8 +1071,12 @@ int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) 
   {
     Scope sc(c, NC_PHASE_INDEX);
     IndexOut io{c->src_offsets, c->group_ptr, c->group_start, c->group_delay, N};
-    index_scatter_soa_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(c->s_src, c->s_d, n, tile_head_off,
-                                                                                    c->d_total_groups, io);
+    if (c->organised_in_blocks)
+      index_scatter_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(block_keys, n, tile_head_off,
+                                                                                  c->d_total_groups, io);
+    else
+      index_scatter_soa_kernel<<<(unsigned)head_tiles, kHeadThreads, 0, c->stream>>>(c->s_src, c->s_d, n, tile_head_off,
+                                                                                      c->d_total_groups, io);
     NC_LAUNCH_CHECK(c, "index_scatter");
     index_finish_kernel<<<(N + 255) / 256, 256, 0, c->stream>>>(c->src_offsets, c->group_ptr, N, c->out_degree,
                                                                c->group_count, c->d_max + 1);
@@ -985,6 +1201,12 @@ int nc_create(const nc_config* cfg, nc_context** out) {
   c->off_w = c->off_tgt + align_up(c->B * 4, 256);
   c->off_d = c->off_w + align_up(c->B * 4, 256);
   c->block_bytes = c->off_d + align_up(c->B * 2, 256);
+  if (cfg->flags & NC_FLAG_ORGANISE_COPASS) {
+    // a block must be able to hold its connections as five arrays (18 B each) and, while the block-sort runs,
+    // as 16-byte records
+    c->off_perm = c->block_bytes;
+    c->block_bytes = std::max(c->off_perm + align_up(c->B * 4, 256), align_up(c->B * 16, 256));
+  }
   c->d_max = (uint32_t*)dev_alloc(c, 8);
   if (!c->d_max) {
     delete c;
@@ -1179,7 +1401,11 @@ int nc_finalize(nc_context* c) {
     c->sort_passes = 0;
   } else {
     int rc;
-    if (c->key_bits > 32) rc = sort_and_index<uint64_t>(c, plan);
+    if (c->cfg.flags & NC_FLAG_ORGANISE_COPASS) {
+      if (c->key_bits > 32)
+        return fail(c, NC_ERR_CAPACITY, "COPASS organisation needs a (source, delay) key of at most 32 bits");
+      rc = organise_copass(c, plan);
+    } else if (c->key_bits > 32) rc = sort_and_index<uint64_t>(c, plan);
     else if (c->cfg.flags & NC_FLAG_SORT_PAIRS) rc = sort_and_index<uint32_t>(c, plan);
     else if (c->cfg.flags & NC_FLAG_SORT_ONESWEEP) rc = sort_carry_and_index(c, plan);
     else rc = sort_split_and_index(c, plan);
@@ -1207,14 +1433,20 @@ int nc_get_connections(nc_context* c, int sorted, nc_connections_view* out) {
   std::memset(out, 0, sizeof(*out));
   out->n = c->n_conns;
   out->block_size = c->B;
-  if (sorted) {
-    if (!c->finalized) return fail(c, NC_ERR_STATE, "sorted view before nc_finalize");
+  if (sorted && !c->finalized) return fail(c, NC_ERR_STATE, "sorted view before nc_finalize");
+  if (!sorted && c->organised_in_blocks)
+    return fail(c, NC_ERR_STATE, "the creation-order view is gone: the blocks were organised in place (COPASS)");
+  if (sorted && !c->organised_in_blocks) {
     out->source = c->s_src;
     out->target = c->s_tgt;
     out->weight = c->s_w;
     out->delay = c->s_d;
     out->perm = c->perm;
     return NC_OK;
+  }
+  if (sorted) {
+    out->off_perm = c->off_perm;
+    if (c->blocks.size() == 1) out->perm = (const uint32_t*)((char*)c->blocks[0] + c->off_perm);
   }
   out->n_blocks = c->blocks.size();
   out->blocks = c->blocks.data();
@@ -1305,9 +1537,11 @@ int nc_read_connections(nc_context* c, int sorted, uint64_t first, uint64_t coun
   if (!c) return NC_ERR_INVALID_ARG;
   if (first + count > c->n_conns) return fail(c, NC_ERR_INVALID_ARG, "nc_read_connections: range outside the connections");
   if (sorted && !c->finalized) return fail(c, NC_ERR_STATE, "sorted view before nc_finalize");
+  if (!sorted && c->organised_in_blocks)
+    return fail(c, NC_ERR_STATE, "the creation-order view is gone: the blocks were organised in place (COPASS)");
   if (count == 0) return NC_OK;
   const cudaMemcpyKind k = cudaMemcpyDeviceToHost;
-  if (sorted) {
+  if (sorted && !c->organised_in_blocks) {
     if (source) NC_CUDA(c, cudaMemcpyAsync(source, c->s_src + first, count * 4, k, c->stream));
     if (target) NC_CUDA(c, cudaMemcpyAsync(target, c->s_tgt + first, count * 4, k, c->stream));
     if (weight) NC_CUDA(c, cudaMemcpyAsync(weight, c->s_w + first, count * 4, k, c->stream));
@@ -1323,6 +1557,7 @@ int nc_read_connections(nc_context* c, int sorted, uint64_t first, uint64_t coun
       if (target) NC_CUDA(c, cudaMemcpyAsync(target + done, (uint32_t*)(b + c->off_tgt) + slot, m * 4, k, c->stream));
       if (weight) NC_CUDA(c, cudaMemcpyAsync(weight + done, (float*)(b + c->off_w) + slot, m * 4, k, c->stream));
       if (delay) NC_CUDA(c, cudaMemcpyAsync(delay + done, (uint16_t*)(b + c->off_d) + slot, m * 2, k, c->stream));
+      if (perm && sorted) NC_CUDA(c, cudaMemcpyAsync(perm + done, (uint32_t*)(b + c->off_perm) + slot, m * 4, k, c->stream));
       pos += m;
       done += m;
     }
@@ -1353,6 +1588,75 @@ int nc_read_degree_histogram(nc_context* c, int kind, uint32_t* per_node_degree,
   if (per_node_degree && c->n_nodes)
     NC_CUDA(c, cudaMemcpyAsync(per_node_degree, dev, (size_t)c->n_nodes * 4, cudaMemcpyDeviceToHost, c->stream));
   return sync_stream(c);
+}
+
+int nc_copass_partition(nc_context* c, const uint32_t* keys, uint64_t n_keys, const uint32_t* start, const uint32_t* len,
+                        uint32_t k, uint32_t m, uint32_t* m_out, nc_copass_info* info) {
+  if (!c) return NC_ERR_INVALID_ARG;
+  if (!keys || !start || !len || !m_out || k == 0) return fail(c, NC_ERR_INVALID_ARG, "nc_copass_partition: NULL argument");
+  if (k > kCopassMaxBlocks) return fail(c, NC_ERR_CAPACITY, "nc_copass_partition: more than 4096 subarrays");
+  if (n_keys > 0xffffffffull) return fail(c, NC_ERR_CAPACITY, "nc_copass_partition: more than 2^32 - 1 keys");
+  uint64_t total = 0;
+  for (uint32_t i = 0; i < k; ++i) {
+    if ((uint64_t)start[i] + len[i] > n_keys) return fail(c, NC_ERR_INVALID_ARG, "nc_copass_partition: subarray outside keys");
+    total += len[i];
+  }
+  if (m == 0 || (uint64_t)m >= total)
+    return fail(c, NC_ERR_INVALID_ARG, "nc_copass_partition: 0 < m < sum of the subarray sizes is required (PAPER.md:464)");
+  const size_t k1 = (size_t)k + 1;
+  uint32_t* d_keys = (uint32_t*)dev_alloc(c, (size_t)n_keys * 4);
+  uint32_t* st = (uint32_t*)dev_alloc(c, 7 * k1 * 4 + sizeof(CopassInfo));
+  auto drop = [&]() {
+    dev_free_later(c, d_keys);
+    dev_free_later(c, st);
+  };
+  if (!d_keys || !st) {
+    drop();
+    return fail(c, NC_ERR_OOM, "out of device memory in nc_copass_partition");
+  }
+  uint32_t *d_start = st, *d_len = st + k1, *d_m = st + 2 * k1, *d_left = st + 3 * k1, *d_right = st + 4 * k1,
+           *d_new_start = st + 5 * k1, *d_new_len = st + 6 * k1;
+  CopassInfo* d_info = (CopassInfo*)(st + 7 * k1);
+  NC_CUDA(c, cudaMemcpyAsync(d_keys, keys, (size_t)n_keys * 4, cudaMemcpyHostToDevice, c->stream));
+  NC_CUDA(c, cudaMemcpyAsync(d_start, start, (size_t)k * 4, cudaMemcpyHostToDevice, c->stream));
+  NC_CUDA(c, cudaMemcpyAsync(d_len, len, (size_t)k * 4, cudaMemcpyHostToDevice, c->stream));
+  const size_t smem = 7 * k1 * 4;
+  auto part = copass_partition_kernel<FlatKeys>;
+  NC_CUDA(c, cudaFuncSetAttribute(part, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  part<<<1, kCopassThreads, smem, c->stream>>>(FlatKeys{d_keys}, k, m, d_start, d_len, 0u, d_m, d_left, d_right,
+                                              d_new_start, d_new_len, d_info, nullptr);
+  NC_LAUNCH_CHECK(c, "copass_partition");
+  CopassInfo h{};
+  NC_CUDA(c, cudaMemcpyAsync(m_out, d_m, (size_t)k * 4, cudaMemcpyDeviceToHost, c->stream));
+  NC_CUDA(c, cudaMemcpyAsync(&h, d_info, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+  drop();
+  const int rc = sync_stream(c);
+  if (rc != NC_OK) return rc;
+  if (info) {
+    info->t = h.t;
+    info->iterations = h.iterations;
+    info->last_step = h.last_step;
+  }
+  return NC_OK;
+}
+
+int nc_get_copass_stats(nc_context* c, nc_copass_stats* out) {
+  if (!c || !out) return NC_ERR_INVALID_ARG;
+  if (!c->finalized || !(c->cfg.flags & NC_FLAG_ORGANISE_COPASS))
+    return fail(c, NC_ERR_STATE, "nc_get_copass_stats: the context was not finalized under NC_FLAG_ORGANISE_COPASS");
+  CopassTotals t{};
+  if (c->d_copass_totals) {
+    NC_CUDA(c, cudaMemcpyAsync(&t, c->d_copass_totals, sizeof(t), cudaMemcpyDeviceToHost, c->stream));
+    const int rc = sync_stream(c);
+    if (rc != NC_OK) return rc;
+  }
+  out->partitions = t.partitions;
+  out->iterations = t.iterations;
+  out->last_step_1 = t.last_step_1;
+  out->last_step_2 = t.last_step_2;
+  out->n_blocks = c->blocks.size();
+  out->aux_bytes = c->copass_aux_bytes;
+  return NC_OK;
 }
 
 int nc_selftest_philox(nc_context* c, uint32_t n, const uint32_t* ctr, const uint32_t* key, uint32_t* out) {
@@ -1393,10 +1697,13 @@ int nc_selftest_fastpath(nc_context* c, double out[4]) {
 int nc_internal_organised_view(nc_context* c, nc_organised_view* out) {
   if (!c || !out) return NC_ERR_INVALID_ARG;
   if (!c->finalized) return fail(c, NC_ERR_STATE, "the connections are not organised yet (nc_finalize)");
+  if (c->organised_in_blocks && c->blocks.size() > 1)
+    return fail(c, NC_ERR_STATE, "spike delivery reads flat target / weight arrays: with COPASS organisation it needs "
+                                 "all connections in one block");
   int rc = ensure_total_groups(c);
   if (rc != NC_OK) return rc;
-  out->target = c->s_tgt;
-  out->weight = c->s_w;
+  out->target = c->organised_in_blocks ? (const uint32_t*)((char*)c->blocks[0] + c->off_tgt) : c->s_tgt;
+  out->weight = c->organised_in_blocks ? (const float*)((char*)c->blocks[0] + c->off_w) : c->s_w;
   out->group_ptr = c->group_ptr;
   out->group_start = c->group_start;
   out->group_delay = c->group_delay;

@@ -142,6 +142,39 @@ struct SoAKeys {
   }
 };
 
+// The organised connections inside their storage blocks (COPASS organisation, nc_copass.cuh): position j is entry
+// j % B of block j / B; source and delay arrays as in the creation-order layout.
+struct BlockKeys {
+  using KeyT = uint64_t;
+  BlockMap map;
+  uint32_t delay_bits;  // always 16
+  __device__ __forceinline__ uint64_t operator[](uint64_t j) const {
+    const BlockAddr a = locate(map, j);
+    return ((uint64_t)*src_ptr(map, a) << 16) | *d_ptr(map, a);
+  }
+  // base % 8 == 0; when B % 8 == 0 the eight positions sit in one block, 16-byte aligned
+  __device__ __forceinline__ void load8(uint64_t base, uint32_t n, uint64_t (&out)[8]) const {
+    if (base + 8 <= n && (map.B & 7) == 0) {
+      const BlockAddr a = locate(map, base);
+      const uint32_t* src = src_ptr(map, a);
+      const uint4 s0 = *reinterpret_cast<const uint4*>(src);
+      const uint4 s1 = *reinterpret_cast<const uint4*>(src + 4);
+      const uint4 d = *reinterpret_cast<const uint4*>(d_ptr(map, a));
+      out[0] = ((uint64_t)s0.x << 16) | (d.x & 0xffffu);
+      out[1] = ((uint64_t)s0.y << 16) | (d.x >> 16);
+      out[2] = ((uint64_t)s0.z << 16) | (d.y & 0xffffu);
+      out[3] = ((uint64_t)s0.w << 16) | (d.y >> 16);
+      out[4] = ((uint64_t)s1.x << 16) | (d.z & 0xffffu);
+      out[5] = ((uint64_t)s1.y << 16) | (d.z >> 16);
+      out[6] = ((uint64_t)s1.z << 16) | (d.w & 0xffffu);
+      out[7] = ((uint64_t)s1.w << 16) | (d.w >> 16);
+    } else {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) out[i] = base + i < n ? (*this)[base + i] : 0ull;
+    }
+  }
+};
+
 // The 8 keys of a thread plus the key just before them: from the lane below, or (lane 0) from memory.
 template <typename Keys>
 __device__ __forceinline__ void load_keys_and_prev(const Keys& keys, uint64_t base, uint32_t n,

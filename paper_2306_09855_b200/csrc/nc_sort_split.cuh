@@ -190,6 +190,7 @@ struct ScatterParams {
   BlockMap map;  // FIRST: records are built from the storage blocks
   uint32_t delay_bits;
   uint32_t n;
+  uint32_t pos_base;  // FIRST: creation position of the first record (0 unless one storage block is sorted on its own)
   const uint4* recs_in;
   uint4* recs_out;
   uint8_t* dig_out;  // !LAST: digit of the NEXT pass for every record written
@@ -260,7 +261,7 @@ __global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(cons
 #pragma unroll
       for (int i = 0; i < ITEMS; ++i) {
         rec[i].x = (s[i] << p.delay_bits) | d[i];
-        rec[i].y = (uint32_t)(tile0 + wbase + i * 32);
+        rec[i].y = p.pos_base + (uint32_t)(tile0 + wbase + i * 32);
       }
     } else {
 #pragma unroll
@@ -270,7 +271,7 @@ __global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(cons
           const BlockAddr a = locate(p.map, tile0 + e);
           const uint32_t s = *src_ptr(p.map, a);
           const uint32_t d = *d_ptr(p.map, a);
-          rec[i] = make_uint4((s << p.delay_bits) | d, (uint32_t)(tile0 + e), *tgt_ptr(p.map, a),
+          rec[i] = make_uint4((s << p.delay_bits) | d, p.pos_base + (uint32_t)(tile0 + e), *tgt_ptr(p.map, a),
                               __float_as_uint(*w_ptr(p.map, a)));
         } else {
           rec[i] = make_uint4(0xffffffffu, 0u, 0u, 0u);

@@ -1,0 +1,198 @@
+"""GPU parity of the COPASS block-sort (include/nc_copass.h): the partition kernel against the
+oracle's step-by-step partition (oracle/copass.cpp) on inputs with long runs of ties, empty subarrays and many
+subarrays; the in-place organisation (NC_FLAG_ORGANISE_COPASS) against the oracle's organised connections and index,
+element by element."""
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+from paper_2306_09855_b200 import workloads as WL
+from tests import parity_util as PU
+
+pytestmark = pytest.mark.gpu
+GOLDEN = Path(__file__).parent / "golden" / "copass_partition.txt"
+
+
+@pytest.fixture(scope="module")
+def nc_mod():
+    from paper_2306_09855_b200 import binding, build
+    build.build()
+    return binding
+
+
+def _flatten(subs):
+    lens = np.array([len(s) for s in subs], dtype=np.uint32)
+    start = np.concatenate([[0], np.cumsum(lens)[:-1]]).astype(np.uint32)
+    keys = np.concatenate([np.asarray(s, dtype=np.uint32) for s in subs])
+    return keys, start, lens
+
+
+def _both(g, oracle_mod, subs, m):
+    keys, start, lens = _flatten(subs)
+    got = g.copass_partition(keys, start, lens, m)
+    want = oracle_mod.copass_partition(keys.astype(np.int64), start, lens, m)
+    assert got[0].tolist() == want[0].astype(int).tolist(), (m, got, want)
+    assert got[1:] == want[1:], (m, got, want)  # threshold, iteration count, which last step
+    return got
+
+
+def test_partition_golden_cases_on_device(nc_mod, oracle_mod):
+    g = nc_mod.NC()
+    for line in [l for l in GOLDEN.read_text().splitlines() if l and not l.startswith("#")]:
+        name, subs, m, want, t, it, last = [f.strip() for f in line.split("|")]
+        subs = [[int(x) for x in s.split()] for s in subs.split(";")]
+        keys, start, lens = _flatten(subs)
+        m_i, got_t, got_it, got_last = g.copass_partition(keys, start, lens, int(m))
+        assert m_i.tolist() == [int(x) for x in want.split()], name
+        assert (got_t, got_it, got_last) == (int(t), int(it), int(last)), name
+    g.close()
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_partition_matches_oracle_small_with_ties(nc_mod, oracle_mod, seed):
+    rng = np.random.default_rng(seed)
+    g = nc_mod.NC()
+    seen = set()
+    for _ in range(12):
+        k = int(rng.integers(1, 12))
+        span = int(rng.choice([2, 6, 60, 2**32 - 1]))
+        subs = [np.sort(rng.integers(0, span, size=int(rng.integers(0, 70)))) for _ in range(k)]
+        total = sum(len(s) for s in subs)
+        if total < 2:
+            continue
+        for m in sorted(set([1, total - 1] + rng.integers(1, total, size=4).tolist())):
+            seen.add(_both(g, oracle_mod, subs, m)[3])
+    assert seen == {1, 2}
+    g.close()
+
+
+def test_partition_matches_oracle_large(nc_mod, oracle_mod):
+    """Sizes at which every search takes several 32-ary steps; many subarrays (more than the CTA has warps, and
+    more than it has threads); keys at both ends of the 32-bit range."""
+    rng = np.random.default_rng(42)
+    g = nc_mod.NC()
+    # 40 subarrays of ~50,000 keys: (source << 6 | delay)-like keys with runs of equal keys
+    subs = [np.sort(rng.integers(0, 2**16, size=int(rng.integers(30000, 70000)))) for _ in range(40)]
+    total = sum(len(s) for s in subs)
+    for m in (1, 77, total // 3, total // 2 + 1, total - 1):
+        _both(g, oracle_mod, subs, m)
+    # 1500 and 4096 short subarrays, some of them empty
+    for k in (1500, 4096):
+        subs = [np.sort(rng.integers(0, 2**32 - 1, size=int(rng.integers(0, 40)))) for _ in range(k)]
+        subs[0] = np.array([0, 0, 2**32 - 1], dtype=np.uint64)
+        total = sum(len(s) for s in subs)
+        for m in (1, total // 2, total - 1):
+            _both(g, oracle_mod, subs, m)
+    # all keys equal: Sec. A4 in the first iteration, the d_i handed out lowest subarray first
+    subs = [np.full(1000, 7)] * 5
+    got = _both(g, oracle_mod, subs, 2500)
+    assert got[0].tolist() == [1000, 1000, 500, 0, 0] and got[3] == 2
+    g.close()
+
+
+def test_partition_argument_errors(nc_mod):
+    g = nc_mod.NC()
+    keys, start, lens = _flatten([[1, 2, 3], [4, 5]])
+    for m in (0, 5, 9):
+        with pytest.raises(nc_mod.NCError) as e:
+            g.copass_partition(keys, start, lens, m)
+        assert e.value.code == nc_mod.ERR_INVALID_ARG
+    with pytest.raises(nc_mod.NCError) as e:
+        g.copass_partition(keys, [0, 3], [3, 5], 2)  # second subarray runs past the keys
+    assert e.value.code == nc_mod.ERR_INVALID_ARG
+    g.close()
+
+
+def copass_parity(net, oracle_mod, nc_mod, B):
+    o = oracle_mod.Oracle(dt_ms=net.dt_ms, block_size=B)
+    WL.run(net, o, finalize=True)
+    g = nc_mod.NC(dt_ms=net.dt_ms, block_size=B, flags=nc_mod.FLAG_ORGANISE_COPASS)
+    WL.run(net, g, finalize=False)
+    scale = PU.weight_scale(net)
+    gu = g.read_connections(sorted=False)
+    rep = PU.compare_connections(gu, o.connections(sorted=False), scale, net.name + " creation order")
+    in_deg = g.read_degree_histogram(0)
+    g.finalize()
+    gs = g.read_connections(sorted=True)
+    if rep["delay_mismatches"] == 0:
+        PU.compare_connections(gs, o.connections(sorted=True), scale, net.name + " organised in place")
+        PU.compare_index(g.read_index(), o.index(), net.name)
+    else:  # a boundary delay moved by one step: the order is the stable sort of the device's own keys
+        key = (gu["source"].astype(np.uint64) << np.uint64(16)) | gu["delay"].astype(np.uint64)
+        perm = np.argsort(key, kind="stable").astype(np.uint32)
+        assert np.array_equal(gs["perm"], perm)
+        for f in ("source", "target", "weight", "delay"):
+            assert np.array_equal(gs[f], gu[f][perm]), f
+    # the blocks were sorted in place: the creation-order view is gone, the block structure is kept
+    with pytest.raises(nc_mod.NCError) as e:
+        g.read_connections(sorted=False)
+    assert e.value.code == nc_mod.ERR_STATE
+    st = g.copass_stats()
+    n = rep["n"]
+    block = B if B else 1 << 24
+    k = (n + block - 1) // block
+    assert st["n_blocks"] == k == o.num_blocks()
+    assert st["partitions"] == max(k - 1, 0) == st["last_step_1"] + st["last_step_2"]
+    v = g.get_connections(sorted=True)
+    assert v.n_blocks == k and v.block_size == block and v.off_perm > v.off_delay
+    # degree histograms still count over the blocks
+    od, om = o.degree_histogram(0)
+    assert np.array_equal(in_deg[0], od) and in_deg[1] == om
+    gd, gm = g.read_degree_histogram(0)
+    assert np.array_equal(gd, od) and gm == om
+    gd, gm = g.read_degree_histogram(1)
+    od, om = o.degree_histogram(1)
+    assert np.array_equal(gd, od) and gm == om
+    g.close()
+    return rep, st
+
+
+@pytest.mark.parametrize("B", [0, 1, 7, 10, 64, 250, 999, 1000])
+def test_copass_config0_tiny(nc_mod, oracle_mod, B):
+    rep, st = copass_parity(WL.config0_tiny(), oracle_mod, nc_mod, B)
+    assert rep["n"] == 1000
+
+
+@pytest.mark.parametrize("rule,scale,B", [("one_to_one", 1.0, 1000), ("all_to_all", 0.15, 300_000),
+                                          ("fixed_indegree", 0.3, 100_000), ("fixed_outdegree", 0.25, 131_072),
+                                          ("fixed_total_number", 0.3, 250_001), ("pairwise_bernoulli", 0.4, 65_536)])
+def test_copass_config1_rules(nc_mod, oracle_mod, rule, scale, B):
+    """Several sort tiles per block, a ragged last block, block sizes that are and are not powers of two."""
+    net = WL.config1_rule(rule, scale=scale)
+    rep, st = copass_parity(net, oracle_mod, nc_mod, B)
+    print(net.name, rep, st)
+    assert st["n_blocks"] >= 3
+
+
+def test_copass_microcircuit_scaled(nc_mod, oracle_mod):
+    """configs[2] at 10 % of the populations, ~3e6 connections in 12 blocks of 2^18."""
+    net = WL.config2_microcircuit(scale=0.1)
+    rep, st = copass_parity(net, oracle_mod, nc_mod, 1 << 18)
+    print(rep, st)
+    assert st["n_blocks"] >= 10 and st["iterations"] >= st["partitions"]
+
+
+def test_copass_uses_a_few_blocks_of_auxiliary_memory(nc_mod):
+    """The point of the algorithm: the organisation step holds a few blocks, not copies of all
+    connections.  2e6 connections in blocks of 2^16: the default path's scratch is > 50 B per connection."""
+    net = WL.config1_rule("fixed_total_number", scale=0.2)
+    B = 1 << 16
+    g = nc_mod.NC(dt_ms=net.dt_ms, block_size=B, flags=nc_mod.FLAG_ORGANISE_COPASS)
+    WL.run(net, g, finalize=True)
+    st = g.copass_stats()
+    n = g.num_connections()
+    assert st["n_blocks"] == (n + B - 1) // B >= 20
+    assert st["aux_bytes"] <= 80 * B + (1 << 20)   # 18 (spare) + 16 (aux) + 33 (sort scratch) B per entry of ONE block
+    assert st["aux_bytes"] < 0.1 * 50 * n
+    g.close()
+
+
+def test_copass_delivery_needs_one_block(nc_mod, oracle_mod):
+    net = WL.config0_tiny()
+    g = nc_mod.NC(dt_ms=net.dt_ms, block_size=100, flags=nc_mod.FLAG_ORGANISE_COPASS)
+    WL.run(net, g, finalize=True)
+    with pytest.raises(nc_mod.NCError) as e:
+        nc_mod.Delivery(g, 64)
+    assert e.value.code == nc_mod.ERR_STATE
+    g.close()
