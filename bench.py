@@ -98,9 +98,12 @@ class ClockSampler(threading.Thread):
                 "reasons": sorted(self.reasons), "samples": len(self.samples)}
 
 
+BLOCK_SIZE = 0  # --block-size: connections per storage block (0 = the library's default 2^24)
+
+
 def one_step(binding, WL, net, flags):
     """The public API call sequence a user makes.  Returns the (still open) context."""
-    g = binding.NC(dt_ms=net.dt_ms, flags=flags)
+    g = binding.NC(dt_ms=net.dt_ms, flags=flags, block_size=BLOCK_SIZE)
     WL.run(net, g)
     return g
 
@@ -213,8 +216,12 @@ def main():
     ap.add_argument("--workload", default="c2")
     ap.add_argument("--sample-scale", type=float, default=0.0, help="cpu baseline sample: population scale of configs[2]")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--flags", type=int, default=0, help="extra NC_FLAG_* bits (e.g. 4 = sort (key, position) pairs + gather)")
+    ap.add_argument("--flags", type=int, default=0, help="extra NC_FLAG_* bits (e.g. 4 = sort (key, position) pairs + gather; "
+                    "16 = COPASS organisation inside the storage blocks)")
+    ap.add_argument("--block-size", type=int, default=0, help="connections per storage block B (0 = 2^24)")
     args = ap.parse_args()
+    global BLOCK_SIZE
+    BLOCK_SIZE = args.block_size
     if args.impl == "reference":
         return run_reference(args)
     if args.workload.startswith("delivery"):
@@ -304,7 +311,17 @@ def main():
     passes = max(1, int(round(per.get("sort_passes", 0))))
     pass_ms = per["sort_pass_ms"] / passes if per.get("sort_pass_ms") else None
     roof = None
-    if pass_ms:
+    copass = bool(flags & binding.FLAG_ORGANISE_COPASS)
+    if copass and per.get("sort_pass_ms"):
+        # every record goes through the digit passes twice: when its block is sorted, and in the auxiliary array
+        P = max(1, int(stats.get("sort_passes") or 1))
+        ach = BYTES["sort_pass"] * 2 * P * n_syn / (per["sort_pass_ms"] * 1e-3) / 1e9
+        roof = {"bound": "hbm", "kernel": "scatter_pass_kernel over one block at a time (COPASS organisation: 2 x "
+                                          f"{P} digit passes per connection, 16 B read + 16 B written each)",
+                "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                "peak_kind": peak_kind, "launch_ms": pass_ms, "launches_per_step": passes}
+        passes = 2 * P
+    elif pass_ms:
         ach = BYTES["sort_pass"] * n_syn / (pass_ms * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": "scatter_pass_kernel (one digit pass carrying the whole connection: 16 B read + "
                                           "16 B written per synapse)",
@@ -321,6 +338,16 @@ def main():
             phases[name] = {"ms": round(ms, 4), "alg_bytes_per_synapse": b, "GBps": round(gbs, 1),
                             "frac_of_measured_peak": round(gbs / peak, 4), "frac_of_8TBps": round(gbs / 8000.0, 4)}
 
+    if per.get("copass_ms", 0.0) > 0:
+        # COPASS organisation (Fig. 6 D-E): per output block the left partitions (B records) and every
+        # record still to the right of it are copied once, 16 B read + 16 B written each
+        Bk = args.block_size or (1 << 24)
+        kb = (n_syn + Bk - 1) // Bk
+        moved = sum(Bk + (n_syn - (b + 1) * Bk) for b in range(kb - 1))
+        gbs = 32 * moved / (per["copass_ms"] * 1e-3) / 1e9
+        phases["copass_moves"] = {"ms": round(per["copass_ms"], 4), "records_moved": moved, "blocks": kb,
+                                  "alg_bytes_per_record_moved": 32, "GBps": round(gbs, 1),
+                                  "frac_of_measured_peak": round(gbs / peak, 4)}
     cpu = None
     if not args.no_cpu_baseline and args.workload.startswith("c2"):
         scale = args.sample_scale if args.sample_scale else 0.5
@@ -338,7 +365,8 @@ def main():
                    if args.workload == "c2" else net.name,
                    "synapses_per_step": n_syn, "parallelism": "replicas only (one independent network per GPU)",
                    "l2": "every step regenerates and re-sorts its own 4.2 GB of connections (>> 126 MB L2); no input is reused",
-                   "key_bits": stats.get("key_bits"), "sort_passes": stats.get("sort_passes"), "flags": flags},
+                   "key_bits": stats.get("key_bits"), "sort_passes": stats.get("sort_passes"), "flags": flags,
+                   "block_size": args.block_size or (1 << 24), "device_bytes_peak": stats.get("bytes_peak")},
         "clocks": clocks, "gpu_launches": launches,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "what": "wall clock of nc_create + populations + all nc_connect + nc_finalize + nc_read_index into host buffers"},

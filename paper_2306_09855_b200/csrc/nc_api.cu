@@ -815,6 +815,7 @@ int sort_split_and_index(nc_context* c, const PassPlan& plan) {
 // COPASS organisation (NC_FLAG_ORGANISE_COPASS; nc_copass.cuh): the connections are sorted inside
 // their storage blocks with auxiliary memory of a few blocks instead of two more copies of everything.
 // ---------------------------------------------------------------------------------------------------------------
+constexpr uint32_t kCopassChunkTiles = 16;  // tiles per scan chunk: a block has few thousand tiles, keep the chunks short
 struct CopassScratch {
   uint4* buf[2];   // intermediate records of the radix passes (one block each)
   uint8_t* dig;    // next-pass digit per record
@@ -827,10 +828,11 @@ struct CopassScratch {
 // creation-order layout (from_storage; map addresses it as block 0; pos_base = its first creation position) or an
 // array of records.  Output: n records at `out`.
 int copass_sort_records(nc_context* c, const PassPlan& plan, const CopassScratch& sc, bool from_storage,
-                        const BlockMap& map, uint32_t pos_base, const uint4* in, uint32_t n, uint4* out) {
+                        const BlockMap& map, uint32_t pos_base, const uint4* in, uint32_t n, uint4* out,
+                        bool have_first_digits = false) {
   const uint32_t kTile = (uint32_t)kSplitShapes[0].warps * 32u * (uint32_t)kSplitShapes[0].items;
   const uint32_t n_tiles = (n + kTile - 1) / kTile;
-  const uint32_t n_chunks = (n_tiles + kScanChunkTiles - 1) / kScanChunkTiles;
+  const uint32_t n_chunks = (n_tiles + kCopassChunkTiles - 1) / kCopassChunkTiles;
   const uint32_t P = plan.n_passes;
   const uint4* cur_in = in;
   for (uint32_t ps = 0; ps < P; ++ps) {
@@ -844,7 +846,7 @@ int copass_sort_records(nc_context* c, const PassPlan& plan, const CopassScratch
         else
           tile_count_first_kernel<false><<<n_tiles, kCountThreads, 0, c->stream>>>(map, n, kTile, c->delay_bits,
                                                                                  plan.shift[0], plan.bits[0], sc.counts);
-      } else if (ps == 0) {
+      } else if (ps == 0 && !have_first_digits) {
         tile_count_recs_kernel<<<n_tiles, kCountThreads, 0, c->stream>>>(in, n, kTile, plan.shift[0], plan.bits[0],
                                                                         sc.counts);
       } else {
@@ -852,11 +854,11 @@ int copass_sort_records(nc_context* c, const PassPlan& plan, const CopassScratch
             sc.dig, n, kTile, n_tiles, sc.counts);
       }
       NC_LAUNCH_CHECK(c, "tile_count");
-      chunk_total_kernel<<<n_chunks, kRadix, 0, c->stream>>>(sc.counts, n_tiles, sc.chunk);
+      chunk_total_kernel<<<n_chunks, kRadix, 0, c->stream>>>(sc.counts, n_tiles, sc.chunk, kCopassChunkTiles);
       NC_LAUNCH_CHECK(c, "chunk_total");
       chunk_scan_kernel<<<1, kRadix * kChunkScanSegs, 0, c->stream>>>(sc.chunk, n_chunks);
       NC_LAUNCH_CHECK(c, "chunk_scan");
-      tile_offsets_kernel<<<n_chunks, kRadix, 0, c->stream>>>(sc.counts, n_tiles, sc.chunk, sc.offs);
+      tile_offsets_kernel<<<n_chunks, kRadix, 0, c->stream>>>(sc.counts, n_tiles, sc.chunk, sc.offs, kCopassChunkTiles);
       NC_LAUNCH_CHECK(c, "tile_offsets");
     }
     {
@@ -893,7 +895,7 @@ int organise_copass(nc_context* c, const PassPlan& plan) {
   const uint32_t big = (uint32_t)std::min<uint64_t>(B, n);  // the largest block (Eq. A3)
   const uint32_t kTile = (uint32_t)kSplitShapes[0].warps * 32u * (uint32_t)kSplitShapes[0].items;
   const uint32_t max_tiles = (big + kTile - 1) / kTile;
-  const uint32_t max_chunks = (max_tiles + kScanChunkTiles - 1) / kScanChunkTiles;
+  const uint32_t max_chunks = (max_tiles + kCopassChunkTiles - 1) / kCopassChunkTiles;
   auto block_n = [&](uint32_t b) { return (uint32_t)std::min<uint64_t>(B, (uint64_t)n - (uint64_t)b * B); };
 
   const uint64_t bytes_before = c->bytes_in_use;
@@ -973,19 +975,19 @@ int organise_copass(nc_context* c, const PassPlan& plan) {
         NC_LAUNCH_CHECK(c, "copass_partition");
         // Fig. 6D
         copass_gather_kernel<<<(N_b + per_cta - 1) / per_cta, kGatherThreads, gather_smem, c->stream>>>(
-            map, k, left_prefix, start[cur], 0u, N_b, aux);
+            map, k, left_prefix, start[cur], 0u, N_b, aux, sc.dig, plan.shift[0], (1u << plan.bits[0]) - 1u);
         NC_LAUNCH_CHECK(c, "copass_gather_left");
         // Fig. 6E, last destination block first: everything a block receives lies at or before it
         for (uint32_t j = k - 1; j > b; --j) {
           const uint32_t cnt = block_n(j);
           copass_gather_kernel<<<(cnt + per_cta - 1) / per_cta, kGatherThreads, gather_smem, c->stream>>>(
-              map, k, start[1 - cur], right_src, (uint32_t)((uint64_t)j * B), cnt, (uint4*)spare);
+              map, k, start[1 - cur], right_src, (uint32_t)((uint64_t)j * B), cnt, (uint4*)spare, nullptr, 0u, 0u);
           NC_LAUNCH_CHECK(c, "copass_shift");
           if ((rc = swap_with_spare(j)) != NC_OK) return rc;
         }
       }
       // Fig. 6F: the auxiliary array, sorted, into block b (all of whose old content has moved)
-      rc = copass_sort_records(c, plan, sc, false, map, 0, aux, N_b, (uint4*)c->blocks[b]);
+      rc = copass_sort_records(c, plan, sc, false, map, 0, aux, N_b, (uint4*)c->blocks[b], true);
       if (rc != NC_OK) return rc;
       cur = 1 - cur;
     }

@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(kCopassThreads) copass_partition_kernel(
 // position src_base[i] + (p - bound[i]).
 //   D: bound = left_prefix, src_base = the subarray starts, p0 = 0, count = N_b      -> out = auxiliary array
 //   E: bound = new_start,   src_base = right_src, p0 = first position of a block     -> out = the spare block
-// 16 bytes per element in, 16 out.
+// 16 bytes per element in, 16 out (+ 1 for the digit side array in D).
 // ---------------------------------------------------------------------------------------------
 constexpr int kGatherThreads = 256;
 constexpr int kGatherItems = 4;
@@ -313,7 +313,9 @@ __global__ void __launch_bounds__(kGatherThreads) copass_gather_kernel(const __g
                                                                       const uint32_t* __restrict__ bound,
                                                                       const uint32_t* __restrict__ src_base,
                                                                       uint32_t p0, uint32_t count,
-                                                                      uint4* __restrict__ out) {
+                                                                      uint4* __restrict__ out,
+                                                                      uint8_t* __restrict__ dig_out, uint32_t dig_shift,
+                                                                      uint32_t dig_mask) {
   extern __shared__ uint32_t sh[];
   uint32_t* b = sh;            // k + 1
   uint32_t* s = sh + k + 1;    // k
@@ -339,7 +341,11 @@ __global__ void __launch_bounds__(kGatherThreads) copass_gather_kernel(const __g
   }
 #pragma unroll
   for (int q = 0; q < kGatherItems; ++q)
-    if (ok[q]) out[j0 + q * kGatherThreads] = v[q];
+    if (ok[q]) {
+      out[j0 + q * kGatherThreads] = v[q];
+      // D: the digit of the first radix pass over the auxiliary array, so that its tile counts read 1 B per record
+      if (dig_out) dig_out[j0 + q * kGatherThreads] = (uint8_t)((v[q].x >> dig_shift) & dig_mask);
+    }
 }
 
 // Digit counts of the first radix pass when the input is an array of records (the auxiliary array).

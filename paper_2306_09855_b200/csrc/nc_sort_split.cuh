@@ -115,12 +115,13 @@ __global__ void __launch_bounds__(kCountThreads) tile_count_bytes_kernel(const u
 // Exclusive scan of counts[tile][digit] in (digit, tile) order -> offs[tile][digit] = first output position
 // of the tile's run of that digit.  Tiles are grouped into chunks of kScanChunkTiles; thread = digit.
 // ---------------------------------------------------------------------------------------------
-constexpr int kScanChunkTiles = 128;
+constexpr uint32_t kScanChunkTiles = 128;  // default; a block-sized sort (nc_copass.cuh) uses shorter chunks
 
 __global__ void __launch_bounds__(kRadix) chunk_total_kernel(const uint16_t* __restrict__ counts, uint32_t n_tiles,
-                                                            uint32_t* __restrict__ chunk_tot) {
-  const uint32_t t0 = blockIdx.x * kScanChunkTiles;
-  const uint32_t t1 = min(t0 + (uint32_t)kScanChunkTiles, n_tiles);
+                                                            uint32_t* __restrict__ chunk_tot,
+                                                            uint32_t chunk_tiles = kScanChunkTiles) {
+  const uint32_t t0 = blockIdx.x * chunk_tiles;
+  const uint32_t t1 = min(t0 + chunk_tiles, n_tiles);
   uint32_t s = 0;
 #pragma unroll 8
   for (uint32_t t = t0; t < t1; ++t) s += counts[(uint64_t)t * kRadix + threadIdx.x];
@@ -171,9 +172,10 @@ __global__ void __launch_bounds__(kRadix * kChunkScanSegs) chunk_scan_kernel(uin
 
 __global__ void __launch_bounds__(kRadix) tile_offsets_kernel(const uint16_t* __restrict__ counts, uint32_t n_tiles,
                                                              const uint32_t* __restrict__ chunk_base,
-                                                             uint32_t* __restrict__ offs) {
-  const uint32_t t0 = blockIdx.x * kScanChunkTiles;
-  const uint32_t t1 = min(t0 + (uint32_t)kScanChunkTiles, n_tiles);
+                                                             uint32_t* __restrict__ offs,
+                                                             uint32_t chunk_tiles = kScanChunkTiles) {
+  const uint32_t t0 = blockIdx.x * chunk_tiles;
+  const uint32_t t1 = min(t0 + chunk_tiles, n_tiles);
   uint32_t run = chunk_base[(uint64_t)blockIdx.x * kRadix + threadIdx.x];
 #pragma unroll 8
   for (uint32_t t = t0; t < t1; ++t) {

@@ -196,3 +196,46 @@ def test_copass_delivery_needs_one_block(nc_mod, oracle_mod):
         nc_mod.Delivery(g, 64)
     assert e.value.code == nc_mod.ERR_STATE
     g.close()
+
+
+def test_copass_full_size_microcircuit(nc_mod):
+    """configs[2] at FULL size (298,880,970 connections, 18 blocks of 2^24) organised in place, in the configuration
+    `bench.py --flags 16` times.  The oracle cannot hold this network in seconds, so the organised blocks are checked
+    against the plain definitions (readings D10, D11) evaluated with numpy on the device's own creation-order arrays,
+    read before nc_finalize: permutation, order, stability, every gathered field, every index array."""
+    net = WL.config2_microcircuit()
+    g = nc_mod.NC(dt_ms=net.dt_ms, flags=nc_mod.FLAG_ORGANISE_COPASS)
+    WL.run(net, g, finalize=False)
+    n = g.num_connections()
+    assert n == 298_880_970
+    u = g.read_connections(sorted=False)
+    g.finalize()
+    st = g.copass_stats()
+    print(st, g.stats())
+    assert st["n_blocks"] == 18 and st["partitions"] == 17
+    assert st["aux_bytes"] < 80 * (1 << 24) + (1 << 22)
+    assert g.stats()["bytes_peak"] < 18 * n + st["aux_bytes"] + (1 << 28)   # never a second copy of the connections
+    s = g.read_connections(sorted=True)
+    perm = s["perm"]
+    seen = np.zeros(n, dtype=bool)
+    seen[perm] = True
+    assert seen.all(), "perm is not a permutation"
+    del seen
+    key = (s["source"].astype(np.uint64) << np.uint64(16)) | s["delay"].astype(np.uint64)
+    dk = key[1:] != key[:-1]
+    assert np.all(key[1:] >= key[:-1]), "not sorted by (source, delay)"
+    assert np.all(dk | (perm[1:] > perm[:-1])), "ties are not in creation order"
+    del key
+    for f in ("source", "target", "weight", "delay"):
+        assert np.array_equal(u[f][perm], s[f]), f
+    idx = g.read_index()
+    out_deg = np.bincount(s["source"], minlength=net.n_nodes)
+    assert np.array_equal(idx["src_offsets"], np.concatenate([[0], np.cumsum(out_deg)]).astype(np.uint32))
+    heads = np.concatenate([[0], np.flatnonzero(dk) + 1]).astype(np.uint32)
+    assert idx["total_groups"] == heads.size
+    assert np.array_equal(idx["group_start"], heads)
+    assert np.array_equal(idx["group_delay"], s["delay"][heads])
+    gcount = np.bincount(s["source"][heads], minlength=net.n_nodes).astype(np.uint32)
+    assert np.array_equal(idx["group_count"], gcount)
+    assert np.array_equal(idx["group_ptr"], np.concatenate([[0], np.cumsum(gcount)]).astype(np.uint32))
+    g.close()
