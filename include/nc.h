@@ -215,6 +215,20 @@ int nc_connect_nodes(nc_context* ctx, const uint32_t* src_nodes, uint32_t n_src,
                      const uint32_t* tgt_nodes, uint32_t n_tgt, nc_range tgt, nc_rule rule,
                      const nc_rule_params* params, const nc_syn_spec* syn, uint64_t seed);
 
+/* The same with per-connection values (weights and delays can "be specified for each connection by an
+ * array having a size equal to the number of connections").  weights[n_values] (fp32, stored as they are) and
+ * delays_ms[n_values] (fp64, in ms; converted like a drawn delay: times 1/dt, rounded half up, at least one step --
+ * readings D8, Q5) are HOST arrays, copied during the call; entry i belongs to connection i_newconns = i of the rule
+ * (Eq. 2).  Either may be NULL: that parameter then follows `syn`, as does nothing else -- sources, targets and the
+ * other parameter are exactly those nc_connect_nodes gives for the same arguments.  n_values must equal N_newconns of
+ * the rule, the delays must be finite and the weights not NaN (NC_ERR_INVALID_ARG), no delay may exceed 65535 steps
+ * (NC_ERR_CAPACITY); pairwise_bernoulli, whose count is not known beforehand, is rejected (NC_ERR_INVALID_ARG).
+ * src_nodes / tgt_nodes as in nc_connect_nodes (NULL = the range). ---- */
+int nc_connect_values(nc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, nc_range src,
+                      const uint32_t* tgt_nodes, uint32_t n_tgt, nc_range tgt, nc_rule rule,
+                      const nc_rule_params* params, const nc_syn_spec* syn, uint64_t seed, const float* weights,
+                      const double* delays_ms, uint64_t n_values);
+
 /* ---- calibration: stable sort by (source, delay), then the group index ---- */
 int nc_finalize(nc_context* ctx);
 

@@ -200,9 +200,27 @@ class Oracle:
         return first.value
 
     def connect_rc(self, src, tgt, rule, degree_or_total=0, p=0.0, weight=(1.0, 0.0, -math.inf, math.inf),
-                   delay_ms=(1.0, 0.0, -math.inf, math.inf), seed=0) -> int:
+                   delay_ms=(1.0, 0.0, -math.inf, math.inf), seed=0, weights=None, delays=None) -> int:
+        """weights / delays: per-connection value arrays (oc_connect_values); None = follow the
+        distributions."""
         rp = _RuleParams(int(degree_or_total), float(p))
         sp = _syn(weight, delay_ms)
+        if weights is not None or delays is not None:
+            sa = None if isinstance(src, tuple) else np.ascontiguousarray(src, dtype=np.uint32)
+            ta = None if isinstance(tgt, tuple) else np.ascontiguousarray(tgt, dtype=np.uint32)
+            wa = None if weights is None else np.ascontiguousarray(weights, dtype=np.float32)
+            da = None if delays is None else np.ascontiguousarray(delays, dtype=np.float64)
+            L = lib()
+            L.oc_connect_values.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, _Range, C.c_void_p, C.c_uint32, _Range,
+                                            C.c_int, C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p, C.c_void_p,
+                                            C.c_uint64]
+            L.oc_connect_values.restype = C.c_int
+            vp = lambda a: None if a is None else a.ctypes.data_as(C.c_void_p)
+            return int(L.oc_connect_values(self._h, vp(sa), 0 if sa is None else sa.size,
+                                           _Range(0, 0) if sa is not None else _Range(*src), vp(ta),
+                                           0 if ta is None else ta.size, _Range(0, 0) if ta is not None else _Range(*tgt),
+                                           int(rule), C.byref(rp), C.byref(sp), int(seed), vp(wa), vp(da),
+                                           (wa if wa is not None else da).size))
         if isinstance(src, tuple) and isinstance(tgt, tuple):
             return int(lib().oc_connect(self._h, _Range(*src), _Range(*tgt), int(rule), C.byref(rp), C.byref(sp),
                                         int(seed)))

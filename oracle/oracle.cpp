@@ -340,6 +340,48 @@ int oc_connect_nodes(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src,
   return OC_OK;
 }
 
+/* "Weights and delays can have identical values for all connections, or be specified for each
+ * connection by an array having a size equal to the number of connections, or be randomly distributed".  The array
+ * form: entry i belongs to connection i_newconns = i (Eq. 2); a NULL array leaves that parameter to `syn`.  The
+ * rule, its random draws and the other parameter are exactly those of oc_connect_nodes.  A given weight is stored
+ * as it is; a given delay in ms goes through reading D8 (times 1/dt, round half up, at least one step). */
+int oc_connect_values(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, oc_range src,
+                      const uint32_t* tgt_nodes, uint32_t n_tgt, oc_range tgt, int rule, const oc_rule_params* params,
+                      const oc_syn_spec* syn, uint64_t seed, const float* weights, const double* delays_ms,
+                      uint64_t n_values) {
+  if (!ctx) return OC_ERR_INVALID_ARG;
+  if (ctx->finalized) return OC_ERR_STATE;
+  if (!weights && !delays_ms) return OC_ERR_INVALID_ARG;
+  if (rule == OC_PAIRWISE_BERNOULLI) return OC_ERR_INVALID_ARG; /* its number of connections is not known beforehand */
+  for (uint64_t i = 0; weights && i < n_values; ++i)
+    if (std::isnan(weights[i])) return OC_ERR_INVALID_ARG;
+  for (uint64_t i = 0; delays_ms && i < n_values; ++i) {
+    if (!std::isfinite(delays_ms[i])) return OC_ERR_INVALID_ARG;
+    if (std::floor(delays_ms[i] * ctx->inv_dt + 0.5) > 65535.0) return OC_ERR_CAPACITY;
+  }
+  const size_t before = ctx->src.size();
+  const uint64_t blocks_before = ctx->n_blocks;
+  int rc = oc_connect_nodes(ctx, src_nodes, n_src, src, tgt_nodes, n_tgt, tgt, rule, params, syn, seed);
+  if (rc != OC_OK) return rc;
+  if (ctx->src.size() - before != n_values) { /* "an array having a size equal to the number of connections" */
+    ctx->src.resize(before); ctx->tgt.resize(before); ctx->w.resize(before); ctx->d.resize(before); ctx->bnd.resize(before);
+    ctx->n_blocks = blocks_before;
+    ctx->n_projections -= 1;
+    return OC_ERR_INVALID_ARG;
+  }
+  for (uint64_t i = 0; i < n_values; ++i) {
+    if (weights) ctx->w[before + i] = weights[i];
+    if (delays_ms) {
+      const double x = delays_ms[i] * ctx->inv_dt;
+      double steps = std::floor(x + 0.5);
+      if (steps < 1.0) steps = 1.0;
+      ctx->d[before + i] = (uint16_t)(int64_t)steps;
+      ctx->bnd[before + i] = std::fabs(x - std::floor(x) - 0.5) < 1e-9 ? 1 : 0;
+    }
+  }
+  return OC_OK;
+}
+
 int oc_num_connections(oc_context* ctx, uint64_t* n) {
   if (!ctx || !n) return OC_ERR_INVALID_ARG;
   *n = ctx->src.size();

@@ -101,6 +101,12 @@ int oc_connect(oc_context* ctx, oc_range src, oc_range tgt, int rule, const oc_r
 int oc_connect_nodes(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, oc_range src,
                      const uint32_t* tgt_nodes, uint32_t n_tgt, oc_range tgt, int rule, const oc_rule_params* params,
                      const oc_syn_spec* syn, uint64_t seed);
+/* per-connection value arrays: HOST arrays of n_values = N_newconns entries, either may be NULL (that
+ * parameter then follows syn); entry i belongs to connection i_newconns = i.  pairwise_bernoulli is rejected. */
+int oc_connect_values(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, oc_range src,
+                      const uint32_t* tgt_nodes, uint32_t n_tgt, oc_range tgt, int rule, const oc_rule_params* params,
+                      const oc_syn_spec* syn, uint64_t seed, const float* weights, const double* delays_ms,
+                      uint64_t n_values);
 int oc_finalize(oc_context* ctx);
 int oc_num_connections(oc_context* ctx, uint64_t* n);
 int oc_num_nodes(oc_context* ctx, uint32_t* n);

@@ -27,7 +27,7 @@ SYMBOLS = (
     "nc_finalize", "nc_num_connections", "nc_num_nodes", "nc_get_connections", "nc_get_index",
     "nc_degree_histogram", "nc_get_stats", "nc_get_timings", "nc_read_connections", "nc_read_index",
     "nc_read_degree_histogram", "nc_selftest_philox", "nc_selftest_fastpath",
-    "nc_connect_nodes",
+    "nc_connect_nodes", "nc_connect_values",
     # include/nc_delivery.h
     "nc_delivery_create", "nc_delivery_destroy", "nc_delivery_step", "nc_delivery_read_spike_array",
     "nc_delivery_counts",
@@ -135,6 +135,8 @@ def load_library():
     L.nc_connect_nodes.argtypes = [vp, vp, C.c_uint32, Range, vp, C.c_uint32, Range, C.c_int, vp, vp, C.c_uint64]
     L.nc_copass_partition.argtypes = [vp, vp, C.c_uint64, vp, vp, C.c_uint32, C.c_uint32, vp, P(CopassInfo)]
     L.nc_get_copass_stats.argtypes = [vp, P(CopassStats)]
+    L.nc_connect_values.argtypes = [vp, vp, C.c_uint32, Range, vp, C.c_uint32, Range, C.c_int, vp, vp, C.c_uint64, vp, vp,
+                                    C.c_uint64]
     L.nc_delivery_create.argtypes = [vp, C.c_uint32, P(vp)]
     L.nc_delivery_destroy.argtypes = [vp]
     L.nc_delivery_step.argtypes = [vp, vp, vp, C.c_uint32, vp]
@@ -254,9 +256,22 @@ class NC:
         return first.value
 
     def connect_rc(self, src, tgt, rule, degree_or_total=0, p=0.0, weight=(1.0, 0.0, -math.inf, math.inf),
-                   delay_ms=(1.0, 0.0, -math.inf, math.inf), seed=0) -> int:
+                   delay_ms=(1.0, 0.0, -math.inf, math.inf), seed=0, weights=None, delays=None) -> int:
+        """weights / delays: per-connection value arrays on the host (nc_connect_values); None = follow the
+        distributions."""
         rp = RuleParams(int(degree_or_total), float(p))
         sp = SynSpec(Dist(*map(float, weight)), Dist(*map(float, delay_ms)))
+        if weights is not None or delays is not None:
+            sa = None if isinstance(src, tuple) else np.ascontiguousarray(src, dtype=np.uint32)
+            ta = None if isinstance(tgt, tuple) else np.ascontiguousarray(tgt, dtype=np.uint32)
+            wa = None if weights is None else np.ascontiguousarray(weights, dtype=np.float32)
+            da = None if delays is None else np.ascontiguousarray(delays, dtype=np.float64)
+            return int(self._L.nc_connect_values(self._h, _ptr(sa), 0 if sa is None else sa.size,
+                                                 Range(0, 0) if sa is not None else Range(*src), _ptr(ta),
+                                                 0 if ta is None else ta.size,
+                                                 Range(0, 0) if ta is not None else Range(*tgt), int(rule), C.byref(rp),
+                                                 C.byref(sp), int(seed), _ptr(wa), _ptr(da),
+                                                 (wa if wa is not None else da).size))
         if isinstance(src, tuple) and isinstance(tgt, tuple):
             return int(self._L.nc_connect(self._h, Range(*src), Range(*tgt), int(rule), C.byref(rp), C.byref(sp), int(seed)))
         # a side that is not a (first, count) tuple is an explicit host array of node ids (nc_connect_nodes)

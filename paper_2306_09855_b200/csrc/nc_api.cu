@@ -1257,7 +1257,9 @@ int nc_create_population(nc_context* c, uint32_t n, uint32_t* first_id) {
 
 // src_nodes / tgt_nodes: HOST arrays of src.count / tgt.count node ids, or NULL for the consecutive range
 static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, const uint32_t* tgt_nodes, nc_range tgt,
-                        nc_rule rule, const nc_rule_params* params, const nc_syn_spec* syn, uint64_t seed) {
+                        nc_rule rule, const nc_rule_params* params, const nc_syn_spec* syn, uint64_t seed,
+                        const float* weights = nullptr, const double* delays_ms = nullptr, uint64_t n_values = 0,
+                        bool with_values = false) {
   if (!c) return NC_ERR_INVALID_ARG;
   if (c->finalized) return fail(c, NC_ERR_STATE, "nc_connect after nc_finalize");
   if (!params || !syn) return fail(c, NC_ERR_INVALID_ARG, "nc_connect: null params");
@@ -1301,8 +1303,23 @@ static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, 
       return fail(c, NC_ERR_INVALID_ARG, "unknown rule");
   }
   if (rule != NC_PAIRWISE_BERNOULLI && n_new > kMaxConns) return fail(c, NC_ERR_CAPACITY, "more than 2^32-1 connections");
-  const double bound = delay_bound_steps(syn->delay_ms, c->inv_dt);
+  double bound = delay_bound_steps(syn->delay_ms, c->inv_dt);
   if (bound > 65535.0) return fail(c, NC_ERR_CAPACITY, "delay can exceed 65535 steps");
+  if (with_values) {  // one value per connection
+    if (!weights && !delays_ms) return fail(c, NC_ERR_INVALID_ARG, "nc_connect_values: no value array given");
+    if (rule == NC_PAIRWISE_BERNOULLI)
+      return fail(c, NC_ERR_INVALID_ARG, "nc_connect_values: pairwise_bernoulli has no connection count known beforehand");
+    if (n_values != n_new)
+      return fail(c, NC_ERR_INVALID_ARG, "nc_connect_values: the arrays must have one entry per connection of the rule");
+    for (uint64_t i = 0; weights && i < n_values; ++i)
+      if (std::isnan(weights[i])) return fail(c, NC_ERR_INVALID_ARG, "nc_connect_values: NaN weight");
+    for (uint64_t i = 0; delays_ms && i < n_values; ++i) {
+      if (!std::isfinite(delays_ms[i])) return fail(c, NC_ERR_INVALID_ARG, "nc_connect_values: delay not finite");
+      const double steps = std::floor(delays_ms[i] * c->inv_dt + 0.5);
+      if (steps > 65535.0) return fail(c, NC_ERR_CAPACITY, "nc_connect_values: a delay exceeds 65535 steps");
+      if (steps > bound) bound = steps;  // the key's delay bits must hold it
+    }
+  }
   if (rule != NC_PAIRWISE_BERNOULLI && c->n_conns + n_new > kMaxConns)
     return fail(c, NC_ERR_CAPACITY, "more than 2^32-1 connections");
 
@@ -1351,6 +1368,18 @@ static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, 
       if (e != cudaSuccess) return fail(c, NC_ERR_CUDA, std::string("launch generate: ") + cudaGetErrorString(e));
       NC_LAUNCH_CHECK(c, "generate");
     }
+    if (with_values) {
+      float* d_w = weights ? (float*)dev_alloc(c, (size_t)n_new * 4) : nullptr;
+      double* d_d = delays_ms ? (double*)dev_alloc(c, (size_t)n_new * 8) : nullptr;
+      dev_free_later(c, d_w);
+      dev_free_later(c, d_d);
+      if ((weights && !d_w) || (delays_ms && !d_d)) return fail(c, NC_ERR_OOM, "out of device memory for the value arrays");
+      if (d_w) NC_CUDA(c, cudaMemcpyAsync(d_w, weights, (size_t)n_new * 4, cudaMemcpyHostToDevice, c->stream));
+      if (d_d) NC_CUDA(c, cudaMemcpyAsync(d_d, delays_ms, (size_t)n_new * 8, cudaMemcpyHostToDevice, c->stream));
+      const unsigned grid = (unsigned)std::min<uint64_t>((n_new + 255) / 256, 148 * 16);
+      set_values_kernel<<<grid, 256, 0, c->stream>>>(gp.map, gp.pos0, n_new, d_w, d_d, c->inv_dt);
+      NC_LAUNCH_CHECK(c, "set_values");
+    }
     c->n_conns += n_new;
   }
   c->n_proj += 1;
@@ -1370,6 +1399,14 @@ int nc_connect_nodes(nc_context* c, const uint32_t* src_nodes, uint32_t n_src, n
   if (src_nodes) src = nc_range{0u, n_src};
   if (tgt_nodes) tgt = nc_range{0u, n_tgt};
   return connect_impl(c, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed);
+}
+
+int nc_connect_values(nc_context* c, const uint32_t* src_nodes, uint32_t n_src, nc_range src, const uint32_t* tgt_nodes,
+                      uint32_t n_tgt, nc_range tgt, nc_rule rule, const nc_rule_params* params, const nc_syn_spec* syn,
+                      uint64_t seed, const float* weights, const double* delays_ms, uint64_t n_values) {
+  if (src_nodes) src = nc_range{0u, n_src};
+  if (tgt_nodes) tgt = nc_range{0u, n_tgt};
+  return connect_impl(c, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed, weights, delays_ms, n_values, true);
 }
 
 int nc_finalize(nc_context* c) {

@@ -431,4 +431,26 @@ __global__ void __launch_bounds__(kBernThreads) bernoulli_write_kernel(const __g
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Per-connection value arrays (weights and delays "specified for each connection by an array having a
+// size equal to the number of connections"): connection i of the projection, at creation position pos0 + i, takes
+// w[i] as it is and / or d_ms[i] through reading D8 in fp64 (one multiply by 1/dt, round half up, at least one
+// step).  Runs after the projection's generate kernel; the arrays come from the host, so PCIe bounds this path.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) set_values_kernel(const __grid_constant__ BlockMap map, uint64_t pos0, uint64_t n,
+                                                        const float* __restrict__ w, const double* __restrict__ d_ms,
+                                                        double inv_dt) {
+  const uint64_t stride = (uint64_t)gridDim.x * 256u;
+  for (uint64_t i = (uint64_t)blockIdx.x * 256u + threadIdx.x; i < n; i += stride) {
+    const BlockAddr a = locate(map, pos0 + i);
+    if (w) *w_ptr(map, a) = w[i];
+    if (d_ms) {
+      const double x = __dmul_rn(d_ms[i], inv_dt);
+      double steps = floor(__dadd_rn(x, 0.5));
+      steps = steps < 1.0 ? 1.0 : (steps > 65535.0 ? 65535.0 : steps);
+      *d_ptr(map, a) = (uint16_t)(int)steps;
+    }
+  }
+}
+
 }  // namespace nc

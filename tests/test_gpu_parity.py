@@ -461,3 +461,48 @@ def test_explicit_node_arrays_parity(nc_mod, oracle_mod):
         assert b.connect_rc(np.array([1, 2, 3]), np.array([4, 5]), WL.RULE_IDS["one_to_one"]) == nc_mod.ERR_INVALID_ARG
         assert b.num_connections() == 0
     g.close(); o.close(); g2.close(); o2.close()
+
+
+def test_value_arrays_parity(nc_mod, oracle_mod):
+    """nc_connect_values: per-connection weight and / or delay arrays, with ranges and with explicit
+    node arrays, mixed with distribution projections, across several storage blocks -- bit-exact against the oracle
+    (a given weight is stored as it is, a given delay goes through the fp64 rule D8), organised order and index too."""
+    rng = np.random.default_rng(29)
+    n_nodes = 2000
+    ids = rng.choice(n_nodes, size=500, replace=False).astype(np.uint32)
+    n1, n2, n3, n4 = 200_000, 500 * 31, 300, 64 * 90
+    calls = [
+        ((0, 2000), (0, 2000), "fixed_total_number", dict(degree_or_total=n1),
+         dict(weights=rng.normal(0, 50, n1).astype(np.float32), delays=rng.uniform(0.0, 12.0, n1))),
+        ((0, 2000), (0, 2000), "fixed_total_number", dict(degree_or_total=30_000), {}),
+        ((100, 700), ids, "fixed_indegree", dict(degree_or_total=31), dict(weights=rng.normal(0, 1, n2).astype(np.float32))),
+        (ids[:300], ids[200:500], "one_to_one", {}, dict(delays=rng.integers(1, 60, n3) * 0.1 + 0.05)),  # on boundaries
+        (ids[:64], (0, 90), "all_to_all", {}, dict(weights=np.arange(n4, dtype=np.float32), delays=np.full(n4, 0.01))),
+    ]
+    o, g = oracle_mod.Oracle(dt_ms=0.1, block_size=50_000), nc_mod.NC(dt_ms=0.1, block_size=50_000)
+    for b in (o, g):
+        b.create_population(n_nodes)
+        for s, t, rule, kw, vals in calls:
+            b.connect(s, t, WL.RULE_IDS[rule], weight=W, delay_ms=D, seed=31, **kw, **vals)
+        b.finalize()
+    gu, ou = g.read_connections(sorted=False), o.connections(sorted=False)
+    rep = PU.compare_connections(gu, ou, 22.0, "value arrays, creation order")
+    assert rep["n"] == n1 + 30_000 + n2 + n3 + n4 and rep["delay_mismatches"] == 0
+    # given values are exact, not merely within tolerance
+    given = np.ones(rep["n"], dtype=bool)
+    given[n1:n1 + 30_000] = False
+    given[n1 + 30_000 + n2:n1 + 30_000 + n2 + n3] = False   # that projection gave delays only
+    assert np.array_equal(gu["weight"][given], ou["weight"][given])
+    PU.compare_connections(g.read_connections(sorted=True), o.connections(sorted=True), 22.0, "value arrays, sorted")
+    PU.compare_index(g.read_index(), o.index(), "value arrays")
+    # errors: same codes as the oracle, context left unchanged
+    g2, o2 = nc_mod.NC(), oracle_mod.Oracle()
+    ftn = WL.RULE_IDS["fixed_total_number"]
+    for b in (g2, o2):
+        b.create_population(20)
+        assert b.connect_rc((0, 20), (0, 20), ftn, degree_or_total=10, weights=np.zeros(9)) == nc_mod.ERR_INVALID_ARG
+        assert b.connect_rc((0, 20), (0, 20), ftn, degree_or_total=10, delays=np.full(10, np.nan)) == nc_mod.ERR_INVALID_ARG
+        assert b.connect_rc((0, 20), (0, 20), ftn, degree_or_total=10, delays=np.full(10, 6553.6)) == nc_mod.ERR_CAPACITY
+        assert b.connect_rc((0, 20), (0, 20), WL.RULE_IDS["pairwise_bernoulli"], p=0.5, weights=np.zeros(200)) == nc_mod.ERR_INVALID_ARG
+        assert b.num_connections() == 0
+    g.close(); o.close(); g2.close(); o2.close()
