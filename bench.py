@@ -217,7 +217,7 @@ def main():
     ap.add_argument("--sample-scale", type=float, default=0.0, help="cpu baseline sample: population scale of configs[2]")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--flags", type=int, default=0, help="extra NC_FLAG_* bits (e.g. 4 = sort (key, position) pairs + gather; "
-                    "16 = COPASS organisation inside the storage blocks)")
+                    "16 = COPASS organisation inside the storage blocks, 48 = the same with the shift of Fig. 6E)")
     ap.add_argument("--block-size", type=int, default=0, help="connections per storage block B (0 = 2^24)")
     args = ap.parse_args()
     global BLOCK_SIZE
@@ -264,6 +264,8 @@ def main():
         n_syn = g.num_connections()
         t = g.timings()  # synchronises this context's stream; the events were recorded on the device
         stats = g.stats()
+        if flags & binding.FLAG_ORGANISE_COPASS:
+            stats["copass"] = g.copass_stats()
         launches += stats["kernel_launches"]
         for k, v in t.items():
             phase_acc[k] = phase_acc.get(k, 0.0) + v
@@ -339,15 +341,18 @@ def main():
                             "frac_of_measured_peak": round(gbs / peak, 4), "frac_of_8TBps": round(gbs / 8000.0, 4)}
 
     if per.get("copass_ms", 0.0) > 0:
-        # COPASS organisation (Fig. 6 D-E): per output block the left partitions (B records) and every
-        # record still to the right of it are copied once, 16 B read + 16 B written each
-        Bk = args.block_size or (1 << 24)
-        kb = (n_syn + Bk - 1) // Bk
-        moved = sum(Bk + (n_syn - (b + 1) * Bk) for b in range(kb - 1))
+        # COPASS organisation (Fig. 6 C-E): partitions plus the record moves (16 B read + 16 B written
+        # each).  Default: gather of every output block + emptying one block into the holes; with NC_FLAG_COPASS_SHIFT
+        # the left partitions and every record still to the right of the block, per output block.
+        cst = stats.get("copass", {})
+        moved = int(cst.get("records_moved", 0))
         gbs = 32 * moved / (per["copass_ms"] * 1e-3) / 1e9
-        phases["copass_moves"] = {"ms": round(per["copass_ms"], 4), "records_moved": moved, "blocks": kb,
-                                  "alg_bytes_per_record_moved": 32, "GBps": round(gbs, 1),
-                                  "frac_of_measured_peak": round(gbs / peak, 4)}
+        phases["copass_partitions_and_moves"] = {
+            "ms": round(per["copass_ms"], 4), "records_moved": moved, "blocks": int(cst.get("n_blocks", 0)),
+            "partitions": int(cst.get("partitions", 0)), "partition_iterations": int(cst.get("iterations", 0)),
+            "aux_bytes": int(cst.get("aux_bytes", 0)),
+            "mode": "shift (Fig. 6E)" if flags & binding.FLAG_COPASS_SHIFT else "hole filling",
+            "alg_bytes_per_record_moved": 32, "GBps": round(gbs, 1), "frac_of_measured_peak": round(gbs / peak, 4)}
     cpu = None
     if not args.no_cpu_baseline and args.workload.startswith("c2"):
         scale = args.sample_scale if args.sample_scale else 0.5

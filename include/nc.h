@@ -77,12 +77,15 @@ enum {
   NC_FLAG_SORT_ONESWEEP = 1u << 3, /* carry the whole connection, but chain the tiles of a digit pass inside the
                                    pass (decoupled look-back) instead of the default count / scan / scatter
                                    kernels per pass */
-  NC_FLAG_ORGANISE_COPASS = 1u << 4 /* organise the connections INSIDE their storage blocks with the COPASS block-sort
+  NC_FLAG_ORGANISE_COPASS = 1u << 4, /* organise the connections INSIDE their storage blocks with the COPASS block-sort
                                    of PAPER.md:426-642 (Appendix A): auxiliary memory of a few blocks instead of two
                                    more copies of all connections.  The organised view then keeps the block structure
                                    (see nc_connections_view) and the creation-order view is gone after nc_finalize.
                                    Needs a (source, delay) key of <= 32 bits and <= 4096 blocks (NC_ERR_CAPACITY).
                                    See include/nc_copass.h. */
+  NC_FLAG_COPASS_SHIFT = 1u << 5   /* with NC_FLAG_ORGANISE_COPASS: follow Fig. 6 C-E to the letter (one partition per
+                                   output block on what the previous extraction left, right partitions shifted
+                                   right) instead of the default extraction by hole filling (include/nc_copass.h) */
 };
 
 typedef struct {

@@ -10,11 +10,18 @@
  *     (Sec. A2-A4); (D) the left partitions are copied to the auxiliary array; (E) the right partitions are shifted
  *     right so that block b becomes free; (F) the auxiliary array is sorted into block b.  The result is the same
  *     stable order as the default path (readings C3, C4, C6 of DESIGN.md), left in the blocks: see
- *     nc_connections_view in nc.h.  Auxiliary device memory: two blocks (the auxiliary array of Eq. A3 and one spare
- *     block that the shift of (E) fills and then swaps in, so that no move overlaps its source) plus the scratch of
- *     the underlying sort for one block -- "the largest between the auxiliary storage requirement of the underlying
- *     sorting algorithm for an array of size m_max and the auxiliary array" -- instead of 50 bytes per
- *     connection.  nc_get_copass_stats reports what the partitions did.
+ *     nc_connections_view in nc.h.  By default step (E) is replaced: all partitions are taken at once on the sorted
+ *     blocks (extraction b needs the first (b+1) N elements, which does not depend on extraction b-1), the subarrays
+ *     are kept as lists of extents ("the subarrays do not need to be stored in contiguous locations"),
+ *     each output block is gathered into a spare block and sorted there, and one block is then emptied into the holes
+ *     the left partitions left behind and becomes the next spare -- about 2 N records move per extraction instead of
+ *     everything to the right of block b.  NC_FLAG_COPASS_SHIFT keeps (C)-(E) to the letter (one partition per output
+ *     block on what the previous extraction left; right partitions shifted right, assembled block by block in a spare
+ *     block so that no move overlaps its source).  Auxiliary device memory: one spare block (two with the shift: the
+ *     auxiliary array of Eq. A3 as well) plus the scratch of the underlying sort for one block -- "the largest
+ *     between the auxiliary storage requirement of the underlying sorting algorithm for an array of size m_max and
+ *     the auxiliary array" -- instead of 50 bytes per connection.  nc_get_copass_stats reports what the
+ *     partitions did.
  *  2. nc_copass_partition: the partition step alone on caller-supplied keys (used by the tests to compare it with
  *     the oracle on inputs the connection keys never produce: long runs of ties, empty subarrays, k up to 4096).
  *
@@ -52,6 +59,7 @@ typedef struct {
   uint32_t last_step_2; /* how many ended in Sec. A4 */
   uint64_t n_blocks;    /* k */
   uint64_t aux_bytes;   /* auxiliary device memory the organisation step held at its peak */
+  uint64_t records_moved; /* records copied by the moves of Fig. 6 D-E (or by gathering and hole filling) */
 } nc_copass_stats;
 
 /* NC_ERR_STATE unless the context was finalized under NC_FLAG_ORGANISE_COPASS. */

@@ -159,7 +159,13 @@ __global__ void __launch_bounds__(kCopassThreads) copass_partition_kernel(
     const Keys keys, uint32_t k, uint32_t m, const uint32_t* __restrict__ start_g, const uint32_t* __restrict__ len_g,
     uint32_t new_base, uint32_t* __restrict__ m_out, uint32_t* __restrict__ left_prefix,
     uint32_t* __restrict__ right_src, uint32_t* __restrict__ new_start, uint32_t* __restrict__ new_len,
-    CopassInfo* __restrict__ info, CopassTotals* __restrict__ totals) {
+    CopassInfo* __restrict__ info, CopassTotals* __restrict__ totals, uint32_t m_step = 0, uint32_t out_stride = 0) {
+  // several independent partitions of the same subarrays in one launch: CTA c takes m + c m_step and writes its
+  // outputs out_stride words further on
+  m += blockIdx.x * m_step;
+  m_out += (size_t)blockIdx.x * out_stride;
+  const bool for_moves = left_prefix != nullptr;  // the shift of Fig. 6E needs the prefixes; hole filling only m_i
+  if (info) info += blockIdx.x;
   extern __shared__ uint32_t sh[];
   const size_t k1 = (size_t)k + 1;  // every array has a spare word for the total of a scan
   uint32_t* start = sh;
@@ -275,25 +281,28 @@ __global__ void __launch_bounds__(kCopassThreads) copass_partition_kernel(
   for (uint32_t i = tid; i < k; i += kCopassThreads) {
     const uint32_t mi = res[i];
     m_out[i] = mi;
-    right_src[i] = start[i] + mi;
-    const uint32_t rest = len[i] - mi;
-    new_len[i] = rest;
-    m_hi[i] = rest;
+    m_hi[i] = len[i] - mi;
+    if (for_moves) {
+      right_src[i] = start[i] + mi;
+      new_len[i] = len[i] - mi;
+    }
   }
   __syncthreads();
-  block_exscan(res, mu_lo, k, 0, tmp32);
-  for (uint32_t i = tid; i < k; i += kCopassThreads) left_prefix[i] = mu_lo[i];
-  if (tid == 0) left_prefix[k] = mu_lo[k];
-  __syncthreads();
-  block_exscan(m_hi, mu_lo, k, new_base, tmp32);
-  for (uint32_t i = tid; i < k; i += kCopassThreads) new_start[i] = mu_lo[i];
+  if (for_moves) {
+    block_exscan(res, mu_lo, k, 0, tmp32);
+    for (uint32_t i = tid; i < k; i += kCopassThreads) left_prefix[i] = mu_lo[i];
+    if (tid == 0) left_prefix[k] = mu_lo[k];
+    __syncthreads();
+    block_exscan(m_hi, mu_lo, k, new_base, tmp32);
+    for (uint32_t i = tid; i < k; i += kCopassThreads) new_start[i] = mu_lo[i];
+  }
   if (tid == 0) {
-    new_start[k] = mu_lo[k];
+    if (for_moves) new_start[k] = mu_lo[k];
     if (info) *info = CopassInfo{t_out_s, iterations, last_step, 0u};
     if (totals) {
-      totals->partitions += 1;
-      totals->iterations += iterations;
-      (last_step == 1 ? totals->last_step_1 : totals->last_step_2) += 1;
+      atomicAdd(&totals->partitions, 1u);
+      atomicAdd(&totals->iterations, iterations);
+      atomicAdd(last_step == 1 ? &totals->last_step_1 : &totals->last_step_2, 1u);
     }
   }
 }
@@ -345,6 +354,61 @@ __global__ void __launch_bounds__(kGatherThreads) copass_gather_kernel(const __g
       out[j0 + q * kGatherThreads] = v[q];
       // D: the digit of the first radix pass over the auxiliary array, so that its tile counts read 1 B per record
       if (dig_out) dig_out[j0 + q * kGatherThreads] = (uint8_t)((v[q].x >> dig_shift) & dig_mask);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Segmented copy for the hole-filling organisation (organise_copass_fill in nc_api.cu): element e (e < total) of
+// the launch belongs to command c with prefix[c] <= e < prefix[c+1] and goes from position src[c] + (e - prefix[c])
+// to position dst[c] + (e - prefix[c]); positions index the PHYSICAL blocks (block id * B + slot, the map's table
+// lists the block pointers by id).  The commands are planned on the host from the partition results.
+// ---------------------------------------------------------------------------------------------
+constexpr uint32_t kSegSmemCmds = 2048;
+
+__global__ void __launch_bounds__(kGatherThreads) copass_segcopy_kernel(const __grid_constant__ BlockMap map,
+                                                                       const uint32_t* __restrict__ src,
+                                                                       const uint32_t* __restrict__ dst,
+                                                                       const uint32_t* __restrict__ prefix,
+                                                                       uint32_t n_cmds, uint32_t total,
+                                                                       uint8_t* __restrict__ dig_out, uint32_t dig_shift,
+                                                                       uint32_t dig_mask) {
+  __shared__ uint32_t s_src[kSegSmemCmds], s_dst[kSegSmemCmds], s_pre[kSegSmemCmds];
+  const uint32_t *ps = src, *pd = dst, *pp = prefix;
+  if (n_cmds <= kSegSmemCmds) {
+    for (uint32_t i = threadIdx.x; i < n_cmds; i += kGatherThreads) {
+      s_src[i] = src[i];
+      s_dst[i] = dst[i];
+      s_pre[i] = prefix[i];
+    }
+    __syncthreads();
+    ps = s_src;
+    pd = s_dst;
+    pp = s_pre;
+  }
+  const uint32_t e0 = blockIdx.x * (kGatherThreads * kGatherItems) + threadIdx.x;
+  uint4 v[kGatherItems];
+  uint32_t to[kGatherItems];
+  bool ok[kGatherItems];
+#pragma unroll
+  for (int q = 0; q < kGatherItems; ++q) {
+    const uint32_t e = e0 + q * kGatherThreads;
+    ok[q] = e < total;
+    if (ok[q]) {
+      uint32_t lo = 0, hi = n_cmds;  // last command with prefix <= e (commands are never empty)
+      while (hi - lo > 1) {
+        const uint32_t mid = (lo + hi) >> 1;
+        if (pp[mid] <= e) lo = mid; else hi = mid;
+      }
+      const uint32_t off = e - pp[lo];
+      v[q] = *rec_ptr(map, ps[lo] + off);
+      to[q] = pd[lo] + off;
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < kGatherItems; ++q)
+    if (ok[q]) {
+      *const_cast<uint4*>(rec_ptr(map, to[q])) = v[q];
+      if (dig_out) dig_out[e0 + q * kGatherThreads] = (uint8_t)((v[q].x >> dig_shift) & dig_mask);
     }
 }
 

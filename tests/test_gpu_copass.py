@@ -104,10 +104,11 @@ def test_partition_argument_errors(nc_mod):
     g.close()
 
 
-def copass_parity(net, oracle_mod, nc_mod, B):
+def copass_parity(net, oracle_mod, nc_mod, B, shift=False):
     o = oracle_mod.Oracle(dt_ms=net.dt_ms, block_size=B)
     WL.run(net, o, finalize=True)
-    g = nc_mod.NC(dt_ms=net.dt_ms, block_size=B, flags=nc_mod.FLAG_ORGANISE_COPASS)
+    flags = nc_mod.FLAG_ORGANISE_COPASS | (nc_mod.FLAG_COPASS_SHIFT if shift else 0)
+    g = nc_mod.NC(dt_ms=net.dt_ms, block_size=B, flags=flags)
     WL.run(net, g, finalize=False)
     scale = PU.weight_scale(net)
     gu = g.read_connections(sorted=False)
@@ -148,19 +149,22 @@ def copass_parity(net, oracle_mod, nc_mod, B):
     return rep, st
 
 
+@pytest.mark.parametrize("shift", [False, True], ids=["fill", "shift"])
 @pytest.mark.parametrize("B", [0, 1, 7, 10, 64, 250, 999, 1000])
-def test_copass_config0_tiny(nc_mod, oracle_mod, B):
-    rep, st = copass_parity(WL.config0_tiny(), oracle_mod, nc_mod, B)
+def test_copass_config0_tiny(nc_mod, oracle_mod, B, shift):
+    """shift = Fig. 6 C-E to the letter; fill = the default extraction by hole filling"""
+    rep, st = copass_parity(WL.config0_tiny(), oracle_mod, nc_mod, B, shift)
     assert rep["n"] == 1000
 
 
 @pytest.mark.parametrize("rule,scale,B", [("one_to_one", 1.0, 1000), ("all_to_all", 0.15, 300_000),
                                           ("fixed_indegree", 0.3, 100_000), ("fixed_outdegree", 0.25, 131_072),
                                           ("fixed_total_number", 0.3, 250_001), ("pairwise_bernoulli", 0.4, 65_536)])
-def test_copass_config1_rules(nc_mod, oracle_mod, rule, scale, B):
+@pytest.mark.parametrize("shift", [False, True], ids=["fill", "shift"])
+def test_copass_config1_rules(nc_mod, oracle_mod, rule, scale, B, shift):
     """Several sort tiles per block, a ragged last block, block sizes that are and are not powers of two."""
     net = WL.config1_rule(rule, scale=scale)
-    rep, st = copass_parity(net, oracle_mod, nc_mod, B)
+    rep, st = copass_parity(net, oracle_mod, nc_mod, B, shift)
     print(net.name, rep, st)
     assert st["n_blocks"] >= 3
 
@@ -168,8 +172,9 @@ def test_copass_config1_rules(nc_mod, oracle_mod, rule, scale, B):
 def test_copass_microcircuit_scaled(nc_mod, oracle_mod):
     """configs[2] at 10 % of the populations, ~3e6 connections in 12 blocks of 2^18."""
     net = WL.config2_microcircuit(scale=0.1)
-    rep, st = copass_parity(net, oracle_mod, nc_mod, 1 << 18)
-    print(rep, st)
+    for shift in (False, True):
+        rep, st = copass_parity(net, oracle_mod, nc_mod, 1 << 18, shift)
+        print(rep, st)
     assert st["n_blocks"] >= 10 and st["iterations"] >= st["partitions"]
 
 
