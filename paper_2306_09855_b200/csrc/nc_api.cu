@@ -1995,13 +1995,18 @@ int nc_selftest_fastpath(nc_context* c, double out[4]) {
 int nc_internal_organised_view(nc_context* c, nc_organised_view* out) {
   if (!c || !out) return NC_ERR_INVALID_ARG;
   if (!c->finalized) return fail(c, NC_ERR_STATE, "the connections are not organised yet (nc_finalize)");
-  if (c->organised_in_blocks && c->blocks.size() > 1)
-    return fail(c, NC_ERR_STATE, "spike delivery reads flat target / weight arrays: with COPASS organisation it needs "
-                                 "all connections in one block");
   int rc = ensure_total_groups(c);
   if (rc != NC_OK) return rc;
-  out->target = c->organised_in_blocks ? (const uint32_t*)((char*)c->blocks[0] + c->off_tgt) : c->s_tgt;
-  out->weight = c->organised_in_blocks ? (const float*)((char*)c->blocks[0] + c->off_w) : c->s_w;
+  std::memset(out, 0, sizeof(*out));
+  if (c->organised_in_blocks) {
+    out->block_table = c->d_table;
+    out->block_size = c->B;
+    out->off_target = c->off_tgt;
+    out->off_weight = c->off_w;
+  } else {
+    out->target = c->s_tgt;
+    out->weight = c->s_w;
+  }
   out->group_ptr = c->group_ptr;
   out->group_start = c->group_start;
   out->group_delay = c->group_delay;

@@ -106,6 +106,9 @@ struct DeliverParams {
   uint32_t capacity;
 };
 
+// BLOCKS: the organised connections live in the storage blocks (COPASS organisation); position c is entry c % B of
+// block c / B, a group may straddle two blocks.
+template <bool BLOCKS>
 __global__ void __launch_bounds__(256) deliver_kernel(const __grid_constant__ DeliverParams p) {
   const uint32_t n_arr = min(*p.n_arr, p.capacity);
   const uint32_t warps = gridDim.x * (256 / 32);
@@ -115,7 +118,17 @@ __global__ void __launch_bounds__(256) deliver_kernel(const __grid_constant__ De
     const uint32_t c0 = p.v.group_start[ent.x];
     const uint32_t c1 = ent.x + 1 < p.v.total_groups ? p.v.group_start[ent.x + 1] : (uint32_t)p.v.n;
     const float m = (float)ent.y;
-    for (uint32_t c = c0 + lane_id(); c < c1; c += 32) atomicAdd(p.input + p.v.target[c], p.v.weight[c] * m);
+    for (uint32_t c = c0 + lane_id(); c < c1; c += 32) {
+      if (BLOCKS) {
+        const uint64_t blk = c / p.v.block_size, slot = c - blk * p.v.block_size;
+        const char* base = reinterpret_cast<const char*>(p.v.block_table[blk]);
+        const uint32_t t = reinterpret_cast<const uint32_t*>(base + p.v.off_target)[slot];
+        const float w = reinterpret_cast<const float*>(base + p.v.off_weight)[slot];
+        atomicAdd(p.input + t, w * m);
+      } else {
+        atomicAdd(p.input + p.v.target[c], p.v.weight[c] * m);
+      }
+    }
     ev += c1 - c0;
   }
   if (lane_id() == 0 && ev) atomicAdd(&p.ctr->events, ev);
@@ -211,7 +224,8 @@ int nc_delivery_step(nc_delivery* d, const uint32_t* d_nodes, const uint32_t* d_
   dp.input = d_input;
   dp.capacity = d->capacity;
   const unsigned dgrid = (unsigned)std::max<uint64_t>(1, std::min<uint64_t>(((uint64_t)d->capacity + 7) / 8, (uint64_t)d->sms * 8));
-  deliver_kernel<<<dgrid, 256, 0, st>>>(dp);
+  if (d->v.block_table) deliver_kernel<true><<<dgrid, 256, 0, st>>>(dp);
+  else deliver_kernel<false><<<dgrid, 256, 0, st>>>(dp);
   d->cur = 1 - d->cur;
   if (cudaPeekAtLastError() != cudaSuccess)
     return nc_internal_fail(d->ctx, NC_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));

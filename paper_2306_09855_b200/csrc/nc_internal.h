@@ -6,8 +6,11 @@
 #include "../../include/nc.h"
 
 struct nc_organised_view {  // borrowed device pointers, valid until nc_destroy
-  const uint32_t* target;
+  const uint32_t* target;       // flat organised arrays; NULL when the organised connections live in the storage blocks
   const float* weight;
+  // COPASS organisation (NC_FLAG_ORGANISE_COPASS): organised position j is entry j % block_size of block j / block_size
+  const uint64_t* block_table;  // device array of block base addresses, NULL for the flat arrays
+  uint64_t block_size, off_target, off_weight;
   const uint32_t* group_ptr;    // [n_nodes + 1]
   const uint32_t* group_start;  // [total_groups]
   const uint16_t* group_delay;  // [total_groups]

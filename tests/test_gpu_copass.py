@@ -193,14 +193,30 @@ def test_copass_uses_a_few_blocks_of_auxiliary_memory(nc_mod):
     g.close()
 
 
-def test_copass_delivery_needs_one_block(nc_mod, oracle_mod):
+def test_delivery_over_copass_blocks(nc_mod, oracle_mod):
+    """Spike delivery (include/nc_delivery.h) over connections organised inside 10 storage blocks: groups straddle
+    blocks; the spike array and every node's input equal the oracle's step by step."""
+    import torch
     net = WL.config0_tiny()
+    o = oracle_mod.Oracle(dt_ms=net.dt_ms, block_size=100)
+    WL.run(net, o)
     g = nc_mod.NC(dt_ms=net.dt_ms, block_size=100, flags=nc_mod.FLAG_ORGANISE_COPASS)
-    WL.run(net, g, finalize=True)
-    with pytest.raises(nc_mod.NCError) as e:
-        nc_mod.Delivery(g, 64)
-    assert e.value.code == nc_mod.ERR_STATE
-    g.close()
+    WL.run(net, g)
+    od, gd = oracle_mod.Delivery(o), nc_mod.Delivery(g, 4096)
+    inp = torch.zeros(net.n_nodes, dtype=torch.float32, device="cuda")
+    rng = np.random.default_rng(4)
+    for k in range(80):
+        nodes = rng.choice(net.n_nodes, size=int(rng.integers(0, 12)) if k < 30 else 0, replace=False).astype(np.uint32)
+        want = np.zeros(net.n_nodes)
+        od.step(nodes, None, want)
+        inp.zero_()
+        gd.step(torch.from_numpy(nodes.astype(np.int32)).cuda(), None, inp)
+        go, gm = gd.read_spike_array()
+        wo, wm = od.spike_array()
+        assert sorted(zip(go.tolist(), gm.tolist())) == sorted(zip(wo.tolist(), wm.tolist())), k
+        assert np.abs(inp.cpu().numpy() - want).max() <= 1e-5 * max(1.0, np.abs(want).max()), k
+    assert gd.counts()["events"] == od.counts()[1] > 0
+    gd.close(); od.close(); g.close(); o.close()
 
 
 def test_copass_full_size_microcircuit(nc_mod):
