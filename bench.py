@@ -245,9 +245,14 @@ def main():
 
     # ---- warm-up (also warms torch's caching allocator: the timed steps allocate from its cache) ----
     n_syn = 0
-    for _ in range(max(args.warmup, 0)):
+    cold_ms = None
+    for w in range(max(args.warmup, 0)):
+        t0 = time.perf_counter()
         g = one_step(binding, WL, net, flags)
         n_syn = g.num_connections()
+        g.synchronize()
+        if w == 0:  # the one cold step: device allocations come from the driver, not from torch's cache
+            cold_ms = 1e3 * (time.perf_counter() - t0)
         g.close()
     barrier()
 
@@ -259,6 +264,7 @@ def main():
     phase_acc, launches, stats = {}, 0, {}
     barrier()
     ev0.record(stream)
+    step_marks = [ev0]
     for _ in range(args.steps):
         g = one_step(binding, WL, net, flags)
         n_syn = g.num_connections()
@@ -270,9 +276,12 @@ def main():
         for k, v in t.items():
             phase_acc[k] = phase_acc.get(k, 0.0) + v
         g.close()
+        step_marks.append(torch.cuda.Event(enable_timing=True))
+        step_marks[-1].record(stream)
     ev1.record(stream)
     barrier()
     total_ms = ev0.elapsed_time(ev1)
+    step_ms = [a.elapsed_time(b) for a, b in zip(step_marks[:-1], step_marks[1:])]
     clocks = sampler.stop()
     total_ms = replicas.max_over_ranks(dist, total_ms, "cuda")
     ms_per_step = total_ms / args.steps
@@ -363,7 +372,8 @@ def main():
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32+f32",
+        "ms_per_step": ms_per_step, "ms_per_step_sd": statistics.pstdev(step_ms) if len(step_ms) > 1 else 0.0,
+        "cold_first_step_ms": cold_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32+f32",
         "data": "synthetic",
         "config": {"workload": f"{net.name}: BASELINE.json configs[2] cortical-microcircuit-shaped network, "
                                f"{net.n_nodes} nodes, {len(net.projections)} fixed_total_number projections, seed 7"
