@@ -21,7 +21,9 @@
  *     auxiliary array of Eq. A3 as well) plus the scratch of the underlying sort for one block -- "the largest
  *     between the auxiliary storage requirement of the underlying sorting algorithm for an array of size m_max and
  *     the auxiliary array" -- instead of 50 bytes per connection.  nc_get_copass_stats reports what the
- *     partitions did.
+ *     partitions did.  The organisation rewrites the blocks: should nc_finalize fail under this flag after it has
+ *     started (NC_ERR_OOM, NC_ERR_CUDA), the connections are lost and every later call but nc_destroy returns
+ *     NC_ERR_STATE; argument and capacity errors are detected before anything is touched.
  *  2. nc_copass_partition: the partition step alone on caller-supplied keys (used by the tests to compare it with
  *     the oracle on inputs the connection keys never produce: long runs of ties, empty subarrays, k up to 4096).
  *

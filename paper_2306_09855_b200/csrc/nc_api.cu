@@ -72,6 +72,7 @@ struct nc_context {
   bool organised_in_blocks = false; // nc_finalize left the organised connections in the storage blocks
   CopassTotals* d_copass_totals = nullptr;
   uint64_t copass_aux_bytes = 0, copass_moved = 0;
+  bool broken = false;  // an in-place organisation failed half way: the connections are lost, only nc_destroy is left
 
   // allocations
   std::unordered_map<void*, size_t> live;
@@ -919,9 +920,7 @@ int copass_extract_fill(nc_context* c, const PassPlan& plan, const CopassScratch
   const uint32_t n = (uint32_t)c->n_conns;
   const uint64_t B = c->B;
   const uint32_t k = (uint32_t)c->blocks.size();
-  if ((uint64_t)(k + 1) * B > 0xffffffffull)
-    return fail(c, NC_ERR_CAPACITY, "COPASS organisation: (blocks + 1) x block_size must stay below 2^32");
-  const size_t k1 = (size_t)k + 1;
+  const size_t k1 = (size_t)k + 1;  // (k + 1) B < 2^32 was checked before anything was rewritten
   auto block_n = [&](uint32_t b) { return (uint32_t)std::min<uint64_t>(B, (uint64_t)n - (uint64_t)b * B); };
 
   // ---- Fig. 6C for every output block at once ----
@@ -1142,6 +1141,8 @@ int organise_copass(nc_context* c, const PassPlan& plan) {
   const uint32_t k = (uint32_t)c->blocks.size();
   if (k > kCopassMaxBlocks)
     return fail(c, NC_ERR_CAPACITY, "COPASS organisation handles at most 4096 storage blocks: raise block_size");
+  if (k > 1 && !(c->cfg.flags & NC_FLAG_COPASS_SHIFT) && (uint64_t)(k + 1) * B > 0xffffffffull)
+    return fail(c, NC_ERR_CAPACITY, "COPASS organisation: (blocks + 1) x block_size must stay below 2^32");
   const uint32_t big = (uint32_t)std::min<uint64_t>(B, n);  // the largest block (Eq. A3)
   const uint32_t kTile = (uint32_t)kSplitShapes[0].warps * 32u * (uint32_t)kSplitShapes[0].items;
   const uint32_t max_tiles = (big + kTile - 1) / kTile;
@@ -1195,7 +1196,9 @@ int organise_copass(nc_context* c, const PassPlan& plan) {
   const BlockMap map = make_map(c);
   int rc;
 
-  // Fig. 6B: every block sorted on its own, creation-order layout -> records
+  // Fig. 6B: every block sorted on its own, creation-order layout -> records.  From here on the blocks are being
+  // rewritten: a failure leaves no usable connections behind.
+  c->broken = true;
   for (uint32_t b = 0; b < k; ++b) {
     BlockMap one = map;
     one.table = c->d_table + b;
@@ -1268,6 +1271,7 @@ int organise_copass(nc_context* c, const PassPlan& plan) {
   }
   c->copass_aux_bytes = c->bytes_in_use - bytes_before;  // nothing of the scratch has been released yet
   c->organised_in_blocks = true;
+  c->broken = false;  // the blocks hold the organised connections
   rc = build_index_from_sorted(c, n, nullptr);
   drop();
   return rc;
@@ -1519,6 +1523,7 @@ static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, 
                         const float* weights = nullptr, const double* delays_ms = nullptr, uint64_t n_values = 0,
                         bool with_values = false) {
   if (!c) return NC_ERR_INVALID_ARG;
+  if (c->broken) return fail(c, NC_ERR_STATE, "nc_connect: a failed in-place organisation left this context without connections; destroy it");
   if (c->finalized) return fail(c, NC_ERR_STATE, "nc_connect after nc_finalize");
   if (!params || !syn) return fail(c, NC_ERR_INVALID_ARG, "nc_connect: null params");
   if (src.count == 0 || tgt.count == 0) return fail(c, NC_ERR_INVALID_ARG, "nc_connect: empty node range");
@@ -1669,6 +1674,7 @@ int nc_connect_values(nc_context* c, const uint32_t* src_nodes, uint32_t n_src, 
 
 int nc_finalize(nc_context* c) {
   if (!c) return NC_ERR_INVALID_ARG;
+  if (c->broken) return fail(c, NC_ERR_STATE, "nc_finalize: a failed in-place organisation left this context without connections; destroy it");
   if (c->finalized) return fail(c, NC_ERR_STATE, "nc_finalize called twice");
   gen_span_end(c);
   const uint32_t N = c->n_nodes;
@@ -1730,6 +1736,7 @@ int nc_get_connections(nc_context* c, int sorted, nc_connections_view* out) {
   std::memset(out, 0, sizeof(*out));
   out->n = c->n_conns;
   out->block_size = c->B;
+  if (c->broken) return fail(c, NC_ERR_STATE, "a failed in-place organisation left this context without connections");
   if (sorted && !c->finalized) return fail(c, NC_ERR_STATE, "sorted view before nc_finalize");
   if (!sorted && c->organised_in_blocks)
     return fail(c, NC_ERR_STATE, "the creation-order view is gone: the blocks were organised in place (COPASS)");
@@ -1834,6 +1841,7 @@ int nc_read_connections(nc_context* c, int sorted, uint64_t first, uint64_t coun
   if (!c) return NC_ERR_INVALID_ARG;
   if (first + count > c->n_conns) return fail(c, NC_ERR_INVALID_ARG, "nc_read_connections: range outside the connections");
   if (sorted && !c->finalized) return fail(c, NC_ERR_STATE, "sorted view before nc_finalize");
+  if (c->broken) return fail(c, NC_ERR_STATE, "a failed in-place organisation left this context without connections");
   if (!sorted && c->organised_in_blocks)
     return fail(c, NC_ERR_STATE, "the creation-order view is gone: the blocks were organised in place (COPASS)");
   if (count == 0) return NC_OK;

@@ -260,3 +260,18 @@ def test_copass_full_size_microcircuit(nc_mod):
     assert np.array_equal(idx["group_count"], gcount)
     assert np.array_equal(idx["group_ptr"], np.concatenate([[0], np.cumsum(gcount)]).astype(np.uint32))
     g.close()
+
+
+def test_copass_capacity_errors_leave_the_connections_intact(nc_mod, oracle_mod):
+    """More than 4096 blocks: NC_ERR_CAPACITY before anything is rewritten -- the creation-order view still reads."""
+    g = nc_mod.NC(dt_ms=0.1, block_size=1, flags=nc_mod.FLAG_ORGANISE_COPASS)
+    o = oracle_mod.Oracle(dt_ms=0.1, block_size=1)
+    for b in (g, o):
+        b.create_population(50)
+        b.connect((0, 50), (0, 50), WL.RULE_IDS["fixed_total_number"], degree_or_total=5000, weight=(1.0, 0.1, 0.0, float("inf")),
+                  delay_ms=(1.5, 0.75, 0.1, float("inf")), seed=8)
+    with pytest.raises(nc_mod.NCError) as e:
+        g.finalize()
+    assert e.value.code == nc_mod.ERR_CAPACITY
+    PU.compare_connections(g.read_connections(sorted=False), o.connections(sorted=False), 1.1, "after a refused finalize")
+    g.close(); o.close()
