@@ -852,8 +852,8 @@ int copass_sort_records(nc_context* c, const PassPlan& plan, const CopassScratch
         tile_count_recs_kernel<<<n_tiles, kCountThreads, 0, c->stream>>>(in, n, kTile, plan.shift[0], plan.bits[0],
                                                                         sc.counts);
       } else {
-        tile_count_bytes_kernel<<<(n_tiles + kCountTilesPerCta - 1) / kCountTilesPerCta, kCountThreads, 0, c->stream>>>(
-            sc.dig, n, kTile, n_tiles, sc.counts);
+        // a block has a few thousand tiles: two per CTA fill the machine, eight would leave most SMs idle
+        tile_count_bytes_kernel<<<(n_tiles + 1) / 2, kCountThreads, 0, c->stream>>>(sc.dig, n, kTile, n_tiles, sc.counts, 2u);
       }
       NC_LAUNCH_CHECK(c, "tile_count");
       chunk_total_kernel<<<n_chunks, kRadix, 0, c->stream>>>(sc.counts, n_tiles, sc.chunk, kCopassChunkTiles);

@@ -80,12 +80,13 @@ constexpr int kCountTilesPerCta = 8;
 
 __global__ void __launch_bounds__(kCountThreads) tile_count_bytes_kernel(const uint8_t* __restrict__ dig, uint32_t n,
                                                                         uint32_t tile_size, uint32_t n_tiles,
-                                                                        uint16_t* __restrict__ counts) {
+                                                                        uint16_t* __restrict__ counts,
+                                                                        uint32_t tiles_per_cta = kCountTilesPerCta) {
   __shared__ uint32_t hist[kRadix];
   hist[threadIdx.x] = 0;
   __syncthreads();
-  for (uint32_t k = 0; k < (uint32_t)kCountTilesPerCta; ++k) {
-    const uint32_t tile = blockIdx.x * kCountTilesPerCta + k;
+  for (uint32_t k = 0; k < tiles_per_cta; ++k) {
+    const uint32_t tile = blockIdx.x * tiles_per_cta + k;
     if (tile >= n_tiles) break;
     const uint64_t tile0 = (uint64_t)tile * tile_size;
     const uint32_t valid = (uint32_t)min((uint64_t)tile_size, (uint64_t)n - tile0);
