@@ -159,7 +159,7 @@ def run_delivery(args):
     torch.cuda.set_device(0)
     rate = float(args.workload.split(":")[1]) if ":" in args.workload else 0.01
     net = WL.config2_microcircuit()
-    g = binding.NC(dt_ms=net.dt_ms)
+    g = binding.NC(dt_ms=net.dt_ms, flags=args.flags, block_size=args.block_size)  # --flags 16: over COPASS-organised blocks
     WL.run(net, g)
     n_nodes, n_syn = g.num_nodes(), g.num_connections()
     rng = np.random.default_rng(2306)
@@ -198,7 +198,7 @@ def run_delivery(args):
             "config": {"workload": f"delivery over configs[2] ({n_nodes} nodes, {n_syn} connections), Bernoulli({rate}) "
                                    "spikes per node per step, raster resident in HBM",
                        "events_per_step": events / args.steps, "spikes_per_step": float(counts[args.warmup:].mean()),
-                       "buffered_at_end": c["buffered"], "dropped": c["dropped"]},
+                       "buffered_at_end": c["buffered"], "dropped": c["dropped"], "flags": args.flags},
             "gpu_launches": 2 * args.steps,
             "roofline": {"bound": "hbm", "kernel": "deliver_kernel (8 B read per delivered connection + one fp32 atomic add)",
                          "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None}}
