@@ -232,6 +232,18 @@ int nc_connect_values(nc_context* ctx, const uint32_t* src_nodes, uint32_t n_src
                       const nc_rule_params* params, const nc_syn_spec* syn, uint64_t seed, const float* weights,
                       const double* delays_ms, uint64_t n_values);
 
+/* Receptor port and synaptic group (a connection "includes the source node index, the target node index,
+ * the receptor port index, the weight, the delay, and the synaptic group index.  The synaptic group index takes
+ * non-zero values only for non-static synapses").  The pair set here (0, 0 at the start) belongs to every connection
+ * the following nc_connect* calls create.  Both are constants of a projection, so the library keeps them per
+ * projection instead of per connection; nc_read_connection_attributes resolves entries first .. first+count-1 of
+ * either view through their creation positions and copies them to HOST arrays (either may be NULL; synchronises).
+ * The library stores and returns them, nothing more: synapses are static and spike delivery (nc_delivery.h) has one
+ * input per node. ---- */
+int nc_set_connection_attributes(nc_context* ctx, uint8_t port, uint8_t syn_group);
+int nc_read_connection_attributes(nc_context* ctx, int sorted, uint64_t first, uint64_t count, uint8_t* port,
+                                  uint8_t* syn_group);
+
 /* ---- calibration: stable sort by (source, delay), then the group index ---- */
 int nc_finalize(nc_context* ctx);
 

@@ -242,6 +242,25 @@ class Oracle:
         if rc != 0:
             raise OracleError(rc)
 
+    def set_connection_attributes(self, port: int, syn_group: int = 0):
+        L = lib()
+        L.oc_set_connection_attributes.argtypes = [C.c_void_p, C.c_uint8, C.c_uint8]
+        rc = L.oc_set_connection_attributes(self._h, int(port), int(syn_group))
+        if rc != 0:
+            raise OracleError(rc)
+
+    def read_connection_attributes(self, sorted: bool = False, first: int = 0, count=None):
+        L = lib()
+        L.oc_read_connection_attributes.argtypes = [C.c_void_p, C.c_int, C.c_uint64, C.c_uint64, C.c_void_p, C.c_void_p]
+        if count is None:
+            count = self.num_connections() - first
+        port, group = np.zeros(count, np.uint8), np.zeros(count, np.uint8)
+        rc = L.oc_read_connection_attributes(self._h, 1 if sorted else 0, int(first), int(count),
+                                             port.ctypes.data_as(C.c_void_p), group.ctypes.data_as(C.c_void_p))
+        if rc != 0:
+            raise OracleError(rc)
+        return port, group
+
     def finalize(self):
         rc = lib().oc_finalize(self._h)
         if rc != 0:

@@ -192,6 +192,8 @@ struct oc_context {
   std::vector<float> w;
   std::vector<uint16_t> d;
   std::vector<uint8_t> bnd;
+  std::vector<uint8_t> port, group; /* receptor port index and synaptic group index of every connection */
+  uint8_t cur_port = 0, cur_group = 0;
   uint64_t n_blocks = 0;
   /* D10: sorted copies. */
   std::vector<uint32_t> perm, ssrc, stgt;
@@ -303,6 +305,8 @@ static int connect_core(oc_context* ctx, uint64_t node_space, oc_range src, oc_r
   ctx->n_blocks += n_newblocks;
   ctx->n_projections += 1;
   ctx->have_in = ctx->have_out = false;
+  ctx->port.resize(ctx->src.size(), ctx->cur_port);   /* the new connections carry the attributes in force */
+  ctx->group.resize(ctx->src.size(), ctx->cur_group);
   return OC_OK;
 }
 
@@ -365,6 +369,7 @@ int oc_connect_values(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src
   if (rc != OC_OK) return rc;
   if (ctx->src.size() - before != n_values) { /* "an array having a size equal to the number of connections" */
     ctx->src.resize(before); ctx->tgt.resize(before); ctx->w.resize(before); ctx->d.resize(before); ctx->bnd.resize(before);
+    ctx->port.resize(before); ctx->group.resize(before);
     ctx->n_blocks = blocks_before;
     ctx->n_projections -= 1;
     return OC_ERR_INVALID_ARG;
@@ -378,6 +383,33 @@ int oc_connect_values(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src
       ctx->d[before + i] = (uint16_t)(int64_t)steps;
       ctx->bnd[before + i] = std::fabs(x - std::floor(x) - 0.5) < 1e-9 ? 1 : 0;
     }
+  }
+  return OC_OK;
+}
+
+/* "The basic structure of a NEST GPU connection includes the source node index, the target node index, the
+ * receptor port index, the weight, the delay, and the synaptic group index.  The synaptic group index takes non-zero
+ * values only for non-static synapses".  Both are set for the connect calls that follow (0, 0 at the start) and
+ * stored with every connection; nothing here interprets them. */
+int oc_set_connection_attributes(oc_context* ctx, uint8_t port, uint8_t syn_group) {
+  if (!ctx) return OC_ERR_INVALID_ARG;
+  if (ctx->finalized) return OC_ERR_STATE;
+  ctx->cur_port = port;
+  ctx->cur_group = syn_group;
+  return OC_OK;
+}
+
+/* entries first .. first+count-1 of the creation-order (sorted = 0) or organised (sorted = 1: entry j is the
+ * connection created at perm[j]) view; either output may be NULL */
+int oc_read_connection_attributes(oc_context* ctx, int sorted, uint64_t first, uint64_t count, uint8_t* port,
+                                  uint8_t* syn_group) {
+  if (!ctx) return OC_ERR_INVALID_ARG;
+  if (sorted && !ctx->finalized) return OC_ERR_STATE;
+  if (first + count > ctx->src.size()) return OC_ERR_INVALID_ARG;
+  for (uint64_t j = 0; j < count; ++j) {
+    const uint64_t pos = sorted ? ctx->perm[first + j] : first + j;
+    if (port) port[j] = ctx->port[pos];
+    if (syn_group) syn_group[j] = ctx->group[pos];
   }
   return OC_OK;
 }

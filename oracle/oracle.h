@@ -107,6 +107,11 @@ int oc_connect_values(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src
                       const uint32_t* tgt_nodes, uint32_t n_tgt, oc_range tgt, int rule, const oc_rule_params* params,
                       const oc_syn_spec* syn, uint64_t seed, const float* weights, const double* delays_ms,
                       uint64_t n_values);
+/* receptor port and synaptic group of the connections created by the connect calls that follow;
+ * oc_read_connection_attributes returns them per connection for either view (HOST arrays, either may be NULL) */
+int oc_set_connection_attributes(oc_context* ctx, uint8_t port, uint8_t syn_group);
+int oc_read_connection_attributes(oc_context* ctx, int sorted, uint64_t first, uint64_t count, uint8_t* port,
+                                  uint8_t* syn_group);
 int oc_finalize(oc_context* ctx);
 int oc_num_connections(oc_context* ctx, uint64_t* n);
 int oc_num_nodes(oc_context* ctx, uint32_t* n);

@@ -27,7 +27,7 @@ SYMBOLS = (
     "nc_finalize", "nc_num_connections", "nc_num_nodes", "nc_get_connections", "nc_get_index",
     "nc_degree_histogram", "nc_get_stats", "nc_get_timings", "nc_read_connections", "nc_read_index",
     "nc_read_degree_histogram", "nc_selftest_philox", "nc_selftest_fastpath",
-    "nc_connect_nodes", "nc_connect_values",
+    "nc_connect_nodes", "nc_connect_values", "nc_set_connection_attributes", "nc_read_connection_attributes",
     # include/nc_delivery.h
     "nc_delivery_create", "nc_delivery_destroy", "nc_delivery_step", "nc_delivery_read_spike_array",
     "nc_delivery_counts",
@@ -138,6 +138,8 @@ def load_library():
     L.nc_get_copass_stats.argtypes = [vp, P(CopassStats)]
     L.nc_connect_values.argtypes = [vp, vp, C.c_uint32, Range, vp, C.c_uint32, Range, C.c_int, vp, vp, C.c_uint64, vp, vp,
                                     C.c_uint64]
+    L.nc_set_connection_attributes.argtypes = [vp, C.c_uint8, C.c_uint8]
+    L.nc_read_connection_attributes.argtypes = [vp, C.c_int, C.c_uint64, C.c_uint64, vp, vp]
     L.nc_delivery_create.argtypes = [vp, C.c_uint32, P(vp)]
     L.nc_delivery_destroy.argtypes = [vp]
     L.nc_delivery_step.argtypes = [vp, vp, vp, C.c_uint32, vp]
@@ -285,6 +287,17 @@ class NC:
 
     def connect(self, *a, **k):
         self._check(self.connect_rc(*a, **k))
+
+    def set_connection_attributes(self, port: int, syn_group: int = 0):
+        self._check(self._L.nc_set_connection_attributes(self._h, int(port), int(syn_group)))
+
+    def read_connection_attributes(self, sorted: bool = False, first: int = 0, count: int | None = None):
+        if count is None:
+            count = self.num_connections() - first
+        port, group = np.zeros(int(count), np.uint8), np.zeros(int(count), np.uint8)
+        self._check(self._L.nc_read_connection_attributes(self._h, 1 if sorted else 0, int(first), int(count), _ptr(port),
+                                                          _ptr(group)))
+        return port, group
 
     def finalize(self):
         self._check(self._L.nc_finalize(self._h))

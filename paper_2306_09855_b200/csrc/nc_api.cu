@@ -72,6 +72,9 @@ struct nc_context {
   bool organised_in_blocks = false; // nc_finalize left the organised connections in the storage blocks
   CopassTotals* d_copass_totals = nullptr;
   uint64_t copass_aux_bytes = 0, copass_moved = 0;
+  uint8_t cur_port = 0, cur_group = 0;       // attributes in force for the next nc_connect*
+  std::vector<uint32_t> proj_first;          // creation position of the first connection of every projection
+  std::vector<uint16_t> proj_attr;           // port | syn_group << 8 of every projection
   bool broken = false;  // an in-place organisation failed half way: the connections are lost, only nc_destroy is left
 
   // allocations
@@ -1646,6 +1649,8 @@ static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, 
     c->n_conns += n_new;
   }
   c->n_proj += 1;
+  c->proj_first.push_back((uint32_t)gp.pos0);
+  c->proj_attr.push_back((uint16_t)(c->cur_port | (c->cur_group << 8)));
   if (bound > (double)c->max_delay_steps) c->max_delay_steps = (uint32_t)bound;
   c->have_in = c->have_out = false;
   return NC_OK;
@@ -1867,6 +1872,44 @@ int nc_read_connections(nc_context* c, int sorted, uint64_t first, uint64_t coun
       done += m;
     }
   }
+  return sync_stream(c);
+}
+
+int nc_set_connection_attributes(nc_context* c, uint8_t port, uint8_t syn_group) {
+  if (!c) return NC_ERR_INVALID_ARG;
+  if (c->finalized) return fail(c, NC_ERR_STATE, "nc_set_connection_attributes after nc_finalize");
+  c->cur_port = port;
+  c->cur_group = syn_group;
+  return NC_OK;
+}
+
+int nc_read_connection_attributes(nc_context* c, int sorted, uint64_t first, uint64_t count, uint8_t* port,
+                                  uint8_t* syn_group) {
+  if (!c) return NC_ERR_INVALID_ARG;
+  if (c->broken) return fail(c, NC_ERR_STATE, "a failed in-place organisation left this context without connections");
+  if (first + count > c->n_conns) return fail(c, NC_ERR_INVALID_ARG, "nc_read_connection_attributes: range outside the connections");
+  if (sorted && !c->finalized) return fail(c, NC_ERR_STATE, "sorted view before nc_finalize");
+  if (!sorted && c->organised_in_blocks)
+    return fail(c, NC_ERR_STATE, "the creation-order view is gone: the blocks were organised in place (COPASS)");
+  if (count == 0 || (!port && !syn_group)) return NC_OK;
+  const uint32_t np = (uint32_t)c->proj_first.size();
+  uint32_t* d_first = (uint32_t*)dev_alloc(c, (size_t)np * 4);
+  uint16_t* d_attr = (uint16_t*)dev_alloc(c, (size_t)np * 2);
+  uint8_t* d_port = port ? (uint8_t*)dev_alloc(c, count) : nullptr;
+  uint8_t* d_group = syn_group ? (uint8_t*)dev_alloc(c, count) : nullptr;
+  dev_free_later(c, d_first); dev_free_later(c, d_attr); dev_free_later(c, d_port); dev_free_later(c, d_group);
+  if (!d_first || !d_attr || (port && !d_port) || (syn_group && !d_group))
+    return fail(c, NC_ERR_OOM, "out of device memory in nc_read_connection_attributes");
+  NC_CUDA(c, cudaMemcpyAsync(d_first, c->proj_first.data(), (size_t)np * 4, cudaMemcpyHostToDevice, c->stream));
+  NC_CUDA(c, cudaMemcpyAsync(d_attr, c->proj_attr.data(), (size_t)np * 2, cudaMemcpyHostToDevice, c->stream));
+  const uint32_t* perm = (sorted && !c->organised_in_blocks) ? c->perm : nullptr;
+  const uint64_t perm_off = (sorted && c->organised_in_blocks) ? c->off_perm : 0;
+  const unsigned grid = (unsigned)std::min<uint64_t>((count + 255) / 256, 148 * 16);
+  attribute_lookup_kernel<<<grid, 256, 0, c->stream>>>(make_map(c), perm, perm_off, first, count, d_first, np, d_attr, d_port,
+                                                       d_group);
+  NC_LAUNCH_CHECK(c, "attribute_lookup");
+  if (port) NC_CUDA(c, cudaMemcpyAsync(port, d_port, count, cudaMemcpyDeviceToHost, c->stream));
+  if (syn_group) NC_CUDA(c, cudaMemcpyAsync(syn_group, d_group, count, cudaMemcpyDeviceToHost, c->stream));
   return sync_stream(c);
 }
 

@@ -420,4 +420,34 @@ __global__ void __launch_bounds__(256) max_u32_kernel(const uint32_t* __restrict
   if (lane_id() == 0 && m) atomicMax(out, m);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Receptor port and synaptic group are constants of a projection: they are kept per projection and an
+// entry of either view is resolved through its creation position (binary search over the projections' first
+// positions).  perm == NULL and perm_off == 0: the creation-order view (position = entry); perm != NULL: the flat
+// organised view; perm_off != 0: the organised view inside the storage blocks (creation positions at perm_off).
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) attribute_lookup_kernel(const __grid_constant__ BlockMap map, const uint32_t* __restrict__ perm,
+                                                              uint64_t perm_off, uint64_t first, uint64_t count,
+                                                              const uint32_t* __restrict__ proj_first, uint32_t n_proj,
+                                                              const uint16_t* __restrict__ proj_attr,
+                                                              uint8_t* __restrict__ port, uint8_t* __restrict__ group) {
+  for (uint64_t j = (uint64_t)blockIdx.x * 256u + threadIdx.x; j < count; j += (uint64_t)gridDim.x * 256u) {
+    uint32_t pos = (uint32_t)(first + j);
+    if (perm) {
+      pos = perm[first + j];
+    } else if (perm_off) {
+      const BlockAddr a = locate(map, first + j);
+      pos = reinterpret_cast<const uint32_t*>(a.base + perm_off)[a.slot];
+    }
+    uint32_t lo = 0, hi = n_proj;  // last projection with proj_first <= pos (empty projections share their start
+    while (hi - lo > 1) {          // with the next one and are skipped by taking the last)
+      const uint32_t mid = (lo + hi) >> 1;
+      if (proj_first[mid] <= pos) lo = mid; else hi = mid;
+    }
+    const uint16_t a = proj_attr[lo];
+    if (port) port[j] = (uint8_t)(a & 0xffu);
+    if (group) group[j] = (uint8_t)(a >> 8);
+  }
+}
+
 }  // namespace nc

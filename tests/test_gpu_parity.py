@@ -506,3 +506,33 @@ def test_value_arrays_parity(nc_mod, oracle_mod):
         assert b.connect_rc((0, 20), (0, 20), WL.RULE_IDS["pairwise_bernoulli"], p=0.5, weights=np.zeros(200)) == nc_mod.ERR_INVALID_ARG
         assert b.num_connections() == 0
     g.close(); o.close(); g2.close(); o2.close()
+
+
+@pytest.mark.parametrize("variant", ["default", "pairs", "copass", "copass_shift"])
+def test_connection_attributes_parity(nc_mod, oracle_mod, variant):
+    """nc_set_connection_attributes / nc_read_connection_attributes (receptor port, synaptic group): the
+    pair in force belongs to the connections of the following connect calls (an empty projection in between included)
+    and is returned for the creation-order and the organised view, flat or inside the storage blocks."""
+    flags = {"default": 0, "pairs": nc_mod.FLAG_SORT_PAIRS, "copass": nc_mod.FLAG_ORGANISE_COPASS,
+             "copass_shift": nc_mod.FLAG_ORGANISE_COPASS | nc_mod.FLAG_COPASS_SHIFT}[variant]
+    o, g = oracle_mod.Oracle(dt_ms=0.1, block_size=3000), nc_mod.NC(dt_ms=0.1, block_size=3000, flags=flags)
+    calls = [((0, 0), "fixed_total_number", dict(degree_or_total=7000)), ((3, 0), "all_to_all", {}),
+             ((9, 9), "pairwise_bernoulli", dict(p=0.0)),  # creates nothing
+             ((255, 7), "pairwise_bernoulli", dict(p=0.3)), ((1, 1), "fixed_indegree", dict(degree_or_total=11))]
+    for b in (o, g):
+        b.create_population(120)
+        for (port, group), rule, kw in calls:
+            b.set_connection_attributes(port, group)
+            b.connect((0, 120), (0, 120), WL.RULE_IDS[rule], weight=W, delay_ms=D, seed=5, **kw)
+    po, go = o.read_connection_attributes(sorted=False)
+    pg, gg = g.read_connection_attributes(sorted=False)
+    assert np.array_equal(pg, po) and np.array_equal(gg, go) and set(po.tolist()) == {0, 3, 255, 1}
+    for b in (o, g):
+        b.finalize()
+    PU.compare_connections(g.read_connections(sorted=True), o.connections(sorted=True), 22.0, "attributes " + variant)
+    po, go = o.read_connection_attributes(sorted=True)
+    pg, gg = g.read_connection_attributes(sorted=True)
+    assert np.array_equal(pg, po) and np.array_equal(gg, go)
+    p2, g2 = g.read_connection_attributes(sorted=True, first=4321, count=5000)
+    assert np.array_equal(p2, po[4321:9321]) and np.array_equal(g2, go[4321:9321])
+    g.close(); o.close()
