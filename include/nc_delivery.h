@@ -9,7 +9,7 @@
  *
  * Readings: F1 one step = advance, collect matured, deliver, then insert the spikes
  * emitted in this step, so a spike emitted in step k reaches a connection of delay d in step k + d; F2 the input of
- * a node is one fp32 accumulator per node (receptor port 0, Q12), every connection adds weight * multiplicity;
+ * a node is one fp32 accumulator per (receptor port, node), every connection adds weight * multiplicity;
  * F3 group indexes in the spike array are global (group_ptr[source] + local index, Eq. 14).
  *
  * Conventions as in nc.h: int status returns, no exceptions; all work is enqueued on the context's stream; the
@@ -32,8 +32,13 @@ typedef struct nc_delivery nc_delivery; /* opaque */
 int nc_delivery_create(nc_context* ctx, uint32_t capacity, nc_delivery** out);
 int nc_delivery_destroy(nc_delivery* d);
 
+/* Number of receptor ports in use: 1 + the largest port any projection was given (nc_set_connection_attributes,
+ * PAPER.md:53); 1 unless ports were set. */
+int nc_delivery_num_ports(nc_delivery* d, uint32_t* n_ports);
+
 /* One simulation step (asynchronous).  d_nodes[n_new]: nodes that emit a spike in this step; d_mult[n_new]: their
- * multiplicities (NULL = 1 each; 0 = no spike).  d_input[n_nodes] (fp32) is ACCUMULATED into with atomic adds, so
+ * multiplicities (NULL = 1 each; 0 = no spike).  d_input[n_ports * n_nodes] (fp32; the input of receptor port p of
+ * node t is entry p * n_nodes + t) is ACCUMULATED into with atomic adds, so
  * the caller zeroes it when a neuron model has consumed it.  A node id >= n_nodes or a full buffer drops the spike
  * and is reported by nc_delivery_counts (never silently). */
 int nc_delivery_step(nc_delivery* d, const uint32_t* d_nodes, const uint32_t* d_mult, uint32_t n_new, float* d_input);

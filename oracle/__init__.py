@@ -348,11 +348,15 @@ class Delivery:
         if rc != 0:
             raise OracleError(rc)
         self.n_nodes = oracle.num_nodes()
+        L.oc_delivery_num_ports.argtypes = [C.c_void_p, C.POINTER(C.c_uint32)]
+        np_ = C.c_uint32()
+        L.oc_delivery_num_ports(self._h, C.byref(np_))
+        self.n_ports = np_.value
 
     def step(self, nodes, mult, input_f64):
         nodes = np.ascontiguousarray(nodes, dtype=np.uint32)
         m = None if mult is None else np.ascontiguousarray(mult, dtype=np.uint32)
-        assert input_f64.dtype == np.float64 and input_f64.size == self.n_nodes and input_f64.flags.c_contiguous
+        assert input_f64.dtype == np.float64 and input_f64.size == self.n_nodes * self.n_ports and input_f64.flags.c_contiguous
         rc = self._L.oc_delivery_step(self._h, nodes.ctypes.data_as(C.c_void_p),
                                       None if m is None else m.ctypes.data_as(C.c_void_p), nodes.size,
                                       input_f64.ctypes.data_as(C.c_void_p))

@@ -1,6 +1,7 @@
 // delivery.cpp -- see delivery.h.  Plain loops in the paper's order; test infrastructure only.
 #include "delivery.h"
 
+#include <algorithm>
 #include <deque>
 #include <vector>
 
@@ -15,6 +16,8 @@ struct oc_delivery {
   oc_index_view idx;
   std::vector<std::deque<Spike>> queue;  // one per node
   std::vector<uint32_t> arr_group, arr_mult;
+  std::vector<uint8_t> port;  // receptor port of every organised connection
+  uint32_t n_ports = 1;
   uint64_t events = 0;
 };
 
@@ -30,6 +33,12 @@ int oc_delivery_create(oc_context* ctx, oc_delivery** out) {
     return rc;
   }
   d->queue.resize(d->idx.n_nodes);
+  d->port.resize(d->conn.n);
+  if (d->conn.n && oc_read_connection_attributes(ctx, 1, 0, d->conn.n, d->port.data(), nullptr) != 0) {
+    delete d;
+    return -1;
+  }
+  for (uint8_t p : d->port) d->n_ports = std::max<uint32_t>(d->n_ports, (uint32_t)p + 1u);
   *out = d;
   return 0;
 }
@@ -64,7 +73,8 @@ int oc_delivery_step(oc_delivery* d, const uint32_t* nodes, const uint32_t* mult
     const uint32_t g = d->arr_group[e];
     const uint64_t c0 = d->idx.group_start[g];
     const uint64_t c1 = g + 1 < d->idx.total_groups ? d->idx.group_start[g + 1] : d->conn.n;
-    for (uint64_t c = c0; c < c1; ++c) input[d->conn.target[c]] += (double)d->conn.weight[c] * (double)d->arr_mult[e];
+    for (uint64_t c = c0; c < c1; ++c)  // reading F2: one input per (receptor port, node), port-major
+      input[(uint64_t)d->port[c] * d->idx.n_nodes + d->conn.target[c]] += (double)d->conn.weight[c] * (double)d->arr_mult[e];
     d->events += c1 - c0;
   }
   // the spikes emitted in this step (a node without outgoing connections buffers nothing)
@@ -80,6 +90,12 @@ int oc_delivery_spike_array(oc_delivery* d, const uint32_t** group, const uint32
   *group = d->arr_group.data();
   *mult = d->arr_mult.data();
   *n = (uint32_t)d->arr_group.size();
+  return 0;
+}
+
+int oc_delivery_num_ports(oc_delivery* d, uint32_t* n_ports) {
+  if (!d || !n_ports) return -1;
+  *n_ports = d->n_ports;
   return 0;
 }
 

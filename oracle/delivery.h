@@ -12,7 +12,7 @@
  *
  * Readings: F1 one step = advance, collect matured, deliver, THEN insert the spikes
  * emitted in this step (time index 0), so a spike emitted in step k reaches a connection of delay d in step k + d;
- * F2 the "input" of a node is one fp accumulator per node (receptor port 0, Q12), summed here in fp64;
+ * F2 the "input" of a node is one fp accumulator per (receptor port, node), summed here in fp64;
  * F3 the group index in the spike array is the global one, group_ptr[source] + local index (Eq. 14).
  */
 #ifndef ORACLE_DELIVERY_H_
@@ -26,11 +26,12 @@ typedef struct oc_delivery oc_delivery;
 /* ctx must be finalized and outlive the delivery object */
 int oc_delivery_create(oc_context* ctx, oc_delivery** out);
 int oc_delivery_destroy(oc_delivery* d);
-/* One step.  nodes/mult: the n_new spikes emitted in this step (mult NULL = 1 each).  input[n_nodes] (fp64) is
- * ACCUMULATED into.  Returns OC_OK or a negative oc status (node out of range). */
+/* One step.  nodes/mult: the n_new spikes emitted in this step (mult NULL = 1 each).  input[n_ports * n_nodes] (fp64,
+ * entry port * n_nodes + node; n_ports = 1 + the largest receptor port in use) is ACCUMULATED into.  Returns OC_OK or a negative oc status (node out of range). */
 int oc_delivery_step(oc_delivery* d, const uint32_t* nodes, const uint32_t* mult, uint32_t n_new, double* input);
 /* the spike array of the last step: global group index and multiplicity per entry, in queue order */
 int oc_delivery_spike_array(oc_delivery* d, const uint32_t** group, const uint32_t** mult, uint32_t* n);
+int oc_delivery_num_ports(oc_delivery* d, uint32_t* n_ports);
 /* spikes still buffered, and connections delivered so far */
 int oc_delivery_counts(oc_delivery* d, uint64_t* buffered, uint64_t* events);
 #ifdef __cplusplus

@@ -30,7 +30,7 @@ SYMBOLS = (
     "nc_connect_nodes", "nc_connect_values", "nc_set_connection_attributes", "nc_read_connection_attributes",
     # include/nc_delivery.h
     "nc_delivery_create", "nc_delivery_destroy", "nc_delivery_step", "nc_delivery_read_spike_array",
-    "nc_delivery_counts",
+    "nc_delivery_counts", "nc_delivery_num_ports",
     # include/nc_copass.h
     "nc_copass_partition", "nc_get_copass_stats",
 )
@@ -142,6 +142,7 @@ def load_library():
     L.nc_read_connection_attributes.argtypes = [vp, C.c_int, C.c_uint64, C.c_uint64, vp, vp]
     L.nc_delivery_create.argtypes = [vp, C.c_uint32, P(vp)]
     L.nc_delivery_destroy.argtypes = [vp]
+    L.nc_delivery_num_ports.argtypes = [vp, P(C.c_uint32)]
     L.nc_delivery_step.argtypes = [vp, vp, vp, C.c_uint32, vp]
     L.nc_delivery_read_spike_array.argtypes = [vp, vp, vp, C.c_uint32, P(C.c_uint32)]
     L.nc_delivery_counts.argtypes = [vp, P(C.c_uint64), P(C.c_uint64), P(C.c_uint64), P(C.c_uint64)]
@@ -409,10 +410,13 @@ class Delivery:
         self._h = C.c_void_p()
         nc._check(self._L.nc_delivery_create(nc._h, int(capacity), C.byref(self._h)))
         self.capacity = int(capacity)
+        n_ports = C.c_uint32()
+        nc._check(self._L.nc_delivery_num_ports(self._h, C.byref(n_ports)))
+        self.n_ports = n_ports.value
 
     def step(self, nodes, mult, input_f32, n_new=None):
         n = int(nodes.numel()) if n_new is None else int(n_new)
-        assert input_f32.is_cuda and input_f32.element_size() == 4 and input_f32.numel() == self._nc.num_nodes()
+        assert input_f32.is_cuda and input_f32.element_size() == 4 and input_f32.numel() == self._nc.num_nodes() * self.n_ports
         assert nodes.is_cuda and nodes.element_size() == 4 and (mult is None or (mult.is_cuda and mult.element_size() == 4))
         self._nc._check(self._L.nc_delivery_step(self._h, nodes.data_ptr() if n else None,
                                                  mult.data_ptr() if (mult is not None and n) else None, n,

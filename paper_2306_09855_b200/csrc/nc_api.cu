@@ -75,6 +75,7 @@ struct nc_context {
   uint8_t cur_port = 0, cur_group = 0;       // attributes in force for the next nc_connect*
   std::vector<uint32_t> proj_first;          // creation position of the first connection of every projection
   std::vector<uint16_t> proj_attr;           // port | syn_group << 8 of every projection
+  uint8_t* d_sorted_port = nullptr;          // port of every organised connection, built on first use by delivery
   bool broken = false;  // an in-place organisation failed half way: the connections are lost, only nc_destroy is left
 
   // allocations
@@ -2057,6 +2058,29 @@ int nc_internal_organised_view(nc_context* c, nc_organised_view* out) {
   } else {
     out->target = c->s_tgt;
     out->weight = c->s_w;
+  }
+  // receptor ports: materialised once, only if some projection uses a port other than 0
+  uint32_t max_port = 0;
+  for (uint16_t a : c->proj_attr) max_port = std::max<uint32_t>(max_port, a & 0xffu);
+  out->n_ports = max_port + 1;
+  if (max_port > 0 && c->n_conns > 0) {
+    if (!c->d_sorted_port) {
+      const uint32_t np = (uint32_t)c->proj_first.size();
+      uint32_t* d_first = (uint32_t*)dev_alloc(c, (size_t)np * 4);
+      uint16_t* d_attr = (uint16_t*)dev_alloc(c, (size_t)np * 2);
+      c->d_sorted_port = (uint8_t*)dev_alloc(c, c->n_conns);
+      dev_free_later(c, d_first);
+      dev_free_later(c, d_attr);
+      if (!d_first || !d_attr || !c->d_sorted_port) return fail(c, NC_ERR_OOM, "out of device memory for the receptor ports");
+      NC_CUDA(c, cudaMemcpyAsync(d_first, c->proj_first.data(), (size_t)np * 4, cudaMemcpyHostToDevice, c->stream));
+      NC_CUDA(c, cudaMemcpyAsync(d_attr, c->proj_attr.data(), (size_t)np * 2, cudaMemcpyHostToDevice, c->stream));
+      const unsigned grid = (unsigned)std::min<uint64_t>((c->n_conns + 255) / 256, 148 * 16);
+      attribute_lookup_kernel<<<grid, 256, 0, c->stream>>>(make_map(c), c->organised_in_blocks ? nullptr : c->perm,
+                                                           c->organised_in_blocks ? c->off_perm : 0, 0, c->n_conns, d_first,
+                                                           np, d_attr, c->d_sorted_port, nullptr);
+      NC_LAUNCH_CHECK(c, "attribute_lookup");
+    }
+    out->port = c->d_sorted_port;
   }
   out->group_ptr = c->group_ptr;
   out->group_start = c->group_start;

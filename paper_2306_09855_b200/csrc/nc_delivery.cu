@@ -124,9 +124,12 @@ __global__ void __launch_bounds__(256) deliver_kernel(const __grid_constant__ De
         const char* base = reinterpret_cast<const char*>(p.v.block_table[blk]);
         const uint32_t t = reinterpret_cast<const uint32_t*>(base + p.v.off_target)[slot];
         const float w = reinterpret_cast<const float*>(base + p.v.off_weight)[slot];
-        atomicAdd(p.input + t, w * m);
+        const uint64_t in = p.v.port ? (uint64_t)p.v.port[c] * p.v.n_nodes + t : t;  // input of (port, node)
+        atomicAdd(p.input + in, w * m);
       } else {
-        atomicAdd(p.input + p.v.target[c], p.v.weight[c] * m);
+        const uint32_t t = p.v.target[c];
+        const uint64_t in = p.v.port ? (uint64_t)p.v.port[c] * p.v.n_nodes + t : t;
+        atomicAdd(p.input + in, p.v.weight[c] * m);
       }
     }
     ev += c1 - c0;
@@ -229,6 +232,12 @@ int nc_delivery_step(nc_delivery* d, const uint32_t* d_nodes, const uint32_t* d_
   d->cur = 1 - d->cur;
   if (cudaPeekAtLastError() != cudaSuccess)
     return nc_internal_fail(d->ctx, NC_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));
+  return NC_OK;
+}
+
+int nc_delivery_num_ports(nc_delivery* d, uint32_t* n_ports) {
+  if (!d || !n_ports) return NC_ERR_INVALID_ARG;
+  *n_ports = d->v.n_ports;
   return NC_OK;
 }
 

@@ -14,6 +14,8 @@ struct nc_organised_view {  // borrowed device pointers, valid until nc_destroy
   const uint32_t* group_ptr;    // [n_nodes + 1]
   const uint32_t* group_start;  // [total_groups]
   const uint16_t* group_delay;  // [total_groups]
+  const uint8_t* port;          // receptor port of every organised connection, NULL when every port is 0
+  uint32_t n_ports;             // 1 + the largest port in use
   uint32_t n_nodes, total_groups;
   uint64_t n;
   cudaStream_t stream;

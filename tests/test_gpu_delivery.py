@@ -104,3 +104,34 @@ def test_delivery_edge_cases(nc_mod, oracle_mod):
     d2.step(torch.tensor([7, 8, 9], dtype=torch.int32, device="cuda"), mult0, inp)  # multiplicity 0 = no spike
     assert d2.counts()["buffered"] == 0
     d.close(); d2.close(); g.close()
+
+
+@pytest.mark.parametrize("copass", [False, True], ids=["flat", "blocks"])
+def test_delivery_with_receptor_ports(nc_mod, oracle_mod, copass):
+    """Projections with different receptor ports (nc_set_connection_attributes): every (port, node) input
+    equals the oracle's, over the flat organised arrays and over COPASS-organised blocks."""
+    import torch
+    o = oracle_mod.Oracle(dt_ms=0.1, block_size=500)
+    g = nc_mod.NC(dt_ms=0.1, block_size=500, flags=nc_mod.FLAG_ORGANISE_COPASS if copass else 0)
+    W, D = (5.0, 1.0, 0.0, float("inf")), (1.0, 0.5, 0.1, float("inf"))
+    for b in (o, g):
+        b.create_population(60)
+        for k, port in enumerate([0, 3, 1, 3, 0]):
+            b.set_connection_attributes(port)
+            b.connect((0, 60), (0, 60), 4, degree_or_total=700, weight=W, delay_ms=D, seed=20 + k)  # fixed_total_number
+        b.finalize()
+    od, gd = oracle_mod.Delivery(o), nc_mod.Delivery(g, 4096)
+    assert gd.n_ports == od.n_ports == 4
+    inp = torch.zeros(4 * 60, dtype=torch.float32, device="cuda")
+    rng = np.random.default_rng(6)
+    for k in range(70):
+        nodes = rng.choice(60, size=int(rng.integers(0, 8)) if k < 30 else 0, replace=False).astype(np.uint32)
+        want = np.zeros(4 * 60)
+        od.step(nodes, None, want)
+        inp.zero_()
+        gd.step(torch.from_numpy(nodes.astype(np.int32)).cuda(), None, inp)
+        got = inp.cpu().numpy()
+        assert np.abs(got - want).max() <= 1e-5 * max(1.0, np.abs(want).max()), k
+        assert not got.reshape(4, 60)[2].any()  # port 2 is unused
+    assert gd.counts()["events"] == od.counts()[1] > 0
+    gd.close(); od.close(); g.close(); o.close()

@@ -120,3 +120,35 @@ def test_groups_mature_in_ascending_delay_order(oracle_mod):
     assert [k for k, _ in order] == [int(x) for x in idx["group_delay"][:G]]
     d.close()
     o.close()
+
+
+def test_delivery_with_receptor_ports_matches_the_definition(oracle_mod):
+    """Connections created under nc/oc_set_connection_attributes(port) deliver into the input of (port, target)
+    (reading F2): the plain definition evaluated per port from the creation-order arrays."""
+    o = oracle_mod.Oracle(dt_ms=0.1)
+    o.create_population(40)
+    W, D = (5.0, 1.0, 0.0, INF), (1.0, 0.5, 0.1, INF)
+    ports = [0, 2, 1, 2]
+    for k, port in enumerate(ports):
+        o.set_connection_attributes(port)
+        o.connect((0, 40), (0, 40), oracle_mod.FIXED_TOTAL_NUMBER, degree_or_total=300, weight=W, delay_ms=D, seed=3 + k)
+    conn = o.connections(sorted=False)
+    port_of = o.read_connection_attributes(sorted=False)[0]
+    assert np.array_equal(port_of, np.repeat(np.array(ports, np.uint8), 300))
+    o.finalize()
+    rng = np.random.default_rng(11)
+    steps, tail = 30, 40
+    raster = _raster(rng, 40, steps, 0.1)
+    want = np.zeros((steps + tail, 3, 40))
+    for p in range(3):
+        sel = port_of == p
+        sub = {f: conn[f][sel] for f in ("source", "target", "weight", "delay")}
+        want[:, p, :] = _definition(sub, 40, raster, steps + tail)
+    d = oracle_mod.Delivery(o)
+    assert d.n_ports == 3
+    for k in range(steps + tail):
+        nodes, mult = raster[k] if k < steps else (np.zeros(0, np.uint32), np.zeros(0, np.uint32))
+        got = np.zeros(3 * 40)
+        d.step(nodes, mult, got)
+        np.testing.assert_allclose(got.reshape(3, 40), want[k], rtol=1e-12, atol=1e-9, err_msg=f"step {k}")
+    d.close(); o.close()
