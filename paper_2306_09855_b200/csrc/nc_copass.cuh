@@ -7,11 +7,19 @@
 //   (C) COPASS partition: a common threshold t and left partition sizes m_i with sum m_i = N_b (Sec. A2-A4)
 //                                                              -> copass_partition_kernel (one CTA, one warp per
 //                                                                 subarray, 32-ary searches)
-//   (D) left partitions -> auxiliary array                     -> copass_gather_kernel
-//   (E) right partitions shifted right, block b freed          -> copass_gather_kernel per destination block into a
+//   (D) left partitions -> auxiliary array                     -> copass_segcopy_kernel (copass_gather_kernel)
+//   (E) right partitions shifted right, block b freed          -> replaced by default: the k-1 partitions are taken at once
+//                                                                 on the sorted blocks, the subarrays are kept as
+//                                                                 extent lists, and after gathering an output block
+//                                                                 ONE block is emptied into the holes the left
+//                                                                 partitions left (copass_segcopy_kernel; host plan
+//                                                                 in nc_api.cu, copass_extract_fill).  The shift to
+//                                                                 the letter (NC_FLAG_COPASS_SHIFT):
+//                                                                 copass_gather_kernel per destination block into a
 //                                                                 spare block, then the two block pointers are
 //                                                                 swapped (no overlapping move, each byte moved once)
-//   (F) auxiliary array sorted into block b                    -> radix passes again
+//   (F) auxiliary array sorted into block b                    -> radix passes again; the last pass writes the block's
+//                                                                 final arrays
 // While this runs a block holds 16-byte records (key, creation position, target, weight), key = (source <<
 // delay_bits) | delay: every move is a 128-bit copy whatever the shift.  Logical positions 0 .. n-1 map to
 // (block, slot) through the same BlockMap as the creation-order storage (pos / B, pos % B).
