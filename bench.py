@@ -6,7 +6,7 @@ cortical-microcircuit-shaped workload (BASELINE.json configs[2]: 77,169 neurons,
     python bench.py --impl reference --steps K --warmup W    # the CPU oracle on a bounded sample
 
 One "step" = one pass of the whole hot path: create the populations, issue all 55 nc_connect calls (rule
-expansion + draws + append into block storage), nc_finalize (histogram, onesweep passes, permute, index).
+expansion + draws + append into block storage), nc_finalize (per-pass digit counts and scans, record-carrying digit passes, index).
 Prints ONE JSON line on rank 0.  See DESIGN.md "Measurement" for how every field is obtained.
 """
 from __future__ import annotations

@@ -165,7 +165,7 @@ typedef struct {
 typedef enum {
   NC_PHASE_GENERATE = 0, /* rule expansion + draws + append (nc_connect) */
   NC_PHASE_HISTOGRAM = 1, /* sort: digit histograms over the packed (source, delay) key */
-  NC_PHASE_SORT = 2,     /* sort: onesweep digit passes */
+  NC_PHASE_SORT = 2,     /* sort: digit passes (scatter kernels) */
   NC_PHASE_PERMUTE = 3,  /* materialise sorted source/target/weight/delay */
   NC_PHASE_INDEX = 4,    /* head flags, scans, group compaction */
   NC_PHASE_DEGREE = 5,   /* nc_degree_histogram */
@@ -176,8 +176,8 @@ typedef enum {
 typedef struct {
   double ms[NC_PHASE_COUNT];          /* device time per phase, summed over the context's life */
   uint32_t launches[NC_PHASE_COUNT];  /* kernels launched per phase */
-  double sort_pass_ms;                /* device time of the onesweep pass kernels alone */
-  uint32_t sort_passes;               /* how many onesweep pass kernels ran */
+  double sort_pass_ms;                /* device time of the digit-pass kernels alone */
+  uint32_t sort_passes;               /* how many digit-pass kernels ran */
 } nc_timings;
 
 typedef struct {
