@@ -275,3 +275,22 @@ def test_copass_capacity_errors_leave_the_connections_intact(nc_mod, oracle_mod)
     assert e.value.code == nc_mod.ERR_CAPACITY
     PU.compare_connections(g.read_connections(sorted=False), o.connections(sorted=False), 1.1, "after a refused finalize")
     g.close(); o.close()
+
+
+@pytest.mark.parametrize("shift", [False, True], ids=["fill", "shift"])
+def test_copass_single_digit_pass_key(nc_mod, oracle_mod, shift):
+    """Four nodes and delays of at most 7 steps: the (source, delay) key has 5 bits, the underlying sort is ONE digit
+    pass -- the path where a sorted block cannot be written over its own input."""
+    flags = nc_mod.FLAG_ORGANISE_COPASS | (nc_mod.FLAG_COPASS_SHIFT if shift else 0)
+    o, g = oracle_mod.Oracle(dt_ms=0.1, block_size=300), nc_mod.NC(dt_ms=0.1, block_size=300, flags=flags)
+    for b in (o, g):
+        b.create_population(4)
+        b.connect((0, 4), (0, 4), WL.RULE_IDS["fixed_total_number"], degree_or_total=2500, weight=(1.0, 0.2, 0.0, float("inf")),
+                  delay_ms=(0.4, 0.1, 0.1, 0.7), seed=12)
+        b.finalize()
+    st = g.stats()
+    assert st["sort_passes"] == 1 and st["key_bits"] <= 8
+    PU.compare_connections(g.read_connections(sorted=True), o.connections(sorted=True), 2.0, "single pass")
+    PU.compare_index(g.read_index(), o.index(), "single pass")
+    assert g.copass_stats()["n_blocks"] == 9
+    g.close(); o.close()
