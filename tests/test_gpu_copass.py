@@ -294,3 +294,18 @@ def test_copass_single_digit_pass_key(nc_mod, oracle_mod, shift):
     PU.compare_index(g.read_index(), o.index(), "single pass")
     assert g.copass_stats()["n_blocks"] == 9
     g.close(); o.close()
+
+
+@pytest.mark.parametrize("shift", [False, True], ids=["fill", "shift"])
+def test_copass_with_the_library_allocator(nc_mod, oracle_mod, shift):
+    """mem.alloc == NULL: cudaMalloc / cudaFree inside the library (no caching allocator underneath the block swaps)."""
+    net = WL.config1_rule("fixed_outdegree", scale=0.1)
+    o = oracle_mod.Oracle(dt_ms=net.dt_ms, block_size=40_000)
+    WL.run(net, o)
+    flags = nc_mod.FLAG_ORGANISE_COPASS | (nc_mod.FLAG_COPASS_SHIFT if shift else 0)
+    g = nc_mod.NC(dt_ms=net.dt_ms, block_size=40_000, flags=flags, use_torch_allocator=False)
+    WL.run(net, g)
+    PU.compare_connections(g.read_connections(sorted=True), o.connections(sorted=True), PU.weight_scale(net), "cudaMalloc")
+    PU.compare_index(g.read_index(), o.index(), "cudaMalloc")
+    assert g.copass_stats()["n_blocks"] >= 4
+    g.close(); o.close()
