@@ -8,12 +8,16 @@
 //                           and the spikes emitted in this step are appended behind them (warp-aggregated atomics);
 //   deliver_kernel        : one warp per spike-array entry, lanes over the connections of the group (coalesced
 //                           reads of target and weight, one float atomic add per connection).
-// Counts stay on the device: the host never waits inside a step.
+// Counts stay on the device: the host never waits inside a step.  Where the device supports cooperative launches the
+// two kernels run as ONE launch per step (fused_step_kernel: a grid-wide barrier between them, the counters of the next
+// step cleared behind it), which halves the cost of a step at biological rates, where a step is launch-bound.
 #include "../../include/nc_delivery.h"
 
+#include <cooperative_groups.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cstdlib>
 #include <new>
 
 #include "nc_common.cuh"
@@ -25,9 +29,9 @@ namespace {
 
 struct Counters {
   uint32_t n_live_a;   // entries of live list A
-  uint32_t n_arr;      // entries of the spike array
+  uint32_t n_arr;      // entries of the spike array (two-kernel step; even steps of the fused step)
   uint32_t n_live_b;   // entries of live list B
-  uint32_t pad_;
+  uint32_t n_arr_odd;  // entries of the spike array, odd steps of the fused step
   unsigned long long events, dropped, bad_nodes;
 };
 
@@ -56,7 +60,7 @@ __device__ __forceinline__ uint32_t warp_reserve(uint32_t* counter, bool want) {
 
 constexpr int kStepThreads = 256;
 
-__global__ void __launch_bounds__(kStepThreads) advance_insert_kernel(const __grid_constant__ StepParams p) {
+__device__ __forceinline__ void advance_insert_body(const StepParams& p) {
   const uint32_t n_live = min(*p.n_live_in, p.capacity);
   const uint32_t total = n_live + p.n_new;
   const uint32_t rounds = (total + gridDim.x * kStepThreads - 1) / (gridDim.x * kStepThreads);
@@ -108,8 +112,12 @@ struct DeliverParams {
 
 // BLOCKS: the organised connections live in the storage blocks (COPASS organisation); position c is entry c % B of
 // block c / B, a group may straddle two blocks.
+__global__ void __launch_bounds__(kStepThreads) advance_insert_kernel(const __grid_constant__ StepParams p) {
+  advance_insert_body(p);
+}
+
 template <bool BLOCKS>
-__global__ void __launch_bounds__(256) deliver_kernel(const __grid_constant__ DeliverParams p) {
+__device__ __forceinline__ void deliver_body(const DeliverParams& p) {
   const uint32_t n_arr = min(*p.n_arr, p.capacity);
   const uint32_t warps = gridDim.x * (256 / 32);
   unsigned long long ev = 0;
@@ -137,6 +145,27 @@ __global__ void __launch_bounds__(256) deliver_kernel(const __grid_constant__ De
   if (lane_id() == 0 && ev) atomicAdd(&p.ctr->events, ev);
 }
 
+template <bool BLOCKS>
+__global__ void __launch_bounds__(256) deliver_kernel(const __grid_constant__ DeliverParams p) {
+  deliver_body<BLOCKS>(p);
+}
+
+// One launch per step (cooperative): advance + insert, a grid-wide barrier, delivery.  The counters the NEXT step
+// appends to are cleared here, after the barrier, when nobody reads them any more: the list counter this step
+// consumed, and the other of the two spike-array counters (the host may still read this step's).
+template <bool BLOCKS>
+__global__ void __launch_bounds__(kStepThreads) fused_step_kernel(const __grid_constant__ StepParams sp,
+                                                                 const __grid_constant__ DeliverParams dp,
+                                                                 uint32_t* clear_a, uint32_t* clear_b) {
+  advance_insert_body(sp);
+  cooperative_groups::this_grid().sync();
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    *clear_a = 0u;
+    *clear_b = 0u;
+  }
+  deliver_body<BLOCKS>(dp);
+}
+
 }  // namespace
 
 struct nc_delivery {
@@ -148,6 +177,8 @@ struct nc_delivery {
   uint2* arr = nullptr;
   Counters* ctr = nullptr;
   int sms = 148;
+  int coop_grid = 0;                  // > 0: one cooperative launch per step with at most this many CTAs
+  uint32_t* last_arr_ctr = nullptr;   // counter of the spike array the last step filled
 };
 
 extern "C" {
@@ -177,6 +208,17 @@ int nc_delivery_create(nc_context* ctx, uint32_t capacity, nc_delivery** out) {
   }
   int dev = 0;
   if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&d->sms, cudaDevAttrMultiProcessorCount, dev);
+  d->last_arr_ctr = &d->ctr->n_arr;
+  // one cooperative launch per step when the device supports it (NC_DELIVERY_TWO_KERNELS=1 keeps the two-kernel step)
+  const char* two = getenv("NC_DELIVERY_TWO_KERNELS");
+  int coop = 0, per_sm = 0;
+  if (!(two && atoi(two) != 0) && cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev) == cudaSuccess && coop) {
+    const cudaError_t e = v.block_table
+                              ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fused_step_kernel<true>, kStepThreads, 0)
+                              : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fused_step_kernel<false>, kStepThreads, 0);
+    if (e == cudaSuccess && per_sm > 0) d->coop_grid = d->sms * std::min(per_sm, 8);
+  }
+  cudaGetLastError();
   *out = d;
   return NC_OK;
 }
@@ -195,19 +237,25 @@ int nc_delivery_destroy(nc_delivery* d) {
 int nc_delivery_step(nc_delivery* d, const uint32_t* d_nodes, const uint32_t* d_mult, uint32_t n_new, float* d_input) {
   if (!d || !d_input || (n_new && !d_nodes)) return NC_ERR_INVALID_ARG;
   cudaStream_t st = d->v.stream;
-  // the spike array and the list that is written in this step start empty; they sit next to each other in Counters
   uint32_t* n_live_in = d->cur == 0 ? &d->ctr->n_live_a : &d->ctr->n_live_b;
   uint32_t* n_live_out = d->cur == 0 ? &d->ctr->n_live_b : &d->ctr->n_live_a;
-  uint32_t* reset_from = d->cur == 0 ? &d->ctr->n_arr : &d->ctr->n_live_a;  // {n_arr, n_live_b} or {n_live_a, n_arr}
-  if (cudaMemsetAsync(reset_from, 0, 8, st) != cudaSuccess) return nc_internal_fail(d->ctx, NC_ERR_CUDA, "cudaMemsetAsync failed");
   d->now += 1;
+  const bool fused = d->coop_grid > 0;
+  // fused step: two spike-array counters used in turn, each cleared by the step before (see fused_step_kernel)
+  uint32_t* n_arr = fused && (d->now & 1u) ? &d->ctr->n_arr_odd : &d->ctr->n_arr;
+  uint32_t* n_arr_next = fused && (d->now & 1u) ? &d->ctr->n_arr : &d->ctr->n_arr_odd;
+  if (!fused) {
+    // the spike array and the list that is written in this step start empty; they sit next to each other in Counters
+    uint32_t* reset_from = d->cur == 0 ? &d->ctr->n_arr : &d->ctr->n_live_a;  // {n_arr, n_live_b} or {n_live_a, n_arr}
+    if (cudaMemsetAsync(reset_from, 0, 8, st) != cudaSuccess) return nc_internal_fail(d->ctx, NC_ERR_CUDA, "cudaMemsetAsync failed");
+  }
   StepParams sp{};
   sp.v = d->v;
   sp.live_in = d->live[d->cur];
   sp.live_out = d->live[1 - d->cur];
   sp.n_live_in = n_live_in;
   sp.n_live_out = n_live_out;
-  sp.n_arr = &d->ctr->n_arr;
+  sp.n_arr = n_arr;
   sp.arr = d->arr;
   sp.ctr = d->ctr;
   sp.new_nodes = d_nodes;
@@ -215,20 +263,30 @@ int nc_delivery_step(nc_delivery* d, const uint32_t* d_nodes, const uint32_t* d_
   sp.n_new = n_new;
   sp.capacity = d->capacity;
   sp.now = d->now;
-  // the number of buffered spikes is only known on the device: a fixed grid strides over them
-  const uint64_t most = (uint64_t)d->capacity + n_new;
-  const unsigned grid = (unsigned)std::max<uint64_t>(1, std::min<uint64_t>((most + kStepThreads - 1) / kStepThreads, (uint64_t)d->sms * 8));
-  advance_insert_kernel<<<grid, kStepThreads, 0, st>>>(sp);
   DeliverParams dp{};
   dp.v = d->v;
-  dp.n_arr = &d->ctr->n_arr;
+  dp.n_arr = n_arr;
   dp.arr = d->arr;
   dp.ctr = d->ctr;
   dp.input = d_input;
   dp.capacity = d->capacity;
+  // the number of buffered spikes is only known on the device: a fixed grid strides over them
+  const uint64_t most = (uint64_t)d->capacity + n_new;
+  const unsigned grid = (unsigned)std::max<uint64_t>(1, std::min<uint64_t>((most + kStepThreads - 1) / kStepThreads, (uint64_t)d->sms * 8));
   const unsigned dgrid = (unsigned)std::max<uint64_t>(1, std::min<uint64_t>(((uint64_t)d->capacity + 7) / 8, (uint64_t)d->sms * 8));
-  if (d->v.block_table) deliver_kernel<true><<<dgrid, 256, 0, st>>>(dp);
-  else deliver_kernel<false><<<dgrid, 256, 0, st>>>(dp);
+  if (fused) {
+    const unsigned g = std::min<unsigned>(std::max(grid, dgrid), (unsigned)d->coop_grid);
+    void* args[] = {(void*)&sp, (void*)&dp, (void*)&n_live_in, (void*)&n_arr_next};
+    const cudaError_t e = d->v.block_table
+                              ? cudaLaunchCooperativeKernel((void*)fused_step_kernel<true>, dim3(g), dim3(kStepThreads), args, 0, st)
+                              : cudaLaunchCooperativeKernel((void*)fused_step_kernel<false>, dim3(g), dim3(kStepThreads), args, 0, st);
+    if (e != cudaSuccess) return nc_internal_fail(d->ctx, NC_ERR_CUDA, cudaGetErrorString(e));
+  } else {
+    advance_insert_kernel<<<grid, kStepThreads, 0, st>>>(sp);
+    if (d->v.block_table) deliver_kernel<true><<<dgrid, 256, 0, st>>>(dp);
+    else deliver_kernel<false><<<dgrid, 256, 0, st>>>(dp);
+  }
+  d->last_arr_ctr = n_arr;
   d->cur = 1 - d->cur;
   if (cudaPeekAtLastError() != cudaSuccess)
     return nc_internal_fail(d->ctx, NC_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));
@@ -245,7 +303,7 @@ int nc_delivery_read_spike_array(nc_delivery* d, uint32_t* group, uint32_t* mult
   if (!d || !n) return NC_ERR_INVALID_ARG;
   cudaStream_t st = d->v.stream;
   uint32_t cnt = 0;
-  if (cudaMemcpyAsync(&cnt, &d->ctr->n_arr, 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+  if (cudaMemcpyAsync(&cnt, d->last_arr_ctr, 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
       cudaStreamSynchronize(st) != cudaSuccess)
     return nc_internal_fail(d->ctx, NC_ERR_CUDA, "reading the spike array failed");
   *n = cnt;
