@@ -43,6 +43,13 @@ int nc_delivery_num_ports(nc_delivery* d, uint32_t* n_ports);
  * and is reported by nc_delivery_counts (never silently). */
 int nc_delivery_step(nc_delivery* d, const uint32_t* d_nodes, const uint32_t* d_mult, uint32_t n_new, float* d_input);
 
+/* n_steps consecutive steps over a raster that is known beforehand (asynchronous): step k emits the spikes
+ * d_nodes[offsets[k] .. offsets[k+1]) (d_mult likewise, or NULL); offsets is a HOST array of n_steps + 1 entries.
+ * The same as n_steps calls of nc_delivery_step, without returning to the caller in between; d_input accumulates
+ * over all of them. */
+int nc_delivery_run(nc_delivery* d, uint32_t n_steps, const uint32_t* d_nodes, const uint32_t* d_mult,
+                    const uint64_t* offsets, float* d_input);
+
 /* The spike array of the last step, in no particular order (synchronises): global group index and multiplicity of
  * each entry; *n = number of entries, of which min(*n, cap) are copied. */
 int nc_delivery_read_spike_array(nc_delivery* d, uint32_t* group, uint32_t* mult, uint32_t cap, uint32_t* n);

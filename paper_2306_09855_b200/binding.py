@@ -30,7 +30,7 @@ SYMBOLS = (
     "nc_connect_nodes", "nc_connect_values", "nc_set_connection_attributes", "nc_read_connection_attributes",
     # include/nc_delivery.h
     "nc_delivery_create", "nc_delivery_destroy", "nc_delivery_step", "nc_delivery_read_spike_array",
-    "nc_delivery_counts", "nc_delivery_num_ports",
+    "nc_delivery_counts", "nc_delivery_num_ports", "nc_delivery_run",
     # include/nc_copass.h
     "nc_copass_partition", "nc_get_copass_stats",
 )
@@ -143,6 +143,7 @@ def load_library():
     L.nc_delivery_create.argtypes = [vp, C.c_uint32, P(vp)]
     L.nc_delivery_destroy.argtypes = [vp]
     L.nc_delivery_num_ports.argtypes = [vp, P(C.c_uint32)]
+    L.nc_delivery_run.argtypes = [vp, C.c_uint32, vp, vp, vp, vp]
     L.nc_delivery_step.argtypes = [vp, vp, vp, C.c_uint32, vp]
     L.nc_delivery_read_spike_array.argtypes = [vp, vp, vp, C.c_uint32, P(C.c_uint32)]
     L.nc_delivery_counts.argtypes = [vp, P(C.c_uint64), P(C.c_uint64), P(C.c_uint64), P(C.c_uint64)]
@@ -421,6 +422,15 @@ class Delivery:
         self._nc._check(self._L.nc_delivery_step(self._h, nodes.data_ptr() if n else None,
                                                  mult.data_ptr() if (mult is not None and n) else None, n,
                                                  input_f32.data_ptr()))
+
+    def run(self, nodes, mult, offsets, input_f32):
+        """nc_delivery_run: len(offsets) - 1 steps over a raster resident on the device (nodes / mult: CUDA tensors;
+        offsets: host integers, step k emits nodes[offsets[k]:offsets[k+1]])."""
+        offs = np.ascontiguousarray(offsets, dtype=np.uint64)
+        assert input_f32.is_cuda and input_f32.numel() == self._nc.num_nodes() * self.n_ports
+        self._nc._check(self._L.nc_delivery_run(self._h, offs.size - 1, nodes.data_ptr(),
+                                                None if mult is None else mult.data_ptr(), _ptr(offs),
+                                                input_f32.data_ptr()))
 
     def read_spike_array(self):
         n = C.c_uint32()

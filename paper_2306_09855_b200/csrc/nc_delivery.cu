@@ -126,23 +126,47 @@ __device__ __forceinline__ void deliver_body(const DeliverParams& p) {
     const uint32_t c0 = p.v.group_start[ent.x];
     const uint32_t c1 = ent.x + 1 < p.v.total_groups ? p.v.group_start[ent.x + 1] : (uint32_t)p.v.n;
     const float m = (float)ent.y;
-    for (uint32_t c = c0 + lane_id(); c < c1; c += 32) {
-      if (BLOCKS) {
-        const uint64_t blk = c / p.v.block_size, slot = c - blk * p.v.block_size;
-        const char* base = reinterpret_cast<const char*>(p.v.block_table[blk]);
-        const uint32_t t = reinterpret_cast<const uint32_t*>(base + p.v.off_target)[slot];
-        const float w = reinterpret_cast<const float*>(base + p.v.off_weight)[slot];
-        const uint64_t in = p.v.port ? (uint64_t)p.v.port[c] * p.v.n_nodes + t : t;  // input of (port, node)
-        atomicAdd(p.input + in, w * m);
-      } else {
-        const uint32_t t = p.v.target[c];
-        const uint64_t in = p.v.port ? (uint64_t)p.v.port[c] * p.v.n_nodes + t : t;
-        atomicAdd(p.input + in, p.v.weight[c] * m);
+    // kUnroll x 32 connections per round: all loads of a round are issued before the first add, so a large group
+    // costs one memory latency per 256 connections instead of one per 32 (the largest groups of configs[2] have
+    // several hundred connections and would otherwise set the duration of the whole step)
+    constexpr int kUnroll = 16;
+    for (uint32_t cb = c0 + lane_id(); cb < c1; cb += 32 * kUnroll) {
+      uint32_t t[kUnroll];
+      float w[kUnroll];
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) {
+        const uint32_t c = cb + 32u * u;
+        t[u] = 0xffffffffu;
+        if (c < c1) {
+          if (BLOCKS) {
+            const uint64_t blk = c / p.v.block_size, slot = c - blk * p.v.block_size;
+            const char* base = reinterpret_cast<const char*>(p.v.block_table[blk]);
+            t[u] = reinterpret_cast<const uint32_t*>(base + p.v.off_target)[slot];
+            w[u] = reinterpret_cast<const float*>(base + p.v.off_weight)[slot];
+          } else {
+            t[u] = p.v.target[c];
+            w[u] = p.v.weight[c];
+          }
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) {
+        const uint32_t c = cb + 32u * u;
+        if (c < c1) {
+          const uint64_t in = p.v.port ? (uint64_t)p.v.port[c] * p.v.n_nodes + t[u] : t[u];  // input of (port, node)
+          atomicAdd(p.input + in, w[u] * m);
+        }
       }
     }
     ev += c1 - c0;
   }
-  if (lane_id() == 0 && ev) atomicAdd(&p.ctr->events, ev);
+  // one atomic per CTA on the event counter (thousands of warps finish within a few microseconds of one another)
+  __shared__ unsigned long long cta_events;
+  if (threadIdx.x == 0) cta_events = 0ull;
+  __syncthreads();
+  if (lane_id() == 0 && ev) atomicAdd(&cta_events, ev);
+  __syncthreads();
+  if (threadIdx.x == 0 && cta_events) atomicAdd(&p.ctr->events, cta_events);
 }
 
 template <bool BLOCKS>
@@ -290,6 +314,19 @@ int nc_delivery_step(nc_delivery* d, const uint32_t* d_nodes, const uint32_t* d_
   d->cur = 1 - d->cur;
   if (cudaPeekAtLastError() != cudaSuccess)
     return nc_internal_fail(d->ctx, NC_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));
+  return NC_OK;
+}
+
+int nc_delivery_run(nc_delivery* d, uint32_t n_steps, const uint32_t* d_nodes, const uint32_t* d_mult,
+                    const uint64_t* offsets, float* d_input) {
+  if (!d || !offsets || !d_input) return NC_ERR_INVALID_ARG;
+  for (uint32_t k = 0; k < n_steps; ++k) {
+    if (offsets[k + 1] < offsets[k] || offsets[k + 1] - offsets[k] > 0xffffffffull) return NC_ERR_INVALID_ARG;
+    const uint32_t n_new = (uint32_t)(offsets[k + 1] - offsets[k]);
+    const int rc = nc_delivery_step(d, n_new ? d_nodes + offsets[k] : nullptr, (d_mult && n_new) ? d_mult + offsets[k] : nullptr,
+                                    n_new, d_input);
+    if (rc != NC_OK) return rc;
+  }
   return NC_OK;
 }
 

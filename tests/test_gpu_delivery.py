@@ -135,3 +135,29 @@ def test_delivery_with_receptor_ports(nc_mod, oracle_mod, copass):
         assert not got.reshape(4, 60)[2].any()  # port 2 is unused
     assert gd.counts()["events"] == od.counts()[1] > 0
     gd.close(); od.close(); g.close(); o.close()
+
+
+def test_run_equals_step_by_step(nc_mod):
+    """nc_delivery_run over a raster known beforehand = the same steps issued one by one."""
+    import torch
+    net = WL.config0_tiny()
+    rng = np.random.default_rng(9)
+    counts = rng.integers(0, 9, size=50)
+    offs = np.concatenate([[0], np.cumsum(counts)]).astype(np.uint64)
+    nodes = np.concatenate([rng.choice(net.n_nodes, size=int(k), replace=False) for k in counts]).astype(np.int32)
+    d_nodes = torch.from_numpy(nodes).cuda()
+    res = []
+    for mode in ("steps", "run"):
+        g = nc_mod.NC(dt_ms=net.dt_ms)
+        WL.run(net, g)
+        d = nc_mod.Delivery(g, 4096)
+        inp = torch.zeros(net.n_nodes, dtype=torch.float32, device="cuda")
+        if mode == "steps":
+            for k in range(50):
+                d.step(d_nodes[int(offs[k]):int(offs[k + 1])], None, inp)
+        else:
+            d.run(d_nodes, None, offs, inp)
+        res.append((inp.cpu().numpy(), d.counts(), sorted(zip(*[a.tolist() for a in d.read_spike_array()]))))
+        d.close(); g.close()
+    assert res[0][1] == res[1][1] and res[0][2] == res[1][2]
+    assert np.abs(res[0][0] - res[1][0]).max() <= 1e-4 * max(1.0, np.abs(res[0][0]).max())  # fp32 atomics reorder
