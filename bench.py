@@ -197,8 +197,8 @@ def run_delivery(args):
                                    "spikes per node per step, raster resident in HBM",
                        "events_per_step": events / args.steps, "spikes_per_step": float(counts[args.warmup:].mean()),
                        "buffered_at_end": c["buffered"], "dropped": c["dropped"], "flags": args.flags},
-            "gpu_launches": 2 * args.steps,
-            "roofline": {"bound": "hbm", "kernel": "deliver_kernel (8 B read per delivered connection + one fp32 atomic add)",
+            "gpu_launches": args.steps * (2 if os.environ.get("NC_DELIVERY_TWO_KERNELS", "0") not in ("", "0") else 1),
+            "roofline": {"bound": "hbm", "kernel": "fused_step_kernel, delivery phase (8 B read per delivered connection + one fp32 atomic add)",
                          "achieved": gbs, "peak": peak, "unit": "GB/s", "frac": gbs / peak, "traffic": None}}
     print(json.dumps(line))
     d.close()
