@@ -28,7 +28,7 @@ extern "C" {
 typedef struct nc_delivery nc_delivery; /* opaque */
 
 /* capacity = the largest number of spikes that may be buffered at once (roughly spikes per step x largest delay in
- * steps).  The context must be finalized (else NC_ERR_STATE).  Allocates 2 x 16 B + 8 B per unit of capacity. */
+ * steps).  The context must be finalized (else NC_ERR_STATE).  Allocates 2 x 16 B + 2 x 8 B per unit of capacity. */
 int nc_delivery_create(nc_context* ctx, uint32_t capacity, nc_delivery** out);
 int nc_delivery_destroy(nc_delivery* d);
 

@@ -43,6 +43,7 @@ struct StepParams {
   uint32_t* n_live_out;
   uint32_t* n_arr;
   uint2* arr;             // (global group, multiplicity)
+  uint2* arr_range;       // (first, one past the last) organised position of the group's connections
   Counters* ctr;
   const uint32_t* new_nodes;
   const uint32_t* new_mult;
@@ -58,6 +59,19 @@ __device__ __forceinline__ uint32_t warp_reserve(uint32_t* counter, bool want) {
   return base + __popc(m & lanemask_lt());
 }
 
+// two reservations at once: both atomics are issued before either result is waited for
+__device__ __forceinline__ void warp_reserve2(uint32_t* counter_a, bool want_a, uint32_t* counter_b, bool want_b,
+                                              uint32_t& slot_a, uint32_t& slot_b) {
+  const uint32_t ma = __ballot_sync(0xffffffffu, want_a), mb = __ballot_sync(0xffffffffu, want_b);
+  uint32_t base_a = 0, base_b = 0;
+  if (ma && lane_id() == (uint32_t)(__ffs(ma) - 1)) base_a = atomicAdd(counter_a, (uint32_t)__popc(ma));
+  if (mb && lane_id() == (uint32_t)(__ffs(mb) - 1)) base_b = atomicAdd(counter_b, (uint32_t)__popc(mb));
+  base_a = __shfl_sync(0xffffffffu, base_a, ma ? __ffs(ma) - 1 : 0);
+  base_b = __shfl_sync(0xffffffffu, base_b, mb ? __ffs(mb) - 1 : 0);
+  slot_a = base_a + __popc(ma & lanemask_lt());
+  slot_b = base_b + __popc(mb & lanemask_lt());
+}
+
 constexpr int kStepThreads = 256;
 
 __device__ __forceinline__ void advance_insert_body(const StepParams& p) {
@@ -69,9 +83,14 @@ __device__ __forceinline__ void advance_insert_body(const StepParams& p) {
     bool keep = false, mature = false, bad = false;
     uint4 sp = make_uint4(0u, 0u, 0u, 0u);
     uint32_t g_mature = 0;
+    uint2 range = make_uint2(0u, 0u);
     if (i < n_live) {
       sp = p.live_in[i];
       const uint32_t end = p.v.group_ptr[sp.x + 1];
+      // where the group's connections lie: fetched together with its delay, so that the delivery phase finds the
+      // range in the spike array instead of chasing group -> group_start after the barrier
+      range.x = p.v.group_start[sp.z];
+      range.y = sp.z + 1 < p.v.total_groups ? p.v.group_start[sp.z + 1] : (uint32_t)p.v.n;
       // time index = steps since emission ("the time indexes of all the spikes are increased by one")
       if (p.v.group_delay[sp.z] == p.now - sp.y) {
         mature = true;
@@ -90,9 +109,12 @@ __device__ __forceinline__ void advance_insert_body(const StepParams& p) {
         sp = make_uint4(s, p.now, g0, m);
       }
     }
-    const uint32_t a = warp_reserve(p.n_arr, mature);
-    if (mature) p.arr[a] = make_uint2(g_mature, sp.w);  // one entry per buffered spike at most: always fits
-    const uint32_t o = warp_reserve(p.n_live_out, keep);
+    uint32_t a, o;
+    warp_reserve2(p.n_arr, mature, p.n_live_out, keep, a, o);
+    if (mature) {  // one entry per buffered spike at most: always fits
+      p.arr[a] = make_uint2(g_mature, sp.w);
+      p.arr_range[a] = range;
+    }
     if (keep) {
       if (o < p.capacity) p.live_out[o] = sp;
       else atomicAdd(&p.ctr->dropped, 1ull);
@@ -105,6 +127,7 @@ struct DeliverParams {
   nc_organised_view v;
   const uint32_t* n_arr;
   const uint2* arr;
+  const uint2* arr_range;
   Counters* ctr;
   float* input;
   uint32_t capacity;
@@ -122,9 +145,8 @@ __device__ __forceinline__ void deliver_body(const DeliverParams& p) {
   const uint32_t warps = gridDim.x * (256 / 32);
   unsigned long long ev = 0;
   for (uint32_t e = blockIdx.x * (256 / 32) + (threadIdx.x >> 5); e < n_arr; e += warps) {
-    const uint2 ent = p.arr[e];
-    const uint32_t c0 = p.v.group_start[ent.x];
-    const uint32_t c1 = ent.x + 1 < p.v.total_groups ? p.v.group_start[ent.x + 1] : (uint32_t)p.v.n;
+    const uint2 ent = p.arr[e], range = p.arr_range[e];
+    const uint32_t c0 = range.x, c1 = range.y;
     const float m = (float)ent.y;
     // kUnroll x 32 connections per round: all loads of a round are issued before the first add, so a large group
     // costs one memory latency per 256 connections instead of one per 32 (the largest groups of configs[2] have
@@ -199,6 +221,7 @@ struct nc_delivery {
   int cur = 0;  // which live list is the input of the next step
   uint4* live[2] = {nullptr, nullptr};
   uint2* arr = nullptr;
+  uint2* arr_range = nullptr;
   Counters* ctr = nullptr;
   int sms = 148;
   int coop_grid = 0;                  // > 0: one cooperative launch per step with at most this many CTAs
@@ -221,8 +244,9 @@ int nc_delivery_create(nc_context* ctx, uint32_t capacity, nc_delivery** out) {
   d->live[0] = (uint4*)nc_internal_alloc(ctx, (size_t)capacity * 16);
   d->live[1] = (uint4*)nc_internal_alloc(ctx, (size_t)capacity * 16);
   d->arr = (uint2*)nc_internal_alloc(ctx, (size_t)capacity * 8);
+  d->arr_range = (uint2*)nc_internal_alloc(ctx, (size_t)capacity * 8);
   d->ctr = (Counters*)nc_internal_alloc(ctx, sizeof(Counters));
-  if (!d->live[0] || !d->live[1] || !d->arr || !d->ctr) {
+  if (!d->live[0] || !d->live[1] || !d->arr || !d->arr_range || !d->ctr) {
     nc_delivery_destroy(d);
     return nc_internal_fail(ctx, NC_ERR_OOM, "out of device memory for the spike buffers");
   }
@@ -253,6 +277,7 @@ int nc_delivery_destroy(nc_delivery* d) {
   nc_internal_free(d->ctx, d->live[0]);
   nc_internal_free(d->ctx, d->live[1]);
   nc_internal_free(d->ctx, d->arr);
+  nc_internal_free(d->ctx, d->arr_range);
   nc_internal_free(d->ctx, d->ctr);
   delete d;
   return NC_OK;
@@ -281,6 +306,7 @@ int nc_delivery_step(nc_delivery* d, const uint32_t* d_nodes, const uint32_t* d_
   sp.n_live_out = n_live_out;
   sp.n_arr = n_arr;
   sp.arr = d->arr;
+  sp.arr_range = d->arr_range;
   sp.ctr = d->ctr;
   sp.new_nodes = d_nodes;
   sp.new_mult = d_mult;
@@ -291,6 +317,7 @@ int nc_delivery_step(nc_delivery* d, const uint32_t* d_nodes, const uint32_t* d_
   dp.v = d->v;
   dp.n_arr = n_arr;
   dp.arr = d->arr;
+  dp.arr_range = d->arr_range;
   dp.ctr = d->ctr;
   dp.input = d_input;
   dp.capacity = d->capacity;
