@@ -171,6 +171,26 @@ def eval_synapse(src, tgt, rule, degree_or_total, p, weight, delay_ms, seed, pro
     return {f: getattr(out, f) for f, _ in _Synapse._fields_}
 
 
+def eval_synapses(src, tgt, rule, degree_or_total, p, weight, delay_ms, seed, projection_id, dt_ms, idx) -> dict:
+    """eval_synapse over an array of indexes (oc_eval_synapse_batch); returns a dict of arrays."""
+    idx = np.ascontiguousarray(idx, dtype=np.uint64)
+    n = idx.size
+    rp = _RuleParams(int(degree_or_total), float(p))
+    sp = _syn(weight, delay_ms)
+    out = {"source": np.empty(n, np.uint32), "target": np.empty(n, np.uint32), "weight": np.empty(n, np.float32),
+           "delay": np.empty(n, np.uint16), "boundary": np.empty(n, np.uint8), "accepted": np.empty(n, np.uint8)}
+    L = lib()
+    L.oc_eval_synapse_batch.argtypes = [_Range, _Range, C.c_int, C.POINTER(_RuleParams), C.POINTER(_SynSpec), C.c_uint64,
+                                        C.c_uint32, C.c_double, C.c_void_p, C.c_uint64] + [C.c_void_p] * 6
+    vp = lambda a: a.ctypes.data_as(C.c_void_p)  # noqa: E731
+    rc = L.oc_eval_synapse_batch(_Range(*src), _Range(*tgt), int(rule), C.byref(rp), C.byref(sp), int(seed),
+                                 int(projection_id), float(dt_ms), vp(idx), n, vp(out["source"]), vp(out["target"]),
+                                 vp(out["weight"]), vp(out["delay"]), vp(out["boundary"]), vp(out["accepted"]))
+    if rc != 0:
+        raise OracleError(rc)
+    return out
+
+
 class Oracle:
     """Same call sequence as the nc_ ABI (create_population / connect / finalize / getters)."""
 
@@ -286,23 +306,35 @@ class Oracle:
         lib().oc_block_slot(self._h, int(pos), C.byref(b), C.byref(s))
         return b.value, s.value
 
-    def connections(self, sorted: bool = False) -> dict:
-        """Arrays are COPIES (safe to keep after further calls)."""
+    def projection_starts(self) -> np.ndarray:
+        """Creation position at which each projection starts, closed by the current number of connections."""
+        L = lib()
+        L.oc_get_projection_starts.argtypes = [C.c_void_p, C.POINTER(C.POINTER(C.c_uint64)), C.POINTER(C.c_uint32)]
+        p, n = C.POINTER(C.c_uint64)(), C.c_uint32()
+        rc = L.oc_get_projection_starts(self._h, C.byref(p), C.byref(n))
+        if rc != 0:
+            raise OracleError(rc)
+        return np.concatenate([_np(p, n.value, np.uint64).astype(np.int64), [self.num_connections()]]).astype(np.int64)
+
+    def connections(self, sorted: bool = False, copy: bool = True) -> dict:
+        """Arrays are COPIES (safe to keep after further calls) unless copy=False (views into the oracle's own
+        vectors, valid until the next connect / finalize / close -- for networks too large to duplicate)."""
         v = _ConnView()
         rc = lib().oc_get_connections(self._h, 1 if sorted else 0, C.byref(v))
         if rc != 0:
             raise OracleError(rc)
         n = v.n
+        cp = (lambda a: a.copy()) if copy else (lambda a: a)
         out = {
-            "source": _np(v.source, n, np.uint32).copy(),
-            "target": _np(v.target, n, np.uint32).copy(),
-            "weight": _np(v.weight, n, np.float32).copy(),
-            "delay": _np(v.delay, n, np.uint16).copy(),
-            "boundary": _np(v.boundary, n, np.uint8).copy(),
+            "source": cp(_np(v.source, n, np.uint32)),
+            "target": cp(_np(v.target, n, np.uint32)),
+            "weight": cp(_np(v.weight, n, np.float32)),
+            "delay": cp(_np(v.delay, n, np.uint16)),
+            "boundary": cp(_np(v.boundary, n, np.uint8)),
             "n": int(n),
         }
         if sorted:
-            out["perm"] = _np(v.perm, n, np.uint32).copy()
+            out["perm"] = cp(_np(v.perm, n, np.uint32))
         return out
 
     def index(self) -> dict:

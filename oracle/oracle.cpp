@@ -186,6 +186,7 @@ struct oc_context {
   double dt_ms, inv_dt;
   uint32_t n_nodes = 0;
   uint32_t n_projections = 0;
+  std::vector<uint64_t> proj_start; /* bookkeeping: creation position of each projection's first connection */
   bool finalized = false;
   /* D9: creation order, flat (position pos lives in block pos / B, slot pos % B). */
   std::vector<uint32_t> src, tgt;
@@ -304,6 +305,7 @@ static int connect_core(oc_context* ctx, uint64_t node_space, oc_range src, oc_r
   const uint64_t n_newblocks = (n_conns + n_newconns + ctx->B - 1) / ctx->B - ctx->n_blocks;
   ctx->n_blocks += n_newblocks;
   ctx->n_projections += 1;
+  ctx->proj_start.push_back(n_before);
   ctx->have_in = ctx->have_out = false;
   ctx->port.resize(ctx->src.size(), ctx->cur_port);   /* the new connections carry the attributes in force */
   ctx->group.resize(ctx->src.size(), ctx->cur_group);
@@ -372,6 +374,7 @@ int oc_connect_values(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src
     ctx->port.resize(before); ctx->group.resize(before);
     ctx->n_blocks = blocks_before;
     ctx->n_projections -= 1;
+    ctx->proj_start.pop_back();
     return OC_ERR_INVALID_ARG;
   }
   for (uint64_t i = 0; i < n_values; ++i) {
@@ -427,6 +430,13 @@ int oc_num_nodes(oc_context* ctx, uint32_t* n) {
 int oc_num_blocks(oc_context* ctx, uint64_t* n_blocks) {
   if (!ctx || !n_blocks) return OC_ERR_INVALID_ARG;
   *n_blocks = ctx->n_blocks;
+  return OC_OK;
+}
+/* bookkeeping for the tests (no arithmetic of the method): creation position at which each projection starts */
+int oc_get_projection_starts(oc_context* ctx, const uint64_t** starts, uint32_t* n_projections) {
+  if (!ctx || !starts || !n_projections) return OC_ERR_INVALID_ARG;
+  *starts = ctx->proj_start.data();
+  *n_projections = (uint32_t)ctx->proj_start.size();
   return OC_OK;
 }
 int oc_block_slot(oc_context* ctx, uint64_t pos, uint64_t* block, uint64_t* slot) {
@@ -551,6 +561,24 @@ int oc_eval_synapse(oc_range src, oc_range tgt, int rule, const oc_rule_params* 
   if (rule == OC_PAIRWISE_BERNOULLI) {
     const uint64_t T = bernoulli_threshold(params->p);
     out->accepted = (uint64_t)oc_bernoulli_trial_word(seed, projection_id, idx) < T ? 1 : 0;
+  }
+  return OC_OK;
+}
+
+/* oc_eval_synapse over an array of indexes (the same function, called in a loop): sampled parity at sizes the
+ * full oracle cannot hold.  Outputs are HOST arrays of n entries; accepted may be NULL. */
+int oc_eval_synapse_batch(oc_range src, oc_range tgt, int rule, const oc_rule_params* params,
+                          const oc_syn_spec* syn, uint64_t seed, uint32_t projection_id, double dt_ms,
+                          const uint64_t* idx, uint64_t n, uint32_t* source, uint32_t* target, float* weight,
+                          uint16_t* delay, uint8_t* boundary, uint8_t* accepted) {
+  if (!idx || !source || !target || !weight || !delay || !boundary) return OC_ERR_INVALID_ARG;
+  for (uint64_t k = 0; k < n; ++k) {
+    oc_synapse sy;
+    const int rc = oc_eval_synapse(src, tgt, rule, params, syn, seed, projection_id, dt_ms, idx[k], &sy);
+    if (rc != OC_OK) return rc;
+    source[k] = sy.source; target[k] = sy.target; weight[k] = sy.weight; delay[k] = sy.delay;
+    boundary[k] = sy.boundary;
+    if (accepted) accepted[k] = sy.accepted;
   }
   return OC_OK;
 }

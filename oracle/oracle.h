@@ -116,6 +116,8 @@ int oc_finalize(oc_context* ctx);
 int oc_num_connections(oc_context* ctx, uint64_t* n);
 int oc_num_nodes(oc_context* ctx, uint32_t* n);
 int oc_num_blocks(oc_context* ctx, uint64_t* n_blocks);          /* Eq. 1 */
+/* test bookkeeping: creation position of the first connection of each successful connect call (n entries) */
+int oc_get_projection_starts(oc_context* ctx, const uint64_t** starts, uint32_t* n_projections);
 int oc_block_slot(oc_context* ctx, uint64_t pos, uint64_t* block, uint64_t* slot); /* reading D9 */
 int oc_get_connections(oc_context* ctx, int sorted, oc_connections_view* out);
 int oc_get_index(oc_context* ctx, oc_index_view* out);
@@ -147,6 +149,12 @@ typedef struct {
 int oc_eval_synapse(oc_range src, oc_range tgt, int rule, const oc_rule_params* params,
                     const oc_syn_spec* syn, uint64_t seed, uint32_t projection_id, double dt_ms,
                     uint64_t idx, oc_synapse* out);
+
+/* the same function over an array of indexes; outputs are HOST arrays of n entries, accepted may be NULL */
+int oc_eval_synapse_batch(oc_range src, oc_range tgt, int rule, const oc_rule_params* params,
+                          const oc_syn_spec* syn, uint64_t seed, uint32_t projection_id, double dt_ms,
+                          const uint64_t* idx, uint64_t n, uint32_t* source, uint32_t* target, float* weight,
+                          uint16_t* delay, uint8_t* boundary, uint8_t* accepted);
 
 #ifdef __cplusplus
 }

@@ -110,14 +110,14 @@ def copass_parity(net, oracle_mod, nc_mod, B, shift=False):
     flags = nc_mod.FLAG_ORGANISE_COPASS | (nc_mod.FLAG_COPASS_SHIFT if shift else 0)
     g = nc_mod.NC(dt_ms=net.dt_ms, block_size=B, flags=flags)
     WL.run(net, g, finalize=False)
-    scale = PU.weight_scale(net)
     gu = g.read_connections(sorted=False)
-    rep = PU.compare_connections(gu, o.connections(sorted=False), scale, net.name + " creation order")
+    rep = PU.compare_connections(gu, o.connections(sorted=False), PU.weight_scale(net, o), net.name + " creation order")
     in_deg = g.read_degree_histogram(0)
     g.finalize()
     gs = g.read_connections(sorted=True)
     if rep["delay_mismatches"] == 0:
-        PU.compare_connections(gs, o.connections(sorted=True), scale, net.name + " organised in place")
+        os_ = o.connections(sorted=True)
+        PU.compare_connections(gs, os_, PU.weight_scale(net, o, os_["perm"]), net.name + " organised in place")
         PU.compare_index(g.read_index(), o.index(), net.name)
     else:  # a boundary delay moved by one step: the order is the stable sort of the device's own keys
         key = (gu["source"].astype(np.uint64) << np.uint64(16)) | gu["delay"].astype(np.uint64)
@@ -305,7 +305,7 @@ def test_copass_with_the_library_allocator(nc_mod, oracle_mod, shift):
     flags = nc_mod.FLAG_ORGANISE_COPASS | (nc_mod.FLAG_COPASS_SHIFT if shift else 0)
     g = nc_mod.NC(dt_ms=net.dt_ms, block_size=40_000, flags=flags, use_torch_allocator=False)
     WL.run(net, g)
-    PU.compare_connections(g.read_connections(sorted=True), o.connections(sorted=True), PU.weight_scale(net), "cudaMalloc")
+    PU.compare_sorted(g, o, net, "cudaMalloc")
     PU.compare_index(g.read_index(), o.index(), "cudaMalloc")
     assert g.copass_stats()["n_blocks"] >= 4
     g.close(); o.close()

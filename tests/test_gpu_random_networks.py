@@ -98,7 +98,9 @@ def test_random_network_all_variants(nc_mod, oracle_mod, seed):
     n = ou["n"]
     o.finalize()
     os_, oi = o.connections(sorted=True), o.index()
-    scale = max(abs(kw["weight"][0]) + kw["weight"][1] for _, _, _, kw in calls)
+    per_proj = [abs(kw["weight"][0]) + kw["weight"][1] for _, _, _, kw in calls]  # the synapse's own projection scale
+    scale = PU.scale_per_connection(per_proj, o)
+    scale_s = scale[os_["perm"]]
     for name in VARIANTS:
         if name.startswith("copass") and B and (n + B - 1) // B > 4096:
             continue
@@ -113,7 +115,7 @@ def test_random_network_all_variants(nc_mod, oracle_mod, seed):
         g.finalize()
         assert g.stats()["n_blocks"] == o.num_blocks(), name
         if n and rep["delay_mismatches"] == 0:
-            PU.compare_connections(g.read_connections(sorted=True), os_, scale, f"seed {seed} {name} organised")
+            PU.compare_connections(g.read_connections(sorted=True), os_, scale_s, f"seed {seed} {name} organised")
         PU.compare_index(g.read_index(), oi, f"seed {seed} {name}") if (n == 0 or rep["delay_mismatches"] == 0) else None
         outd = g.read_degree_histogram(1)
         od, om = o.degree_histogram(1)
