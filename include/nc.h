@@ -83,9 +83,14 @@ enum {
                                    (see nc_connections_view) and the creation-order view is gone after nc_finalize.
                                    Needs a (source, delay) key of <= 32 bits and <= 4096 blocks (NC_ERR_CAPACITY).
                                    See include/nc_copass.h. */
-  NC_FLAG_COPASS_SHIFT = 1u << 5   /* with NC_FLAG_ORGANISE_COPASS: follow Fig. 6 C-E to the letter (one partition per
+  NC_FLAG_COPASS_SHIFT = 1u << 5,  /* with NC_FLAG_ORGANISE_COPASS: follow Fig. 6 C-E to the letter (one partition per
                                    output block on what the previous extraction left, right partitions shifted
                                    right) instead of the default extraction by hole filling (include/nc_copass.h) */
+  NC_FLAG_SORT_BULK = 1u << 6      /* default organisation path, but every digit pass runs as a persistent kernel fed by
+                                   the bulk-async copy engine (cp.async.bulk loads of whole tiles tracked by mbarriers,
+                                   one bulk store per digit run) instead of one CTA per tile with ordinary loads and
+                                   stores.  Same result bit for bit; measured on par, kept selectable.
+                                   The first pass takes this form only when block_size is a multiple of 4096. */
 };
 
 typedef struct {

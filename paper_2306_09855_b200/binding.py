@@ -19,6 +19,7 @@ LIB_PATH = _HERE / "libnc.so"
 OK, ERR_INVALID_ARG, ERR_STATE, ERR_CAPACITY, ERR_OOM, ERR_CUDA = 0, -1, -2, -3, -4, -5
 ONE_TO_ONE, ALL_TO_ALL, FIXED_INDEGREE, FIXED_OUTDEGREE, FIXED_TOTAL_NUMBER, PAIRWISE_BERNOULLI = range(6)
 FLAG_TIMING, FLAG_EXACT_FP64, FLAG_SORT_PAIRS, FLAG_SORT_ONESWEEP, FLAG_ORGANISE_COPASS, FLAG_COPASS_SHIFT = 1, 2, 4, 8, 16, 32
+FLAG_SORT_BULK = 64
 PHASES = ("generate", "histogram", "sort", "permute", "index", "degree", "copass")
 
 # every symbol include/nc.h declares (checked by tests/test_abi.py against the header and the library)

@@ -19,6 +19,7 @@
 #include "nc_index.cuh"
 #include "nc_sort.cuh"
 #include "nc_sort_split.cuh"
+#include "nc_sort_bulk.cuh"
 #include "nc_copass.cuh"
 #include "../../include/nc_copass.h"
 
@@ -726,9 +727,22 @@ int launch_scatter_pass(nc_context* c, const ScatterParams& sp, uint32_t n_tiles
   }
 }
 
+// NC_FLAG_SORT_BULK: the same pass as a persistent kernel fed by cp.async.bulk (nc_sort_bulk.cuh), one CTA per SM.
+template <bool FIRST, bool LAST>
+int launch_scatter_bulk(nc_context* c, const ScatterParams& sp, uint32_t n_tiles) {
+  auto kern = scatter_bulk_kernel<FIRST, LAST>;
+  NC_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BulkSmem)));
+  int sms = 0;
+  NC_CUDA(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device));
+  kern<<<std::min<uint32_t>(n_tiles, (uint32_t)sms), kBulkWarps * 32, sizeof(BulkSmem), c->stream>>>(sp, n_tiles);
+  NC_LAUNCH_CHECK(c, "scatter_bulk");
+  return NC_OK;
+}
+
 int sort_split_and_index(nc_context* c, const PassPlan& plan) {
   const uint32_t n = (uint32_t)c->n_conns;
-  const int variant = split_variant();
+  const bool bulk = (c->cfg.flags & NC_FLAG_SORT_BULK) != 0;
+  const int variant = bulk ? 0 : split_variant();  // the bulk kernel works on the tiles of shape 0
   const uint32_t kSplitTile = (uint32_t)kSplitShapes[variant].warps * 32u * (uint32_t)kSplitShapes[variant].items;
   const uint32_t n_tiles = (uint32_t)(((uint64_t)n + kSplitTile - 1) / kSplitTile);
   const uint32_t n_chunks = (n_tiles + kScanChunkTiles - 1) / kScanChunkTiles;
@@ -803,10 +817,12 @@ int sort_split_and_index(nc_context* c, const PassPlan& plan) {
       sp.next_bits = last ? 0 : plan.bits[ps + 1];
       sp.offs = offs;
       int rc;
-      if (first && last) rc = launch_scatter_pass<true, true>(c, sp, n_tiles, variant);
-      else if (first) rc = launch_scatter_pass<true, false>(c, sp, n_tiles, variant);
-      else if (last) rc = launch_scatter_pass<false, true>(c, sp, n_tiles, variant);
-      else rc = launch_scatter_pass<false, false>(c, sp, n_tiles, variant);
+      static_assert(kBulkTile == 8 * 32 * 16, "the bulk kernel shares the tiles (and their offsets) of split shape 0");
+      const bool bulk_first = bulk && c->B % kBulkTile == 0;  // a tile of the first pass must lie inside one block
+      if (first && last) rc = bulk_first ? launch_scatter_bulk<true, true>(c, sp, n_tiles) : launch_scatter_pass<true, true>(c, sp, n_tiles, variant);
+      else if (first) rc = bulk_first ? launch_scatter_bulk<true, false>(c, sp, n_tiles) : launch_scatter_pass<true, false>(c, sp, n_tiles, variant);
+      else if (last) rc = bulk ? launch_scatter_bulk<false, true>(c, sp, n_tiles) : launch_scatter_pass<false, true>(c, sp, n_tiles, variant);
+      else rc = bulk ? launch_scatter_bulk<false, false>(c, sp, n_tiles) : launch_scatter_pass<false, false>(c, sp, n_tiles, variant);
       if (rc != NC_OK) return rc;
       cur = dst;
     }

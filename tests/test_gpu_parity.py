@@ -97,6 +97,16 @@ def test_onesweep_lookback_variant_parity(nc_mod, oracle_mod):
         assert rep["n"] > 300_000
 
 
+def test_bulk_fed_persistent_variant_parity(nc_mod, oracle_mod):
+    """NC_FLAG_SORT_BULK: every digit pass as a persistent kernel fed by cp.async.bulk (nc_sort_bulk.cuh): first pass from
+    the SoA slices of the storage blocks (B a multiple of the tile) or through the default kernel (odd B), middle
+    passes with one bulk store per digit run, last pass into the final arrays; ragged last tile; several blocks."""
+    for net, B in ((WL.config2_microcircuit(scale=0.06), 0), (WL.config1_rule("fixed_indegree", scale=0.2), 1 << 16),
+                   (WL.config1_rule("fixed_total_number", scale=0.05), 100_003), (WL.config0_tiny(), 64)):
+        rep, _ = PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_BULK, B=B)
+        assert rep["n"] >= 1000
+
+
 def test_single_pass_key(nc_mod, oracle_mod):
     """<= 8 key bits: one digit pass that is both the first and the last (storage blocks -> final arrays)."""
     net = WL.Network("narrow", [16])
@@ -108,6 +118,7 @@ def test_single_pass_key(nc_mod, oracle_mod):
     PU.full_parity(net, oracle_mod, nc_mod)
     PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_PAIRS)
     PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_ONESWEEP)
+    PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_BULK)
 
 
 def test_block_sizes_paper_default_and_odd(nc_mod, oracle_mod):
