@@ -279,9 +279,16 @@ int nc_read_degree_histogram(nc_context* ctx, int kind, uint32_t* per_node_degre
  *   2^24 values of u1 and of u2 (D5, D6).  out[0] = max |r32 - r64| / (bound on it that the delay guard band
  *   assumes), out[1], out[2] = the same ratio for sin and cos, out[3] = max |r32 - r64| (the fp32 weight is off by
  *   at most sd_w (out[3] + r |cos32 - cos|)).  The guard band is sound iff out[0..2] < 1; the GPU tests require
- *   < 0.25 and out[3] < 4e-6. */
+ *   < 0.25 and out[3] < 4e-6.
+ * nc_selftest_guard: with NC_GUARD=1 in the environment at nc_create, every device buffer of the library lies between two
+ *   256-byte guard zones that are compared when the buffer is released (a stand-in where compute-sanitizer cannot be
+ *   run: writes up to 256 bytes outside a buffer are counted, reported on stderr, and make nc_destroy return
+ *   NC_ERR_STATE).  The self-test writes one byte behind a scratch buffer (offset = 1) or before it (offset = -1) or
+ *   nowhere (0) and returns in *violations how many guard zones were found overwritten when it was released.
+ *   NC_ERR_STATE when guards are off. */
 int nc_selftest_philox(nc_context* ctx, uint32_t n, const uint32_t* ctr, const uint32_t* key, uint32_t* out);
 int nc_selftest_fastpath(nc_context* ctx, double out[4]);
+int nc_selftest_guard(nc_context* ctx, int offset, uint64_t* violations);
 
 #ifdef __cplusplus
 }

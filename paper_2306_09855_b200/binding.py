@@ -8,6 +8,7 @@ the built library or without a GPU, creating a context raises.
 from __future__ import annotations
 
 import ctypes as C
+import weakref
 import math
 from pathlib import Path
 
@@ -27,7 +28,7 @@ SYMBOLS = (
     "nc_create", "nc_destroy", "nc_last_error", "nc_synchronize", "nc_create_population", "nc_connect",
     "nc_finalize", "nc_num_connections", "nc_num_nodes", "nc_get_connections", "nc_get_index",
     "nc_degree_histogram", "nc_get_stats", "nc_get_timings", "nc_read_connections", "nc_read_index",
-    "nc_read_degree_histogram", "nc_selftest_philox", "nc_selftest_fastpath",
+    "nc_read_degree_histogram", "nc_selftest_philox", "nc_selftest_fastpath", "nc_selftest_guard",
     "nc_connect_nodes", "nc_connect_values", "nc_set_connection_attributes", "nc_read_connection_attributes",
     # include/nc_delivery.h
     "nc_delivery_create", "nc_delivery_destroy", "nc_delivery_step", "nc_delivery_read_spike_array",
@@ -134,6 +135,7 @@ def load_library():
     L.nc_read_degree_histogram.argtypes = [vp, C.c_int, vp, P(C.c_uint32)]
     L.nc_selftest_philox.argtypes = [vp, C.c_uint32, vp, vp, vp]
     L.nc_selftest_fastpath.argtypes = [vp, P(C.c_double)]
+    L.nc_selftest_guard.argtypes = [vp, C.c_int, P(C.c_uint64)]
     L.nc_connect_nodes.argtypes = [vp, vp, C.c_uint32, Range, vp, C.c_uint32, Range, C.c_int, vp, vp, C.c_uint64]
     L.nc_copass_partition.argtypes = [vp, vp, C.c_uint64, vp, vp, C.c_uint32, C.c_uint32, vp, P(CopassInfo)]
     L.nc_get_copass_stats.argtypes = [vp, P(CopassStats)]
@@ -226,6 +228,7 @@ class NC:
         cfg.device = torch.cuda.current_device()
         cfg.flags = int(flags)
         self._h = C.c_void_p()
+        self._deliveries = weakref.WeakSet()  # closed before the context: they allocate from it (nc_delivery.h)
         rc = self._L.nc_create(C.byref(cfg), C.byref(self._h))
         if rc != 0:
             raise NCError(rc, "nc_create failed")
@@ -237,8 +240,17 @@ class NC:
 
     def close(self):
         if getattr(self, "_h", None):
-            self._L.nc_destroy(self._h)
+            for d in list(getattr(self, "_deliveries", ())):
+                d.close()
+            rc = self._L.nc_destroy(self._h)
             self._h = C.c_void_p()
+            if rc != 0:  # NC_GUARD=1: a guard zone around one of the library's buffers was overwritten
+                raise NCError(rc, "nc_destroy: guard zone violation (see stderr)")
+
+    def guard_violations(self) -> int:
+        self._L.nc_internal_guard_violations.restype = C.c_uint64
+        self._L.nc_internal_guard_violations.argtypes = [C.c_void_p]
+        return int(self._L.nc_internal_guard_violations(self._h))
 
     def __del__(self):
         try:
@@ -396,6 +408,11 @@ class NC:
         self._check(self._L.nc_selftest_philox(self._h, ctr.shape[0], _ptr(ctr), _ptr(key), _ptr(out)))
         return out
 
+    def selftest_guard(self, offset: int) -> int:
+        v = C.c_uint64()
+        self._check(self._L.nc_selftest_guard(self._h, int(offset), C.byref(v)))
+        return v.value
+
     def selftest_fastpath(self):
         out = (C.c_double * 4)()
         self._check(self._L.nc_selftest_fastpath(self._h, out))
@@ -415,6 +432,7 @@ class Delivery:
         n_ports = C.c_uint32()
         nc._check(self._L.nc_delivery_num_ports(self._h, C.byref(n_ports)))
         self.n_ports = n_ports.value
+        nc._deliveries.add(self)
 
     def step(self, nodes, mult, input_f32, n_new=None):
         n = int(nodes.numel()) if n_new is None else int(n_new)

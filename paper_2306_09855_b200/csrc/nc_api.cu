@@ -80,6 +80,8 @@ struct nc_context {
   bool broken = false;  // an in-place organisation failed half way: the connections are lost, only nc_destroy is left
 
   // allocations
+  bool guard = false;           // NC_GUARD=1: every allocation sits between two 256-byte guard zones checked when it is freed
+  uint64_t guard_violations = 0;
   std::unordered_map<void*, size_t> live;
   std::vector<void*> deferred;  // scratch to release at the next point the stream is known idle
   uint64_t bytes_in_use = 0, bytes_peak = 0;
@@ -128,16 +130,29 @@ int fail(nc_context* c, int code, const std::string& msg) {
       return fail(ctx, NC_ERR_CUDA, std::string("launch ") + name + ": " + cudaGetErrorString(e_)); \
   } while (0)
 
+// Guard zones (NC_GUARD=1 in the environment; compute-sanitizer is not available on every box): an allocation of n bytes
+// becomes 256 guard bytes | n bytes rounded up to 256 | 256 guard bytes, the guards filled with 0xA5 on the context's
+// stream and compared when the allocation is freed.  A kernel that writes up to 256 bytes before or behind a buffer of
+// the library is then counted (nc_internal_guard_violations) and reported on stderr instead of going unnoticed.
+constexpr size_t kGuardBytes = 256;
+
 void* dev_alloc(nc_context* c, size_t bytes) {
   if (bytes == 0) bytes = 256;
+  const size_t body = c->guard ? (bytes + 255) / 256 * 256 : bytes;
+  const size_t total = c->guard ? body + 2 * kGuardBytes : bytes;
   void* p = nullptr;
   if (c->cfg.mem.alloc) {
-    p = c->cfg.mem.alloc(c->cfg.mem.user, bytes);
+    p = c->cfg.mem.alloc(c->cfg.mem.user, total);
   } else {
-    if (cudaMalloc(&p, bytes) != cudaSuccess) {
+    if (cudaMalloc(&p, total) != cudaSuccess) {
       cudaGetLastError();
       p = nullptr;
     }
+  }
+  if (p && c->guard) {
+    cudaMemsetAsync(p, 0xA5, kGuardBytes, c->stream);
+    cudaMemsetAsync((char*)p + kGuardBytes + body, 0xA5, kGuardBytes, c->stream);
+    p = (char*)p + kGuardBytes;
   }
   if (p) {
     c->live[p] = bytes;
@@ -149,10 +164,28 @@ void* dev_alloc(nc_context* c, size_t bytes) {
 
 void dev_free(nc_context* c, void* p) {
   if (!p) return;
+  size_t bytes = 0;
   auto it = c->live.find(p);
   if (it != c->live.end()) {
+    bytes = it->second;
     c->bytes_in_use -= it->second;
     c->live.erase(it);
+  }
+  if (c->guard) {
+    const size_t body = (bytes + 255) / 256 * 256;
+    unsigned char g[2][kGuardBytes];
+    cudaStreamSynchronize(c->stream);
+    cudaMemcpy(g[0], (char*)p - kGuardBytes, kGuardBytes, cudaMemcpyDeviceToHost);
+    cudaMemcpy(g[1], (char*)p + body, kGuardBytes, cudaMemcpyDeviceToHost);
+    for (int side = 0; side < 2; ++side)
+      for (size_t i = 0; i < kGuardBytes; ++i)
+        if (g[side][i] != 0xA5) {
+          ++c->guard_violations;
+          fprintf(stderr, "libnc guard: byte %zu %s an allocation of %zu bytes was overwritten\n", side ? i : kGuardBytes - i,
+                  side ? "behind" : "before", bytes);
+          break;
+        }
+    p = (char*)p - kGuardBytes;
   }
   if (c->cfg.mem.alloc) {
     c->cfg.mem.free(c->cfg.mem.user, p);
@@ -1478,6 +1511,10 @@ int nc_create(const nc_config* cfg, nc_context** out) {
   c->cfg = *cfg;
   c->device = dev;
   c->stream = (cudaStream_t)cfg->cuda_stream;
+  {
+    const char* e = getenv("NC_GUARD");
+    c->guard = e && atoi(e) != 0;
+  }
   c->B = cfg->block_size ? cfg->block_size : (1ull << 24);  // Q10
   c->dt = cfg->dt_ms;
   c->inv_dt = 1.0 / cfg->dt_ms;  // Q5: computed once
@@ -1517,8 +1554,9 @@ int nc_destroy(nc_context* c) {
   std::vector<void*> all;
   for (auto& kv : c->live) all.push_back(kv.first);
   for (void* p : all) dev_free(c, p);
+  const bool clean = c->guard_violations == 0;
   delete c;
-  return NC_OK;
+  return clean ? NC_OK : NC_ERR_STATE;  // NC_GUARD=1: something wrote outside a buffer of the library
 }
 
 const char* nc_last_error(nc_context* c) { return c ? c->err.c_str() : "null context"; }
@@ -2044,6 +2082,24 @@ int nc_selftest_philox(nc_context* c, uint32_t n, const uint32_t* ctr, const uin
   return rc;
 }
 
+namespace {
+__global__ void poke_kernel(unsigned char* p) { *p = 0x11; }
+}  // namespace
+
+int nc_selftest_guard(nc_context* c, int offset, uint64_t* violations) {
+  if (!c || !violations) return NC_ERR_INVALID_ARG;
+  if (!c->guard) return fail(c, NC_ERR_STATE, "nc_selftest_guard: NC_GUARD was not set when the context was created");
+  unsigned char* d = (unsigned char*)dev_alloc(c, 1000);
+  if (!d) return fail(c, NC_ERR_OOM, "selftest: out of device memory");
+  if (offset > 0) poke_kernel<<<1, 1, 0, c->stream>>>(d + 1024);  // first byte behind the body (1000 rounded up to 1024)
+  if (offset < 0) poke_kernel<<<1, 1, 0, c->stream>>>(d - 1);
+  const uint64_t before = c->guard_violations;
+  dev_free(c, d);
+  *violations = c->guard_violations - before;
+  c->guard_violations = before;  // a deliberate poke is not a finding
+  return NC_OK;
+}
+
 int nc_selftest_fastpath(nc_context* c, double out[4]) {
   if (!c || !out) return NC_ERR_INVALID_ARG;
   double* d = (double*)dev_alloc(c, 32);
@@ -2110,3 +2166,4 @@ int nc_internal_organised_view(nc_context* c, nc_organised_view* out) {
 void* nc_internal_alloc(nc_context* c, size_t bytes) { return dev_alloc(c, bytes); }
 void nc_internal_free(nc_context* c, void* p) { dev_free(c, p); }
 int nc_internal_fail(nc_context* c, int code, const char* msg) { return fail(c, code, msg); }
+extern "C" uint64_t nc_internal_guard_violations(nc_context* c) { return c ? c->guard_violations : 0; }
