@@ -132,7 +132,9 @@ typedef struct {
  *              blocks is a HOST array of n_blocks device base pointers; inside a block the four arrays
  *              start at byte offsets off_source/off_target/off_weight/off_delay.  Creation position pos
  *              is entry pos % block_size of block pos / block_size (D9).  The flat pointers are NULL
- *              unless n_blocks == 1, in which case they point into that single block.
+ *              unless n_blocks == 1, in which case they point into that single block.  The block pointers stay valid
+ *              until nc_destroy; the HOST array `blocks` itself is valid until the next nc_connect* call (which may
+ *              append to it and move it) -- ask for the view again after connecting.
  *  sorted = 1 under NC_FLAG_ORGANISE_COPASS: the organised connections stay in the storage blocks: sorted position j
  *              is entry j % block_size of block j / block_size, the view is filled as for sorted = 0 plus
  *              off_perm (creation positions), and sorted = 0 is NC_ERR_STATE after nc_finalize (the blocks were
@@ -216,7 +218,8 @@ int nc_connect(nc_context* ctx, nc_range src, nc_range tgt, nc_rule rule, const 
 /* The same with explicit node arrays ("If the indexes of source or target nodes are not consecutive but
  * are explicitly given by an array, the above formulas are used to derive the indexes of the array elements from
  * which to extract the node indexes").  src_nodes / tgt_nodes are HOST arrays of n_src / n_tgt node ids (copied
- * during the call; ids may repeat and need not be sorted; every id must be a created node, else NC_ERR_INVALID_ARG);
+ * during the call -- the call waits for the upload, pageable or page-locked, so the arrays may be reused on return;
+ * ids may repeat and need not be sorted; every id must be a created node, else NC_ERR_INVALID_ARG);
  * a NULL array means "use the range argument of that side".  Rule formulas and random draws are those of nc_connect
  * with N_sources = n_src, N_targets = n_tgt and s0 = t0 = 0; the result indexes the arrays. ---- */
 int nc_connect_nodes(nc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, nc_range src,

@@ -427,10 +427,14 @@ int connect_bernoulli(nc_context* c, GenParams gp, double p, uint32_t seed_lo, u
     bernoulli_trials_kernel<<<(unsigned)n_tiles, kBernThreads, 0, c->stream>>>(bp);
     NC_LAUNCH_CHECK(c, "bernoulli_trials");
     int rc = device_scan(c, tile_count, tile_off, n_tiles, partial, d_total);
-    if (rc != NC_OK) return rc;
+    if (rc != NC_OK) {
+      drop();
+      return rc;
+    }
     NC_CUDA(c, cudaMemcpyAsync(&total, d_total, 8, cudaMemcpyDeviceToHost, c->stream));
   }
   NC_CUDA(c, cudaStreamSynchronize(c->stream));  // the exact count decides the allocation
+  release_deferred(c);  // the stream is idle: scratch of earlier calls (masks, tables) goes back before the blocks are reserved
   if (c->n_conns + total > kMaxConns) {
     drop();
     return fail(c, NC_ERR_CAPACITY, "more than 2^32-1 connections");
@@ -589,6 +593,7 @@ int sort_and_index(nc_context* c, const PassPlan& plan) {
     NC_CUDA(c, cudaMemcpyAsync(&lookback_error, tickets + kMaxPasses, 4, cudaMemcpyDeviceToHost, c->stream));
   }
   NC_CUDA(c, cudaStreamSynchronize(c->stream));  // total_groups sizes the group arrays
+  release_deferred(c);
   if (lookback_error) {
     drop_scratch(cur);
     return fail(c, NC_ERR_CUDA, "onesweep look-back timed out");
@@ -1006,6 +1011,7 @@ int copass_extract_fill(nc_context* c, const PassPlan& plan, const CopassScratch
     NC_CUDA(c, cudaMemcpyAsync(d_phys, phys.data(), k1 * 8, cudaMemcpyHostToDevice, c->stream));
   }
   NC_CUDA(c, cudaStreamSynchronize(c->stream));  // the one wait of the organisation step: the plan needs the m_i
+  release_deferred(c);
 
   // ---- plan (host): extents of every original block, holes per physical block, copy commands per step ----
   struct Step {
@@ -1370,6 +1376,8 @@ int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) 
     NC_CUDA(c, cudaMemcpyAsync(&total_groups, c->d_total_groups, 8, cudaMemcpyDeviceToHost, c->stream));
     if (lookback_flag) NC_CUDA(c, cudaMemcpyAsync(&lookback_error, lookback_flag, 4, cudaMemcpyDeviceToHost, c->stream));
     NC_CUDA(c, cudaStreamSynchronize(c->stream));  // total_groups sizes the group arrays
+  release_deferred(c);
+    release_deferred(c);
     if (lookback_error) {
       drop();
       return fail(c, NC_ERR_CUDA, "onesweep look-back timed out");
@@ -1703,6 +1711,12 @@ static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, 
     }
     c->n_conns += n_new;
   }
+  if (src_nodes || tgt_nodes || with_values) {
+    // nc.h: the host arrays are copied DURING the call.  From page-locked memory cudaMemcpyAsync returns before the copy
+    // has run, so wait here; this also releases the device copies (and any older scratch) right away.
+    const int rc = sync_stream(c);
+    if (rc != NC_OK) return rc;
+  }
   c->n_proj += 1;
   c->proj_first.push_back((uint32_t)gp.pos0);
   c->proj_attr.push_back((uint16_t)(c->cur_port | (c->cur_group << 8)));
@@ -1732,6 +1746,18 @@ int nc_connect_values(nc_context* c, const uint32_t* src_nodes, uint32_t n_src, 
   return connect_impl(c, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed, weights, delays_ms, n_values, true);
 }
 
+// A failed nc_finalize keeps nothing: the index and organised arrays it had assigned are released (kernels of the failed
+// attempt may still run, hence the deferred release) so that a retry starts clean and nothing stays allocated twice.
+static void drop_finalize_outputs(nc_context* c) {
+  void** outs[] = {(void**)&c->src_offsets, (void**)&c->group_ptr, (void**)&c->group_count, (void**)&c->group_start,
+                   (void**)&c->group_delay, (void**)&c->s_src,     (void**)&c->s_tgt,       (void**)&c->s_w,
+                   (void**)&c->s_d,         (void**)&c->perm};
+  for (void** o : outs) {
+    dev_free_later(c, *o);
+    *o = nullptr;
+  }
+}
+
 int nc_finalize(nc_context* c) {
   if (!c) return NC_ERR_INVALID_ARG;
   if (c->broken) return fail(c, NC_ERR_STATE, "nc_finalize: a failed in-place organisation left this context without connections; destroy it");
@@ -1742,8 +1768,10 @@ int nc_finalize(nc_context* c) {
   c->group_ptr = (uint32_t*)dev_alloc(c, ((size_t)N + 1) * 4);
   c->group_count = (uint32_t*)dev_alloc(c, (size_t)N * 4);
   if (!c->out_degree) c->out_degree = (uint32_t*)dev_alloc(c, (size_t)N * 4);
-  if (!c->src_offsets || !c->group_ptr || !c->group_count || !c->out_degree)
+  if (!c->src_offsets || !c->group_ptr || !c->group_count || !c->out_degree) {
+    drop_finalize_outputs(c);
     return fail(c, NC_ERR_OOM, "out of device memory for the index");
+  }
   NC_CUDA(c, cudaMemsetAsync(c->d_max + 1, 0, 4, c->stream));
 
   // key-width plan: source bits from the node count, delay bits from the analytic bound (Q6)
@@ -1765,14 +1793,19 @@ int nc_finalize(nc_context* c) {
   } else {
     int rc;
     if (c->cfg.flags & NC_FLAG_ORGANISE_COPASS) {
-      if (c->key_bits > 32)
+      if (c->key_bits > 32) {
+        drop_finalize_outputs(c);
         return fail(c, NC_ERR_CAPACITY, "COPASS organisation needs a (source, delay) key of at most 32 bits");
+      }
       rc = organise_copass(c, plan);
     } else if (c->key_bits > 32) rc = sort_and_index<uint64_t>(c, plan);
     else if (c->cfg.flags & NC_FLAG_SORT_PAIRS) rc = sort_and_index<uint32_t>(c, plan);
     else if (c->cfg.flags & NC_FLAG_SORT_ONESWEEP) rc = sort_carry_and_index(c, plan);
     else rc = sort_split_and_index(c, plan);
-    if (rc != NC_OK) return rc;
+    if (rc != NC_OK) {
+      drop_finalize_outputs(c);
+      return rc;
+    }
   }
   c->finalized = true;
   c->have_out = true;

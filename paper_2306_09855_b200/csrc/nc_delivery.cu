@@ -15,6 +15,7 @@
 
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
+#include <cstddef>
 
 #include <algorithm>
 #include <cstdlib>
@@ -34,6 +35,9 @@ struct Counters {
   uint32_t n_arr_odd;  // entries of the spike array, odd steps of the fused step
   unsigned long long events, dropped, bad_nodes;
 };
+// the two-kernel step clears {n_arr, n_live_b} or {n_live_a, n_arr} with ONE 8-byte memset (nc_delivery_step)
+static_assert(offsetof(Counters, n_live_a) == 0 && offsetof(Counters, n_arr) == 4 && offsetof(Counters, n_live_b) == 8,
+              "nc_delivery_step resets two neighbouring counters at once");
 
 struct StepParams {
   nc_organised_view v;
@@ -288,11 +292,11 @@ int nc_delivery_step(nc_delivery* d, const uint32_t* d_nodes, const uint32_t* d_
   cudaStream_t st = d->v.stream;
   uint32_t* n_live_in = d->cur == 0 ? &d->ctr->n_live_a : &d->ctr->n_live_b;
   uint32_t* n_live_out = d->cur == 0 ? &d->ctr->n_live_b : &d->ctr->n_live_a;
-  d->now += 1;
+  const uint32_t now = d->now + 1;  // committed only once the step has been launched
   const bool fused = d->coop_grid > 0;
   // fused step: two spike-array counters used in turn, each cleared by the step before (see fused_step_kernel)
-  uint32_t* n_arr = fused && (d->now & 1u) ? &d->ctr->n_arr_odd : &d->ctr->n_arr;
-  uint32_t* n_arr_next = fused && (d->now & 1u) ? &d->ctr->n_arr : &d->ctr->n_arr_odd;
+  uint32_t* n_arr = fused && (now & 1u) ? &d->ctr->n_arr_odd : &d->ctr->n_arr;
+  uint32_t* n_arr_next = fused && (now & 1u) ? &d->ctr->n_arr : &d->ctr->n_arr_odd;
   if (!fused) {
     // the spike array and the list that is written in this step start empty; they sit next to each other in Counters
     uint32_t* reset_from = d->cur == 0 ? &d->ctr->n_arr : &d->ctr->n_live_a;  // {n_arr, n_live_b} or {n_live_a, n_arr}
@@ -312,7 +316,7 @@ int nc_delivery_step(nc_delivery* d, const uint32_t* d_nodes, const uint32_t* d_
   sp.new_mult = d_mult;
   sp.n_new = n_new;
   sp.capacity = d->capacity;
-  sp.now = d->now;
+  sp.now = now;
   DeliverParams dp{};
   dp.v = d->v;
   dp.n_arr = n_arr;
@@ -337,10 +341,11 @@ int nc_delivery_step(nc_delivery* d, const uint32_t* d_nodes, const uint32_t* d_
     if (d->v.block_table) deliver_kernel<true><<<dgrid, 256, 0, st>>>(dp);
     else deliver_kernel<false><<<dgrid, 256, 0, st>>>(dp);
   }
-  d->last_arr_ctr = n_arr;
-  d->cur = 1 - d->cur;
   if (cudaPeekAtLastError() != cudaSuccess)
     return nc_internal_fail(d->ctx, NC_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));
+  d->now = now;
+  d->last_arr_ctr = n_arr;
+  d->cur = 1 - d->cur;
   return NC_OK;
 }
 

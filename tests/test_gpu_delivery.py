@@ -21,6 +21,14 @@ def nc_mod():
     return binding
 
 
+@pytest.fixture(params=["fused", "two_kernels"], autouse=True)
+def delivery_form(request, monkeypatch):
+    """every test runs over the cooperative one-launch step and over the two-kernel step (the fallback when cooperative
+    launch is unavailable; nc_delivery_create reads NC_DELIVERY_TWO_KERNELS)"""
+    monkeypatch.setenv("NC_DELIVERY_TWO_KERNELS", "1" if request.param == "two_kernels" else "0")
+    return request.param
+
+
 def _raster(rng, n_nodes, steps, rate, max_mult):
     out = []
     for _ in range(steps):

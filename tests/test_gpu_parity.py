@@ -569,3 +569,20 @@ def test_connection_attributes_parity(nc_mod, oracle_mod, variant):
     p2, g2 = g.read_connection_attributes(sorted=True, first=4321, count=5000)
     assert np.array_equal(p2, po[4321:9321]) and np.array_equal(g2, go[4321:9321])
     g.close(); o.close()
+
+
+def test_scratch_of_earlier_connect_calls_is_released(nc_mod):
+    """Scratch queued for release (Bernoulli masks and tile tables, uploaded node and value arrays) goes back at the next
+    point the stream is known idle, so the bytes held do not grow with the number of projections beyond the connections
+    themselves (the masks of configs[4] would otherwise stay allocated through nc_finalize)."""
+    g = nc_mod.NC(block_size=1 << 16)
+    a = g.create_population(3000)
+    held = []
+    for k in range(6):
+        g.connect((a, 3000), (a, 3000), nc_mod.PAIRWISE_BERNOULLI, p=0.01, weight=(1.0, 0.1, 0.0, math.inf),
+                  delay_ms=(1.0, 0.2, 0.1, math.inf), seed=5)
+        st = g.stats()
+        held.append(st["bytes_in_use"] - st["n_blocks"] * 14 * (1 << 16))
+    # one call's scratch (9e6 trials: 1.1 MB mask + tables) may be pending, never several
+    assert max(held[1:]) <= held[0] + (1 << 20), held
+    g.close()
