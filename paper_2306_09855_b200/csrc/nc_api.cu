@@ -94,6 +94,7 @@ struct nc_context {
   uint16_t* group_delay = nullptr;
   uint32_t total_groups = 0;
   uint64_t* d_total_groups = nullptr;  // device scalar; total_groups is fetched on first use (no sync in nc_finalize)
+  uint32_t* d_index_error = nullptr;   // set by index_fused_kernel if its look-back ever gave up; read with total_groups
   bool total_groups_pending = false;
   uint32_t *out_degree = nullptr, *in_degree = nullptr, *d_max = nullptr;  // d_max: [2] device scalars
   bool have_in = false, have_out = false;
@@ -1337,6 +1338,16 @@ int organise_copass(nc_context* c, const PassPlan& plan) {
 }
 
 // a12-a14 over the final source / delay arrays.
+// NC_INDEX_FUSED=1 selects the single-read index (index_fused_kernel: count, look-back across tiles and write in one kernel).
+// Measured on B200, configs[2]: 1.16 - 1.20 ms against 0.72 ms for count / scan / scatter (two streaming reads at 8 CTAs per
+// SM): a tile cannot write before the tiles before it have counted, so each CTA sits through one load latency, two block
+// scans and a look-back with nothing to overlap them (tiles of 4096 with 1184 in flight and tiles of 16384 with 148 in
+// flight measure the same).  Kept selectable and parity-tested; not the default.
+bool index_fused() {
+  const char* e = getenv("NC_INDEX_FUSED");
+  return e && atoi(e) != 0;
+}
+
 int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) {
   const uint32_t N = c->n_nodes;
   const uint64_t head_tiles = ((uint64_t)n + kHeadTile - 1) / kHeadTile;
@@ -1344,7 +1355,7 @@ int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) 
   uint32_t* tile_heads = (uint32_t*)dev_alloc(c, head_tiles * 4);
   uint32_t* tile_head_off = (uint32_t*)dev_alloc(c, head_tiles * 4);
   uint32_t* head_partial = (uint32_t*)dev_alloc(c, head_chunks * 4);
-  if (!c->d_total_groups) c->d_total_groups = (uint64_t*)dev_alloc(c, 8);
+  if (!c->d_total_groups) c->d_total_groups = (uint64_t*)dev_alloc(c, 16);  // total_groups | index error flag
   auto drop = [&]() {
     dev_free_later(c, tile_heads); dev_free_later(c, tile_head_off); dev_free_later(c, head_partial);
   };
@@ -1359,6 +1370,30 @@ int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) 
   const bool presize = !lookback_flag && bound * 6 <= std::max<uint64_t>((uint64_t)n * 2, 1u << 20);
   const SoAKeys keys{c->s_src, c->s_d, 16u};
   const BlockKeys block_keys{make_map(c), 16u};
+  if (presize && !c->organised_in_blocks && index_fused()) {
+    // one read of the keys: heads counted, chained across tiles by look-back and written by the same kernel
+    const uint64_t tiles = ((uint64_t)n + kFusedTile - 1) / kFusedTile;
+    uint64_t* status = (uint64_t*)dev_alloc(c, tiles * 8 + 16);  // [tiles] status words | ticket | error flag
+    c->group_start = (uint32_t*)dev_alloc(c, (size_t)bound * 4);
+    c->group_delay = (uint16_t*)dev_alloc(c, (size_t)bound * 2);
+    drop();
+    dev_free_later(c, status);
+    if (!status || !c->group_start || !c->group_delay) return fail(c, NC_ERR_OOM, "out of device memory for the index");
+    uint32_t* ticket = reinterpret_cast<uint32_t*>(status + tiles);
+    c->d_index_error = reinterpret_cast<uint32_t*>(c->d_total_groups + 1);  // read back together with total_groups
+    Scope sc(c, NC_PHASE_INDEX);
+    NC_CUDA(c, cudaMemsetAsync(status, 0, tiles * 8 + 16, c->stream));
+    NC_CUDA(c, cudaMemsetAsync(c->d_index_error, 0, 4, c->stream));
+    IndexOut io{c->src_offsets, c->group_ptr, c->group_start, c->group_delay, N};
+    index_fused_kernel<<<(unsigned)tiles, kFusedThreads, 0, c->stream>>>(c->s_src, c->s_d, n, status, ticket, c->d_total_groups,
+                                                                     c->d_index_error, io);
+    NC_LAUNCH_CHECK(c, "index_fused");
+    index_finish_kernel<<<(N + 255) / 256, 256, 0, c->stream>>>(c->src_offsets, c->group_ptr, N, c->out_degree,
+                                                               c->group_count, c->d_max + 1);
+    NC_LAUNCH_CHECK(c, "index_finish");
+    c->total_groups_pending = true;
+    return NC_OK;
+  }
   {
     Scope sc(c, NC_PHASE_INDEX);
     if (c->organised_in_blocks)
@@ -1376,7 +1411,6 @@ int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) 
     NC_CUDA(c, cudaMemcpyAsync(&total_groups, c->d_total_groups, 8, cudaMemcpyDeviceToHost, c->stream));
     if (lookback_flag) NC_CUDA(c, cudaMemcpyAsync(&lookback_error, lookback_flag, 4, cudaMemcpyDeviceToHost, c->stream));
     NC_CUDA(c, cudaStreamSynchronize(c->stream));  // total_groups sizes the group arrays
-  release_deferred(c);
     release_deferred(c);
     if (lookback_error) {
       drop();
@@ -1415,9 +1449,12 @@ int build_index_from_sorted(nc_context* c, uint32_t n, uint32_t* lookback_flag) 
 int ensure_total_groups(nc_context* c) {
   if (!c->total_groups_pending) return NC_OK;
   uint64_t total_groups = 0;
+  uint32_t index_error = 0;
   NC_CUDA(c, cudaMemcpyAsync(&total_groups, c->d_total_groups, 8, cudaMemcpyDeviceToHost, c->stream));
+  if (c->d_index_error) NC_CUDA(c, cudaMemcpyAsync(&index_error, c->d_index_error, 4, cudaMemcpyDeviceToHost, c->stream));
   int rc = sync_stream(c);
   if (rc != NC_OK) return rc;
+  if (index_error) return fail(c, NC_ERR_CUDA, "index look-back timed out");
   c->total_groups = (uint32_t)total_groups;
   c->total_groups_pending = false;
   return NC_OK;

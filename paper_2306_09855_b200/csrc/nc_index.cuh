@@ -36,6 +36,28 @@ __device__ __forceinline__ uint32_t block_exclusive_scan_256(uint32_t v, uint32_
   return base + inc - v;
 }
 
+template <int THREADS>
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* warp_tmp /*[THREADS / 32]*/, uint32_t& total) {
+  uint32_t inc = v;
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d);
+    if (lane_id() >= (uint32_t)d) inc += t;
+  }
+  __syncthreads();  // protect warp_tmp against a previous use
+  if (lane_id() == 31) warp_tmp[threadIdx.x >> 5] = inc;
+  __syncthreads();
+  uint32_t base = 0, tot = 0;
+#pragma unroll
+  for (uint32_t w = 0; w < THREADS / 32; ++w) {
+    const uint32_t t = warp_tmp[w];
+    if (w < (threadIdx.x >> 5)) base += t;
+    tot += t;
+  }
+  total = tot;
+  return base + inc - v;
+}
+
 __global__ void __launch_bounds__(kScanThreads) scan_reduce_kernel(const uint32_t* __restrict__ in, uint64_t n,
                                                                   uint32_t* __restrict__ partial) {
   __shared__ uint32_t warp_tmp[kScanThreads / 32];
@@ -379,6 +401,178 @@ __global__ void __launch_bounds__(kHeadThreads) index_scatter_soa_kernel(const u
     for (uint64_t node = (uint64_t)sl + 1; node <= out.n_nodes; ++node) {
       out.src_offsets[node] = n;
       out.group_ptr[node] = tg;
+    }
+  }
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// The whole index in ONE read of the final source / delay arrays (NC_INDEX_FUSED=1; needs group arrays sized from the
+// analytic bound; measured slower than the two streaming reads, see build_index_from_sorted): a tile of kFusedTile positions keeps its keys in registers, counts its heads, chains the
+// count to the tiles before it with a decoupled look-back (one status word per tile: a warp polls 32 predecessors per
+// load), and writes group_start / group_delay / src_offsets / group_ptr with the keys it still holds.  Replaces
+// head_count_kernel + the three scan kernels + index_scatter_soa_kernel (two reads of the keys).
+//   status word: bits 0..31 heads | bit 32 = aggregate of this tile published | bit 33 = inclusive prefix published
+// Tiles are handed out by a ticket so that a tile only ever waits on tiles that already run.
+// ---------------------------------------------------------------------------------------------
+constexpr int kFusedChunks = 2;  // chunks of 8 consecutive positions per thread
+constexpr int kFusedThreads = 1024;  // one CTA per SM: 148 tiles in flight, so a look-back walks at most 5 polls of 32
+constexpr int kFusedTile = kFusedThreads * 8 * kFusedChunks;
+constexpr uint64_t kStatAggregate = 1ull << 32, kStatInclusive = 2ull << 32;
+
+__global__ void __launch_bounds__(kFusedThreads) index_fused_kernel(const uint32_t* __restrict__ src,
+                                                                  const uint16_t* __restrict__ dly, uint32_t n,
+                                                                  uint64_t* __restrict__ status, uint32_t* __restrict__ ticket,
+                                                                  uint64_t* __restrict__ total_groups,
+                                                                  uint32_t* __restrict__ error_flag,
+                                                                  const __grid_constant__ IndexOut out) {
+  __shared__ uint32_t warp_tmp[kFusedThreads / 32];
+  __shared__ uint32_t sh_tile, sh_prefix;
+  if (threadIdx.x == 0) sh_tile = atomicAdd(ticket, 1u);
+  __syncthreads();
+  const uint32_t tile = sh_tile;
+  uint32_t s[kFusedChunks][9], d[kFusedChunks][9], cnt[kFusedChunks], heads[kFusedChunks], first_src[kFusedChunks];
+  uint32_t my_heads = 0;
+#pragma unroll
+  for (int c = 0; c < kFusedChunks; ++c) {
+    // chunk c of the tile: thread t owns positions tile * kFusedTile + c * 8 * kFusedThreads + t * 8 .. + 7
+    const uint64_t base64 = (uint64_t)tile * kFusedTile + (uint64_t)c * (kFusedThreads * 8) + threadIdx.x * 8u;
+    const uint32_t base = (uint32_t)base64;
+    const bool in_range = base64 < n;
+#pragma unroll
+    for (int i = 0; i < 9; ++i) s[c][i] = d[c][i] = 0;
+    cnt[c] = 0;
+    if (in_range) {
+      if (n - base >= 8u) {
+        const uint4 s0 = *reinterpret_cast<const uint4*>(src + base);
+        const uint4 s1 = *reinterpret_cast<const uint4*>(src + base + 4);
+        const uint4 dd = *reinterpret_cast<const uint4*>(dly + base);
+        s[c][1] = s0.x; s[c][2] = s0.y; s[c][3] = s0.z; s[c][4] = s0.w; s[c][5] = s1.x; s[c][6] = s1.y; s[c][7] = s1.z; s[c][8] = s1.w;
+        d[c][1] = dd.x & 0xffffu; d[c][2] = dd.x >> 16; d[c][3] = dd.y & 0xffffu; d[c][4] = dd.y >> 16;
+        d[c][5] = dd.z & 0xffffu; d[c][6] = dd.z >> 16; d[c][7] = dd.w & 0xffffu; d[c][8] = dd.w >> 16;
+        cnt[c] = 8;
+      } else {
+        cnt[c] = n - base;
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+          if ((uint32_t)i < cnt[c]) {
+            s[c][i + 1] = src[base + i];
+            d[c][i + 1] = dly[base + i];
+          }
+      }
+    }
+    const uint32_t up_s = __shfl_up_sync(0xffffffffu, s[c][8], 1), up_d = __shfl_up_sync(0xffffffffu, d[c][8], 1);
+    s[c][0] = up_s;
+    d[c][0] = up_d;
+    if (lane_id() == 0 && in_range && base > 0) {
+      s[c][0] = src[base - 1];
+      d[c][0] = dly[base - 1];
+    }
+    uint32_t h = 0, f = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const bool new_s = s[c][i + 1] != s[c][i];
+      if (new_s | (d[c][i + 1] != d[c][i])) h |= 1u << i;
+      if (new_s) f |= 1u << i;
+    }
+    if (in_range && base == 0) {  // position 0 is a head and the first connection of its source
+      h |= 1u;
+      f |= 1u;
+    }
+    const uint32_t live = cnt[c] >= 8 ? 0xffu : ((1u << cnt[c]) - 1u);
+    heads[c] = h & live;
+    first_src[c] = f & live;
+    my_heads += __popc(heads[c]);
+  }
+  // exclusive scan in POSITION order: chunk 0 of every thread precedes chunk 1 of any thread
+  uint32_t tot0, tot1;
+  const uint32_t ex0 = block_exclusive_scan<kFusedThreads>(__popc(heads[0]), warp_tmp, tot0);
+  const uint32_t ex1 = block_exclusive_scan<kFusedThreads>(__popc(heads[1]), warp_tmp, tot1) + tot0;
+  const uint32_t tile_total = tot0 + tot1;
+  static_assert(kFusedChunks == 2, "the scan above is written for two chunks");
+  (void)my_heads;
+
+  // ---- chain the tile's head count to the tiles before it ----
+  if (threadIdx.x < 32) {
+    uint64_t* my_status = status + tile;
+    uint32_t excl = 0;
+    if (tile == 0) {
+      if (threadIdx.x == 0) st_relaxed_u64(my_status, kStatInclusive | tile_total);
+    } else {
+      if (threadIdx.x == 0) st_relaxed_u64(my_status, kStatAggregate | tile_total);
+      int64_t t = (int64_t)tile - 1;
+      uint32_t spins = 0;
+      while (true) {
+        const int64_t mine = t - (int64_t)lane_id();
+        const uint64_t w = mine >= 0 ? ld_relaxed_u64(status + mine) : kStatInclusive;  // before tile 0: prefix 0
+        const uint32_t ready = __ballot_sync(0xffffffffu, (w >> 32) != 0);
+        const uint32_t incl = __ballot_sync(0xffffffffu, (w >> 33) != 0);
+        // usable: the run of ready predecessors starting at lane 0, up to and including the first inclusive one
+        const uint32_t run = __ffs(~ready) - 1;  // 32 when all are ready (ffs(0) = 0 -> wraps to 0xffffffff: handled below)
+        uint32_t usable = ready == 0xffffffffu ? 32u : run;
+        const uint32_t first_incl = incl ? (uint32_t)__ffs(incl) - 1u : 32u;
+        const bool done = first_incl < usable;
+        if (done) usable = first_incl + 1;
+        uint32_t v = lane_id() < usable ? (uint32_t)w : 0u;
+        v = __reduce_add_sync(0xffffffffu, v);
+        excl += v;
+        if (done) break;
+        t -= usable;
+        if (usable == 0) {
+          if (++spins > (1u << 22)) {  // a predecessor is lost: report instead of hanging the device
+            if (lane_id() == 0) *error_flag = 1u;
+            break;
+          }
+          __nanosleep(20);
+        }
+      }
+      if (threadIdx.x == 0) st_relaxed_u64(my_status, kStatInclusive | (uint64_t)(excl + tile_total));
+    }
+    if (threadIdx.x == 0) sh_prefix = excl;
+  }
+  __syncthreads();
+  const uint32_t prefix = sh_prefix;
+  const uint64_t tile_end = (uint64_t)tile * kFusedTile + kFusedTile;
+  if (threadIdx.x == 0 && tile_end >= n && (uint64_t)tile * kFusedTile < n) *total_groups = (uint64_t)prefix + tile_total;
+
+#pragma unroll
+  for (int c = 0; c < kFusedChunks; ++c) {
+    const uint32_t base = tile * (uint32_t)kFusedTile + (uint32_t)c * (kFusedThreads * 8) + threadIdx.x * 8u;
+    uint32_t g = prefix + (c == 0 ? ex0 : ex1);
+    uint32_t m = heads[c];
+    while (m) {
+      const int i = __ffs(m) - 1;
+      m &= m - 1;
+      const uint32_t j = base + i;
+      uint32_t si = s[c][1], di = d[c][1], sp = s[c][0];
+#pragma unroll
+      for (int q = 1; q < 8; ++q)
+        if (i == q) {
+          si = s[c][q + 1];
+          di = d[c][q + 1];
+          sp = s[c][q];
+        }
+      out.group_start[g] = j;
+      out.group_delay[g] = (uint16_t)di;
+      if (first_src[c] & (1u << i)) {
+        const uint32_t lo = j == 0 ? 0u : sp + 1u;  // nodes in between have no outgoing connection (Q9)
+        for (uint32_t node = lo; node <= si; ++node) {
+          out.src_offsets[node] = j;
+          out.group_ptr[node] = g;
+        }
+      }
+      ++g;
+    }
+    if (cnt[c] > 0 && base + cnt[c] == n) {  // nodes after the last source, and the closing entries
+      uint32_t sl = s[c][1];
+#pragma unroll
+      for (int q = 1; q < 8; ++q)
+        if (cnt[c] == (uint32_t)q + 1) sl = s[c][q + 1];
+      const uint32_t tg = prefix + tile_total;  // this is the last tile: its inclusive prefix is the number of groups
+      for (uint64_t node = (uint64_t)sl + 1; node <= out.n_nodes; ++node) {
+        out.src_offsets[node] = n;
+        out.group_ptr[node] = tg;
+      }
     }
   }
 }

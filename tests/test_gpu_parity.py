@@ -586,3 +586,12 @@ def test_scratch_of_earlier_connect_calls_is_released(nc_mod):
     # one call's scratch (9e6 trials: 1.1 MB mask + tables) may be pending, never several
     assert max(held[1:]) <= held[0] + (1 << 20), held
     g.close()
+
+
+def test_single_read_index_variant_parity(nc_mod, oracle_mod, monkeypatch):
+    """NC_INDEX_FUSED=1: heads counted, chained across tiles by look-back and written by one kernel (one read of the
+    organised keys instead of two).  Several tiles, sources without connections, a ragged last tile."""
+    monkeypatch.setenv("NC_INDEX_FUSED", "1")
+    for net in (WL.config2_microcircuit(scale=0.06), WL.config1_rule("fixed_outdegree", scale=0.2), WL.config0_tiny()):
+        rep, _ = PU.full_parity(net, oracle_mod, nc_mod)
+        assert rep["n"] >= 1000
