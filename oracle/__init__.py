@@ -262,6 +262,13 @@ class Oracle:
         if rc != 0:
             raise OracleError(rc)
 
+    def set_rule_flags(self, flags: int):
+        L = lib()
+        L.oc_set_rule_flags.argtypes = [C.c_void_p, C.c_uint32]
+        rc = L.oc_set_rule_flags(self._h, int(flags))
+        if rc != 0:
+            raise OracleError(rc)
+
     def set_connection_attributes(self, port: int, syn_group: int = 0):
         L = lib()
         L.oc_set_connection_attributes.argtypes = [C.c_void_p, C.c_uint8, C.c_uint8]
@@ -468,3 +475,15 @@ def copass_block_sort(keys, vals, sizes, max_extract=None):
     if rc != 0:
         raise OracleError(rc)
     return keys, vals, sub_start, sub_len, {f: getattr(st, f) for f, _ in _CopassStats._fields_}
+
+
+NO_AUTAPSES, NO_MULTAPSES = 1, 2
+
+
+def keyed_permutation(M: int, k: int, keys) -> int:
+    """oc_keyed_permutation (reading A5)."""
+    L = lib()
+    L.oc_keyed_permutation.restype = C.c_uint32
+    L.oc_keyed_permutation.argtypes = [C.c_uint32, C.c_uint32, C.POINTER(C.c_uint32)]
+    arr = (C.c_uint32 * 4)(*[int(x) & 0xffffffff for x in keys])
+    return int(L.oc_keyed_permutation(int(M), int(k), arr))

@@ -81,6 +81,37 @@ double max_delay_steps(const oc_dist& d, double inv_dt) {
   return std::floor(top * inv_dt + 0.5);
 }
 
+/* Reading A5: a permutation of [0, M) keyed by four words -- cycle walking over a balanced Feistel network of
+ * 6 + ceil(24 / h) rounds on 2h bits (narrow halves need more rounds: a two-round differential trail has probability 2^-h). */
+uint32_t mix32(uint32_t v) {
+  v ^= v >> 16;
+  v *= 0x7feb352du;
+  v ^= v >> 15;
+  v *= 0x846ca68bu;
+  v ^= v >> 16;
+  return v;
+}
+uint32_t keyed_permutation(uint32_t M, uint32_t k, const uint32_t keys[4]) {
+  if (M <= 1) return 0;
+  uint32_t bits = 0;
+  for (uint32_t v = M - 1; v; v >>= 1) ++bits;
+  const uint32_t h = std::max<uint32_t>(1, (bits + 1) / 2);
+  const uint32_t mask = (1u << h) - 1u; /* h <= 16 */
+  uint32_t x = k;
+  do {
+    uint32_t L = x >> h, R = x & mask;
+    const uint32_t rounds = 6 + (24 + h - 1) / h;
+    for (uint32_t r = 0; r < rounds; ++r) {
+      const uint32_t key_r = keys[r & 3] + r * 0x9E3779B9u;
+      const uint32_t nR = L ^ (mix32(R ^ key_r) & mask);
+      L = R;
+      R = nR;
+    }
+    x = (L << h) | R;
+  } while (x >= M);
+  return x;
+}
+
 struct Projection {
   oc_range src, tgt;
   int rule;
@@ -195,6 +226,7 @@ struct oc_context {
   std::vector<uint8_t> bnd;
   std::vector<uint8_t> port, group; /* receptor port index and synaptic group index of every connection */
   uint8_t cur_port = 0, cur_group = 0;
+  uint32_t rule_flags = 0; /* OC_NO_AUTAPSES | OC_NO_MULTAPSES for the connect calls that follow (readings A1-A6) */
   uint64_t n_blocks = 0;
   /* D10: sorted copies. */
   std::vector<uint32_t> perm, ssrc, stgt;
@@ -312,9 +344,157 @@ static int connect_core(oc_context* ctx, uint64_t node_space, oc_range src, oc_r
   return OC_OK;
 }
 
+
+/* Readings A1-A6: a connect call with autapses and / or multapses prohibited.  src / tgt are index ranges into the node
+ * arrays when those are given (first = 0), node ranges otherwise. */
+static int connect_flagged(oc_context* ctx, const uint32_t* src_nodes, oc_range src, const uint32_t* tgt_nodes, oc_range tgt,
+                           int rule, const oc_rule_params* params, const oc_syn_spec* syn, uint64_t seed, uint32_t flags) {
+  if (ctx->finalized) return OC_ERR_STATE;
+  const bool no_aut = (flags & OC_NO_AUTAPSES) != 0, no_mult = (flags & OC_NO_MULTAPSES) != 0;
+  uint64_t n_iter = 0;
+  const uint64_t space = std::max<uint64_t>(ctx->n_nodes, std::max<uint64_t>(src_nodes ? src.count : 0, tgt_nodes ? tgt.count : 0));
+  int rc = validate((uint32_t)std::min<uint64_t>(space, 0xffffffffull), src, tgt, rule, params, syn, ctx->inv_dt, &n_iter);
+  if (rc != OC_OK) return rc;
+  auto sid = [&](uint64_t sl) -> uint32_t { return src_nodes ? src_nodes[sl] : (uint32_t)(src.first + sl); };
+  auto tid = [&](uint64_t tl) -> uint32_t { return tgt_nodes ? tgt_nodes[tl] : (uint32_t)(tgt.first + tl); };
+  /* A1: no repeated ids in explicit arrays */
+  for (int side = 0; side < 2; ++side) {
+    const uint32_t* a = side ? tgt_nodes : src_nodes;
+    if (!a) continue;
+    std::vector<uint32_t> v(a, a + (side ? tgt.count : src.count));
+    std::sort(v.begin(), v.end());
+    if (std::adjacent_find(v.begin(), v.end()) != v.end()) return OC_ERR_INVALID_ARG;
+  }
+  /* index of a node id among the sources / targets, or -1 */
+  auto find_in = [&](bool in_src, uint32_t id) -> int64_t {
+    const uint32_t* a = in_src ? src_nodes : tgt_nodes;
+    const oc_range r = in_src ? src : tgt;
+    if (!a) return (id >= r.first && (uint64_t)id < (uint64_t)r.first + r.count) ? (int64_t)(id - r.first) : -1;
+    for (uint32_t k = 0; k < r.count; ++k)
+      if (a[k] == id) return k;
+    return -1;
+  };
+  const uint64_t K = params->degree_or_total;
+  if (rule == OC_FIXED_TOTAL_NUMBER && no_mult) return OC_ERR_INVALID_ARG; /* A6 */
+  /* feasibility */
+  if (rule == OC_FIXED_INDEGREE || rule == OC_FIXED_OUTDEGREE) {
+    const bool indeg = rule == OC_FIXED_INDEGREE;
+    const uint64_t n_fixed = indeg ? tgt.count : src.count, n_part = indeg ? src.count : tgt.count;
+    for (uint64_t f = 0; f < n_fixed; ++f) {
+      const uint32_t fid = indeg ? tid(f) : sid(f);
+      const uint64_t e = (no_aut && find_in(indeg, fid) >= 0) ? 1 : 0;
+      const uint64_t M = n_part - e;
+      if (no_mult ? K > M : (K > 0 && M == 0)) return OC_ERR_INVALID_ARG;
+    }
+  }
+  if (rule == OC_FIXED_TOTAL_NUMBER && no_aut && K > 0 && src.count == 1 && tgt.count == 1 && sid(0) == tid(0))
+    return OC_ERR_INVALID_ARG;
+
+  Projection pr{src, tgt, rule, *params, *syn, seed, ctx->n_projections};
+  const uint64_t n_before = ctx->src.size();
+  auto rollback = [&]() {
+    ctx->src.resize(n_before); ctx->tgt.resize(n_before); ctx->w.resize(n_before); ctx->d.resize(n_before); ctx->bnd.resize(n_before);
+  };
+  auto append = [&](uint64_t idx, uint32_t s_id, uint32_t t_id) { /* weight and delay: words 2, 3 of Philox(idx, stream 0) */
+    oc_synapse sy;
+    eval_synapse(pr, ctx->inv_dt, idx, &sy);
+    ctx->src.push_back(s_id);
+    ctx->tgt.push_back(t_id);
+    ctx->w.push_back(sy.weight);
+    ctx->d.push_back(sy.delay);
+    ctx->bnd.push_back(sy.boundary);
+  };
+  try {
+    if (rule == OC_ONE_TO_ONE || rule == OC_ALL_TO_ALL || rule == OC_PAIRWISE_BERNOULLI) { /* A2 */
+      const uint64_t T = rule == OC_PAIRWISE_BERNOULLI ? bernoulli_threshold(params->p) : 0;
+      uint32_t tw[4] = {0, 0, 0, 0};
+      for (uint64_t q = 0; q < n_iter; ++q) {
+        if (rule == OC_PAIRWISE_BERNOULLI) {
+          if ((q & 3) == 0) philox_stream(seed, pr.id, 1u, q >> 2, tw);
+          if (!((uint64_t)tw[q & 3] < T)) continue;
+        }
+        const uint64_t sl = rule == OC_ONE_TO_ONE ? q : q / tgt.count, tl = rule == OC_ONE_TO_ONE ? q : q % tgt.count;
+        if (no_aut && sid(sl) == tid(tl)) continue;
+        if (ctx->src.size() >= 0xffffffffull) {
+          rollback();
+          return OC_ERR_CAPACITY;
+        }
+        append(q, sid(sl), tid(tl));
+      }
+    } else {
+      if (n_before + n_iter > 0xffffffffull) return OC_ERR_CAPACITY;
+      const bool indeg = rule == OC_FIXED_INDEGREE, outdeg = rule == OC_FIXED_OUTDEGREE;
+      for (uint64_t i = 0; i < n_iter; ++i) {
+        uint32_t w[4];
+        if (rule == OC_FIXED_TOTAL_NUMBER) { /* A4 */
+          uint64_t sl = 0, tl = 0;
+          for (uint32_t a = 0;; ++a) {
+            philox_stream(seed, pr.id, a == 0 ? 0u : 1u + a, i, w);
+            sl = bounded(w[0], src.count);
+            tl = bounded(w[1], tgt.count);
+            if (sid(sl) != tid(tl)) break;
+            if (a == 63) { /* never reached in practice: take the next target, cyclically */
+              tl = (tl + 1) % tgt.count;
+              if (sid(sl) == tid(tl)) sl = (sl + 1) % src.count;
+              break;
+            }
+          }
+          append(i, sid(sl), tid(tl));
+          continue;
+        }
+        const uint64_t f = i / K, k = i % K; /* fixed node number and which of its K partners */
+        const uint32_t fid = indeg ? tid(f) : sid(f);
+        const uint32_t n_part = indeg ? src.count : tgt.count;
+        uint64_t x = 0;
+        if (!no_mult) { /* A3 */
+          for (uint32_t a = 0;; ++a) {
+            philox_stream(seed, pr.id, a == 0 ? 0u : 1u + a, i, w);
+            x = bounded(indeg ? w[0] : w[1], n_part);
+            if ((indeg ? sid(x) : tid(x)) != fid) break;
+            if (a == 63) {
+              x = (x + 1) % n_part;
+              break;
+            }
+          }
+        } else { /* A5 */
+          const int64_t z = no_aut ? find_in(indeg, fid) : -1;
+          const uint32_t M = n_part - (z >= 0 ? 1u : 0u);
+          philox_stream(seed, pr.id, 2u, f, w);
+          x = keyed_permutation(M, (uint32_t)k, w);
+          if (z >= 0 && x >= (uint64_t)z) x += 1;
+        }
+        (void)outdeg;
+        if (indeg) append(i, sid(x), fid);
+        else append(i, fid, tid(x));
+      }
+    }
+  } catch (const std::bad_alloc&) {
+    rollback();
+    return OC_ERR_OOM;
+  }
+  const uint64_t n_newconns = ctx->src.size() - n_before;
+  const uint64_t n_newblocks = (n_before + n_newconns + ctx->B - 1) / ctx->B - ctx->n_blocks; /* Eq. 1 */
+  ctx->n_blocks += n_newblocks;
+  ctx->n_projections += 1;
+  ctx->proj_start.push_back(n_before);
+  ctx->have_in = ctx->have_out = false;
+  ctx->port.resize(ctx->src.size(), ctx->cur_port);
+  ctx->group.resize(ctx->src.size(), ctx->cur_group);
+  return OC_OK;
+}
+
+int oc_set_rule_flags(oc_context* ctx, uint32_t flags) {
+  if (!ctx || (flags & ~3u)) return OC_ERR_INVALID_ARG;
+  if (ctx->finalized) return OC_ERR_STATE;
+  ctx->rule_flags = flags;
+  return OC_OK;
+}
+uint32_t oc_keyed_permutation(uint32_t M, uint32_t k, const uint32_t keys[4]) { return keyed_permutation(M, k, keys); }
+
 int oc_connect(oc_context* ctx, oc_range src, oc_range tgt, int rule, const oc_rule_params* params,
                const oc_syn_spec* syn, uint64_t seed) {
   if (!ctx) return OC_ERR_INVALID_ARG;
+  if (ctx->rule_flags) return connect_flagged(ctx, nullptr, src, nullptr, tgt, rule, params, syn, seed, ctx->rule_flags);
   return connect_core(ctx, ctx->n_nodes, src, tgt, rule, params, syn, seed);
 }
 
@@ -335,6 +515,7 @@ int oc_connect_nodes(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src,
   if ((!src_nodes && (uint64_t)src.first + src.count > ctx->n_nodes) ||
       (!tgt_nodes && (uint64_t)tgt.first + tgt.count > ctx->n_nodes))
     return OC_ERR_INVALID_ARG;
+  if (ctx->rule_flags) return connect_flagged(ctx, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed, ctx->rule_flags);
   const uint64_t space = std::max<uint64_t>(ctx->n_nodes, std::max<uint64_t>(src_nodes ? n_src : 0, tgt_nodes ? n_tgt : 0));
   const size_t before = ctx->src.size();
   int rc = connect_core(ctx, space, src, tgt, rule, params, syn, seed);
@@ -359,6 +540,8 @@ int oc_connect_values(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src
   if (ctx->finalized) return OC_ERR_STATE;
   if (!weights && !delays_ms) return OC_ERR_INVALID_ARG;
   if (rule == OC_PAIRWISE_BERNOULLI) return OC_ERR_INVALID_ARG; /* its number of connections is not known beforehand */
+  if ((ctx->rule_flags & OC_NO_AUTAPSES) && (rule == OC_ONE_TO_ONE || rule == OC_ALL_TO_ALL))
+    return OC_ERR_INVALID_ARG; /* reading A2: nor is it when pairs with equal ids are left out */
   for (uint64_t i = 0; weights && i < n_values; ++i)
     if (std::isnan(weights[i])) return OC_ERR_INVALID_ARG;
   for (uint64_t i = 0; delays_ms && i < n_values; ++i) {

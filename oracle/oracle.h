@@ -112,6 +112,36 @@ int oc_connect_values(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src
 int oc_set_connection_attributes(oc_context* ctx, uint8_t port, uint8_t syn_group);
 int oc_read_connection_attributes(oc_context* ctx, int sorted, uint64_t first, uint64_t count, uint8_t* port,
                                   uint8_t* syn_group);
+/* Prohibiting autapses and multapses ("Autapses and multapses are currently always allowed in NEST GPU;
+ * therefore another useful addition would be the possibility to prohibit them (for example, using a flag as in the CPU
+ * version of NEST)"; PAPER.md:47, 148 for the allowed default).  The flags hold for the connect calls that follow
+ * (0 at the start).  Readings A1-A6 of DESIGN.md section 8c:
+ *  A1 an autapse is a connection whose source node id equals its target node id; a multapse is a second connection of
+ *     the SAME connect call with the same (source id, target id).  With either flag set, explicit node arrays must not
+ *     repeat an id (OC_ERR_INVALID_ARG).
+ *  A2 one_to_one, all_to_all, pairwise_bernoulli: every pair occurs at most once, so OC_NO_MULTAPSES changes nothing;
+ *     under OC_NO_AUTAPSES the pairs with equal ids are left out, the others keep their pair index q for the synapse
+ *     stream (same weight and delay as without the flag) and take consecutive creation positions in ascending q.
+ *  A3 fixed_indegree / fixed_outdegree under OC_NO_AUTAPSES alone: connection i redraws its random partner until its id
+ *     differs from the fixed node's: attempt 0 is the draw of the unflagged rule (stream 0), attempt a >= 1 takes the
+ *     same word of Philox(idx = i, stream = 1 + a); after 64 attempts the next partner index (cyclically) is taken.
+ *  A4 fixed_total_number under OC_NO_AUTAPSES: the same with both coordinates redrawn (words 0 and 1).
+ *  A5 fixed_indegree / fixed_outdegree under OC_NO_MULTAPSES: the K partners of fixed node number f are the first K values
+ *     of a keyed permutation of the M allowed partner indexes, partner(f, k) = skip(perm_M(k; keys(f))), where
+ *     M = N_partners - e, e = 1 iff OC_NO_AUTAPSES is also set and f's id is among the partners (at index z), and
+ *     skip(x) = x + (e and x >= z).  keys(f) = the four words of Philox(idx = f, stream = 2).  K > M is
+ *     OC_ERR_INVALID_ARG.  perm_M: oc_keyed_permutation below.
+ *  A6 fixed_total_number under OC_NO_MULTAPSES is not offered (OC_ERR_INVALID_ARG).
+ * Weight and delay of connection i always come from words 2 and 3 of Philox(idx = i, stream 0) (D5-D8). */
+enum { OC_NO_AUTAPSES = 1, OC_NO_MULTAPSES = 2 };
+int oc_set_rule_flags(oc_context* ctx, uint32_t flags);
+/* perm_M(k; keys), k < M: a permutation of [0, M) by cycle walking over a balanced Feistel network on 2h bits,
+ * h = max(1, ceil(bits(M - 1) / 2)): x = k; repeat { (L, R) = (x >> h, x & (2^h - 1)); 6 + ceil(24 / h) rounds
+ * r = 0, 1, ...: (L, R) <- (R, L ^ (mix32(R ^ key_r) & (2^h - 1))), key_r = keys[r & 3] + r * 0x9E3779B9; x = L << h | R }
+ * until x < M.  (Narrow halves get more rounds: a two-round differential trail of the network has probability 2^-h, and
+ * tests/test_oracle_flags.py sees the resulting excess of neighbouring pairs with six rounds on a 4-bit domain.)
+ * mix32(v): v ^= v >> 16; v *= 0x7feb352d; v ^= v >> 15; v *= 0x846ca68b; v ^= v >> 16. */
+uint32_t oc_keyed_permutation(uint32_t M, uint32_t k, const uint32_t keys[4]);
 int oc_finalize(oc_context* ctx);
 int oc_num_connections(oc_context* ctx, uint64_t* n);
 int oc_num_nodes(oc_context* ctx, uint32_t* n);
