@@ -215,6 +215,34 @@ int nc_create_population(nc_context* ctx, uint32_t n, uint32_t* first_id);
 int nc_connect(nc_context* ctx, nc_range src, nc_range tgt, nc_rule rule, const nc_rule_params* params,
                const nc_syn_spec* syn, uint64_t seed);
 
+/* Prohibiting autapses and multapses ("Autapses and multapses are currently always allowed in NEST GPU;
+ * therefore another useful addition would be the possibility to prohibit them (for example, using a flag as in the CPU
+ * version of NEST)"; PAPER.md:47, 148 for the allowed default).  The flags hold for the nc_connect* calls that follow
+ * (0 at nc_create).  Readings:
+ *  A1 an autapse is a connection whose source node id equals its target node id; a multapse is a second connection of the
+ *     SAME connect call with the same (source id, target id).  With either flag set, explicit node arrays must not repeat
+ *     an id (NC_ERR_INVALID_ARG).
+ *  A2 one_to_one, all_to_all, pairwise_bernoulli: every pair occurs at most once, so NC_NO_MULTAPSES changes nothing;
+ *     under NC_NO_AUTAPSES the pairs with equal ids are left out, the others keep their pair index q for the synapse stream
+ *     (same weight and delay as without the flag) and take consecutive creation positions in ascending q; the call then
+ *     waits for its exact count like pairwise_bernoulli, and nc_connect_values refuses these two rules.
+ *  A3 fixed_indegree / fixed_outdegree under NC_NO_AUTAPSES alone: connection i redraws its random partner until its id
+ *     differs from the fixed node's: attempt 0 is the draw of the unflagged rule (stream 0), attempt a >= 1 takes the same
+ *     word of Philox(idx = i, stream = 1 + a); after 64 attempts the next partner index (cyclically) is taken.  Only the
+ *     connections that were autapses change.
+ *  A4 fixed_total_number under NC_NO_AUTAPSES: the same with both coordinates redrawn (words 0 and 1).
+ *  A5 fixed_indegree / fixed_outdegree under NC_NO_MULTAPSES: the K partners of fixed node number f are the first K values
+ *     of a keyed permutation of the M allowed partner indexes, partner(f, k) = skip(perm_M(k; keys(f))), M = N_partners - e,
+ *     e = 1 iff NC_NO_AUTAPSES is also set and f's id is among the partners (at index z), skip(x) = x + (e and x >= z),
+ *     keys(f) = the four words of Philox(idx = f, stream 2).  perm_M: cycle walking over a balanced Feistel network on 2h
+ *     bits, h = max(1, ceil(bits(M - 1) / 2)), 6 + ceil(24 / h) rounds (L, R) <- (R, L ^ (mix32(R ^ key_r) & (2^h - 1))),
+ *     key_r = keys[r & 3] + r * 0x9E3779B9, mix32(v): v ^= v >> 16; v *= 0x7feb352d; v ^= v >> 15; v *= 0x846ca68b;
+ *     v ^= v >> 16.  K > M for some fixed node is NC_ERR_INVALID_ARG.
+ *  A6 fixed_total_number under NC_NO_MULTAPSES is not offered (NC_ERR_INVALID_ARG).
+ * Weight and delay of connection i always come from words 2 and 3 of Philox(idx = i, stream 0) (D5-D8). ---- */
+enum { NC_NO_AUTAPSES = 1u, NC_NO_MULTAPSES = 2u };
+int nc_set_rule_flags(nc_context* ctx, uint32_t flags);
+
 /* The same with explicit node arrays ("If the indexes of source or target nodes are not consecutive but
  * are explicitly given by an array, the above formulas are used to derive the indexes of the array elements from
  * which to extract the node indexes").  src_nodes / tgt_nodes are HOST arrays of n_src / n_tgt node ids (copied

@@ -21,6 +21,7 @@ OK, ERR_INVALID_ARG, ERR_STATE, ERR_CAPACITY, ERR_OOM, ERR_CUDA = 0, -1, -2, -3,
 ONE_TO_ONE, ALL_TO_ALL, FIXED_INDEGREE, FIXED_OUTDEGREE, FIXED_TOTAL_NUMBER, PAIRWISE_BERNOULLI = range(6)
 FLAG_TIMING, FLAG_EXACT_FP64, FLAG_SORT_PAIRS, FLAG_SORT_ONESWEEP, FLAG_ORGANISE_COPASS, FLAG_COPASS_SHIFT = 1, 2, 4, 8, 16, 32
 FLAG_SORT_BULK = 64
+NO_AUTAPSES, NO_MULTAPSES = 1, 2  # nc_set_rule_flags
 PHASES = ("generate", "histogram", "sort", "permute", "index", "degree", "copass")
 
 # every symbol include/nc.h declares (checked by tests/test_abi.py against the header and the library)
@@ -30,6 +31,7 @@ SYMBOLS = (
     "nc_degree_histogram", "nc_get_stats", "nc_get_timings", "nc_read_connections", "nc_read_index",
     "nc_read_degree_histogram", "nc_selftest_philox", "nc_selftest_fastpath", "nc_selftest_guard",
     "nc_connect_nodes", "nc_connect_values", "nc_set_connection_attributes", "nc_read_connection_attributes",
+    "nc_set_rule_flags",
     # include/nc_delivery.h
     "nc_delivery_create", "nc_delivery_destroy", "nc_delivery_step", "nc_delivery_read_spike_array",
     "nc_delivery_counts", "nc_delivery_num_ports", "nc_delivery_run",
@@ -302,6 +304,10 @@ class NC:
 
     def connect(self, *a, **k):
         self._check(self.connect_rc(*a, **k))
+
+    def set_rule_flags(self, flags: int):
+        self._L.nc_set_rule_flags.argtypes = [C.c_void_p, C.c_uint32]
+        self._check(self._L.nc_set_rule_flags(self._h, int(flags)))
 
     def set_connection_attributes(self, port: int, syn_group: int = 0):
         self._check(self._L.nc_set_connection_attributes(self._h, int(port), int(syn_group)))

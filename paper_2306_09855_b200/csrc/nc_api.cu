@@ -16,6 +16,7 @@
 #include "nc_common.cuh"
 #include "nc_internal.h"
 #include "nc_generate.cuh"
+#include "nc_flags.cuh"
 #include "nc_index.cuh"
 #include "nc_sort.cuh"
 #include "nc_sort_split.cuh"
@@ -74,6 +75,7 @@ struct nc_context {
   CopassTotals* d_copass_totals = nullptr;
   uint64_t copass_aux_bytes = 0, copass_moved = 0;
   uint8_t cur_port = 0, cur_group = 0;       // attributes in force for the next nc_connect*
+  uint32_t rule_flags = 0;                   // NC_NO_AUTAPSES | NC_NO_MULTAPSES for the next nc_connect*
   std::vector<uint32_t> proj_first;          // creation position of the first connection of every projection
   std::vector<uint16_t> proj_attr;           // port | syn_group << 8 of every projection
   uint8_t* d_sorted_port = nullptr;          // port of every organised connection, built on first use by delivery
@@ -394,9 +396,13 @@ int device_scan(nc_context* c, const uint32_t* in, uint32_t* out, uint64_t n, ui
   return NC_OK;
 }
 
-int connect_bernoulli(nc_context* c, GenParams gp, double p, uint32_t seed_lo, uint32_t seed_hi) {
-  const uint64_t n_pairs = (uint64_t)gp.n_src * gp.n_tgt;
-  const uint64_t T = (uint64_t)std::floor(std::ldexp(p, 32));  // Q14
+// Pair-mask path: pairwise_bernoulli (trials = true), and -- reading A2 -- one_to_one / all_to_all with the equal-id
+// pairs left out (trials = false: every pair accepted, then the autapses cleared).  self_tgt: device array for
+// pair_mask_clear_autapses_kernel when node arrays are in use, NULL for ranges.
+int connect_bernoulli(nc_context* c, GenParams gp, double p, uint32_t seed_lo, uint32_t seed_hi, bool trials = true,
+                      bool one_to_one = false, bool no_autapses = false, const uint32_t* self_tgt = nullptr) {
+  const uint64_t n_pairs = one_to_one ? (uint64_t)gp.n_src : (uint64_t)gp.n_src * gp.n_tgt;
+  const uint64_t T = trials ? (uint64_t)std::floor(std::ldexp(p, 32)) : (1ull << 32);  // Q14
   if (T == 0) return NC_OK;                                    // realised probability 0: nothing to create
   const uint64_t n_tiles = (n_pairs + kBernTile - 1) / kBernTile;
   if (n_tiles > 0x7fffffffull) return fail(c, NC_ERR_CAPACITY, "pairwise_bernoulli: too many pairs for one call");
@@ -419,14 +425,33 @@ int connect_bernoulli(nc_context* c, GenParams gp, double p, uint32_t seed_lo, u
   gen_span_end(c);
   {
     Scope sc(c, NC_PHASE_GENERATE);
-    BernParams bp{};
-    bp.n_pairs = n_pairs;
-    bp.threshold = T;
-    bp.rng = make_philox_stream(seed_lo, seed_hi, c->n_proj, 1u);
-    bp.mask = mask;
-    bp.tile_count = tile_count;
-    bernoulli_trials_kernel<<<(unsigned)n_tiles, kBernThreads, 0, c->stream>>>(bp);
-    NC_LAUNCH_CHECK(c, "bernoulli_trials");
+    PairMaskParams pm{};
+    pm.n_pairs = n_pairs;
+    pm.n_src = gp.n_src;
+    pm.n_tgt = gp.n_tgt;
+    pm.s0 = gp.s0;
+    pm.t0 = gp.t0;
+    pm.one_to_one = one_to_one ? 1u : 0u;
+    pm.self_tgt = self_tgt;
+    pm.mask = mask;
+    pm.tile_count = tile_count;
+    if (trials) {
+      BernParams bp{};
+      bp.n_pairs = n_pairs;
+      bp.threshold = T;
+      bp.rng = make_philox_stream(seed_lo, seed_hi, c->n_proj, 1u);
+      bp.mask = mask;
+      bp.tile_count = tile_count;
+      bernoulli_trials_kernel<<<(unsigned)n_tiles, kBernThreads, 0, c->stream>>>(bp);
+      NC_LAUNCH_CHECK(c, "bernoulli_trials");
+    } else {
+      pair_mask_fill_kernel<<<(unsigned)n_tiles, kBernThreads, 0, c->stream>>>(pm);
+      NC_LAUNCH_CHECK(c, "pair_mask_fill");
+    }
+    if (no_autapses) {
+      pair_mask_clear_autapses_kernel<<<(gp.n_src + 255) / 256, 256, 0, c->stream>>>(pm);
+      NC_LAUNCH_CHECK(c, "pair_mask_clear_autapses");
+    }
     int rc = device_scan(c, tile_count, tile_off, n_tiles, partial, d_total);
     if (rc != NC_OK) {
       drop();
@@ -453,6 +478,7 @@ int connect_bernoulli(nc_context* c, GenParams gp, double p, uint32_t seed_lo, u
     wp.g.pos0 = c->n_conns;
     wp.g.n = total;
     wp.n_pairs = n_pairs;
+    wp.one_to_one = one_to_one ? 1u : 0u;
     wp.mask = mask;
     wp.tile_offset = tile_off;
     bernoulli_write_kernel<<<(unsigned)n_tiles, kBernThreads, 0, c->stream>>>(wp);
@@ -1689,6 +1715,73 @@ static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, 
   if (rule != NC_PAIRWISE_BERNOULLI && c->n_conns + n_new > kMaxConns)
     return fail(c, NC_ERR_CAPACITY, "more than 2^32-1 connections");
 
+  // ---- autapses / multapses prohibited (readings A1-A6): checks that need no device work ----
+  const uint32_t rflags = c->rule_flags;
+  const bool no_aut = (rflags & NC_NO_AUTAPSES) != 0, no_mult = (rflags & NC_NO_MULTAPSES) != 0;
+  std::vector<uint32_t> self_host;  // A2: per source its equal-id target index; A5: per fixed node its index among the partners
+  bool need_self = false;
+  if (rflags) {
+    if (with_values && no_aut && (rule == NC_ONE_TO_ONE || rule == NC_ALL_TO_ALL))
+      return fail(c, NC_ERR_INVALID_ARG, "nc_connect_values: without autapses the number of connections of this rule is not known beforehand");
+    if (rule == NC_FIXED_TOTAL_NUMBER && no_mult)
+      return fail(c, NC_ERR_INVALID_ARG, "fixed_total_number cannot prohibit multapses (reading A6)");
+    for (int side = 0; side < 2; ++side) {  // A1: node arrays must not repeat an id
+      const uint32_t* a = side ? tgt_nodes : src_nodes;
+      if (!a) continue;
+      std::vector<uint32_t> v(a, a + (side ? tgt.count : src.count));
+      std::sort(v.begin(), v.end());
+      if (std::adjacent_find(v.begin(), v.end()) != v.end())
+        return fail(c, NC_ERR_INVALID_ARG, "nc_connect_nodes: a node array repeats an id while autapses or multapses are prohibited");
+    }
+    // index of a node id among the sources (side 0) or targets (side 1), or kNoIndex
+    std::unordered_map<uint32_t, uint32_t> where[2];
+    for (int side = 0; side < 2; ++side) {
+      const uint32_t* a = side ? tgt_nodes : src_nodes;
+      const uint32_t cnt = side ? tgt.count : src.count;
+      for (uint32_t k = 0; a && k < cnt; ++k) where[side][a[k]] = k;
+    }
+    auto find_in = [&](int side, uint32_t id) -> uint32_t {
+      const uint32_t* a = side ? tgt_nodes : src_nodes;
+      const nc_range r = side ? tgt : src;
+      if (!a) return (id >= r.first && (uint64_t)id < (uint64_t)r.first + r.count) ? id - r.first : kNoIndex;
+      auto it = where[side].find(id);
+      return it == where[side].end() ? kNoIndex : it->second;
+    };
+    auto id_of = [&](int side, uint32_t k) -> uint32_t {
+      const uint32_t* a = side ? tgt_nodes : src_nodes;
+      return a ? a[k] : (side ? tgt.first : src.first) + k;
+    };
+    const bool arrays = src_nodes || tgt_nodes;
+    if (rule == NC_FIXED_INDEGREE || rule == NC_FIXED_OUTDEGREE) {
+      const int fixed_side = rule == NC_FIXED_INDEGREE ? 1 : 0, part_side = 1 - fixed_side;
+      const uint32_t n_fixed = fixed_side ? tgt.count : src.count, n_part = part_side ? tgt.count : src.count;
+      bool any_self = false;
+      if (no_aut) {
+        if (arrays) {
+          self_host.resize(n_fixed);
+          for (uint32_t f = 0; f < n_fixed; ++f) {
+            self_host[f] = find_in(part_side, id_of(fixed_side, f));
+            any_self = any_self || self_host[f] != kNoIndex;
+          }
+          need_self = no_mult;  // only the permutation (A5) needs the index on the device; the redraws compare ids
+        } else {
+          const uint64_t a0 = fixed_side ? tgt.first : src.first, b0 = part_side ? tgt.first : src.first;
+          any_self = a0 < b0 + n_part && b0 < a0 + n_fixed;  // the ranges overlap
+        }
+      }
+      const uint64_t M_min = (uint64_t)n_part - (any_self ? 1 : 0);
+      if (no_mult ? K > M_min : (K > 0 && M_min == 0))
+        return fail(c, NC_ERR_INVALID_ARG, "more distinct partners asked for than the rule allows (readings A3, A5)");
+    } else if (rule == NC_FIXED_TOTAL_NUMBER) {
+      if (no_aut && K > 0 && src.count == 1 && tgt.count == 1 && id_of(0, 0) == id_of(1, 0))
+        return fail(c, NC_ERR_INVALID_ARG, "fixed_total_number: the only pair is an autapse");
+    } else if (no_aut && arrays) {  // A2 with node arrays: which target index carries each source's id
+      self_host.resize(src.count);
+      for (uint32_t k = 0; k < src.count; ++k) self_host[k] = find_in(1, id_of(0, k));
+      need_self = true;
+    }
+  }
+
   GenParams gp{};
   gp.pos0 = c->n_conns;
   gp.n = n_new;
@@ -1714,9 +1807,61 @@ static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, 
     (side == 0 ? gp.src_nodes : gp.tgt_nodes) = dev;
   }
 
-  if (rule == NC_PAIRWISE_BERNOULLI) {
-    int rc = connect_bernoulli(c, gp, params->p, seed_lo, seed_hi);
+  uint32_t* d_self = nullptr;
+  if (need_self) {
+    d_self = (uint32_t*)dev_alloc(c, self_host.size() * 4);
+    if (!d_self) return fail(c, NC_ERR_OOM, "out of device memory for the self-index array");
+    dev_free_later(c, d_self);
+    NC_CUDA(c, cudaMemcpyAsync(d_self, self_host.data(), self_host.size() * 4, cudaMemcpyHostToDevice, c->stream));
+  }
+  const bool pair_rule = rule == NC_PAIRWISE_BERNOULLI || rule == NC_ONE_TO_ONE || rule == NC_ALL_TO_ALL;
+  if (rule == NC_PAIRWISE_BERNOULLI || (no_aut && pair_rule)) {
+    // reading A2: under NC_NO_AUTAPSES one_to_one and all_to_all also go through the pair mask (count, reserve, ordered write)
+    int rc = connect_bernoulli(c, gp, params->p, seed_lo, seed_hi, rule == NC_PAIRWISE_BERNOULLI, rule == NC_ONE_TO_ONE, no_aut,
+                               d_self);
     if (rc != NC_OK) return rc;
+    if (need_self) {
+      rc = sync_stream(c);  // self_host is read by the upload
+      if (rc != NC_OK) return rc;
+    }
+  } else if (rflags && !pair_rule && n_new > 0) {
+    // readings A3-A5: the random-partner rules under the flags
+    int rc = reserve_blocks(c, n_new);
+    if (rc != NC_OK) return rc;
+    gp.map = make_map(c);
+    gen_span_end(c);
+    {
+      Scope sc(c, NC_PHASE_GENERATE);
+      FlagGenParams fp{};
+      fp.g = gp;
+      fp.rule = rule == NC_FIXED_INDEGREE ? (uint32_t)kFixedIndegree
+                                          : rule == NC_FIXED_OUTDEGREE ? (uint32_t)kFixedOutdegree : (uint32_t)kFixedTotalNumber;
+      fp.flags = rflags;
+      fp.seed_lo = seed_lo;
+      fp.seed_hi = seed_hi;
+      fp.proj = c->n_proj;
+      fp.self_idx = d_self;
+      const unsigned grid = (unsigned)std::min<uint64_t>((n_new + 255) / 256, 148 * 32);
+      generate_flagged_kernel<<<grid, 256, 0, c->stream>>>(fp);
+      NC_LAUNCH_CHECK(c, "generate_flagged");
+    }
+    if (with_values) {
+      float* d_w = weights ? (float*)dev_alloc(c, (size_t)n_new * 4) : nullptr;
+      double* d_d = delays_ms ? (double*)dev_alloc(c, (size_t)n_new * 8) : nullptr;
+      dev_free_later(c, d_w);
+      dev_free_later(c, d_d);
+      if ((weights && !d_w) || (delays_ms && !d_d)) return fail(c, NC_ERR_OOM, "out of device memory for the value arrays");
+      if (d_w) NC_CUDA(c, cudaMemcpyAsync(d_w, weights, (size_t)n_new * 4, cudaMemcpyHostToDevice, c->stream));
+      if (d_d) NC_CUDA(c, cudaMemcpyAsync(d_d, delays_ms, (size_t)n_new * 8, cudaMemcpyHostToDevice, c->stream));
+      const unsigned vgrid = (unsigned)std::min<uint64_t>((n_new + 255) / 256, 148 * 16);
+      set_values_kernel<<<vgrid, 256, 0, c->stream>>>(gp.map, gp.pos0, n_new, d_w, d_d, c->inv_dt);
+      NC_LAUNCH_CHECK(c, "set_values");
+    }
+    c->n_conns += n_new;
+    if (need_self) {
+      rc = sync_stream(c);
+      if (rc != NC_OK) return rc;
+    }
   } else if (n_new > 0) {
     int rc = reserve_blocks(c, n_new);
     if (rc != NC_OK) return rc;
@@ -1759,6 +1904,14 @@ static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, 
   c->proj_attr.push_back((uint16_t)(c->cur_port | (c->cur_group << 8)));
   if (bound > (double)c->max_delay_steps) c->max_delay_steps = (uint32_t)bound;
   c->have_in = c->have_out = false;
+  return NC_OK;
+}
+
+int nc_set_rule_flags(nc_context* c, uint32_t flags) {
+  if (!c) return NC_ERR_INVALID_ARG;
+  if (flags & ~(uint32_t)(NC_NO_AUTAPSES | NC_NO_MULTAPSES)) return fail(c, NC_ERR_INVALID_ARG, "nc_set_rule_flags: unknown flag");
+  if (c->finalized) return fail(c, NC_ERR_STATE, "nc_set_rule_flags after nc_finalize");
+  c->rule_flags = flags;
   return NC_OK;
 }
 

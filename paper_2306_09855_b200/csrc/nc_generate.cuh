@@ -357,6 +357,7 @@ __global__ void __launch_bounds__(kBernThreads) bernoulli_trials_kernel(const __
 struct BernWriteParams {
   GenParams g;                 // pos0 = N_conns before the call, n = accepted total
   uint64_t n_pairs;
+  uint32_t one_to_one;         // pair q is (q, q) (one_to_one through the pair-mask path, nc_flags.cuh) instead of source-major
   const uint32_t* mask;
   const uint32_t* tile_offset; // exclusive scan of tile_count
 };
@@ -423,6 +424,10 @@ __global__ void __launch_bounds__(kBernThreads) bernoulli_write_kernel(const __g
     draw_weight_delay(rnd.z, rnd.w, p.g.syn, wgt, dly);
     const BlockAddr a = locate(p.g.map, out0 + k);
     uint32_t s = p.g.s0 + (uint32_t)row0 + dq, t = p.g.t0 + col;
+    if (p.one_to_one) {
+      s = p.g.s0 + (uint32_t)q;
+      t = p.g.t0 + (uint32_t)q;
+    }
     map_nodes(p.g, s, t);
     *src_ptr(p.g.map, a) = s;
     *tgt_ptr(p.g.map, a) = t;
