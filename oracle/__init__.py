@@ -262,6 +262,13 @@ class Oracle:
         if rc != 0:
             raise OracleError(rc)
 
+    def set_shard(self, first: int, count: int):
+        L = lib()
+        L.oc_set_shard.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32]
+        rc = L.oc_set_shard(self._h, int(first), int(count))
+        if rc != 0:
+            raise OracleError(rc)
+
     def set_rule_flags(self, flags: int):
         L = lib()
         L.oc_set_rule_flags.argtypes = [C.c_void_p, C.c_uint32]

@@ -227,6 +227,8 @@ struct oc_context {
   std::vector<uint8_t> port, group; /* receptor port index and synaptic group index of every connection */
   uint8_t cur_port = 0, cur_group = 0;
   uint32_t rule_flags = 0; /* OC_NO_AUTAPSES | OC_NO_MULTAPSES for the connect calls that follow (readings A1-A6) */
+  bool sharded = false;    /* reading S1: keep only the connections whose target id lies in [shard_first, shard_first + shard_count) */
+  uint32_t shard_first = 0, shard_count = 0;
   uint64_t n_blocks = 0;
   /* D10: sorted copies. */
   std::vector<uint32_t> perm, ssrc, stgt;
@@ -491,8 +493,8 @@ int oc_set_rule_flags(oc_context* ctx, uint32_t flags) {
 }
 uint32_t oc_keyed_permutation(uint32_t M, uint32_t k, const uint32_t keys[4]) { return keyed_permutation(M, k, keys); }
 
-int oc_connect(oc_context* ctx, oc_range src, oc_range tgt, int rule, const oc_rule_params* params,
-               const oc_syn_spec* syn, uint64_t seed) {
+static int connect_impl(oc_context* ctx, oc_range src, oc_range tgt, int rule, const oc_rule_params* params,
+                        const oc_syn_spec* syn, uint64_t seed) {
   if (!ctx) return OC_ERR_INVALID_ARG;
   if (ctx->rule_flags) return connect_flagged(ctx, nullptr, src, nullptr, tgt, rule, params, syn, seed, ctx->rule_flags);
   return connect_core(ctx, ctx->n_nodes, src, tgt, rule, params, syn, seed);
@@ -501,9 +503,9 @@ int oc_connect(oc_context* ctx, oc_range src, oc_range tgt, int rule, const oc_r
 /* "If the indexes of source or target nodes are not consecutive but are explicitly given by an array,
  * the above formulas are used to derive the indexes of the array elements from which to extract the node indexes."
  * So: run the rule over the index ranges 0..n_src-1 / 0..n_tgt-1 (s0 = t0 = 0), then look every result up. */
-int oc_connect_nodes(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, oc_range src,
-                     const uint32_t* tgt_nodes, uint32_t n_tgt, oc_range tgt, int rule, const oc_rule_params* params,
-                     const oc_syn_spec* syn, uint64_t seed) {
+static int connect_nodes_impl(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, oc_range src,
+                              const uint32_t* tgt_nodes, uint32_t n_tgt, oc_range tgt, int rule, const oc_rule_params* params,
+                              const oc_syn_spec* syn, uint64_t seed) {
   if (!ctx) return OC_ERR_INVALID_ARG;
   if (ctx->finalized) return OC_ERR_STATE;
   for (uint32_t k = 0; src_nodes && k < n_src; ++k)
@@ -532,10 +534,10 @@ int oc_connect_nodes(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src,
  * form: entry i belongs to connection i_newconns = i (Eq. 2); a NULL array leaves that parameter to `syn`.  The
  * rule, its random draws and the other parameter are exactly those of oc_connect_nodes.  A given weight is stored
  * as it is; a given delay in ms goes through reading D8 (times 1/dt, round half up, at least one step). */
-int oc_connect_values(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, oc_range src,
-                      const uint32_t* tgt_nodes, uint32_t n_tgt, oc_range tgt, int rule, const oc_rule_params* params,
-                      const oc_syn_spec* syn, uint64_t seed, const float* weights, const double* delays_ms,
-                      uint64_t n_values) {
+static int connect_values_impl(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, oc_range src,
+                               const uint32_t* tgt_nodes, uint32_t n_tgt, oc_range tgt, int rule, const oc_rule_params* params,
+                               const oc_syn_spec* syn, uint64_t seed, const float* weights, const double* delays_ms,
+                               uint64_t n_values) {
   if (!ctx) return OC_ERR_INVALID_ARG;
   if (ctx->finalized) return OC_ERR_STATE;
   if (!weights && !delays_ms) return OC_ERR_INVALID_ARG;
@@ -550,7 +552,7 @@ int oc_connect_values(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src
   }
   const size_t before = ctx->src.size();
   const uint64_t blocks_before = ctx->n_blocks;
-  int rc = oc_connect_nodes(ctx, src_nodes, n_src, src, tgt_nodes, n_tgt, tgt, rule, params, syn, seed);
+  int rc = connect_nodes_impl(ctx, src_nodes, n_src, src, tgt_nodes, n_tgt, tgt, rule, params, syn, seed);
   if (rc != OC_OK) return rc;
   if (ctx->src.size() - before != n_values) { /* "an array having a size equal to the number of connections" */
     ctx->src.resize(before); ctx->tgt.resize(before); ctx->w.resize(before); ctx->d.resize(before); ctx->bnd.resize(before);
@@ -571,6 +573,66 @@ int oc_connect_values(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src
     }
   }
   return OC_OK;
+}
+
+
+/* Reading S1 ("future work is required to extend the algorithm to employing multiple GPUs"):
+ * a context that holds ONE SHARD of a network keeps, of every connect call, exactly the connections whose target id lies
+ * in [first, first + count) -- the nodes this shard owns -- in the order the full call creates them, with the full call's
+ * random numbers (Philox indices are those of the full call) and projection ids.  Everything after that (Eq. 1 blocks,
+ * sort, index) runs on what was kept.  Here: generate the full call, then erase what is not owned. */
+static void apply_shard(oc_context* ctx, size_t before) {
+  if (!ctx->sharded) return;
+  size_t o = before;
+  for (size_t j = before; j < ctx->src.size(); ++j) {
+    const uint32_t t = ctx->tgt[j];
+    if (t >= ctx->shard_first && (uint64_t)t < (uint64_t)ctx->shard_first + ctx->shard_count) {
+      ctx->src[o] = ctx->src[j]; ctx->tgt[o] = ctx->tgt[j]; ctx->w[o] = ctx->w[j]; ctx->d[o] = ctx->d[j];
+      ctx->bnd[o] = ctx->bnd[j]; ctx->port[o] = ctx->port[j]; ctx->group[o] = ctx->group[j];
+      ++o;
+    }
+  }
+  ctx->src.resize(o); ctx->tgt.resize(o); ctx->w.resize(o); ctx->d.resize(o); ctx->bnd.resize(o);
+  ctx->port.resize(o); ctx->group.resize(o);
+  ctx->n_blocks = (o + ctx->B - 1) / ctx->B; /* Eq. 1 over what this shard holds */
+}
+
+int oc_set_shard(oc_context* ctx, uint32_t first, uint32_t count) {
+  if (!ctx) return OC_ERR_INVALID_ARG;
+  if (ctx->finalized || !ctx->src.empty() || ctx->n_projections) return OC_ERR_STATE; /* before the first connect call */
+  ctx->sharded = true;
+  ctx->shard_first = first;
+  ctx->shard_count = count;
+  return OC_OK;
+}
+
+int oc_connect(oc_context* ctx, oc_range src, oc_range tgt, int rule, const oc_rule_params* params,
+               const oc_syn_spec* syn, uint64_t seed) {
+  if (!ctx) return OC_ERR_INVALID_ARG;
+  const size_t before = ctx->src.size();
+  const int rc = connect_impl(ctx, src, tgt, rule, params, syn, seed);
+  if (rc == OC_OK) apply_shard(ctx, before);
+  return rc;
+}
+int oc_connect_nodes(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, oc_range src,
+                     const uint32_t* tgt_nodes, uint32_t n_tgt, oc_range tgt, int rule, const oc_rule_params* params,
+                     const oc_syn_spec* syn, uint64_t seed) {
+  if (!ctx) return OC_ERR_INVALID_ARG;
+  const size_t before = ctx->src.size();
+  const int rc = connect_nodes_impl(ctx, src_nodes, n_src, src, tgt_nodes, n_tgt, tgt, rule, params, syn, seed);
+  if (rc == OC_OK) apply_shard(ctx, before);
+  return rc;
+}
+int oc_connect_values(oc_context* ctx, const uint32_t* src_nodes, uint32_t n_src, oc_range src,
+                      const uint32_t* tgt_nodes, uint32_t n_tgt, oc_range tgt, int rule, const oc_rule_params* params,
+                      const oc_syn_spec* syn, uint64_t seed, const float* weights, const double* delays_ms,
+                      uint64_t n_values) {
+  if (!ctx) return OC_ERR_INVALID_ARG;
+  const size_t before = ctx->src.size();
+  const int rc = connect_values_impl(ctx, src_nodes, n_src, src, tgt_nodes, n_tgt, tgt, rule, params, syn, seed, weights,
+                                     delays_ms, n_values);
+  if (rc == OC_OK) apply_shard(ctx, before);
+  return rc;
 }
 
 /* "The basic structure of a NEST GPU connection includes the source node index, the target node index, the

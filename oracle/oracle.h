@@ -134,6 +134,10 @@ int oc_read_connection_attributes(oc_context* ctx, int sorted, uint64_t first, u
  *  A6 fixed_total_number under OC_NO_MULTAPSES is not offered (OC_ERR_INVALID_ARG).
  * Weight and delay of connection i always come from words 2 and 3 of Philox(idx = i, stream 0) (D5-D8). */
 enum { OC_NO_AUTAPSES = 1, OC_NO_MULTAPSES = 2 };
+/* Reading S1: this context holds ONE SHARD of the network: of every connect call it keeps
+ * exactly the connections whose target id lies in [first, first + count), in the order the full call creates them and with
+ * the full call's random numbers and projection ids.  To be called before the first connect call. */
+int oc_set_shard(oc_context* ctx, uint32_t first, uint32_t count);
 int oc_set_rule_flags(oc_context* ctx, uint32_t flags);
 /* perm_M(k; keys), k < M: a permutation of [0, M) by cycle walking over a balanced Feistel network on 2h bits,
  * h = max(1, ceil(bits(M - 1) / 2)): x = k; repeat { (L, R) = (x >> h, x & (2^h - 1)); 6 + ceil(24 / h) rounds
