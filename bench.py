@@ -32,14 +32,19 @@ BYTES = {"generate": 14, "histogram": 8, "sort_pass": 32, "permute": 26, "index"
 
 
 def ncu_traffic_per_launch():
-    """dram__bytes_read.sum + dram__bytes_write.sum of one scatter pass, from the committed ncu --set full capture."""
+    """(dram__bytes_read.sum + dram__bytes_write.sum of one middle scatter pass, where it was captured) from the committed
+    ncu --set full capture.  The figure is a property of the kernel source at that commit, so the file names the commit and
+    the bench line repeats it: a reader can see at once whether the kernel has changed since."""
+    out, where = None, None
     try:
-        for line in open(os.path.join(ROOT, "profiles", "r01_scatter_traffic.txt")):
+        for line in open(os.path.join(ROOT, "profiles", "r02_scatter_traffic.txt")):
             if line.startswith("traffic_bytes_per_launch"):
-                return float(line.split("=")[1])
+                out = float(line.split("=")[1])
+            if line.startswith("captured_at"):
+                where = line.split("=", 1)[1].strip()
     except Exception:
         pass
-    return None
+    return out, where
 
 
 def workload(name: str):
@@ -101,27 +106,62 @@ class ClockSampler(threading.Thread):
 BLOCK_SIZE = 0  # --block-size: connections per storage block (0 = the library's default 2^24)
 
 
+SHARD = None  # --sharded: (world, rank)
+
+
 def one_step(binding, WL, net, flags):
     """The public API call sequence a user makes.  Returns the (still open) context."""
     g = binding.NC(dt_ms=net.dt_ms, flags=flags, block_size=BLOCK_SIZE)
-    WL.run(net, g)
+    if SHARD is not None:
+        from paper_2306_09855_b200 import sharding
+        sharding.build_shard(net, g, *SHARD)
+    else:
+        WL.run(net, g)
     return g
 
 
+def cpu_model():
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+PHASE_SPLIT = {}  # filled by cpu_oracle_sample: seconds of the last step's generate / sort + index
+
+
 def cpu_oracle_sample(sample_scale: float, steps: int = 1):
-    """The oracle as it stands, one thread, on a bounded sample of the same workload."""
+    """The oracle as it stands, one thread pinned to one core, on a bounded sample of the same workload.
+    generate = the connect calls, organise = oc_finalize (stable sort + index)."""
     import oracle
     from paper_2306_09855_b200 import workloads as WL
     net = WL.config2_microcircuit(scale=sample_scale)
     oracle.build()
+    old_aff = None
+    try:
+        old_aff = os.sched_getaffinity(0)
+        os.sched_setaffinity(0, {sorted(old_aff)[-1]})
+    except Exception:
+        old_aff = None
     times, n = [], 0
-    for _ in range(steps):
-        t0 = time.perf_counter()
-        o = oracle.Oracle(dt_ms=net.dt_ms)
-        WL.run(net, o)
-        n = o.num_connections()
-        times.append(time.perf_counter() - t0)
-        o.close()
+    try:
+        for _ in range(steps):
+            t0 = time.perf_counter()
+            o = oracle.Oracle(dt_ms=net.dt_ms)
+            WL.run(net, o, finalize=False)
+            t1 = time.perf_counter()
+            o.finalize()
+            t2 = time.perf_counter()
+            n = o.num_connections()
+            times.append(t2 - t0)
+            PHASE_SPLIT.update(generate_s=t1 - t0, sort_index_s=t2 - t1)
+            o.close()
+    finally:
+        if old_aff is not None:
+            os.sched_setaffinity(0, old_aff)
     return net, n, times
 
 
@@ -141,7 +181,9 @@ def run_reference(args):
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "configs[2] cortical-microcircuit-shaped, fixed_total_number, seed 7 (bounded sample)",
                    "sample": sample},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                         "phases_s": {k: round(v, 2) for k, v in PHASE_SPLIT.items()},
+                         "pinned": "one thread on one core (sched_setaffinity)", "cpu_model": cpu_model(), "host_cpus": os.cpu_count()},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -217,6 +259,8 @@ def main():
     ap.add_argument("--flags", type=int, default=0, help="extra NC_FLAG_* bits (e.g. 4 = sort (key, position) pairs + gather; "
                     "16 = COPASS organisation inside the storage blocks, 48 = the same with the shift of Fig. 6E)")
     ap.add_argument("--block-size", type=int, default=0, help="connections per storage block B (0 = 2^24)")
+    ap.add_argument("--sharded", action="store_true", help="strong scaling: the ranks build the shards of ONE network "
+                    "(nc_set_shard: rank r keeps the connections whose target it owns) instead of one replica each")
     args = ap.parse_args()
     global BLOCK_SIZE
     BLOCK_SIZE = args.block_size
@@ -240,6 +284,9 @@ def main():
     net = workload(args.workload)
     stream = torch.cuda.current_stream()
     flags = binding.FLAG_TIMING | args.flags
+    if args.sharded:
+        global SHARD
+        SHARD = (world, rank)
 
     # ---- warm-up (also warms torch's caching allocator: the timed steps allocate from its cache) ----
     n_syn = 0
@@ -284,6 +331,10 @@ def main():
     total_ms = replicas.max_over_ranks(dist, total_ms, "cuda")
     ms_per_step = total_ms / args.steps
     value = replicas.whole_job_rate(n_syn, args.steps, world, total_ms)
+    if args.sharded:  # the ranks hold one network between them: its size is the sum of the shards
+        from paper_2306_09855_b200 import sharding
+        n_total = sum(sharding.shard_sizes(dist, n_syn, "cuda"))
+        value = n_total * args.steps / (total_ms * 1e-3)
 
     # ---- end to end through the public API with host buffers: context creation, host descriptors in,
     #      index arrays read back into host memory, wall clock ----
@@ -335,7 +386,8 @@ def main():
         roof = {"bound": "hbm", "kernel": "scatter_pass_kernel (one digit pass carrying the whole connection: 16 B read + "
                                           "16 B written per synapse)",
                 "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": ncu_traffic_per_launch() if args.workload == "c2" and not args.flags else None,
+                "traffic": ncu_traffic_per_launch()[0] if args.workload == "c2" and not args.flags else None,
+                "traffic_captured_at": ncu_traffic_per_launch()[1] if args.workload == "c2" and not args.flags else None,
                 "peak_kind": peak_kind,
                 "launch_ms": pass_ms, "launches_per_step": passes}
     phases = {}
@@ -366,17 +418,21 @@ def main():
         snet, sn, st = cpu_oracle_sample(scale)
         cpu = {"value": sn / st[0], "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"configs[2] with populations scaled x{scale:g}: {snet.n_nodes} nodes, {sn} synapses, generate+sort+index, {st[0]:.1f} s",
-               "host_cpus": os.cpu_count()}
+               "phases_s": {k: round(v, 2) for k, v in PHASE_SPLIT.items()},
+               "pinned": "one thread on one core (sched_setaffinity)", "cpu_model": cpu_model(), "host_cpus": os.cpu_count()}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "ms_per_step_sd": statistics.pstdev(step_ms) if len(step_ms) > 1 else 0.0,
-        "cold_first_step_ms": cold_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u32+f32",
+        "cold_first_step_ms": cold_ms, "higher_is_better": True, "scaling": "strong" if args.sharded else "weak",
+        "vs_baseline": None, "dtype": "u32+f32",
         "data": "synthetic",
         "config": {"workload": f"{net.name}: BASELINE.json configs[2] cortical-microcircuit-shaped network, "
                                f"{net.n_nodes} nodes, {len(net.projections)} fixed_total_number projections, seed 7"
                    if args.workload == "c2" else net.name,
-                   "synapses_per_step": n_syn, "parallelism": "replicas only (one independent network per GPU)",
+                   "synapses_per_step": n_syn,
+                   "parallelism": (f"one network in {world} shards by target node (nc_set_shard), no data-path collective"
+                                   if args.sharded else "replicas only (one independent network per GPU)"),
                    "l2": "every step regenerates and re-sorts its own 4.2 GB of connections (>> 126 MB L2); no input is reused",
                    "key_bits": stats.get("key_bits"), "sort_passes": stats.get("sort_passes"), "flags": flags,
                    "block_size": args.block_size or (1 << 24), "device_bytes_peak": stats.get("bytes_peak")},

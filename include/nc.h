@@ -243,6 +243,18 @@ int nc_connect(nc_context* ctx, nc_range src, nc_range tgt, nc_rule rule, const 
 enum { NC_NO_AUTAPSES = 1u, NC_NO_MULTAPSES = 2u };
 int nc_set_rule_flags(nc_context* ctx, uint32_t flags);
 
+/* One shard of a network per context ("future work is required to extend the algorithm to employing multiple
+ * GPUs"; reading S1): after nc_set_shard(first, count) every nc_connect* call keeps exactly the connections whose TARGET id
+ * lies in first .. first + count - 1 -- the nodes this shard owns -- in the order the full call creates them, with the full
+ * call's random numbers (Philox indices are those of the full call) and projection ids; Eq. 1, the sort and the index then
+ * run over what was kept, so perm refers to the shard's own creation positions.  One process per GPU builds one shard;
+ * the shards of a partition of the nodes together hold every connection of the unsharded network exactly once, each in the
+ * unsharded order (creation order and organised order), without any exchange between ranks: a rank draws the random
+ * numbers of the connections it does not own as well and skips them (owner-computes with redundant generation).  A call
+ * is staged in full on the device first (14 B per connection of the FULL call, released afterwards) and waits for the
+ * owned count.  To be called before the first nc_connect*; node ids outside the created nodes own nothing. ---- */
+int nc_set_shard(nc_context* ctx, uint32_t first, uint32_t count);
+
 /* The same with explicit node arrays ("If the indexes of source or target nodes are not consecutive but
  * are explicitly given by an array, the above formulas are used to derive the indexes of the array elements from
  * which to extract the node indexes").  src_nodes / tgt_nodes are HOST arrays of n_src / n_tgt node ids (copied

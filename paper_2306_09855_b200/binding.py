@@ -31,7 +31,7 @@ SYMBOLS = (
     "nc_degree_histogram", "nc_get_stats", "nc_get_timings", "nc_read_connections", "nc_read_index",
     "nc_read_degree_histogram", "nc_selftest_philox", "nc_selftest_fastpath", "nc_selftest_guard",
     "nc_connect_nodes", "nc_connect_values", "nc_set_connection_attributes", "nc_read_connection_attributes",
-    "nc_set_rule_flags",
+    "nc_set_rule_flags", "nc_set_shard",
     # include/nc_delivery.h
     "nc_delivery_create", "nc_delivery_destroy", "nc_delivery_step", "nc_delivery_read_spike_array",
     "nc_delivery_counts", "nc_delivery_num_ports", "nc_delivery_run",
@@ -304,6 +304,10 @@ class NC:
 
     def connect(self, *a, **k):
         self._check(self.connect_rc(*a, **k))
+
+    def set_shard(self, first: int, count: int):
+        self._L.nc_set_shard.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32]
+        self._check(self._L.nc_set_shard(self._h, int(first), int(count)))
 
     def set_rule_flags(self, flags: int):
         self._L.nc_set_rule_flags.argtypes = [C.c_void_p, C.c_uint32]

@@ -17,6 +17,7 @@
 #include "nc_internal.h"
 #include "nc_generate.cuh"
 #include "nc_flags.cuh"
+#include "nc_shard.cuh"
 #include "nc_index.cuh"
 #include "nc_sort.cuh"
 #include "nc_sort_split.cuh"
@@ -76,6 +77,13 @@ struct nc_context {
   uint64_t copass_aux_bytes = 0, copass_moved = 0;
   uint8_t cur_port = 0, cur_group = 0;       // attributes in force for the next nc_connect*
   uint32_t rule_flags = 0;                   // NC_NO_AUTAPSES | NC_NO_MULTAPSES for the next nc_connect*
+  bool sharded = false;                      // nc_set_shard: keep only connections whose target id is in the owned range
+  uint32_t shard_first = 0, shard_count = 0;
+  std::vector<void*> stage_blocks;           // sharded contexts: staging blocks, kept from call to call (released by nc_finalize)
+  uint64_t* stage_table = nullptr;
+  size_t stage_cap = 0;
+  uint64_t stage_n = 0;                      // connections staged and not yet filtered (flush_shard)
+  std::vector<std::pair<uint32_t, uint64_t>> stage_pending;  // (projection, its first staged position) of the staged calls
   std::vector<uint32_t> proj_first;          // creation position of the first connection of every projection
   std::vector<uint16_t> proj_attr;           // port | syn_group << 8 of every projection
   uint8_t* d_sorted_port = nullptr;          // port of every organised connection, built on first use by delivery
@@ -1647,7 +1655,7 @@ int nc_create_population(nc_context* c, uint32_t n, uint32_t* first_id) {
 }
 
 // src_nodes / tgt_nodes: HOST arrays of src.count / tgt.count node ids, or NULL for the consecutive range
-static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, const uint32_t* tgt_nodes, nc_range tgt,
+static int connect_core(nc_context* c, const uint32_t* src_nodes, nc_range src, const uint32_t* tgt_nodes, nc_range tgt,
                         nc_rule rule, const nc_rule_params* params, const nc_syn_spec* syn, uint64_t seed,
                         const float* weights = nullptr, const double* delays_ms = nullptr, uint64_t n_values = 0,
                         bool with_values = false) {
@@ -1907,6 +1915,130 @@ static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, 
   return NC_OK;
 }
 
+// Reading S1 (nc_set_shard): connect calls run in full into staging blocks; flush_shard then keeps what this shard owns
+// (nc_shard.cuh).  Calls are batched -- the filter runs when kShardFlush connections are staged, at nc_finalize and before
+// anything reads the storage -- so a network of many small projections costs one wait per batch, not one per call.
+constexpr uint64_t kShardFlush = 1ull << 28;  // 3.8 GB of staged connections
+
+static int flush_shard(nc_context* c) {
+  if (!c->sharded || c->stage_n == 0) {
+    c->stage_pending.clear();
+    return NC_OK;
+  }
+  const uint64_t n_full = c->stage_n;
+  const uint64_t tiles = (n_full + kOwnTile - 1) / kOwnTile;
+  const uint64_t chunks = (tiles + kScanChunk - 1) / kScanChunk;
+  const size_t n_q = c->stage_pending.size();
+  uint32_t* tile_count = (uint32_t*)dev_alloc(c, tiles * 4);
+  uint32_t* tile_off = (uint32_t*)dev_alloc(c, tiles * 4);
+  uint32_t* partial = (uint32_t*)dev_alloc(c, chunks * 4);
+  uint64_t* d_total = (uint64_t*)dev_alloc(c, 8);
+  uint64_t* d_query = (uint64_t*)dev_alloc(c, (n_q + 1) * 16);  // [n_q] staged start positions | [n_q] owned connections before each
+  auto drop = [&]() {
+    dev_free_later(c, tile_count); dev_free_later(c, tile_off); dev_free_later(c, partial); dev_free_later(c, d_total);
+    dev_free_later(c, d_query);
+  };
+  if (!tile_count || !tile_off || !partial || !d_total || !d_query) {
+    drop();
+    return fail(c, NC_ERR_OOM, "out of device memory for the shard filter");
+  }
+  ShardFilterParams fp{};
+  fp.stage = make_map(c);
+  fp.stage.table = c->stage_table;
+  fp.n = n_full;
+  fp.first = c->shard_first;
+  fp.count = c->shard_count;
+  fp.tile_count = tile_count;
+  fp.tile_offset = tile_off;
+  uint64_t total = 0;
+  std::vector<uint64_t> starts(n_q), before(n_q);
+  for (size_t k = 0; k < n_q; ++k) starts[k] = c->stage_pending[k].second;
+  gen_span_end(c);
+  {
+    Scope sc(c, NC_PHASE_GENERATE);
+    owned_count_kernel<<<(unsigned)tiles, kOwnThreads, 0, c->stream>>>(fp);
+    NC_LAUNCH_CHECK(c, "owned_count");
+    int rc = device_scan(c, tile_count, tile_off, tiles, partial, d_total);
+    if (rc != NC_OK) {
+      drop();
+      return rc;
+    }
+    if (n_q) {
+      NC_CUDA(c, cudaMemcpyAsync(d_query, starts.data(), n_q * 8, cudaMemcpyHostToDevice, c->stream));
+      owned_before_kernel<<<(unsigned)((n_q + 7) / 8), 256, 0, c->stream>>>(fp, d_query, (uint32_t)n_q, d_query + n_q);
+      NC_LAUNCH_CHECK(c, "owned_before");
+      NC_CUDA(c, cudaMemcpyAsync(before.data(), d_query + n_q, n_q * 8, cudaMemcpyDeviceToHost, c->stream));
+    }
+    NC_CUDA(c, cudaMemcpyAsync(&total, d_total, 8, cudaMemcpyDeviceToHost, c->stream));
+  }
+  NC_CUDA(c, cudaStreamSynchronize(c->stream));  // the exact count decides the allocation
+  if (c->n_conns + total > kMaxConns) {
+    drop();
+    return fail(c, NC_ERR_CAPACITY, "more than 2^32-1 connections in this shard");
+  }
+  int rc = reserve_blocks(c, total);
+  if (rc != NC_OK) {
+    drop();
+    return rc;
+  }
+  if (total > 0) {
+    Scope sc(c, NC_PHASE_GENERATE);
+    fp.store = make_map(c);
+    fp.pos0 = c->n_conns;
+    owned_copy_kernel<<<(unsigned)tiles, kOwnThreads, 0, c->stream>>>(fp);
+    NC_LAUNCH_CHECK(c, "owned_copy");
+  }
+  for (size_t k = 0; k < n_q; ++k)  // a projection starts where the first connection kept from it (or after it) went
+    c->proj_first[c->stage_pending[k].first] = (uint32_t)(c->n_conns + before[k]);
+  c->n_conns += total;
+  c->stage_n = 0;
+  c->stage_pending.clear();
+  drop();
+  return NC_OK;
+}
+
+static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, const uint32_t* tgt_nodes, nc_range tgt,
+                        nc_rule rule, const nc_rule_params* params, const nc_syn_spec* syn, uint64_t seed,
+                        const float* weights = nullptr, const double* delays_ms = nullptr, uint64_t n_values = 0,
+                        bool with_values = false) {
+  if (!c || !c->sharded || c->broken || c->finalized)  // not sharded, or let the ordinary path report the state
+    return connect_core(c, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed, weights, delays_ms, n_values, with_values);
+  // swap in the staging storage: the generators append the full projection behind what is already staged
+  std::vector<void*> real_blocks;
+  real_blocks.swap(c->blocks);
+  c->blocks.swap(c->stage_blocks);
+  uint64_t* real_table = c->d_table;
+  const size_t real_cap = c->table_cap;
+  const uint64_t real_n = c->n_conns;
+  c->d_table = c->stage_table;
+  c->table_cap = c->stage_cap;
+  c->n_conns = c->stage_n;
+  const uint32_t proj_before = c->n_proj;
+  const uint64_t stage_start = c->stage_n;
+  const int rc = connect_core(c, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed, weights, delays_ms, n_values, with_values);
+  c->stage_blocks.swap(c->blocks);
+  c->stage_table = c->d_table;
+  c->stage_cap = c->table_cap;
+  c->stage_n = c->n_conns;
+  c->blocks.swap(real_blocks);
+  c->d_table = real_table;
+  c->table_cap = real_cap;
+  c->n_conns = real_n;
+  if (rc != NC_OK) return rc;
+  if (c->n_proj > proj_before) c->stage_pending.push_back({proj_before, stage_start});
+  return c->stage_n >= kShardFlush ? flush_shard(c) : NC_OK;
+}
+
+int nc_set_shard(nc_context* c, uint32_t first, uint32_t count) {
+  if (!c) return NC_ERR_INVALID_ARG;
+  if (c->finalized || c->n_conns || c->n_proj) return fail(c, NC_ERR_STATE, "nc_set_shard: only before the first nc_connect*");
+  if (c->cfg.flags & NC_FLAG_ORGANISE_COPASS) {}  // any organisation works: the filter runs before it
+  c->sharded = true;
+  c->shard_first = first;
+  c->shard_count = count;
+  return NC_OK;
+}
+
 int nc_set_rule_flags(nc_context* c, uint32_t flags) {
   if (!c) return NC_ERR_INVALID_ARG;
   if (flags & ~(uint32_t)(NC_NO_AUTAPSES | NC_NO_MULTAPSES)) return fail(c, NC_ERR_INVALID_ARG, "nc_set_rule_flags: unknown flag");
@@ -1953,6 +2085,15 @@ int nc_finalize(nc_context* c) {
   if (c->broken) return fail(c, NC_ERR_STATE, "nc_finalize: a failed in-place organisation left this context without connections; destroy it");
   if (c->finalized) return fail(c, NC_ERR_STATE, "nc_finalize called twice");
   gen_span_end(c);
+  {
+    const int frc = flush_shard(c);
+    if (frc != NC_OK) return frc;
+  }
+  for (void* b : c->stage_blocks) dev_free_later(c, b);  // a sharded context's staging is not needed any more
+  c->stage_blocks.clear();
+  dev_free_later(c, c->stage_table);
+  c->stage_table = nullptr;
+  c->stage_cap = 0;
   const uint32_t N = c->n_nodes;
   c->src_offsets = (uint32_t*)dev_alloc(c, ((size_t)N + 1) * 4);
   c->group_ptr = (uint32_t*)dev_alloc(c, ((size_t)N + 1) * 4);
@@ -2003,6 +2144,10 @@ int nc_finalize(nc_context* c) {
 }
 
 int nc_num_connections(nc_context* c, uint64_t* n) {
+  if (c && c->sharded && c->stage_n) {  // staged connect calls of a sharded context: filter them first
+    const int frc = flush_shard(c);
+    if (frc != NC_OK) return frc;
+  }
   if (!c || !n) return NC_ERR_INVALID_ARG;
   *n = c->n_conns;  // pairwise_bernoulli already waited for its count inside nc_connect
   return NC_OK;
@@ -2015,6 +2160,10 @@ int nc_num_nodes(nc_context* c, uint32_t* n) {
 }
 
 int nc_get_connections(nc_context* c, int sorted, nc_connections_view* out) {
+  if (c && c->sharded && c->stage_n) {  // staged connect calls of a sharded context: filter them first
+    const int frc = flush_shard(c);
+    if (frc != NC_OK) return frc;
+  }
   if (!c || !out) return NC_ERR_INVALID_ARG;
   std::memset(out, 0, sizeof(*out));
   out->n = c->n_conns;
@@ -2067,6 +2216,10 @@ int nc_get_index(nc_context* c, nc_index_view* out) {
 }
 
 int nc_degree_histogram(nc_context* c, int kind, const uint32_t** per_node_degree, uint32_t* max_degree) {
+  if (c && c->sharded && c->stage_n) {  // staged connect calls of a sharded context: filter them first
+    const int frc = flush_shard(c);
+    if (frc != NC_OK) return frc;
+  }
   if (!c || (kind != 0 && kind != 1)) return fail(c, NC_ERR_INVALID_ARG, "nc_degree_histogram: bad argument");
   const uint32_t N = c->n_nodes;
   bool& have = kind == 0 ? c->have_in : c->have_out;
@@ -2098,6 +2251,10 @@ int nc_degree_histogram(nc_context* c, int kind, const uint32_t** per_node_degre
 }
 
 int nc_get_stats(nc_context* c, nc_stats* out) {
+  if (c && c->sharded && c->stage_n) {  // staged connect calls of a sharded context: filter them first
+    const int frc = flush_shard(c);
+    if (frc != NC_OK) return frc;
+  }
   if (!c || !out) return NC_ERR_INVALID_ARG;
   out->kernel_launches = c->launches;
   out->bytes_in_use = c->bytes_in_use;
@@ -2121,6 +2278,10 @@ int nc_get_timings(nc_context* c, nc_timings* out) {
 
 int nc_read_connections(nc_context* c, int sorted, uint64_t first, uint64_t count, uint32_t* source, uint32_t* target,
                         float* weight, uint16_t* delay, uint32_t* perm) {
+  if (c && c->sharded && c->stage_n) {
+    const int frc = flush_shard(c);
+    if (frc != NC_OK) return frc;
+  }
   if (!c) return NC_ERR_INVALID_ARG;
   if (first + count > c->n_conns) return fail(c, NC_ERR_INVALID_ARG, "nc_read_connections: range outside the connections");
   if (sorted && !c->finalized) return fail(c, NC_ERR_STATE, "sorted view before nc_finalize");
@@ -2163,6 +2324,10 @@ int nc_set_connection_attributes(nc_context* c, uint8_t port, uint8_t syn_group)
 
 int nc_read_connection_attributes(nc_context* c, int sorted, uint64_t first, uint64_t count, uint8_t* port,
                                   uint8_t* syn_group) {
+  if (c && c->sharded && c->stage_n) {
+    const int frc = flush_shard(c);
+    if (frc != NC_OK) return frc;
+  }
   if (!c) return NC_ERR_INVALID_ARG;
   if (c->broken) return fail(c, NC_ERR_STATE, "a failed in-place organisation left this context without connections");
   if (first + count > c->n_conns) return fail(c, NC_ERR_INVALID_ARG, "nc_read_connection_attributes: range outside the connections");

@@ -82,10 +82,13 @@ def delay(mean: float, sd: float, lo: float = 0.1) -> Dist:
     return (mean, sd, lo, INF)
 
 
-def run(net: Network, backend, finalize: bool = True):
+def run(net: Network, backend, finalize: bool = True, shard=None):
     """Replay the recipe: populations in listed order, projections in listed order (projection_id =
-    issue order)."""
+    issue order).  shard = (first node id, count): the backend keeps only the connections whose target
+    it owns (nc_set_shard)."""
     firsts = [backend.create_population(n) for n in net.populations]
+    if shard is not None:
+        backend.set_shard(*shard)
     for pr in net.projections:
         backend.connect(
             (firsts[pr.src_pop], net.populations[pr.src_pop]),

@@ -1,0 +1,99 @@
+"""GPU parity of sharded construction (nc_set_shard; reading S1) against the oracle's shard filter: every
+shard of a node partition is built in its own context (one after the other on this one GPU: the shards share nothing and
+wait on nothing) and compared element by element -- creation order, organised order, permutation, index, block count --
+under the default and the COPASS organisation; the shard sizes add up to the unsharded network."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2306_09855_b200 import workloads as WL
+from tests import parity_util as PU
+
+pytestmark = pytest.mark.gpu
+INF = math.inf
+
+
+@pytest.fixture(scope="module")
+def nc_mod():
+    from paper_2306_09855_b200 import binding, build
+    build.build()
+    return binding
+
+
+@pytest.mark.parametrize("world", [2, 5])
+def test_microcircuit_shards(nc_mod, oracle_mod, world):
+    net = WL.config2_microcircuit(scale=0.05)
+    full = oracle_mod.Oracle(dt_ms=net.dt_ms)
+    WL.run(net, full, finalize=False)
+    n_full = full.num_connections()
+    full.close()
+    bounds = [net.n_nodes * r // world for r in range(world + 1)]
+    total = 0
+    for r in range(world):
+        o = oracle_mod.Oracle(dt_ms=net.dt_ms, block_size=1 << 16)
+        g = nc_mod.NC(dt_ms=net.dt_ms, block_size=1 << 16)
+        shard = (bounds[r], bounds[r + 1] - bounds[r])
+        WL.run(net, o, finalize=False, shard=shard)
+        WL.run(net, g, finalize=False, shard=shard)
+        assert g.num_connections() == o.num_connections()
+        total += g.num_connections()
+        PU.compare_connections(g.read_connections(sorted=False), o.connections(sorted=False), PU.weight_scale(net, o), f"shard {r} creation order")
+        o.finalize()
+        g.finalize()
+        assert g.stats()["n_blocks"] == o.num_blocks()
+        PU.compare_sorted(g, o, net, f"shard {r}")
+        PU.compare_index(g.read_index(), o.index(), f"shard {r}")
+        g.close()
+        o.close()
+    assert total == n_full
+
+
+def test_every_rule_flags_arrays_values_in_a_shard(nc_mod, oracle_mod):
+    rng = np.random.default_rng(4)
+    N = 240
+    arr = rng.permutation(N)[:90].astype(np.uint32)
+    W, D = (20.0, 2.0, 0.0, INF), (1.5, 0.75, 0.1, INF)
+    R = WL.RULE_IDS
+    calls = [(0, (0, 120), (60, 120), "fixed_total_number", dict(degree_or_total=9000)),
+             (0, (0, 100), (100, 100), "one_to_one", {}),
+             (0, (10, 40), (0, 240), "all_to_all", {}),
+             (3, (0, 240), (0, 240), "fixed_indegree", dict(degree_or_total=20)),
+             (1, arr, (0, 200), "pairwise_bernoulli", dict(p=0.2)),
+             (0, (0, 50), arr, "fixed_outdegree", dict(degree_or_total=30, weights=rng.normal(0, 3, 1500).astype(np.float32))),
+             (0, (200, 40), (200, 40), "pairwise_bernoulli", dict(p=0.0))]
+    for flags in (0, nc_mod.FLAG_ORGANISE_COPASS):
+        for first, count in ((0, 80), (80, 80), (160, 80), (0, 240), (300, 10)):
+            o = oracle_mod.Oracle(dt_ms=0.1, block_size=1000)
+            g = nc_mod.NC(dt_ms=0.1, block_size=1000, flags=flags)
+            for b in (o, g):
+                b.create_population(N)
+                b.set_shard(first, count)
+                for k, (rf, src, tgt, rule, kw) in enumerate(calls):
+                    b.set_rule_flags(rf)
+                    b.set_connection_attributes(k % 3, k)  # attributes follow their projection through staging and filter
+                    b.connect(src, tgt, R[rule], weight=W, delay_ms=D, seed=10 + k, **kw)
+            n = o.num_connections()
+            assert g.num_connections() == n
+            scale = PU.scale_per_connection([22.0] * len(calls), o)
+            if n and not flags:
+                PU.compare_connections(g.read_connections(sorted=False), o.connections(sorted=False), scale, "creation order")
+            o.finalize()
+            g.finalize()
+            assert g.stats()["n_blocks"] == o.num_blocks()
+            if n:
+                os_ = o.connections(sorted=True)
+                PU.compare_connections(g.read_connections(sorted=True), os_, scale[os_["perm"]], "organised")
+            PU.compare_index(g.read_index(), o.index(), "index")
+            if n:
+                gp, gg = g.read_connection_attributes(sorted=True)
+                op, og = o.read_connection_attributes(sorted=True)
+                assert np.array_equal(gp, op) and np.array_equal(gg, og)
+            g.close()
+            o.close()
+    g = nc_mod.NC()
+    g.create_population(5)
+    g.connect((0, 5), (0, 5), R["all_to_all"], weight=W, delay_ms=D)
+    with pytest.raises(nc_mod.NCError):
+        g.set_shard(0, 2)
+    g.close()
