@@ -23,7 +23,8 @@ NVCC_FLAGS = [
 
 
 def sources():
-    return sorted(CSRC.glob("*.cu")), sorted(CSRC.glob("*.cuh")) + [HERE.parent / "include" / "nc.h"]
+    return sorted(CSRC.glob("*.cu")), (sorted(CSRC.glob("*.cuh")) + sorted(CSRC.glob("*.inl")) + sorted(CSRC.glob("*.h")) +
+                                     sorted((HERE.parent / "include").glob("*.h")))
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:
