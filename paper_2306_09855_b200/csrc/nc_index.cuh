@@ -373,14 +373,8 @@ __global__ void __launch_bounds__(kHeadThreads) index_scatter_soa_kernel(const u
     const int i = __ffs(m) - 1;
     m &= m - 1;
     const uint32_t j = base + i;
-    uint32_t si = s[1], di = d[1], sp = s[0];
-#pragma unroll
-    for (int q = 1; q < 8; ++q)
-      if (i == q) {
-        si = s[q + 1];
-        di = d[q + 1];
-        sp = s[q];
-      }
+    // heads are ~1 % of the positions: their keys are re-read (cache hits) instead of selected out of the registers
+    const uint32_t si = __ldg(src + j), di = __ldg(dly + j), sp = j ? __ldg(src + j - 1) : 0u;
     out.group_start[g] = j;
     out.group_delay[g] = (uint16_t)di;
     if (first_of_source & (1u << i)) {

@@ -12,6 +12,8 @@
 //               per piece), persistent CTAs with static or ticketed tiles -- the ceiling of a TMA-fed pass.
 //   atomorder : whether same-address shared-memory atomics of ONE warp instruction return their old values in ascending
 //               lane order (the property a rank-by-atomic variant of the pass would rest on).
+//   red       : the ceiling of spike delivery's inner loop: read a target and a weight (8 B), one fp32
+//               red.global.add into one of 77,169 accumulators (the node count of configs[2]), nothing else.
 //   pipes     : issue cost of IMAD.WIDE.U32, IMAD, LOP3, FFMA per warp instruction per SM sub-partition, the figures
 //               behind the integer-pipe bound of the generators.
 #include <cuda_runtime.h>
@@ -194,6 +196,20 @@ __global__ void atom_order(unsigned long long* out /* [0] violations, [1] same-a
 }
 
 // ---------------------------------------------------------------------------------------------------------------
+// red: scattered fp32 reductions into a small L2-resident array
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void fill_targets(uint32_t* tgt, float* w, uint32_t n, uint32_t n_nodes) {
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    tgt[i] = mix(i * 2654435761u + 99u) % n_nodes;
+    w[i] = 1.0f;
+  }
+}
+__global__ void __launch_bounds__(256) red_kernel(const uint32_t* __restrict__ tgt, const float* __restrict__ w, uint32_t n,
+                                                  float* __restrict__ acc) {
+  for (uint32_t i = blockIdx.x * 256u + threadIdx.x; i < n; i += gridDim.x * 256u) atomicAdd(acc + tgt[i], w[i]);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // pipes: N independent chains of one instruction per thread, timed with clock64 by every warp; the figure printed is
 // cycles per warp instruction per SM sub-partition with `warps` resident warps per sub-partition.
 // ---------------------------------------------------------------------------------------------------------------
@@ -346,6 +362,32 @@ int main(int argc, char** argv) {
     }
     printf("atomorder violations total: %llu\n", total);
     cudaFree(d);
+  }
+
+  if (all || !strcmp(what, "red")) {
+    printf("\n## red: n x (4 B target + 4 B weight read, one red.global.add.f32) into 77,169 accumulators\n");
+    printf("| events | us | events/s | GB/s of the 8 B per event |\n|---|---|---|---|\n");
+    const uint32_t n_nodes = 77169, n_max = 1u << 26;
+    uint32_t* tgt;
+    float *w, *acc;
+    CK(cudaMalloc(&tgt, (size_t)n_max * 4));
+    CK(cudaMalloc(&w, (size_t)n_max * 4));
+    CK(cudaMalloc(&acc, n_nodes * 4));
+    CK(cudaMemset(acc, 0, n_nodes * 4));
+    fill_targets<<<1184, 256>>>(tgt, w, n_max, n_nodes);
+    for (uint32_t n : {240000u, 3000000u, 15000000u, 1u << 26}) {
+      float best = 1e9f;
+      for (int r = 0; r < 5; ++r) {
+        t.start();
+        red_kernel<<<(n + 255) / 256 < 148 * 8 ? (n + 255) / 256 : 148 * 8, 256>>>(tgt, w, n, acc);
+        best = fminf(best, t.stop());
+      }
+      CK(cudaGetLastError());
+      printf("| %u | %.1f | %.3g | %.0f |\n", n, best * 1e3, n / (best * 1e-3), 8.0 * n / best * 1e-6);
+    }
+    cudaFree(tgt);
+    cudaFree(w);
+    cudaFree(acc);
   }
 
   if (all || !strcmp(what, "pipes")) {

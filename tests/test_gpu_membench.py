@@ -63,3 +63,8 @@ def test_pipe_rates(membench):
     assert wide, out
     cyc = float(wide[0].strip("|").split("|")[-1])
     assert 1.0 < cyc < 16.0, out
+
+
+def test_scattered_reduction_ceiling(membench):
+    out = _run(membench, "red")
+    assert len(_rows(out)) == 4, out
