@@ -200,7 +200,7 @@ typedef struct {
 
 /* ---- lifecycle ---- */
 int nc_create(const nc_config* cfg, nc_context** out);
-int nc_destroy(nc_context* ctx);
+int nc_destroy(nc_context* ctx); /* NC_ERR_STATE, nothing destroyed, while nc_delivery objects of the context exist (nc_delivery.h) */
 const char* nc_last_error(nc_context* ctx);
 int nc_synchronize(nc_context* ctx);
 

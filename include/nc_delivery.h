@@ -13,7 +13,8 @@
  * F3 group indexes in the spike array are global (group_ptr[source] + local index, Eq. 14).
  *
  * Conventions as in nc.h: int status returns, no exceptions; all work is enqueued on the context's stream; the
- * nc_delivery object borrows the context's sorted arrays and index and must be destroyed before the context.
+ * nc_delivery object borrows the context's sorted arrays and index and allocates from it: it must be destroyed before the
+ * context, and nc_destroy returns NC_ERR_STATE (destroying nothing) while a delivery object of the context still exists.
  * Pointers named d_* are DEVICE pointers owned by the caller; the others are HOST pointers.
  */
 #ifndef NC_DELIVERY_H_

@@ -96,6 +96,7 @@ struct nc_context {
   bool broken = false;  // an in-place organisation failed half way: the connections are lost, only nc_destroy is left
 
   // allocations
+  int attached = 0;             // delivery objects that allocate from this context (nc_destroy refuses while any exists)
   bool guard = false;           // NC_GUARD=1: every allocation sits between two 256-byte guard zones checked when it is freed
   uint64_t guard_violations = 0;
   std::unordered_map<void*, size_t> live;
@@ -190,6 +191,8 @@ int nc_create(const nc_config* cfg, nc_context** out) {
 
 int nc_destroy(nc_context* c) {
   if (!c) return NC_OK;
+  if (c->attached > 0)  // their buffers live in this context: destroying it first would leave them dangling
+    return fail(c, NC_ERR_STATE, "nc_destroy: nc_delivery objects of this context still exist; destroy them first");
   gen_span_end(c);
   cudaStreamSynchronize(c->stream);
   for (Span& s : c->spans) {
@@ -709,4 +712,7 @@ int nc_internal_organised_view(nc_context* c, nc_organised_view* out) {
 void* nc_internal_alloc(nc_context* c, size_t bytes) { return dev_alloc(c, bytes); }
 void nc_internal_free(nc_context* c, void* p) { dev_free(c, p); }
 int nc_internal_fail(nc_context* c, int code, const char* msg) { return fail(c, code, msg); }
+void nc_internal_attach(nc_context* c, int delta) {
+  if (c) c->attached += delta;
+}
 extern "C" uint64_t nc_internal_guard_violations(nc_context* c) { return c ? c->guard_violations : 0; }

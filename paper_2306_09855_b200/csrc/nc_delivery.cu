@@ -230,6 +230,7 @@ struct nc_delivery {
   int sms = 148;
   int coop_grid = 0;                  // > 0: one cooperative launch per step with at most this many CTAs
   uint32_t* last_arr_ctr = nullptr;   // counter of the spike array the last step filled
+  bool attached = false;              // counted in the context (nc_destroy refuses while deliveries exist)
 };
 
 extern "C" {
@@ -271,6 +272,8 @@ int nc_delivery_create(nc_context* ctx, uint32_t capacity, nc_delivery** out) {
     if (e == cudaSuccess && per_sm > 0) d->coop_grid = d->sms * std::min(per_sm, 8);
   }
   cudaGetLastError();
+  nc_internal_attach(ctx, +1);
+  d->attached = true;
   *out = d;
   return NC_OK;
 }
@@ -283,6 +286,7 @@ int nc_delivery_destroy(nc_delivery* d) {
   nc_internal_free(d->ctx, d->arr);
   nc_internal_free(d->ctx, d->arr_range);
   nc_internal_free(d->ctx, d->ctr);
+  if (d->attached) nc_internal_attach(d->ctx, -1);
   delete d;
   return NC_OK;
 }

@@ -24,3 +24,4 @@ int nc_internal_organised_view(nc_context* c, nc_organised_view* out);  // NC_ER
 void* nc_internal_alloc(nc_context* c, size_t bytes);
 void nc_internal_free(nc_context* c, void* p);
 int nc_internal_fail(nc_context* c, int code, const char* msg);
+void nc_internal_attach(nc_context* c, int delta);  // a delivery object was created on (+1) / destroyed from (-1) this context

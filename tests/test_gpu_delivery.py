@@ -169,3 +169,17 @@ def test_run_equals_step_by_step(nc_mod):
         d.close(); g.close()
     assert res[0][1] == res[1][1] and res[0][2] == res[1][2]
     assert np.abs(res[0][0] - res[1][0]).max() <= 1e-4 * max(1.0, np.abs(res[0][0]).max())  # fp32 atomics reorder
+
+
+def test_context_cannot_be_destroyed_under_a_delivery(nc_mod):
+    """nc_destroy refuses (NC_ERR_STATE, nothing freed) while a delivery object of the context exists; the binding's
+    NC.close() closes its deliveries first."""
+    import ctypes as C
+    net = WL.config0_tiny()
+    g = nc_mod.NC(dt_ms=net.dt_ms)
+    WL.run(net, g)
+    d = nc_mod.Delivery(g, 256)
+    assert g._L.nc_destroy(g._h) == nc_mod.ERR_STATE  # raw call: the context stays alive and usable
+    assert g.num_connections() == 1000
+    g.close()            # closes d first, then the context
+    assert not d._h
