@@ -48,6 +48,8 @@ struct GenParams {
   uint64_t div_magic;  // floor(2^64 / div) + 1
   PhiloxStream rng;    // synapse stream (stream 0) of this projection
   SynConst syn;
+  uint32_t i_first;    // i_newconns of the first connection this launch creates (a shard generates a sub-range of a call's
+                       // indexes, nc_set_shard); 0 for a whole call
 };
 
 // Weight and delay on the fp64 path: D5, D6, D7, D8 evaluated in the order the readings state, with explicit
@@ -227,7 +229,7 @@ __global__ void __launch_bounds__(kGenThreads) generate_kernel(const __grid_cons
   const bool interior = (p.map.B & 3) == 0 && tile0 >= p.pos0 && tile0 + kGenTile <= end && a0.slot + kGenTile <= p.map.B;
   if (interior) {
     // N_newconns <= 2^32 - 1 for these rules, so i fits 32 bits
-    const uint32_t i_thread = (uint32_t)(tile0 - p.pos0) + threadIdx.x * 4;
+    const uint32_t i_thread = p.i_first + (uint32_t)(tile0 - p.pos0) + threadIdx.x * 4;
     const uint64_t slot = a0.slot + threadIdx.x * 4;
     uint4* const sp = reinterpret_cast<uint4*>(reinterpret_cast<uint32_t*>(a0.base) + slot);
     uint4* const tp = reinterpret_cast<uint4*>(reinterpret_cast<uint32_t*>(a0.base + p.map.off_tgt) + slot);
@@ -281,7 +283,7 @@ __global__ void __launch_bounds__(kGenThreads) generate_kernel(const __grid_cons
     for (int k = 0; k < kGenGroups * 4; ++k) {
       const uint64_t pos = tile0 + (uint64_t)(k >> 2) * (kGenThreads * 4) + threadIdx.x * 4 + (k & 3);
       if (pos < p.pos0 || pos >= end) continue;
-      const uint32_t i = (uint32_t)(pos - p.pos0);  // i_newconns (Eq. 3)
+      const uint32_t i = p.i_first + (uint32_t)(pos - p.pos0);  // i_newconns (Eq. 3)
       uint32_t quo, rem, s, t, dly;
       float wgt;
       split_index<RULE>(p, i, quo, rem);

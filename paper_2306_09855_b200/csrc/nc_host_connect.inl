@@ -105,7 +105,9 @@ extern "C" {
 static int connect_core(nc_context* c, const uint32_t* src_nodes, nc_range src, const uint32_t* tgt_nodes, nc_range tgt,
                         nc_rule rule, const nc_rule_params* params, const nc_syn_spec* syn, uint64_t seed,
                         const float* weights = nullptr, const double* delays_ms = nullptr, uint64_t n_values = 0,
-                        bool with_values = false) {
+                        bool with_values = false, bool sub = false, uint64_t sub_first = 0, uint64_t sub_count = 0) {
+  // sub: create only connections sub_first .. sub_first + sub_count - 1 of the call (a shard's owned index sub-range; the
+  // caller guarantees a rule whose indexes it may cut, no value arrays, no rule flags)
   if (!c) return NC_ERR_INVALID_ARG;
   if (c->broken) return fail(c, NC_ERR_STATE, "nc_connect: a failed in-place organisation left this context without connections; destroy it");
   if (c->finalized) return fail(c, NC_ERR_STATE, "nc_connect after nc_finalize");
@@ -167,6 +169,7 @@ static int connect_core(nc_context* c, const uint32_t* src_nodes, nc_range src, 
       if (steps > bound) bound = steps;  // the key's delay bits must hold it
     }
   }
+  if (sub) n_new = sub_count;  // every check above was made on the whole call
   if (rule != NC_PAIRWISE_BERNOULLI && c->n_conns + n_new > kMaxConns)
     return fail(c, NC_ERR_CAPACITY, "more than 2^32-1 connections");
 
@@ -240,6 +243,7 @@ static int connect_core(nc_context* c, const uint32_t* src_nodes, nc_range src, 
   GenParams gp{};
   gp.pos0 = c->n_conns;
   gp.n = n_new;
+  gp.i_first = sub ? (uint32_t)sub_first : 0u;
   gp.s0 = src.first;
   gp.n_src = src.count;
   gp.t0 = tgt.first;
@@ -450,6 +454,20 @@ static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, 
                         bool with_values = false) {
   if (!c || !c->sharded || c->broken || c->finalized)  // not sharded, or let the ordinary path report the state
     return connect_core(c, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed, weights, delays_ms, n_values, with_values);
+  // Rules whose target is the slow deterministic coordinate of the index (one_to_one: t = t0 + i; fixed_indegree:
+  // t = t0 + i div K) over a target RANGE: the connections this shard owns are one contiguous index sub-range of the call,
+  // generated directly into the storage -- no staging, no filter, no redundant draws ("each GPU generates the
+  // index sub-range whose deterministic coordinate it owns").
+  if ((rule == NC_ONE_TO_ONE || rule == NC_FIXED_INDEGREE) && !tgt_nodes && !with_values && c->rule_flags == 0 && params &&
+      tgt.count > 0 && (uint64_t)tgt.first + tgt.count <= c->n_nodes) {
+    const uint64_t own_lo = std::max<uint64_t>(c->shard_first, tgt.first);
+    const uint64_t own_hi = std::min<uint64_t>((uint64_t)c->shard_first + c->shard_count, (uint64_t)tgt.first + tgt.count);
+    const uint64_t per = rule == NC_ONE_TO_ONE ? 1 : params->degree_or_total;
+    const uint64_t first = own_hi > own_lo ? (own_lo - tgt.first) * per : 0, count = own_hi > own_lo ? (own_hi - own_lo) * per : 0;
+    const int rc = flush_shard(c);  // what is staged comes before this call in creation order
+    if (rc != NC_OK) return rc;
+    return connect_core(c, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed, nullptr, nullptr, 0, false, true, first, count);
+  }
   // swap in the staging storage: the generators append the full projection behind what is already staged
   std::vector<void*> real_blocks;
   real_blocks.swap(c->blocks);

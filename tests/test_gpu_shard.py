@@ -97,3 +97,33 @@ def test_every_rule_flags_arrays_values_in_a_shard(nc_mod, oracle_mod):
     with pytest.raises(nc_mod.NCError):
         g.set_shard(0, 2)
     g.close()
+
+
+@pytest.mark.parametrize("B", [0, 4097, 1000])
+def test_fixed_indegree_and_one_to_one_shards_take_the_direct_path(nc_mod, oracle_mod, B):
+    """Target-range calls of one_to_one / fixed_indegree: a shard generates its owned index sub-range directly (no staging);
+    mixed with calls that go through staging, so the creation order across both mechanisms is checked too."""
+    net = WL.config3_large_indegree(scale=0.02)  # 1600 + 400 nodes, K = 160 / 40
+    W, D = (20.0, 2.0, 0.0, INF), (1.5, 0.75, 0.1, INF)
+    R = WL.RULE_IDS
+    for first, count in ((0, 700), (700, 613), (1313, 687), (0, 2000)):
+        o = oracle_mod.Oracle(dt_ms=0.1, block_size=B)
+        g = nc_mod.NC(dt_ms=0.1, block_size=B)
+        for b in (o, g):
+            WL.run(net, b, finalize=False, shard=(first, count))
+            b.connect((0, 300), (500, 900), R["fixed_total_number"], degree_or_total=20000, weight=W, delay_ms=D, seed=3)  # staged
+            b.connect((100, 1900), (100, 1900), R["one_to_one"], weight=W, delay_ms=D, seed=4)                              # direct
+            b.connect((0, 2000), (650, 100), R["fixed_indegree"], degree_or_total=33, weight=W, delay_ms=D, seed=5)         # direct
+            b.connect((0, 50), (0, 2000), R["all_to_all"], weight=W, delay_ms=D, seed=6)                                    # staged
+        n = o.num_connections()
+        assert g.num_connections() == n and n > 0
+        scale = PU.scale_per_connection([22.0] * (len(net.projections) + 4), o)
+        PU.compare_connections(g.read_connections(sorted=False), o.connections(sorted=False), scale, "creation order", max_mismatch=1)
+        o.finalize()
+        g.finalize()
+        assert g.stats()["n_blocks"] == o.num_blocks()
+        os_ = o.connections(sorted=True)
+        PU.compare_connections(g.read_connections(sorted=True), os_, scale[os_["perm"]], "organised", max_mismatch=1)
+        PU.compare_index(g.read_index(), o.index(), "index")
+        g.close()
+        o.close()
