@@ -308,13 +308,43 @@ int launch_scatter_pass(nc_context* c, const ScatterParams& sp, uint32_t n_tiles
 }
 
 // NC_FLAG_SORT_BULK: the same pass as a persistent kernel fed by cp.async.bulk (nc_sort_bulk.cuh), one CTA per SM.
+// Checked once per context, on its device: whether the bulk kernel may take ranks from returning shared atomics.
+int atomic_rank_usable(nc_context* c) {
+  if (c->atomic_rank >= 0) return NC_OK;
+  const char* e = getenv("NC_BULK_BALLOT_RANK");
+  if (e && atoi(e) != 0) {
+    c->atomic_rank = 0;
+    return NC_OK;
+  }
+  uint32_t* d = (uint32_t*)dev_alloc(c, 4);
+  if (!d) return fail(c, NC_ERR_OOM, "out of device memory");
+  uint32_t bad = 1;
+  NC_CUDA(c, cudaMemsetAsync(d, 0, 4, c->stream));
+  atomic_lane_order_kernel<<<296, 256, 0, c->stream>>>(d, 256);
+  NC_LAUNCH_CHECK(c, "atomic_lane_order");
+  NC_CUDA(c, cudaMemcpyAsync(&bad, d, 4, cudaMemcpyDeviceToHost, c->stream));
+  NC_CUDA(c, cudaStreamSynchronize(c->stream));
+  dev_free(c, d);
+  c->atomic_rank = bad == 0 ? 1 : 0;
+  return NC_OK;
+}
+
 template <bool FIRST, bool LAST>
 int launch_scatter_bulk(nc_context* c, const ScatterParams& sp, uint32_t n_tiles) {
-  auto kern = scatter_bulk_kernel<FIRST, LAST>;
-  NC_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BulkSmem)));
+  int rc = atomic_rank_usable(c);
+  if (rc != NC_OK) return rc;
   int sms = 0;
   NC_CUDA(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device));
-  kern<<<std::min<uint32_t>(n_tiles, (uint32_t)sms), kBulkWarps * 32, sizeof(BulkSmem), c->stream>>>(sp, n_tiles);
+  const uint32_t grid = std::min<uint32_t>(n_tiles, (uint32_t)sms);
+  if (c->atomic_rank) {
+    auto kern = scatter_bulk_kernel<FIRST, LAST, true>;
+    NC_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BulkSmem)));
+    kern<<<grid, kBulkWarps * 32, sizeof(BulkSmem), c->stream>>>(sp, n_tiles);
+  } else {
+    auto kern = scatter_bulk_kernel<FIRST, LAST, false>;
+    NC_CUDA(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(BulkSmem)));
+    kern<<<grid, kBulkWarps * 32, sizeof(BulkSmem), c->stream>>>(sp, n_tiles);
+  }
   NC_LAUNCH_CHECK(c, "scatter_bulk");
   return NC_OK;
 }

@@ -69,8 +69,33 @@ struct BulkSmem {
   uint64_t full[kBulkBuffers];
 };
 
+// Do the lanes of ONE shared-memory atomicAdd instruction that hit the same address get their old values in ascending lane
+// order?  (Not documented; measured true on B200, tests/cuda/membench.cu `atomorder`.)  The bulk kernel's ATOMIC_RANK form
+// takes a record's rank among the equal digits of its warp from exactly that; nc_create checks it on the device it runs on
+// and the ballot form is used wherever the check fails.
+__global__ void __launch_bounds__(256) atomic_lane_order_kernel(uint32_t* violations, uint32_t iters) {
+  __shared__ uint32_t hist[8][kRadix];
+  const uint32_t warp = threadIdx.x >> 5, lane = lane_id();
+  for (int i = lane; i < kRadix; i += 32) hist[warp][i] = 0;
+  __syncwarp();
+  uint32_t bad = 0;
+  for (uint32_t it = 0; it < iters; ++it) {
+    uint32_t x = (blockIdx.x * 256u + threadIdx.x) * 2654435761u + it * 40503u;
+    x ^= x >> 15;
+    x *= 0x846ca68bu;
+    const uint32_t d = (x >> 16) % ((it & 3u) == 0 ? 2u : (it & 3u) == 1 ? 8u : kRadix);
+    const uint32_t old = atomicAdd(&hist[warp][d], 1u);
+    const uint32_t peers = __match_any_sync(0xffffffffu, d);
+    // among equal digits the returned values must ascend with the lane: old = (value before the instruction) + (peers below)
+    const uint32_t lowest = __shfl_sync(0xffffffffu, old, __ffs(peers) - 1);
+    if (old != lowest + (uint32_t)__popc(peers & lanemask_lt())) ++bad;
+  }
+  if (bad) atomicAdd(violations, bad);
+}
+
 // FIRST requires every tile to lie inside one storage block with 16-byte aligned slices (B % kBulkTile == 0).
-template <bool FIRST, bool LAST>
+// ATOMIC_RANK: rank from one returning shared atomicAdd per record (see above) instead of a histogram round + eight ballots.
+template <bool FIRST, bool LAST, bool ATOMIC_RANK>
 __global__ void __launch_bounds__(kBulkWarps * 32, 1) scatter_bulk_kernel(const __grid_constant__ ScatterParams p,
                                                                          uint32_t n_tiles) {
   constexpr int kT = kBulkWarps * 32;
@@ -142,8 +167,9 @@ __global__ void __launch_bounds__(kBulkWarps * 32, 1) scatter_bulk_kernel(const 
         rec[i] = e < valid ? buf[e] : make_uint4(0xffffffffu, 0u, 0u, 0u);
       }
     }
+    uint32_t rk[ITEMS];
 #pragma unroll
-    for (int i = 0; i < ITEMS; ++i) atomicAdd(&my_hist[(rec[i].x >> p.shift) & mask], 1u);
+    for (int i = 0; i < ITEMS; ++i) rk[i] = atomicAdd(&my_hist[(rec[i].x >> p.shift) & mask], 1u);  // ATOMIC_RANK uses the value
     // the bulk stores of the previous tile may still read their buffer; those of the tile before it must have, before
     // its buffer (the one the next tile lands in) is refilled
     if (!LAST) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
@@ -184,15 +210,23 @@ __global__ void __launch_bounds__(kBulkWarps * 32, 1) scatter_bulk_kernel(const 
     __syncthreads();
 
     // ---- stable rank, records back into the SAME buffer in tile-sorted order ----
+    if (ATOMIC_RANK) {
+      // my_hist[d] now holds the tile position of the warp's first record of digit d; rk[i] the record's rank behind it
 #pragma unroll
-    for (int i = 0; i < ITEMS; ++i) {
-      const uint32_t d = (rec[i].x >> p.shift) & mask;
-      const uint32_t peers = peers_of<kMatchBallot>(d, nullptr);
-      const uint32_t below = __popc(peers & lanemask_lt());
-      uint32_t old = 0;
-      if (below == 0) old = atomicAdd(&my_hist[d], (uint32_t)__popc(peers));
-      old = __shfl_sync(0xffffffffu, old, __ffs(peers) - 1);
-      buf[old + below] = rec[i];
+      for (int i = 0; i < ITEMS; ++i) rk[i] += my_hist[(rec[i].x >> p.shift) & mask];
+#pragma unroll
+      for (int i = 0; i < ITEMS; ++i) buf[rk[i]] = rec[i];
+    } else {
+#pragma unroll
+      for (int i = 0; i < ITEMS; ++i) {
+        const uint32_t d = (rec[i].x >> p.shift) & mask;
+        const uint32_t peers = peers_of<kMatchBallot>(d, nullptr);
+        const uint32_t below = __popc(peers & lanemask_lt());
+        uint32_t old = 0;
+        if (below == 0) old = atomicAdd(&my_hist[d], (uint32_t)__popc(peers));
+        old = __shfl_sync(0xffffffffu, old, __ffs(peers) - 1);
+        buf[old + below] = rec[i];
+      }
     }
     if (!LAST) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // the copy engine reads what was just written
     __syncthreads();
