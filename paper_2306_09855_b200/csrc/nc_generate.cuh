@@ -323,6 +323,9 @@ struct BernParams {
   uint32_t* tile_count;   // [n_tiles]
 };
 
+// T32: the threshold fits 32 bits (p < 1), so a trial is one 32-bit compare; T = 2^32 (p = 1, every word is below it) keeps
+// the 64-bit compare.
+template <bool T32>
 __global__ void __launch_bounds__(kBernThreads) bernoulli_trials_kernel(const __grid_constant__ BernParams p) {
   const uint64_t gt = (uint64_t)blockIdx.x * kBernThreads + threadIdx.x;
   const uint64_t q0 = gt * kBernTrialsPerThread;
@@ -333,10 +336,18 @@ __global__ void __launch_bounds__(kBernThreads) bernoulli_trials_kernel(const __
     for (int j = 0; j < kBernTrialsPerThread / 4; ++j) {
       const uint64_t c = c0 + j;
       const Philox4 r = philox_stream<false>((uint32_t)c, (uint32_t)(c >> 32), p.rng);
-      m |= ((uint64_t)r.x < p.threshold ? 1u : 0u) << (4 * j + 0);
-      m |= ((uint64_t)r.y < p.threshold ? 1u : 0u) << (4 * j + 1);
-      m |= ((uint64_t)r.z < p.threshold ? 1u : 0u) << (4 * j + 2);
-      m |= ((uint64_t)r.w < p.threshold ? 1u : 0u) << (4 * j + 3);
+      if (T32) {
+        const uint32_t t = (uint32_t)p.threshold;
+        m |= (r.x < t ? 1u : 0u) << (4 * j + 0);
+        m |= (r.y < t ? 1u : 0u) << (4 * j + 1);
+        m |= (r.z < t ? 1u : 0u) << (4 * j + 2);
+        m |= (r.w < t ? 1u : 0u) << (4 * j + 3);
+      } else {
+        m |= ((uint64_t)r.x < p.threshold ? 1u : 0u) << (4 * j + 0);
+        m |= ((uint64_t)r.y < p.threshold ? 1u : 0u) << (4 * j + 1);
+        m |= ((uint64_t)r.z < p.threshold ? 1u : 0u) << (4 * j + 2);
+        m |= ((uint64_t)r.w < p.threshold ? 1u : 0u) << (4 * j + 3);
+      }
     }
     const uint64_t left = p.n_pairs - q0;
     if (left < 32) m &= (1u << (uint32_t)left) - 1u;

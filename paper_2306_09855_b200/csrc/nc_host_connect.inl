@@ -51,7 +51,8 @@ int connect_bernoulli(nc_context* c, GenParams gp, double p, uint32_t seed_lo, u
       bp.rng = make_philox_stream(seed_lo, seed_hi, c->n_proj, 1u);
       bp.mask = mask;
       bp.tile_count = tile_count;
-      bernoulli_trials_kernel<<<(unsigned)n_tiles, kBernThreads, 0, c->stream>>>(bp);
+      if (T < (1ull << 32)) bernoulli_trials_kernel<true><<<(unsigned)n_tiles, kBernThreads, 0, c->stream>>>(bp);
+      else bernoulli_trials_kernel<false><<<(unsigned)n_tiles, kBernThreads, 0, c->stream>>>(bp);
       NC_LAUNCH_CHECK(c, "bernoulli_trials");
     } else {
       pair_mask_fill_kernel<<<(unsigned)n_tiles, kBernThreads, 0, c->stream>>>(pm);
