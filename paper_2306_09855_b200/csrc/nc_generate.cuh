@@ -332,17 +332,28 @@ __global__ void __launch_bounds__(kBernThreads) bernoulli_trials_kernel(const __
   uint32_t m = 0;
   if (q0 < p.n_pairs) {
     const uint64_t c0 = q0 >> 2;
+    if (T32) {
+      // mask built from the carry flag of (T - 1) - word, which is set iff the subtraction does not borrow, i.e. iff
+      // word < T (T >= 1 here): m = 2 m + (word < T), two instructions per trial; trials are taken from the last to the
+      // first so that trial k ends up in bit k
+      const uint32_t t = (uint32_t)p.threshold - 1u;
 #pragma unroll
-    for (int j = 0; j < kBernTrialsPerThread / 4; ++j) {
-      const uint64_t c = c0 + j;
-      const Philox4 r = philox_stream<false>((uint32_t)c, (uint32_t)(c >> 32), p.rng);
-      if (T32) {
-        const uint32_t t = (uint32_t)p.threshold;
-        m |= (r.x < t ? 1u : 0u) << (4 * j + 0);
-        m |= (r.y < t ? 1u : 0u) << (4 * j + 1);
-        m |= (r.z < t ? 1u : 0u) << (4 * j + 2);
-        m |= (r.w < t ? 1u : 0u) << (4 * j + 3);
-      } else {
+      for (int j = kBernTrialsPerThread / 4 - 1; j >= 0; --j) {
+        const uint64_t c = c0 + j;
+        const Philox4 r = philox_stream<false>((uint32_t)c, (uint32_t)(c >> 32), p.rng);
+        asm("{\n .reg .u32 d;\n"
+            " sub.cc.u32 d, %5, %1;\n addc.u32 %0, %0, %0;\n"
+            " sub.cc.u32 d, %5, %2;\n addc.u32 %0, %0, %0;\n"
+            " sub.cc.u32 d, %5, %3;\n addc.u32 %0, %0, %0;\n"
+            " sub.cc.u32 d, %5, %4;\n addc.u32 %0, %0, %0;\n}"
+            : "+r"(m)
+            : "r"(r.w), "r"(r.z), "r"(r.y), "r"(r.x), "r"(t));
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < kBernTrialsPerThread / 4; ++j) {
+        const uint64_t c = c0 + j;
+        const Philox4 r = philox_stream<false>((uint32_t)c, (uint32_t)(c >> 32), p.rng);
         m |= ((uint64_t)r.x < p.threshold ? 1u : 0u) << (4 * j + 0);
         m |= ((uint64_t)r.y < p.threshold ? 1u : 0u) << (4 * j + 1);
         m |= ((uint64_t)r.z < p.threshold ? 1u : 0u) << (4 * j + 2);
