@@ -389,7 +389,10 @@ def main():
                 "traffic": ncu_traffic_per_launch()[0] if args.workload == "c2" and not args.flags else None,
                 "traffic_captured_at": ncu_traffic_per_launch()[1] if args.workload == "c2" and not args.flags else None,
                 "peak_kind": peak_kind,
-                "launch_ms": pass_ms, "launches_per_step": passes}
+                "launch_ms": pass_ms, "launches_per_step": passes,
+                "context": "peak is a streaming copy; the pass writes ~256-byte runs that start inside 32-byte sectors, and a "
+                           "copy kernel with that write pattern and no ranking reaches 5050-5390 GB/s on a B200 "
+                           "(tests/cuda/membench.cu `pattern`, profiles/r02_scatter.md)"}
     phases = {}
     for name, b in (("generate", BYTES["generate"]), ("histogram", BYTES["histogram"]), ("sort", BYTES["sort_pass"] * passes),
                     ("permute", BYTES["permute"]), ("index", BYTES["index"])):
