@@ -18,10 +18,14 @@
 // A buffer is refilled once the bulk stores that read it have completed their shared-memory reads
 // (cp.async.bulk.wait_group.read).
 //
-// Measured on B200 (profiles/r02_scatter.md): on par with the default kernel on the middle pass (1.87-1.90 ms against
-// 1.91 ms) and not faster, because the pass is bound by how the memory system takes runs that start inside a sector,
-// not by how the SM is fed; a bulk store costs its issuing warp ~70 cycles, and separating the ranking warps from
-// store-issuing warps, ticketed tiles, and several consumer groups all measured slower.
+// Measured on B200 (profiles/r02_scatter.md): 7.23 ms of digit passes per configs[2] step against 5.95 ms for the default
+// kernels (the middle pass alone was on par in the working harness, 1.86 - 1.90 against 1.91 ms; the first pass with its four
+// SoA slices and the last pass with ordinary stores from one CTA per SM are slower).  Not faster, because the pass is bound by
+// how the memory system takes runs that start inside a sector, not by how the SM is fed; a bulk store costs its issuing warp
+// ~70 cycles, and separating the ranking warps from store-issuing warps, ticketed tiles, and several consumer groups all
+// measured slower.
+//   rank   : (in place of the ballots above) one returning shared atomicAdd per record once atomic_lane_order_kernel has
+//            confirmed on the device that same-address lanes are served in ascending lane order; the ballot form otherwise.
 #pragma once
 
 #include "nc_sort_split.cuh"
