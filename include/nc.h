@@ -86,11 +86,20 @@ enum {
   NC_FLAG_COPASS_SHIFT = 1u << 5,  /* with NC_FLAG_ORGANISE_COPASS: follow Fig. 6 C-E to the letter (one partition per
                                    output block on what the previous extraction left, right partitions shifted
                                    right) instead of the default extraction by hole filling (include/nc_copass.h) */
-  NC_FLAG_SORT_BULK = 1u << 6      /* default organisation path, but every digit pass runs as a persistent kernel fed by
+  NC_FLAG_SORT_BULK = 1u << 6,     /* default organisation path, but every digit pass runs as a persistent kernel fed by
                                    the bulk-async copy engine (cp.async.bulk loads of whole tiles tracked by mbarriers,
                                    one bulk store per digit run) instead of one CTA per tile with ordinary loads and
                                    stores.  Same result bit for bit; measured on par, kept selectable.
                                    The first pass takes this form only when block_size is a multiple of 4096. */
+  NC_FLAG_SORT_BUCKETS = 1u << 7   /* bucket-first organisation (keys of at most 32 bits): one stable pass scatters the
+                                   connections into at most 256 buckets of consecutive source ids, then every bucket is
+                                   sorted on its own by the remaining key bits with its intermediate records in a slot
+                                   meant to stay in the L2 cache (66 instead of 102 bytes of device-memory traffic per
+                                   connection for configs[2] if it does).  Same result bit for bit.  nc_finalize waits
+                                   for the device once (the 256 bucket sizes); with other than two in-bucket passes it
+                                   spreads the buckets over up to three CUDA streams of its own, joined again before it
+                                   returns.  Measured SLOWER than the default on a B200 (the pass is bound by the SM, not
+                                   by HBM); kept selectable as the evidence. */
 };
 
 typedef struct {

@@ -21,6 +21,7 @@ OK, ERR_INVALID_ARG, ERR_STATE, ERR_CAPACITY, ERR_OOM, ERR_CUDA = 0, -1, -2, -3,
 ONE_TO_ONE, ALL_TO_ALL, FIXED_INDEGREE, FIXED_OUTDEGREE, FIXED_TOTAL_NUMBER, PAIRWISE_BERNOULLI = range(6)
 FLAG_TIMING, FLAG_EXACT_FP64, FLAG_SORT_PAIRS, FLAG_SORT_ONESWEEP, FLAG_ORGANISE_COPASS, FLAG_COPASS_SHIFT = 1, 2, 4, 8, 16, 32
 FLAG_SORT_BULK = 64
+FLAG_SORT_BUCKETS = 128
 NO_AUTAPSES, NO_MULTAPSES = 1, 2  # nc_set_rule_flags
 PHASES = ("generate", "histogram", "sort", "permute", "index", "degree", "copass")
 

@@ -15,6 +15,8 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <map>
+#include <mutex>
 #include <string>
 #include <unordered_map>
 #include <vector>
@@ -28,6 +30,7 @@
 #include "nc_sort.cuh"
 #include "nc_sort_split.cuh"
 #include "nc_sort_bulk.cuh"
+#include "nc_sort_msd.cuh"
 #include "nc_copass.cuh"
 #include "../../include/nc_copass.h"
 
@@ -129,6 +132,7 @@ struct nc_context {
 
 #include "nc_host_common.inl"
 #include "nc_host_organise.inl"
+#include "nc_host_msd.inl"
 #include "nc_host_copass.inl"
 #include "nc_host_index.inl"
 
@@ -291,6 +295,7 @@ int nc_finalize(nc_context* c) {
     } else if (c->key_bits > 32) rc = sort_and_index<uint64_t>(c, plan);
     else if (c->cfg.flags & NC_FLAG_SORT_PAIRS) rc = sort_and_index<uint32_t>(c, plan);
     else if (c->cfg.flags & NC_FLAG_SORT_ONESWEEP) rc = sort_carry_and_index(c, plan);
+    else if (c->cfg.flags & NC_FLAG_SORT_BUCKETS) rc = sort_msd_and_index(c);
     else rc = sort_split_and_index(c, plan);
     if (rc != NC_OK) {
       drop_finalize_outputs(c);

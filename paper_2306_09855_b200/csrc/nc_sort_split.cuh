@@ -205,7 +205,65 @@ struct ScatterParams {
   uint32_t shift, bits;            // this pass's digit
   uint32_t next_shift, next_bits;  // the next pass's digit
   const uint32_t* offs;            // [n_tiles][256]
+  // bucket-first organisation (nc_sort_msd.cuh; MODE != 0 of scatter_pass_kernel)
+  uint32_t msd_mul;                // MODE 1: bucket of a key = min(umulhi(source, msd_mul), 255)
+  const uint32_t* key_base_tab;    // MODE 1: [256] smallest key of every bucket (the next pass's digits are relative to it)
+  uint32_t key_base;               // MODE 2, 3: smallest key of the bucket this launch sorts; digits are those of key - key_base
+  const uint16_t* counts;          // MODE 2, 3: [n_tiles][256] digit counts of the tiles and
+  const uint32_t* chunk_base;      //            [n_chunks][256] first output position of every chunk of kSegChunkTiles tiles
 };
+
+// MODE of scatter_pass_kernel: 0 = a digit pass over the whole array (offsets from the scan kernels);
+// 1 = the bucket pass of nc_sort_msd.cuh (digit = bucket of the source); 2 / 3 = a digit pass inside ONE bucket whose records
+// come from HBM / from an L2-resident slot (offsets from chunk bases + the counts of the tiles before it in its chunk; L2
+// eviction-priority hints on the loads and stores).
+constexpr uint32_t kSegChunkTiles = 8;
+
+template <int MODE>
+__device__ __forceinline__ uint32_t pass_digit(uint32_t key, const ScatterParams& p, uint32_t mask) {
+  if (MODE == 1) return min(__umulhi(key >> p.delay_bits, p.msd_mul), (uint32_t)kRadix - 1u);
+  if (MODE >= 2) return ((key - p.key_base) >> p.shift) & mask;
+  return (key >> p.shift) & mask;
+}
+
+// L2 eviction-priority hints (H: 0 none, 1 evict_first, 2 evict_last)
+template <int H>
+__device__ __forceinline__ uint64_t l2_policy() {
+  uint64_t pol = 0;
+  if (H == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  if (H == 2) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+template <int H, bool PAST_L1 = false>
+__device__ __forceinline__ uint4 ld_hint(const uint4* q, uint64_t pol) {
+  if (H == 0) return PAST_L1 ? __ldcg(q) : *q;
+  uint4 r;
+  if (PAST_L1)
+    asm volatile("ld.global.cg.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(q), "l"(pol));
+  else
+    asm volatile("ld.global.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(q), "l"(pol));
+  return r;
+}
+template <int H>
+__device__ __forceinline__ void st_hint(uint4* q, const uint4& v, uint64_t pol) {
+  if (H == 0) *q = v;
+  else asm volatile("st.global.L2::cache_hint.v4.b32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(q), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(pol) : "memory");
+}
+template <int H>
+__device__ __forceinline__ void st_hint(uint32_t* q, uint32_t v, uint64_t pol) {
+  if (H == 0) *q = v;
+  else asm volatile("st.global.L2::cache_hint.b32 [%0], %1, %2;" ::"l"(q), "r"(v), "l"(pol) : "memory");
+}
+template <int H>
+__device__ __forceinline__ void st_hint(uint16_t* q, uint16_t v, uint64_t pol) {
+  if (H == 0) *q = v;
+  else asm volatile("st.global.L2::cache_hint.b16 [%0], %1, %2;" ::"l"(q), "h"(v), "l"(pol) : "memory");
+}
+template <int H>
+__device__ __forceinline__ void st_hint(uint8_t* q, uint8_t v, uint64_t pol) {
+  if (H == 0) *q = v;
+  else asm volatile("st.global.L2::cache_hint.b8 [%0], %1, %2;" ::"l"(q), "r"((uint32_t)v), "l"(pol) : "memory");
+}
 
 template <int WARPS, int ITEMS, bool SMEM_MATCH>
 struct ScatterSmem {
@@ -217,14 +275,30 @@ struct ScatterSmem {
   uint32_t scan_tmp[kRadix / 32];
 };
 
-template <bool FIRST, bool LAST, int WARPS, int ITEMS, int MIN_CTAS, int MATCH>
-__global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(const __grid_constant__ ScatterParams p) {
+// One tile of a pass.  COHERENT (in-bucket passes run by the persistent kernel of nc_sort_msd.cuh): what other CTAs of the SAME
+// launch wrote -- the offsets and, in MODE 3, the records -- is read past the L1.
+struct NoHook {
+  __device__ __forceinline__ void operator()() const {}
+};
+
+// ATOMIC_RANK: a record's place among the equal digits of its warp comes from ONE returning shared atomicAdd per record instead
+// of eight ballots + a leader's atomic + a shuffle; rests on the lanes of one atomic instruction being served in ascending lane
+// order (nc_sort_bulk.cuh, atomic_lane_order_kernel), so only where the context has checked that.
+template <bool FIRST, bool LAST, int WARPS, int ITEMS, int MATCH, int MODE, bool COHERENT, typename Hook = NoHook,
+          bool ATOMIC_RANK = false>
+__device__ __forceinline__ void scatter_tile(const ScatterParams& p, const uint32_t tile,
+                                             ScatterSmem<WARPS, ITEMS, MATCH == kMatchSmem>& sm, Hook hook = Hook()) {
   using Smem = ScatterSmem<WARPS, ITEMS, MATCH == kMatchSmem>;
+  static_assert(MODE == 0 || (MODE == 1 && FIRST && !LAST) || (MODE >= 2 && !FIRST), "bucket pass: from the blocks; in-bucket: records");
+  // in-bucket passes: what comes from HBM is read once (evict_first), what goes to the slot the next pass reads stays
+  // (evict_last), the final arrays are not read again by this step (evict_first)
+  constexpr int kLoadHint = MODE == 2 ? 1 : MODE == 3 ? 2 : 0;
+  constexpr int kStoreHint = MODE >= 2 ? (LAST ? 1 : 2) : 0;
+  const uint64_t lpol = l2_policy<kLoadHint>(), spol = l2_policy<kStoreHint>();
+  const uint32_t pad_key = MODE >= 2 ? p.key_base - 1u : 0xffffffffu;  // its digits are the largest of every pass
   constexpr int kThreads = WARPS * 32;
   constexpr int kTile = Smem::kTile;
   static_assert(kThreads >= kRadix, "one thread per digit is needed for the in-tile scan");
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
 
   const uint32_t warp = threadIdx.x >> 5, lane = lane_id();
   {
@@ -232,12 +306,24 @@ __global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(cons
     uint4* z = reinterpret_cast<uint4*>(&sm.warp_hist[0][0]);
     for (int i = threadIdx.x; i < kZero; i += kThreads) z[i] = make_uint4(0u, 0u, 0u, 0u);
   }
-  const uint32_t tile = blockIdx.x;
   const uint64_t tile0 = (uint64_t)tile * kTile;
   const uint32_t valid = (uint32_t)min((uint64_t)kTile, (uint64_t)p.n - tile0);
   const uint32_t mask = (1u << p.bits) - 1u;
   // first output position of this tile's run of digit threadIdx.x: fetched now, needed after the histogram
-  const uint32_t out0 = threadIdx.x < kRadix ? __ldg(p.offs + (uint64_t)tile * kRadix + threadIdx.x) : 0u;
+  uint32_t out0 = 0u;
+  if (threadIdx.x < kRadix) {
+    if (MODE >= 2) {
+      const uint32_t chunk = tile / kSegChunkTiles, k = tile % kSegChunkTiles;
+      const uint32_t* bp = p.chunk_base + (uint64_t)chunk * kRadix + threadIdx.x;
+      out0 = COHERENT ? __ldcg(bp) : __ldg(bp);
+      const uint16_t* cp = p.counts + (uint64_t)chunk * kSegChunkTiles * kRadix + threadIdx.x;
+#pragma unroll
+      for (uint32_t kk = 0; kk + 1 < kSegChunkTiles; ++kk)
+        if (kk < k) out0 += COHERENT ? __ldcg(cp + kk * kRadix) : __ldg(cp + kk * kRadix);
+    } else {
+      out0 = __ldg(p.offs + (uint64_t)tile * kRadix + threadIdx.x);
+    }
+  }
 
   // ---- load records, warp-striped: element (warp, i, lane) is tile position warp*ITEMS*32 + i*32 + lane ----
   uint4 rec[ITEMS];
@@ -285,19 +371,20 @@ __global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(cons
     const uint4* in = p.recs_in + tile0 + wbase;
     if (valid == kTile) {
 #pragma unroll
-      for (int i = 0; i < ITEMS; ++i) rec[i] = in[i * 32];
+      for (int i = 0; i < ITEMS; ++i) rec[i] = ld_hint<kLoadHint, COHERENT && MODE == 3>(in + i * 32, lpol);
     } else {
 #pragma unroll
       for (int i = 0; i < ITEMS; ++i) {
         // padding sorts behind every real record of the tile and is never written out
-        rec[i] = wbase + i * 32 < valid ? in[i * 32] : make_uint4(0xffffffffu, 0u, 0u, 0u);
+        rec[i] = wbase + i * 32 < valid ? ld_hint<kLoadHint, COHERENT && MODE == 3>(in + i * 32, lpol) : make_uint4(pad_key, 0u, 0u, 0u);
       }
     }
   }
   __syncthreads();  // the counters are zero
+  hook();           // (persistent kernel: bookkeeping of one thread, behind the record loads that are in flight now)
   // ---- per-warp digit histogram with fire-and-forget shared-memory atomics ----
 #pragma unroll
-  for (int i = 0; i < ITEMS; ++i) atomicAdd(&my_hist[(rec[i].x >> p.shift) & mask], 1u);
+  for (int i = 0; i < ITEMS; ++i) atomicAdd(&my_hist[pass_digit<MODE>(rec[i].x, p, mask)], 1u);
   __syncthreads();
 
   // ---- per digit: exclusive scan over the warps; exclusive scan over the digits -> where each digit's run
@@ -335,15 +422,23 @@ __global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(cons
   // ---- stable rank + scatter into shared memory in one go: the lowest lane of each group of equal digits
   //      bumps the warp's running offset for that digit (atomics of one warp to one address retire in
   //      program order, so items keep their position order) and the group shares the old value ----
+  if (ATOMIC_RANK) {
+    uint32_t at[ITEMS];
 #pragma unroll
-  for (int i = 0; i < ITEMS; ++i) {
-    const uint32_t d = (rec[i].x >> p.shift) & mask;
-    const uint32_t peers = peers_of<MATCH>(d, sm.warp_masks[MATCH == kMatchSmem ? warp : 0]);
-    const uint32_t below = __popc(peers & lanemask_lt());
-    uint32_t old = 0;
-    if (below == 0) old = atomicAdd(&my_hist[d], (uint32_t)__popc(peers));
-    old = __shfl_sync(0xffffffffu, old, __ffs(peers) - 1);
-    sm.recs[old + below] = rec[i];
+    for (int i = 0; i < ITEMS; ++i) at[i] = atomicAdd(&my_hist[pass_digit<MODE>(rec[i].x, p, mask)], 1u);
+#pragma unroll
+    for (int i = 0; i < ITEMS; ++i) sm.recs[at[i]] = rec[i];
+  } else {
+#pragma unroll
+    for (int i = 0; i < ITEMS; ++i) {
+      const uint32_t d = pass_digit<MODE>(rec[i].x, p, mask);
+      const uint32_t peers = peers_of<MATCH>(d, sm.warp_masks[MATCH == kMatchSmem ? warp : 0]);
+      const uint32_t below = __popc(peers & lanemask_lt());
+      uint32_t old = 0;
+      if (below == 0) old = atomicAdd(&my_hist[d], (uint32_t)__popc(peers));
+      old = __shfl_sync(0xffffffffu, old, __ffs(peers) - 1);
+      sm.recs[old + below] = rec[i];
+    }
   }
 
   if (LAST) {
@@ -355,12 +450,12 @@ __global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(cons
       const uint32_t j = i * kThreads + threadIdx.x;
       if (j < valid) {
         const uint4 r = sm.recs[j];
-        const uint32_t g = sm.global_off[(r.x >> p.shift) & mask] + j;
-        p.out_src[g] = r.x >> p.delay_bits;
-        p.out_d[g] = (uint16_t)(r.x & dmask);
-        p.out_tgt[g] = r.z;
-        p.out_w[g] = __uint_as_float(r.w);
-        p.out_perm[g] = r.y;
+        const uint32_t g = sm.global_off[pass_digit<MODE>(r.x, p, mask)] + j;
+        st_hint<kStoreHint>(p.out_src + g, r.x >> p.delay_bits, spol);
+        st_hint<kStoreHint>(p.out_d + g, (uint16_t)(r.x & dmask), spol);
+        st_hint<kStoreHint>(p.out_tgt + g, r.z, spol);
+        st_hint<kStoreHint>(reinterpret_cast<uint32_t*>(p.out_w) + g, r.w, spol);
+        st_hint<kStoreHint>(p.out_perm + g, r.y, spol);
       }
     }
   } else {
@@ -373,12 +468,22 @@ __global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(cons
       const uint32_t j = i * kThreads + threadIdx.x;
       if (j < valid) {
         const uint4 r = sm.recs[j];
-        const uint32_t g = sm.global_off[(r.x >> p.shift) & mask] + j;
-        p.recs_out[g] = r;
-        p.dig_out[g] = (uint8_t)((r.x >> p.next_shift) & next_mask);
+        const uint32_t d = pass_digit<MODE>(r.x, p, mask);
+        const uint32_t g = sm.global_off[d] + j;
+        st_hint<kStoreHint>(p.recs_out + g, r, spol);
+        // the next pass's digit: of the key itself, or (bucket-first organisation) of the key relative to its bucket's first
+        const uint32_t rel = MODE == 1 ? r.x - __ldg(p.key_base_tab + d) : MODE >= 2 ? r.x - p.key_base : r.x;
+        st_hint<kStoreHint>(p.dig_out + g, (uint8_t)((rel >> p.next_shift) & next_mask), spol);
       }
     }
   }
+}
+
+template <bool FIRST, bool LAST, int WARPS, int ITEMS, int MIN_CTAS, int MATCH, int MODE = 0>
+__global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(const __grid_constant__ ScatterParams p) {
+  using Smem = ScatterSmem<WARPS, ITEMS, MATCH == kMatchSmem>;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  scatter_tile<FIRST, LAST, WARPS, ITEMS, MATCH, MODE, false>(p, blockIdx.x, *reinterpret_cast<Smem*>(smem_raw));
 }
 
 }  // namespace nc

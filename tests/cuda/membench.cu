@@ -8,6 +8,11 @@
 //               a 128-byte line (what a stable radix scatter of 16-byte records produces: a run of tile t ends where
 //               the run of tile t + 1 begins).  R > 1: one CTA writes R consecutive tiles, so the two parts of a shared
 //               line are written by the same SM one tile period apart.
+//   ring      : whether two consecutive digit passes can keep their intermediate array in the 126 MB L2 when the data is
+//               processed group by group (a group = one bucket of an MSD first pass): per group, copy HBM -> ring slot
+//               (256-byte pieces, 256 streams inside the group) and ring slot -> HBM (512-byte pieces, 128 streams),
+//               groups alternating over CUDA streams so that the two kernels of neighbouring groups overlap; against
+//               the same launches with a full-size intermediate array, and against the two full-array passes.
 //   bulk      : the same pattern moved by cp.async.bulk alone (bulk load of a tile into shared memory, one bulk store
 //               per piece), persistent CTAs with static or ticketed tiles -- the ceiling of a TMA-fed pass.
 //   atomorder : whether same-address shared-memory atomics of ONE warp instruction return their old values in ascending
@@ -72,6 +77,52 @@ __global__ void __launch_bounds__(256) pattern_copy(const uint4* __restrict__ in
       const uint32_t s = c % S, q = c / S;
       out[(uint64_t)s * region + (((uint64_t)tile * per + q) << cr_shift) + o + sh] = r[i];
     }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// ring: the copy of `pattern` with L2 eviction-priority hints on its loads (LH) and stores (SH): 0 none, 1 evict_first,
+// 2 evict_last
+// ---------------------------------------------------------------------------------------------------------------
+template <int H>
+__device__ __forceinline__ uint64_t l2_policy() {
+  uint64_t pol = 0;
+  if (H == 1) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  if (H == 2) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+
+template <int LH, int SH>
+__global__ void __launch_bounds__(256) pattern_copy_hint(const uint4* __restrict__ in, uint4* __restrict__ out, uint32_t n_tiles,
+                                                         uint32_t S, uint32_t cr_shift, uint32_t region, uint32_t sh) {
+  const uint32_t cpt = kTileRecs >> cr_shift, per = cpt / S;
+  const uint32_t tile = blockIdx.x;
+  if (tile >= n_tiles) return;
+  const uint64_t lpol = l2_policy<LH>(), spol = l2_policy<SH>();
+  uint4 r[16];
+  const uint4* src = in + (uint64_t)tile * kTileRecs;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    const uint4* q = src + i * 256 + threadIdx.x;
+    if (LH == 0)
+      r[i] = *q;
+    else
+      asm volatile("ld.global.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
+                   : "=r"(r[i].x), "=r"(r[i].y), "=r"(r[i].z), "=r"(r[i].w)
+                   : "l"(q), "l"(lpol));
+  }
+#pragma unroll
+  for (int i = 0; i < 16; ++i) {
+    const uint32_t j = i * 256 + threadIdx.x;
+    const uint32_t c = j >> cr_shift, o = j & ((1u << cr_shift) - 1u);
+    const uint32_t s = c % S, q = c / S;
+    uint4* dst = out + (uint64_t)s * region + (((uint64_t)tile * per + q) << cr_shift) + o + sh;
+    if (SH == 0)
+      *dst = r[i];
+    else
+      asm volatile("st.global.L2::cache_hint.v4.b32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(dst), "r"(r[i].x), "r"(r[i].y), "r"(r[i].z),
+                   "r"(r[i].w), "l"(spol)
+                   : "memory");
   }
 }
 
@@ -345,6 +396,99 @@ int main(int argc, char** argv) {
       cudaFree(per_cta);
     }
     cudaFree(in);
+    cudaFree(out);
+  }
+
+  if (all || !strcmp(what, "ring")) {
+    const uint32_t n_tiles = 72960;
+    const uint64_t n = (uint64_t)n_tiles * kTileRecs;
+    uint4 *in, *tmp, *out;
+    CK(cudaMalloc(&in, n * 16));
+    CK(cudaMalloc(&tmp, n * 16 + (1 << 20)));
+    CK(cudaMalloc(&out, n * 16 + (1 << 20)));
+    CK(cudaMemset(in, 1, n * 16));
+    printf("\n## ring: two passes over %.2f GB (pass 1: 256 B pieces into 256 streams, pass 2: 512 B pieces into 128 streams, every piece\n"
+           "## starting 16 B into a sector), whole-array launches against per-group launches; 'ring' = the intermediate array is one\n"
+           "## slot per CUDA stream, reused by every group, 'full' = every group has its own part of a full-size intermediate array\n",
+           n * 16e-9);
+    printf("| group MB | CUDA streams | intermediate | hints (load 1, store 1, load 2, store 2) | ms | GB/s of 64 B per record |\n|---|---|---|---|---|---|\n");
+    {
+      float best = 1e9f;
+      for (int r = 0; r < 3; ++r) {
+        t.start();
+        pattern_copy_hint<0, 0><<<n_tiles, 256>>>(in, tmp, n_tiles, 256, 4, (uint32_t)(n / 256), 1);
+        pattern_copy_hint<0, 0><<<n_tiles, 256>>>(tmp, out, n_tiles, 128, 5, (uint32_t)(n / 128), 1);
+        best = fminf(best, t.stop());
+      }
+      CK(cudaGetLastError());
+      printf("| whole array | 1 | full | none | %.3f | %.0f |\n", best, 64.0 * n / best * 1e-6);
+    }
+    cudaStream_t st[4];
+    cudaEvent_t fork, join[4];
+    CK(cudaEventCreateWithFlags(&fork, cudaEventDisableTiming));
+    for (int q = 0; q < 4; ++q) {
+      CK(cudaStreamCreateWithFlags(&st[q], cudaStreamNonBlocking));
+      CK(cudaEventCreateWithFlags(&join[q], cudaEventDisableTiming));
+    }
+    struct Case {
+      uint32_t gt;  // tiles per group
+      int ns, ring, hints;
+    };
+    // hints: 0 = none; else decimal digits (load 1, store 1, load 2, store 2), 0 none / 1 evict_first / 2 evict_last
+    const Case cases[] = {{512, 2, 0, 0},    {512, 2, 1, 0},    {512, 2, 1, 1211}, {512, 2, 1, 1221}, {512, 2, 1, 1201},
+                          {512, 2, 1, 1210}, {512, 2, 1, 210},  {512, 2, 1, 1200}, {512, 2, 0, 1211}, {256, 2, 0, 0},
+                          {256, 2, 1, 0},    {256, 2, 1, 1211}, {256, 3, 1, 1211}, {256, 3, 1, 1221}, {256, 3, 1, 1201},
+                          {128, 4, 1, 1211}, {768, 2, 1, 1211}, {1024, 2, 1, 1211}, {256, 1, 1, 1211}};
+    for (const Case& c : cases) {
+      float best = 1e9f;
+      for (int r = 0; r < 3; ++r) {
+        t.start();
+        CK(cudaEventRecord(fork, 0));
+        for (int q = 0; q < c.ns; ++q) CK(cudaStreamWaitEvent(st[q], fork, 0));
+        uint32_t g = 0;
+        for (uint32_t t0 = 0; t0 < n_tiles; t0 += c.gt, ++g) {
+          const uint32_t gt = n_tiles - t0 < c.gt ? n_tiles - t0 : c.gt;
+          const int q = g % c.ns;
+          const uint64_t recs = (uint64_t)gt * kTileRecs;
+          const uint4* gin = in + (uint64_t)t0 * kTileRecs;
+          uint4* gtmp = c.ring ? tmp + (uint64_t)q * ((uint64_t)c.gt * kTileRecs + 4096) : tmp + (uint64_t)t0 * kTileRecs;
+          uint4* gout = out + (uint64_t)t0 * kTileRecs;
+          const uint32_t r1 = (uint32_t)(recs / 256), r2 = (uint32_t)(recs / 128);
+#define NC_P1(L, S) pattern_copy_hint<L, S><<<gt, 256, 0, st[q]>>>(gin, gtmp, gt, 256, 4, r1, 1)
+#define NC_P2(L, S) pattern_copy_hint<L, S><<<gt, 256, 0, st[q]>>>(gtmp, gout, gt, 128, 5, r2, 1)
+          switch (c.hints / 100) {
+            case 12: NC_P1(1, 2); break;
+            case 2: NC_P1(0, 2); break;
+            default: NC_P1(0, 0); break;
+          }
+          switch (c.hints % 100) {
+            case 11: NC_P2(1, 1); break;
+            case 21: NC_P2(2, 1); break;
+            case 1: NC_P2(0, 1); break;
+            case 10: NC_P2(1, 0); break;
+            default: NC_P2(0, 0); break;
+          }
+#undef NC_P1
+#undef NC_P2
+        }
+        for (int q = 0; q < c.ns; ++q) {
+          CK(cudaEventRecord(join[q], st[q]));
+          CK(cudaStreamWaitEvent(0, join[q], 0));
+        }
+        best = fminf(best, t.stop());
+      }
+      CK(cudaGetLastError());
+      const char* hn[] = {"none", "evict_first", "evict_last"};
+      printf("| %u | %d | %s | %s, %s, %s, %s | %.3f | %.0f |\n", c.gt / 16, c.ns, c.ring ? "ring" : "full", hn[c.hints / 1000],
+             hn[c.hints / 100 % 10], hn[c.hints / 10 % 10], hn[c.hints % 10], best, 64.0 * n / best * 1e-6);
+    }
+    for (int q = 0; q < 4; ++q) {
+      cudaStreamDestroy(st[q]);
+      cudaEventDestroy(join[q]);
+    }
+    cudaEventDestroy(fork);
+    cudaFree(in);
+    cudaFree(tmp);
     cudaFree(out);
   }
 

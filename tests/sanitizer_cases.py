@@ -4,7 +4,7 @@
     compute-sanitizer --tool racecheck python tests/sanitizer_cases.py
     compute-sanitizer --tool synccheck python tests/sanitizer_cases.py
 
-configs[0] and scaled configs[1] rules through every organisation variant (default, pairs, single-pass look-back, bulk-fed,
+configs[0] and scaled configs[1] rules through every organisation variant (default, pairs, single-pass look-back, bulk-fed, bucket-first,
 both COPASS modes) with the usual element-by-element comparison against the oracle, then spike delivery in its fused
 (cooperative) and two-kernel forms.  Exit code 0 = every parity check held; the sanitizer's own report says whether it saw
 a hazard.  profiles/r02_sanitizer.md holds the outcome.  Not collected by pytest (no test_ prefix)."""
@@ -25,7 +25,7 @@ def main():
     assert torch.cuda.is_available()
     which = sys.argv[1] if len(sys.argv) > 1 else "all"
     variants = {"default": 0, "pairs": binding.FLAG_SORT_PAIRS, "onesweep": binding.FLAG_SORT_ONESWEEP,
-                "bulk": binding.FLAG_SORT_BULK, "copass": binding.FLAG_ORGANISE_COPASS,
+                "bulk": binding.FLAG_SORT_BULK, "buckets": binding.FLAG_SORT_BUCKETS, "copass": binding.FLAG_ORGANISE_COPASS,
                 "copass_shift": binding.FLAG_ORGANISE_COPASS | binding.FLAG_COPASS_SHIFT}
     if which in ("all", "organise"):
         nets = [(WL.config0_tiny(), 0), (WL.config0_tiny(), 64), (WL.config0_tiny(), 10)]

@@ -2,7 +2,8 @@
 (gpurun_out/membench.txt).  They are the measurements behind two bounds DESIGN.md states:
   * the ceiling of a digit pass's write pattern (runs of 16-byte records that start inside a 32-byte sector) against an
     aligned copy -- section 6.3;
-  * the issue cost of the Philox multiplies -- section 6.1.
+  * the issue cost of the Philox multiplies -- section 6.1;
+  * what keeping a pass's intermediate array in the L2 can gain (section `ring`) -- section 6.3, bucket-first organisation.
 Assertions are deliberately loose (they check that the tables exist and say what DESIGN.md relies on, not absolute rates)."""
 import re
 import subprocess
@@ -50,6 +51,17 @@ def test_write_pattern_ceiling(membench):
     # pieces that start inside a sector cost bandwidth: this is the pattern a scatter pass of 16-byte records writes
     assert sector_split < 0.9 * aligned, out
     assert rows[(256, 256, 32, 1)] > sector_split, out
+
+
+def test_l2_resident_intermediate(membench):
+    """Two passes with the intermediate array kept in the L2 group by group against two whole-array passes (DESIGN.md 6.3,
+    bucket-first organisation): the memory system alone gains from it."""
+    out = _run(membench, "ring")
+    rows = [l for l in out.splitlines() if l.startswith("|") and ("ring" in l or "full" in l) and not l.startswith("| group")]
+    ms = lambda l: float(l.strip("|").split("|")[-2])
+    whole = ms([l for l in rows if l.startswith("| whole array")][0])
+    best_ring = min(ms(l) for l in rows if "| ring |" in l)
+    assert best_ring < 0.85 * whole, out
 
 
 def test_bulk_copy_path(membench):

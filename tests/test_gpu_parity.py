@@ -107,6 +107,56 @@ def test_bulk_fed_persistent_variant_parity(nc_mod, oracle_mod):
         assert rep["n"] >= 1000
 
 
+def test_bucket_first_variant_parity(nc_mod, oracle_mod, monkeypatch):
+    """NC_FLAG_SORT_BUCKETS (nc_sort_msd.cuh): one pass into <= 256 buckets of consecutive sources, then every bucket sorted on
+    its own with its intermediate records in an L2-resident slot.  Same connections, permutation and index as the oracle:
+    several storage blocks, odd B (scalar first pass), tiny networks (most buckets empty, N < 256), one, two and three
+    in-bucket passes, the persistent kernel and the per-bucket launches over 1 - 4 CUDA streams, one bucket that holds
+    everything."""
+    for net, B in ((WL.config2_microcircuit(scale=0.06), 0), (WL.config1_rule("fixed_indegree", scale=0.2), 1 << 16),
+                   (WL.config1_rule("fixed_total_number", scale=0.05), 100_003), (WL.config0_tiny(), 64),
+                   (WL.config1_rule("pairwise_bernoulli", scale=0.1), 0)):
+        for lanes in (None, "1", "2", "3", "4"):  # None: the persistent kernel where it applies (two in-bucket passes)
+            if lanes is None:
+                monkeypatch.delenv("NC_BUCKET_LANES", raising=False)
+            else:
+                monkeypatch.setenv("NC_BUCKET_LANES", lanes)
+            rep, _ = PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_BUCKETS, B=B)
+            assert rep["n"] >= 1000
+    monkeypatch.delenv("NC_BUCKET_LANES")
+    # 16 nodes, delays up to 15 steps: 4 delay bits + 1 -> one in-bucket pass
+    net = WL.Network("narrow", [16])
+    net.projections = [WL.Projection(0, 0, "fixed_total_number", degree_or_total=100_000, weight=W,
+                                     delay_ms=(0.5, 0.3, 0.1, 1.5), seed=8)]
+    o, g = PU.build_both(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_BUCKETS)
+    assert g.stats()["sort_passes"] == 2
+    g.close(); o.close()
+    PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_BUCKETS)
+    # 3,000,000 nodes x delays up to 2^9 steps: 14 source bits left in a bucket + 10 delay bits -> three in-bucket passes
+    net = WL.Network("wide", [3_000_000])
+    net.projections = [WL.Projection(0, 0, "fixed_total_number", degree_or_total=1_500_000, weight=W,
+                                     delay_ms=(20.0, 15.0, 0.1, 51.0), seed=11)]
+    o, g = PU.build_both(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_BUCKETS)
+    assert g.stats()["sort_passes"] == 4
+    g.close(); o.close()
+    PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_BUCKETS)
+    # every connection from 3 neighbouring sources of 100,000: one bucket holds everything
+    net = WL.Network("one_bucket", [100_000])
+    net.projections = [WL.Projection(0, 0, "fixed_total_number", degree_or_total=2000, weight=W, delay_ms=(1.5, 0.75, 0.1, 4.0), seed=3)]
+    o = oracle_mod.Oracle(dt_ms=net.dt_ms)
+    g = nc_mod.NC(dt_ms=net.dt_ms, flags=nc_mod.FLAG_SORT_BUCKETS)
+    for b in (o, g):
+        b.create_population(100_000)
+        b.connect((0, 100_000), (0, 100_000), WL.RULE_IDS["fixed_total_number"], degree_or_total=2000, weight=(1.0, 0.0, 0.0, float("inf")),
+                  delay_ms=(1.5, 0.75, 0.1, 4.0), seed=3)
+        b.connect((5000, 3), (0, 100_000), WL.RULE_IDS["all_to_all"], weight=(1.0, 0.0, 0.0, float("inf")),
+                  delay_ms=(1.5, 0.75, 0.1, 4.0), seed=4)
+        b.finalize()
+    PU.compare_connections(g.read_connections(sorted=True), o.connections(sorted=True), 1.0, "one bucket")
+    PU.compare_index(g.read_index(), o.index(), "one bucket")
+    g.close(); o.close()
+
+
 def test_single_pass_key(nc_mod, oracle_mod):
     """<= 8 key bits: one digit pass that is both the first and the last (storage blocks -> final arrays)."""
     net = WL.Network("narrow", [16])

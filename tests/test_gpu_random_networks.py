@@ -82,7 +82,7 @@ def build(b, pops, calls):
         b.connect(src, tgt, rule, **kw)
 
 
-VARIANTS = ["default", "pairs", "onesweep", "bulk", "copass", "copass_shift"]
+VARIANTS = ["default", "pairs", "onesweep", "bulk", "buckets", "copass", "copass_shift"]
 
 
 @pytest.mark.parametrize("seed", range(24))
@@ -91,7 +91,7 @@ def test_random_network_all_variants(nc_mod, oracle_mod, seed):
     rng = np.random.default_rng(seed)
     B = int(rng.choice([0, 1 << 12, 1000, 4097, 257]))
     flags = {"default": 0, "pairs": nc_mod.FLAG_SORT_PAIRS, "onesweep": nc_mod.FLAG_SORT_ONESWEEP, "bulk": nc_mod.FLAG_SORT_BULK,
-             "copass": nc_mod.FLAG_ORGANISE_COPASS, "copass_shift": nc_mod.FLAG_ORGANISE_COPASS | nc_mod.FLAG_COPASS_SHIFT}
+             "buckets": nc_mod.FLAG_SORT_BUCKETS, "copass": nc_mod.FLAG_ORGANISE_COPASS, "copass_shift": nc_mod.FLAG_ORGANISE_COPASS | nc_mod.FLAG_COPASS_SHIFT}
     o = oracle_mod.Oracle(dt_ms=0.1, block_size=B)
     build(o, pops, calls)
     ou = o.connections(sorted=False)
