@@ -392,7 +392,9 @@ def main():
                 "launch_ms": pass_ms, "launches_per_step": passes,
                 "context": "peak is a streaming copy; the pass writes ~256-byte runs that start inside 32-byte sectors, and a "
                            "copy kernel with that write pattern and no ranking reaches 5050-5390 GB/s on a B200 "
-                           "(tests/cuda/membench.cu `pattern`, profiles/r02_scatter.md)"}
+                           "(tests/cuda/membench.cu `pattern`, profiles/r02_scatter.md); the SM side of the pass (7.9 us per "
+                           "tile of 4096 records, 296 tiles in flight) sits at the same rate even with the records in the L2 "
+                           "(profiles/r02_buckets.md)"}
     phases = {}
     for name, b in (("generate", BYTES["generate"]), ("histogram", BYTES["histogram"]), ("sort", BYTES["sort_pass"] * passes),
                     ("permute", BYTES["permute"]), ("index", BYTES["index"])):
