@@ -50,6 +50,28 @@ def test_struct_layouts_match_header():
     assert [int(v) for v in out] == want
 
 
+def test_constants_match_header():
+    """the binding's status codes, NC_FLAG_* bits and rule flags are the header's values (compiled by gcc)."""
+    import subprocess
+    import tempfile
+    from paper_2306_09855_b200 import binding as b
+    pairs = [("NC_OK", b.OK), ("NC_ERR_INVALID_ARG", b.ERR_INVALID_ARG), ("NC_ERR_STATE", b.ERR_STATE),
+             ("NC_ERR_CAPACITY", b.ERR_CAPACITY), ("NC_ERR_OOM", b.ERR_OOM), ("NC_ERR_CUDA", b.ERR_CUDA),
+             ("NC_FLAG_TIMING", b.FLAG_TIMING), ("NC_FLAG_EXACT_FP64", b.FLAG_EXACT_FP64), ("NC_FLAG_SORT_PAIRS", b.FLAG_SORT_PAIRS),
+             ("NC_FLAG_SORT_ONESWEEP", b.FLAG_SORT_ONESWEEP), ("NC_FLAG_ORGANISE_COPASS", b.FLAG_ORGANISE_COPASS),
+             ("NC_FLAG_COPASS_SHIFT", b.FLAG_COPASS_SHIFT), ("NC_FLAG_SORT_BULK", b.FLAG_SORT_BULK),
+             ("NC_FLAG_SORT_BUCKETS", b.FLAG_SORT_BUCKETS), ("NC_NO_AUTAPSES", b.NO_AUTAPSES), ("NC_NO_MULTAPSES", b.NO_MULTAPSES)]
+    header = re.sub(r"/\*.*?\*/", "", (ROOT / "include" / "nc.h").read_text(), flags=re.S)
+    declared = set(re.findall(r"\b(NC_FLAG_[A-Z_0-9]+)\s*=", header))
+    assert declared == {n for n, _ in pairs if n.startswith("NC_FLAG_")}, "a flag of nc.h has no constant in binding.py"
+    src = '#include "nc.h"\n#include <stdio.h>\nint main(){' + "".join(f'printf("%d\\n",(int){n});' for n, _ in pairs) + "return 0;}"
+    with tempfile.TemporaryDirectory() as d:
+        (Path(d) / "t.c").write_text(src)
+        subprocess.run(["gcc", "-I", str(ROOT / "include"), "-o", f"{d}/t", f"{d}/t.c"], check=True)
+        out = subprocess.run([f"{d}/t"], check=True, capture_output=True, text=True).stdout.split()
+    assert [int(v) for v in out] == [v for _, v in pairs]
+
+
 def test_no_cpu_fallback_without_gpu(lib):
     import torch
     if torch.cuda.is_available():
