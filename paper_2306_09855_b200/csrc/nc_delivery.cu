@@ -54,16 +54,8 @@ struct StepParams {
   uint32_t n_new, capacity, now;
 };
 
-// append `item` for the lanes with `want` set; returns false for the lanes that did not fit
-__device__ __forceinline__ uint32_t warp_reserve(uint32_t* counter, bool want) {
-  const uint32_t m = __ballot_sync(0xffffffffu, want);
-  uint32_t base = 0;
-  if (m && lane_id() == (uint32_t)(__ffs(m) - 1)) base = atomicAdd(counter, (uint32_t)__popc(m));
-  base = __shfl_sync(0xffffffffu, base, m ? __ffs(m) - 1 : 0);
-  return base + __popc(m & lanemask_lt());
-}
-
-// two reservations at once: both atomics are issued before either result is waited for
+// a slot for the lanes with want_a set and one for those with want_b set: two warp-aggregated reservations at once, both
+// atomics issued before either result is waited for
 __device__ __forceinline__ void warp_reserve2(uint32_t* counter_a, bool want_a, uint32_t* counter_b, bool want_b,
                                               uint32_t& slot_a, uint32_t& slot_b) {
   const uint32_t ma = __ballot_sync(0xffffffffu, want_a), mb = __ballot_sync(0xffffffffu, want_b);

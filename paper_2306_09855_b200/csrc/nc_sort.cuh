@@ -239,7 +239,7 @@ __global__ void __launch_bounds__(THREADS) onesweep_kernel(const __grid_constant
   constexpr int kTile = Smem::kTile;
   constexpr int kWarps = Smem::kWarps;
   static_assert(THREADS >= kRadix, "one thread per digit is needed for the look-back");
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
 
   const uint32_t warp = threadIdx.x >> 5, lane = lane_id();
@@ -407,7 +407,7 @@ __global__ void __launch_bounds__(THREADS, MIN_CTAS) onesweep_rec_kernel(const _
   constexpr int kTile = Smem::kTile;
   constexpr int kWarps = Smem::kWarps;
   static_assert(THREADS >= kRadix, "one thread per digit is needed for the look-back");
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
 
   const uint32_t warp = threadIdx.x >> 5, lane = lane_id();

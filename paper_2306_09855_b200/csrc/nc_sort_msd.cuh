@@ -310,7 +310,7 @@ __global__ void __launch_bounds__(kBsThreads, kBsCtas) bucket_sort_kernel(const 
   constexpr uint32_t kTile = Smem::kTile;
   static_assert(kTile == kBsTile && kSegChunkTiles * kRadix * 4 <= sizeof(Smem::recs), "the count histograms live in the record staging");
   constexpr uint32_t kNone = 0xffffffffu;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
   __shared__ ScatterParams sp;
   // the item being worked on and the one claimed ahead of it: segment (0 count 1, 1 scatter 1, 2 count 2, 3 scatter 2; kNone = no

@@ -482,7 +482,7 @@ __device__ __forceinline__ void scatter_tile(const ScatterParams& p, const uint3
 template <bool FIRST, bool LAST, int WARPS, int ITEMS, int MIN_CTAS, int MATCH, int MODE = 0>
 __global__ void __launch_bounds__(WARPS * 32, MIN_CTAS) scatter_pass_kernel(const __grid_constant__ ScatterParams p) {
   using Smem = ScatterSmem<WARPS, ITEMS, MATCH == kMatchSmem>;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   scatter_tile<FIRST, LAST, WARPS, ITEMS, MATCH, MODE, false>(p, blockIdx.x, *reinterpret_cast<Smem*>(smem_raw));
 }
 
