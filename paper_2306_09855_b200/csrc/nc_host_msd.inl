@@ -266,7 +266,8 @@ int sort_msd_and_index(nc_context* c) {
       int per_sm = 0, sms = 0;
       NC_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, kBsThreads, sizeof(BsSmem)));
       NC_CUDA(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device));
-      const uint32_t grid = std::min<uint32_t>(n_items, (uint32_t)std::max(1, per_sm) * (uint32_t)sms);
+      uint32_t grid = std::min<uint32_t>(n_items, (uint32_t)std::max(1, per_sm) * (uint32_t)sms);
+      if (const char* e = getenv("NC_BUCKET_GRID")) grid = std::max(1, std::min<int>(atoi(e), (int)grid));  // experiments
       // NC_BUCKET_DEBUG=1: thread 0 of every CTA reports where its cycles went (profiles/r02_buckets.md); waits for the kernel
       unsigned long long* d_prof = getenv("NC_BUCKET_DEBUG") ? (unsigned long long*)dev_alloc(c, (size_t)grid * 64) : nullptr;
       bp.prof = d_prof;

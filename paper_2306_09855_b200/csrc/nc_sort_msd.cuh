@@ -317,11 +317,15 @@ __global__ void __launch_bounds__(kBsThreads, kBsCtas) bucket_sort_kernel(const 
   // more work), bucket, index in the segment, whether everything it waits for had happened when it was claimed
   __shared__ uint32_t items[2][4];
   __shared__ uint32_t scratch[16];
+  __shared__ uint32_t s_bsize[kRadix], s_round_first[kRadix + 4];  // the tables thread 0 walks for every item (nb <= 256)
+  for (uint32_t i = threadIdx.x; i < p.nb; i += kBsThreads) s_bsize[i] = __ldg(p.bsize + i);
+  for (uint32_t i = threadIdx.x; i < p.nb + 4; i += kBsThreads) s_round_first[i] = __ldg(p.round_first + i);
+  __syncthreads();
   // thread 0 only
   uint32_t round = 0;            // tickets only grow
   uint32_t* pending = nullptr;   // counter of finished tiles to bump for the previous scatter item, once its stores are done
 
-  auto tiles_of = [&](uint32_t b) { return (__ldg(p.bsize + b) + kTile - 1) / kTile; };
+  auto tiles_of = [&](uint32_t b) { return (s_bsize[b] + kTile - 1) / kTile; };
   // what an item waits for: always items with smaller tickets
   auto deps = [&](uint32_t seg, uint32_t b, bool block) -> bool {
     uint32_t* sy = p.sync + (uint64_t)b * kBsSyncWords;
@@ -336,9 +340,13 @@ __global__ void __launch_bounds__(kBsThreads, kBsCtas) bucket_sort_kernel(const 
     if (seg == 1) addr[k] = sy + kBsReady1, want[k++] = 1u;
     if (seg == 2) addr[k] = sy + kBsTiles1, want[k++] = tiles_of(b);
     if (seg == 3) addr[k] = sy + kBsReady2, want[k++] = 1u;
-    for (uint32_t i = 0; i < k; ++i) {
-      if (block) wait_at_least(addr[i], want[i]);
-      else if (ld_acquire_u32(addr[i]) < want[i]) return false;
+    if (block) {
+      for (uint32_t i = 0; i < k; ++i) wait_at_least(addr[i], want[i]);
+    } else {
+      uint32_t have[2] = {0xffffffffu, 0xffffffffu};  // both loads in flight together
+      for (uint32_t i = 0; i < k; ++i) have[i] = ld_acquire_u32(addr[i]);
+      for (uint32_t i = 0; i < k; ++i)
+        if (have[i] < want[i]) return false;
     }
     return true;
   };
@@ -349,14 +357,14 @@ __global__ void __launch_bounds__(kBsThreads, kBsCtas) bucket_sort_kernel(const 
       pending = nullptr;
     }
   };
-  auto claim = [&](uint32_t* it) {
-    const uint32_t t = atomicAdd(p.ticket, 1u);
+  // claiming an item: the ticket is taken early (one atomic round trip), decoded and checked for what it waits for later
+  auto decode = [&](uint32_t t, uint32_t* it) {
     if (t >= p.n_items) {
       it[0] = kNone;
       return;
     }
-    while (t >= __ldg(p.round_first + round + 1)) ++round;
-    uint32_t o = t - __ldg(p.round_first + round), seg = 0, b = 0;
+    while (t >= s_round_first[round + 1]) ++round;
+    uint32_t o = t - s_round_first[round], seg = 0, b = 0;
     for (; seg < 4; ++seg) {
       if (round < seg || round - seg >= p.nb) continue;
       b = round - seg;
@@ -373,7 +381,7 @@ __global__ void __launch_bounds__(kBsThreads, kBsCtas) bucket_sort_kernel(const 
 
   unsigned long long pf[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   const long long t_start = clock64();
-  if (threadIdx.x == 0) claim(items[0]);
+  if (threadIdx.x == 0) decode(atomicAdd(p.ticket, 1u), items[0]);
   for (uint32_t iter = 0;; ++iter) {
     __syncthreads();  // the previous item is done with the shared memory; this item's description is there
     const uint32_t* it = items[iter & 1];
@@ -393,7 +401,7 @@ __global__ void __launch_bounds__(kBsThreads, kBsCtas) bucket_sort_kernel(const 
       if (seg & 1) {
         const uint32_t ps = seg >> 1, start = __ldg(p.bstart + b);
         sp.delay_bits = p.delay_bits;
-        sp.n = __ldg(p.bsize + b);
+        sp.n = s_bsize[b];
         sp.recs_in = ps == 0 ? p.recs + start : p.slot[slot];
         sp.recs_out = p.slot[slot];
         sp.dig_out = p.slot_dig[slot];
@@ -412,11 +420,15 @@ __global__ void __launch_bounds__(kBsThreads, kBsCtas) bucket_sort_kernel(const 
       }
     }
     __syncthreads();
-    // behind the loads of this item: signal the previous one, claim the next one
+    // the next item's ticket: asked for now, looked at in the hook
+    uint32_t next_ticket = 0;
+    if (threadIdx.x == 0) next_ticket = atomicAdd(p.ticket, 1u);
+    // between the ranking and the stores of this item (this thread's loads are back, so the fence costs nothing): signal the
+    // previous item, whose stores were issued a whole tile ago, and work out the next one
     auto hook = [&]() {
       if (threadIdx.x == 0) {
         flush();
-        claim(next);
+        decode(next_ticket, next);
       }
     };
     const long long t_item = clock64();
@@ -428,7 +440,7 @@ __global__ void __launch_bounds__(kBsThreads, kBsCtas) bucket_sort_kernel(const 
       pf[2] += clock64() - t_item;
     } else {
       hook();
-      const uint32_t ps = seg >> 1, n = __ldg(p.bsize + b);
+      const uint32_t ps = seg >> 1, n = s_bsize[b];
       const uint32_t tiles = (n + kTile - 1) / kTile, chunks = (tiles + kSegChunkTiles - 1) / kSegChunkTiles;
       const uint8_t* dig = ps == 0 ? p.dig + __ldg(p.bstart + b) : p.slot_dig[slot];
       bucket_count_chunk(dig, n, idx, chunks, p.counts[ps][slot], p.chunk_base[ps][slot], sy + (ps == 0 ? kBsCount1 : kBsCount2),

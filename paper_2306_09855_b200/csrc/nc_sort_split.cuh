@@ -287,7 +287,7 @@ struct NoHook {
 template <bool FIRST, bool LAST, int WARPS, int ITEMS, int MATCH, int MODE, bool COHERENT, typename Hook = NoHook,
           bool ATOMIC_RANK = false>
 __device__ __forceinline__ void scatter_tile(const ScatterParams& p, const uint32_t tile,
-                                             ScatterSmem<WARPS, ITEMS, MATCH == kMatchSmem>& sm, Hook hook = Hook()) {
+                                             ScatterSmem<WARPS, ITEMS, MATCH == kMatchSmem>& sm, Hook late_hook = Hook()) {
   using Smem = ScatterSmem<WARPS, ITEMS, MATCH == kMatchSmem>;
   static_assert(MODE == 0 || (MODE == 1 && FIRST && !LAST) || (MODE >= 2 && !FIRST), "bucket pass: from the blocks; in-bucket: records");
   // in-bucket passes: what comes from HBM is read once (evict_first), what goes to the slot the next pass reads stays
@@ -381,7 +381,6 @@ __device__ __forceinline__ void scatter_tile(const ScatterParams& p, const uint3
     }
   }
   __syncthreads();  // the counters are zero
-  hook();           // (persistent kernel: bookkeeping of one thread, behind the record loads that are in flight now)
   // ---- per-warp digit histogram with fire-and-forget shared-memory atomics ----
 #pragma unroll
   for (int i = 0; i < ITEMS; ++i) atomicAdd(&my_hist[pass_digit<MODE>(rec[i].x, p, mask)], 1u);
@@ -443,6 +442,7 @@ __device__ __forceinline__ void scatter_tile(const ScatterParams& p, const uint3
 
   if (LAST) {
     __syncthreads();
+    late_hook();  // (persistent kernel: bookkeeping of one thread; its loads have returned, the stores are not issued yet)
     // ---- final arrays: consecutive threads write consecutive records of a digit run ----
     const uint32_t dmask = (1u << p.delay_bits) - 1u;
 #pragma unroll
@@ -460,6 +460,7 @@ __device__ __forceinline__ void scatter_tile(const ScatterParams& p, const uint3
     }
   } else {
     __syncthreads();
+    late_hook();
     // ---- records and the next pass's digit of each: consecutive threads write consecutive records of a run.
     //      (One TMA bulk copy per run was measured slower: the 32 copies a warp issues are serialised.) ----
     const uint32_t next_mask = (1u << p.next_bits) - 1u;
