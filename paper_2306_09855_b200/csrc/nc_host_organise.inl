@@ -273,10 +273,13 @@ int sort_carry_and_index(nc_context* c, const PassPlan& plan) {
 
 // Default organisation step for keys of <= 32 bits (nc_sort_split.cuh): per digit pass, per-tile digit counts ->
 // scan -> scatter of whole connections; the last pass writes the sorted SoA arrays; then the index.
+// Launch shapes of the scatter pass, NC_SPLIT_VARIANT=k in the environment (measured on B200): 0 the default,
+// 2 CTAs x 8 warps x 16 records; 1 three CTAs x 12 warps x 8 records (tiles of 3072); 2 one CTA x 16 warps x 16 records (tiles of
+// 8192: 512-byte runs, but one CTA's phases do not overlap).
 struct SplitShape {
   int warps, items;
 };
-constexpr SplitShape kSplitShapes[] = {{8, 16}, {12, 8}};
+constexpr SplitShape kSplitShapes[] = {{8, 16}, {12, 8}, {16, 16}};
 
 int split_variant() {
   const char* e = getenv("NC_SPLIT_VARIANT");
@@ -303,6 +306,7 @@ template <bool FIRST, bool LAST>
 int launch_scatter_pass(nc_context* c, const ScatterParams& sp, uint32_t n_tiles, int variant) {
   switch (variant) {
     case 1: return launch_scatter_shape<FIRST, LAST, 12, 8, 3>(c, sp, n_tiles);
+    case 2: return launch_scatter_shape<FIRST, LAST, 16, 16, 1>(c, sp, n_tiles);
     default: return launch_scatter_shape<FIRST, LAST, 8, 16, 2>(c, sp, n_tiles);
   }
 }
