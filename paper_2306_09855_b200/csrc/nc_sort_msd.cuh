@@ -15,7 +15,7 @@
 //            HBM traffic per connection if the slots never left the L2: 14 + 16 + 1 (pass A) and 16 + 1 + 18 (pass B) = 66 B
 //            instead of 102 B for three whole-array passes.
 //
-// MEASURED (B200, configs[2], profiles/r02_buckets.md): it loses.  Organisation takes 8.4 ms against 6.7 ms for the default
+// MEASURED (B200, configs[2], profiles/r02_buckets.md): it loses.  Organisation takes 8.5 ms against 6.7 ms for the default
 // path.  tests/cuda/membench.cu, section `ring`, shows that the MEMORY SYSTEM gains from the arrangement (two passes as plain
 // copies: 3.43 ms whole-array, 2.29 ms with the intermediate in L2 slots), but a tile of scatter_pass_kernel costs 8.8 us of
 // SM time with its records in the L2 and 7.9 us with them in HBM: the pass is bound by the SM's shared-memory pipe (ranking and
