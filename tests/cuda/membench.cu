@@ -344,7 +344,7 @@ int main(int argc, char** argv) {
       const Case cases[] = {{4, 256, 0, 1}, {4, 256, 2, 1}, {4, 256, 4, 1}, {4, 256, 1, 1}, {4, 256, 3, 1}, {4, 16, 1, 1},
                             {4, 64, 1, 1},  {4, 128, 1, 1}, {5, 128, 0, 1}, {5, 128, 1, 1}, {6, 64, 0, 1},  {6, 64, 1, 1},
                             {3, 256, 0, 1}, {3, 256, 1, 1}, {4, 256, 1, 2}, {4, 256, 1, 4}, {4, 256, 1, 16},
-                            {4, 256, 2, 8}, {4, 256, 0, 8}};
+                            {4, 256, 2, 8}, {4, 256, 0, 8}, {0, 256, 0, 1}, {1, 256, 0, 1}, {2, 256, 1, 1}};
       for (const Case& c : cases) {
         float best = 1e9f;
         for (int r = 0; r < 4; ++r) {
