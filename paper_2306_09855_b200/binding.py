@@ -38,6 +38,8 @@ SYMBOLS = (
     "nc_delivery_counts", "nc_delivery_num_ports", "nc_delivery_run",
     # include/nc_copass.h
     "nc_copass_partition", "nc_get_copass_stats",
+    # include/nc_static.h
+    "nc_index_static",
 )
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_void_p, C.c_size_t)
@@ -153,6 +155,8 @@ def load_library():
     L.nc_delivery_step.argtypes = [vp, vp, vp, C.c_uint32, vp]
     L.nc_delivery_read_spike_array.argtypes = [vp, vp, vp, C.c_uint32, P(C.c_uint32)]
     L.nc_delivery_counts.argtypes = [vp, P(C.c_uint64), P(C.c_uint64), P(C.c_uint64), P(C.c_uint64)]
+    L.nc_index_static.argtypes = [vp, vp, C.c_uint64, C.c_uint32, vp, vp, vp, vp, vp, C.c_uint64, vp, vp, vp, C.c_char_p,
+                                  C.c_size_t]
     for name in SYMBOLS:
         if name != "nc_last_error":
             getattr(L, name).restype = C.c_int
@@ -168,6 +172,29 @@ class NCError(RuntimeError):
 
 def _ptr(a):
     return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+INDEX_STATIC_MAX_CONNECTIONS = 1 << 30  # NC_INDEX_STATIC_MAX_CONNECTIONS (include/nc_static.h)
+INDEX_STATIC_LOOKBACK, INDEX_STATIC_GROUPS = 1, 2
+
+
+def index_static(d_source, d_delay, n, n_nodes, d_src_offsets, d_group_ptr, d_group_count, d_group_start, d_group_delay,
+                 group_capacity, d_total_groups, d_error, stream=None):
+    """nc_index_static (include/nc_static.h): the group index over organised connections, built without any device
+    allocation -- for callers that cannot allocate where they need it (a loop with a latency budget, a process whose own
+    pool already owns the whole card).  The scratch is an array inside the library image, shared by all calls on a
+    device: calls that overlap on the GPU race.  Every d_* argument is a raw device address (int; tensor.data_ptr()) or
+    None where the header allows NULL; the caller owns those buffers.  The work is enqueued on `stream` (a torch stream;
+    default: the current one) of the current device and not waited for.  Raises NCError with the library's message,
+    e.g. ERR_CAPACITY for n > INDEX_STATIC_MAX_CONNECTIONS."""
+    import torch
+    L = load_library()
+    s = stream if stream is not None else torch.cuda.current_stream()
+    msg = C.create_string_buffer(512)
+    rc = L.nc_index_static(d_source, d_delay, int(n), int(n_nodes), d_src_offsets, d_group_ptr, d_group_count, d_group_start,
+                           d_group_delay, int(group_capacity), d_total_groups, d_error, s.cuda_stream, msg, 512)
+    if rc != 0:
+        raise NCError(rc, msg.value.decode())
 
 
 def _host_buffer(n, dtype):
