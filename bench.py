@@ -31,20 +31,33 @@ UNIT = "synapses/s"
 BYTES = {"generate": 14, "histogram": 8, "sort_pass": 32, "permute": 26, "index": 12}
 
 
+TRAFFIC_FILE = os.path.join("profiles", "r03_scatter_traffic.txt")
+KERNEL_FILE = os.path.join("paper_2306_09855_b200", "csrc", "nc_sort_split.cuh")
+
+
+def kernel_file_sha256():
+    import hashlib
+    return hashlib.sha256(open(os.path.join(ROOT, KERNEL_FILE), "rb").read()).hexdigest()
+
+
 def ncu_traffic_per_launch():
-    """(dram__bytes_read.sum + dram__bytes_write.sum of one middle scatter pass, where it was captured) from the committed
-    ncu --set full capture.  The figure is a property of the kernel source at that commit, so the file names the commit and
-    the bench line repeats it: a reader can see at once whether the kernel has changed since."""
-    out, where = None, None
+    """(dram__bytes_read.sum + dram__bytes_write.sum of one middle scatter pass, where it was captured, stale?) from the
+    committed ncu --set full capture.  The figure is a property of the kernel source: the file records the SHA-256 of
+    nc_sort_split.cuh as it was when ncu ran, and the figure is only reported while the shipped file still has that hash
+    (the GPU box has no .git, so a content hash and not a commit id); otherwise traffic is null and traffic_stale true."""
+    out, where, sha = None, None, None
     try:
-        for line in open(os.path.join(ROOT, "profiles", "r02_scatter_traffic.txt")):
+        for line in open(os.path.join(ROOT, TRAFFIC_FILE)):
             if line.startswith("traffic_bytes_per_launch"):
                 out = float(line.split("=")[1])
             if line.startswith("captured_at"):
                 where = line.split("=", 1)[1].strip()
+            if line.startswith("kernel_file_sha256"):
+                sha = line.split("=", 1)[1].strip()
     except Exception:
         pass
-    return out, where
+    stale = out is None or sha is None or sha != kernel_file_sha256()
+    return (None if stale else out), where, stale
 
 
 def workload(name: str):
@@ -383,11 +396,12 @@ def main():
         passes = 2 * P
     elif pass_ms:
         ach = BYTES["sort_pass"] * n_syn / (pass_ms * 1e-3) / 1e9
+        # the ncu figure belongs to the default path on configs[2]; stale = the kernel file changed since it was captured
+        traffic = ncu_traffic_per_launch() if args.workload == "c2" and not args.flags else (None, None, None)
         roof = {"bound": "hbm", "kernel": "scatter_pass_kernel (one digit pass carrying the whole connection: 16 B read + "
                                           "16 B written per synapse)",
                 "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": ncu_traffic_per_launch()[0] if args.workload == "c2" and not args.flags else None,
-                "traffic_captured_at": ncu_traffic_per_launch()[1] if args.workload == "c2" and not args.flags else None,
+                "traffic": traffic[0], "traffic_captured_at": traffic[1], "traffic_stale": traffic[2],
                 "peak_kind": peak_kind,
                 "launch_ms": pass_ms, "launches_per_step": passes,
                 "context": "peak is a streaming copy; the pass writes ~256-byte runs that start inside 32-byte sectors, and a "
@@ -419,7 +433,7 @@ def main():
             "alg_bytes_per_record_moved": 32, "GBps": round(gbs, 1), "frac_of_measured_peak": round(gbs / peak, 4)}
     cpu = None
     if not args.no_cpu_baseline and args.workload.startswith("c2"):
-        scale = args.sample_scale if args.sample_scale else 0.5
+        scale = args.sample_scale if args.sample_scale else 1.0  # the bench's own inputs: all of configs[2] (~90 s on one core)
         snet, sn, st = cpu_oracle_sample(scale)
         cpu = {"value": sn / st[0], "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": f"configs[2] with populations scaled x{scale:g}: {snet.n_nodes} nodes, {sn} synapses, generate+sort+index, {st[0]:.1f} s",
@@ -436,7 +450,9 @@ def main():
                                f"{net.n_nodes} nodes, {len(net.projections)} fixed_total_number projections, seed 7"
                    if args.workload == "c2" else net.name,
                    "synapses_per_step": n_syn,
-                   "parallelism": (f"one network in {world} shards by target node (nc_set_shard), no data-path collective"
+                   "parallelism": (f"one network in {world} shards by target node (nc_set_shard), no data-path collective; every "
+                                   "rank generates the FULL call of the random-target rules and filters it (redundant generation: "
+                                   "that part does not shrink with the number of ranks); never measured on more than one GPU"
                                    if args.sharded else "replicas only (one independent network per GPU)"),
                    "l2": "every step regenerates and re-sorts its own 4.2 GB of connections (>> 126 MB L2); no input is reused",
                    "key_bits": stats.get("key_bits"), "sort_passes": stats.get("sort_passes"), "flags": flags,

@@ -124,6 +124,14 @@ def test_golden_misc_vectors(oracle_mod):
             o = oracle_mod.eval_synapse((0, 20683), (0, 20683), oracle_mod.FIXED_TOTAL_NUMBER, 3, 0.0,
                                         (1, 0, -INF, INF), (1, 0, -INF, INF), 7, 0, 0.1, i)
             assert (o["source"], o["target"]) == (s, t)
+        elif r[0] == "fod":  # pins which Philox word fixed_outdegree takes its target from (oracle.cpp, Eqs. 8-9)
+            i, w0, w1, s, t, t_w0 = int(r[1]), int(r[2], 16), int(r[3], 16), int(r[4]), int(r[5]), int(r[6])
+            words = oracle_mod.philox4x32_10((i, 0, 0, 0), (42, 0))
+            assert words[0] == w0 and words[1] == w1
+            assert (w1 * 8000) >> 32 == t and (w0 * 8000) >> 32 == t_w0 and t != t_w0  # the file is consistent with itself
+            o = oracle_mod.eval_synapse((0, 8000), (0, 8000), oracle_mod.FIXED_OUTDEGREE, 1000, 0.0,
+                                        (1, 0, -INF, INF), (1, 0, -INF, INF), 42, 0, 0.1, i)
+            assert (o["source"], o["target"]) == (s, t)
         elif r[0] == "bern_T":
             assert oracle_mod.bernoulli_threshold(0.1) == int(r[1], 16)
         elif r[0] == "bern_words_idx2":
