@@ -45,7 +45,7 @@ typedef enum {
 } nc_status;
 
 /* Connection rules: Eqs. 4-13, names as in Senk et al. 2022.
- * Autapses and multapses are always allowed. */
+ * Autapses and multapses are allowed unless nc_set_rule_flags prohibits them. */
 typedef enum {
   NC_ONE_TO_ONE = 0,         /* Eqs. 4-5:   s = s0 + i,            t = t0 + i            N = N_src = N_tgt */
   NC_ALL_TO_ALL = 1,         /* Eqs. 6-7:   s = s0 + i / N_tgt,    t = t0 + i % N_tgt    N = N_src N_tgt  */
@@ -259,9 +259,14 @@ int nc_set_rule_flags(nc_context* ctx, uint32_t flags);
  * run over what was kept, so perm refers to the shard's own creation positions.  One process per GPU builds one shard;
  * the shards of a partition of the nodes together hold every connection of the unsharded network exactly once, each in the
  * unsharded order (creation order and organised order), without any exchange between ranks: a rank draws the random
- * numbers of the connections it does not own as well and skips them (owner-computes with redundant generation).  A call
- * is staged in full on the device first (14 B per connection of the FULL call, released afterwards) and waits for the
- * owned count.  To be called before the first nc_connect*; node ids outside the created nodes own nothing. ---- */
+ * numbers of the connections it does not own as well and skips them (owner-computes with redundant generation; only
+ * one_to_one, fixed_indegree and all_to_all over a target range generate just the owned connections -- an index sub-range,
+ * or for all_to_all the owned target columns of every source -- without flags or value arrays).  Any other call is staged in
+ * full on the device first, 14 B per connection of the FULL call, in staging blocks that are reused from call to call and
+ * released by nc_finalize; staged calls are filtered in batches (after 2^28 staged connections, before a call that would
+ * not fit behind them, and by every query), which waits for the owned count.  Generation time, filter time and staging
+ * memory of such calls therefore do not shrink with the number of shards.  To be called before the first nc_connect*;
+ * first + count <= 2^32 (NC_ERR_INVALID_ARG); node ids outside the created nodes own nothing. ---- */
 int nc_set_shard(nc_context* ctx, uint32_t first, uint32_t count);
 
 /* The same with explicit node arrays ("If the indexes of source or target nodes are not consecutive but
@@ -295,8 +300,8 @@ int nc_connect_values(nc_context* ctx, const uint32_t* src_nodes, uint32_t n_src
  * the following nc_connect* calls create.  Both are constants of a projection, so the library keeps them per
  * projection instead of per connection; nc_read_connection_attributes resolves entries first .. first+count-1 of
  * either view through their creation positions and copies them to HOST arrays (either may be NULL; synchronises).
- * The library stores and returns them, nothing more: synapses are static and spike delivery (nc_delivery.h) has one
- * input per node. ---- */
+ * The library stores and returns them; synapses are static, and spike delivery (nc_delivery.h) adds a connection's weight
+ * to input [port * n_nodes + target], one fp32 accumulator per (receptor port, node), 1 + the largest port in use ports. ---- */
 int nc_set_connection_attributes(nc_context* ctx, uint8_t port, uint8_t syn_group);
 int nc_read_connection_attributes(nc_context* ctx, int sorted, uint64_t first, uint64_t count, uint8_t* port,
                                   uint8_t* syn_group);

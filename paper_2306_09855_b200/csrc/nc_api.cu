@@ -99,7 +99,7 @@ struct nc_context {
   bool broken = false;  // an in-place organisation failed half way: the connections are lost, only nc_destroy is left
 
   // allocations
-  int atomic_rank = -1;         // NC_FLAG_SORT_BULK: -1 not checked yet, 1 ranks from returning shared atomics are usable, 0 ballots
+  int atomic_rank = -1;         // NC_FLAG_SORT_BULK / _BUCKETS: -1 not decided yet, 0 ranks from ballots (default), 1 from returning shared atomics (NC_ATOMIC_RANK=1 and the device check passed)
   int attached = 0;             // delivery objects that allocate from this context (nc_destroy refuses while any exists)
   bool guard = false;           // NC_GUARD=1: every allocation sits between two 256-byte guard zones checked when it is freed
   uint64_t guard_violations = 0;

@@ -17,7 +17,8 @@ enum Rule : int {
   kFixedIndegree = 2,
   kFixedOutdegree = 3,
   kFixedTotalNumber = 4,
-  kPairwiseBernoulli = 5
+  kPairwiseBernoulli = 5,
+  kAllToAllSub = 6  // all_to_all restricted to a strip of target columns (a shard's owned targets, nc_set_shard): internal
 };
 
 // Constants of one projection's weight and delay transforms (D7, D8).
@@ -50,6 +51,10 @@ struct GenParams {
   SynConst syn;
   uint32_t i_first;    // i_newconns of the first connection this launch creates (a shard generates a sub-range of a call's
                        // indexes, nc_set_shard); 0 for a whole call
+  // kAllToAllSub: the launch creates, source by source, only target columns sub_off .. sub_off + sub_w - 1 of the call's
+  // N_src x N_tgt grid (div = sub_w).  Local index j -> row j / sub_w, column sub_off + j % sub_w; the connection keeps the
+  // index of the FULL call, i = row * n_tgt + column, for its random numbers (reading S1).
+  uint32_t sub_w, sub_off;
 };
 
 // Weight and delay on the fp64 path: D5, D6, D7, D8 evaluated in the order the readings state, with explicit
@@ -182,6 +187,9 @@ __device__ __forceinline__ void rule_coords(const GenParams& p, uint32_t i, uint
   } else if (RULE == kAllToAll) {  // Eqs. 6-7
     s = p.s0 + quo;
     t = p.t0 + rem;
+  } else if (RULE == kAllToAllSub) {  // Eqs. 6-7 over the owned strip of columns
+    s = p.s0 + quo;
+    t = p.t0 + p.sub_off + rem;
   } else if (RULE == kFixedOutdegree) {  // Eqs. 8-9
     s = p.s0 + quo;
     t = p.t0 + bounded(wy, p.n_tgt);
@@ -197,10 +205,17 @@ __device__ __forceinline__ void rule_coords(const GenParams& p, uint32_t i, uint
 template <int RULE>
 __device__ __forceinline__ void split_index(const GenParams& p, uint32_t i, uint32_t& quo, uint32_t& rem) {
   quo = rem = 0;
-  if (RULE == kAllToAll || RULE == kFixedIndegree || RULE == kFixedOutdegree) {
+  if (RULE == kAllToAll || RULE == kAllToAllSub || RULE == kFixedIndegree || RULE == kFixedOutdegree) {
     quo = p.div == 1 ? i : div_magic(i, p.div_magic);
     rem = i - quo * p.div;
   }
+}
+
+// Index of the connection in its (full) connect call, which keys its random numbers: the launch's own index except for a
+// strip of all_to_all columns.
+template <int RULE>
+__device__ __forceinline__ uint32_t philox_index(const GenParams& p, uint32_t i, uint32_t quo, uint32_t rem) {
+  return RULE == kAllToAllSub ? quo * p.n_tgt + p.sub_off + rem : i;
 }
 
 // Redo synapse i of the projection in fp64 and overwrite its weight and delay at creation position pos.
@@ -246,10 +261,10 @@ __global__ void __launch_bounds__(kGenThreads) generate_kernel(const __grid_cons
       bool series = false;
 #pragma unroll
       for (int e = 0; e < 4; ++e) {
-        const Philox4 rnd = philox_stream<true>(i0 + e, 0u, p.rng);
+        const Philox4 rnd = philox_stream<true>(philox_index<RULE>(p, i0 + e, quo, rem), 0u, p.rng);
         rule_coords<RULE>(p, i0 + e, quo, rem, rnd.x, rnd.y, src[e], tgt[e]);
         if (ARR) map_nodes(p, src[e], tgt[e]);
-        if (RULE == kAllToAll || RULE == kFixedIndegree || RULE == kFixedOutdegree) {
+        if (RULE == kAllToAll || RULE == kAllToAllSub || RULE == kFixedIndegree || RULE == kFixedOutdegree) {
           if (++rem == p.div) {
             rem = 0;
             ++quo;
@@ -277,7 +292,13 @@ __global__ void __launch_bounds__(kGenThreads) generate_kernel(const __grid_cons
       const int b = __ffs(redo) - 1;
       redo &= redo - 1;
       const uint32_t off = (uint32_t)(b >> 2) * (kGenThreads * 4) + (b & 3);
-      redo_fp64(p, i_thread + off, tile0 + threadIdx.x * 4 + off);
+      uint32_t ri = i_thread + off;
+      if (RULE == kAllToAllSub) {
+        uint32_t q, r;
+        split_index<RULE>(p, ri, q, r);
+        ri = philox_index<RULE>(p, ri, q, r);
+      }
+      redo_fp64(p, ri, tile0 + threadIdx.x * 4 + off);
     }
   } else {
     for (int k = 0; k < kGenGroups * 4; ++k) {
@@ -287,7 +308,7 @@ __global__ void __launch_bounds__(kGenThreads) generate_kernel(const __grid_cons
       uint32_t quo, rem, s, t, dly;
       float wgt;
       split_index<RULE>(p, i, quo, rem);
-      const Philox4 rnd = philox_stream<true>(i, 0u, p.rng);
+      const Philox4 rnd = philox_stream<true>(philox_index<RULE>(p, i, quo, rem), 0u, p.rng);
       rule_coords<RULE>(p, i, quo, rem, rnd.x, rnd.y, s, t);
       if (ARR) map_nodes(p, s, t);
       draw_weight_delay(rnd.z, rnd.w, p.syn, wgt, dly);
@@ -333,22 +354,24 @@ __global__ void __launch_bounds__(kBernThreads) bernoulli_trials_kernel(const __
   if (q0 < p.n_pairs) {
     const uint64_t c0 = q0 >> 2;
     if (T32) {
-      // mask built from the carry flag of (T - 1) - word, which is set iff the subtraction does not borrow, i.e. iff
-      // word < T (T >= 1 here): m = 2 m + (word < T), two instructions per trial; trials are taken from the last to the
-      // first so that trial k ends up in bit k
-      const uint32_t t = (uint32_t)p.threshold - 1u;
+      // The COMPLEMENT of the mask is built from the carry-out of the addition word + (2^32 - T), which is 1 iff word >= T
+      // (1 <= T < 2^32 here): m' = 2 m' + (word >= T), two instructions per trial, one complement at the end; trials are
+      // taken from the last to the first so that trial k ends up in bit k.  add.cc / addc rather than sub.cc / addc: PTX
+      // defines the carry-out of add.cc and that addc adds it; it does not say what addc sees after a sub.cc.
+      const uint32_t neg_t = 0u - (uint32_t)p.threshold;
 #pragma unroll
       for (int j = kBernTrialsPerThread / 4 - 1; j >= 0; --j) {
         const uint64_t c = c0 + j;
         const Philox4 r = philox_stream<false>((uint32_t)c, (uint32_t)(c >> 32), p.rng);
         asm("{\n .reg .u32 d;\n"
-            " sub.cc.u32 d, %5, %1;\n addc.u32 %0, %0, %0;\n"
-            " sub.cc.u32 d, %5, %2;\n addc.u32 %0, %0, %0;\n"
-            " sub.cc.u32 d, %5, %3;\n addc.u32 %0, %0, %0;\n"
-            " sub.cc.u32 d, %5, %4;\n addc.u32 %0, %0, %0;\n}"
+            " add.cc.u32 d, %1, %5;\n addc.u32 %0, %0, %0;\n"
+            " add.cc.u32 d, %2, %5;\n addc.u32 %0, %0, %0;\n"
+            " add.cc.u32 d, %3, %5;\n addc.u32 %0, %0, %0;\n"
+            " add.cc.u32 d, %4, %5;\n addc.u32 %0, %0, %0;\n}"
             : "+r"(m)
-            : "r"(r.w), "r"(r.z), "r"(r.y), "r"(r.x), "r"(t));
+            : "r"(r.w), "r"(r.z), "r"(r.y), "r"(r.x), "r"(neg_t));
       }
+      m = ~m;
     } else {
 #pragma unroll
       for (int j = 0; j < kBernTrialsPerThread / 4; ++j) {

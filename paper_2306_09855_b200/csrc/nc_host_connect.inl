@@ -106,9 +106,11 @@ extern "C" {
 static int connect_core(nc_context* c, const uint32_t* src_nodes, nc_range src, const uint32_t* tgt_nodes, nc_range tgt,
                         nc_rule rule, const nc_rule_params* params, const nc_syn_spec* syn, uint64_t seed,
                         const float* weights = nullptr, const double* delays_ms = nullptr, uint64_t n_values = 0,
-                        bool with_values = false, bool sub = false, uint64_t sub_first = 0, uint64_t sub_count = 0) {
+                        bool with_values = false, bool sub = false, uint64_t sub_first = 0, uint64_t sub_count = 0,
+                        uint32_t sub_w = 0, uint32_t sub_off = 0) {
   // sub: create only connections sub_first .. sub_first + sub_count - 1 of the call (a shard's owned index sub-range; the
-  // caller guarantees a rule whose indexes it may cut, no value arrays, no rule flags)
+  // caller guarantees a rule whose indexes it may cut, no value arrays, no rule flags).  sub_w > 0 (all_to_all only): the
+  // sub_count = N_src * sub_w connections whose target is one of columns sub_off .. sub_off + sub_w - 1 instead, row by row
   if (!c) return NC_ERR_INVALID_ARG;
   if (c->broken) return fail(c, NC_ERR_STATE, "nc_connect: a failed in-place organisation left this context without connections; destroy it");
   if (c->finalized) return fail(c, NC_ERR_STATE, "nc_connect after nc_finalize");
@@ -250,7 +252,9 @@ static int connect_core(nc_context* c, const uint32_t* src_nodes, nc_range src, 
   gp.t0 = tgt.first;
   gp.n_tgt = tgt.count;
   gp.K = (uint32_t)K;
-  gp.div = rule == NC_ALL_TO_ALL ? tgt.count : (rule == NC_FIXED_INDEGREE || rule == NC_FIXED_OUTDEGREE) ? (uint32_t)K : 1u;
+  gp.div = rule == NC_ALL_TO_ALL ? (sub_w ? sub_w : tgt.count) : (rule == NC_FIXED_INDEGREE || rule == NC_FIXED_OUTDEGREE) ? (uint32_t)K : 1u;
+  gp.sub_w = rule == NC_ALL_TO_ALL ? sub_w : 0u;
+  gp.sub_off = sub_off;
   gp.div_magic = make_div_magic(gp.div);
   const uint32_t seed_lo = (uint32_t)(seed & 0xffffffffull), seed_hi = (uint32_t)(seed >> 32);
   gp.rng = make_philox_stream(seed_lo, seed_hi, c->n_proj, 0u);  // D2: synapse stream
@@ -331,7 +335,7 @@ static int connect_core(nc_context* c, const uint32_t* src_nodes, nc_range src, 
       cudaError_t e;
       switch (rule) {
         case NC_ONE_TO_ONE: e = launch_generate<kOneToOne>(c, gp); break;
-        case NC_ALL_TO_ALL: e = launch_generate<kAllToAll>(c, gp); break;
+        case NC_ALL_TO_ALL: e = gp.sub_w ? launch_generate<kAllToAllSub>(c, gp) : launch_generate<kAllToAll>(c, gp); break;
         case NC_FIXED_INDEGREE: e = launch_generate<kFixedIndegree>(c, gp); break;
         case NC_FIXED_OUTDEGREE: e = launch_generate<kFixedOutdegree>(c, gp); break;
         default: e = launch_generate<kFixedTotalNumber>(c, gp); break;
@@ -455,6 +459,7 @@ static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, 
                         bool with_values = false) {
   if (!c || !c->sharded || c->broken || c->finalized)  // not sharded, or let the ordinary path report the state
     return connect_core(c, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed, weights, delays_ms, n_values, with_values);
+  // (all_to_all, whose owned part is a strip of columns, follows below.)
   // Rules whose target is the slow deterministic coordinate of the index (one_to_one: t = t0 + i; fixed_indegree:
   // t = t0 + i div K) over a target RANGE: the connections this shard owns are one contiguous index sub-range of the call,
   // generated directly into the storage -- no staging, no filter, no redundant draws ("each GPU generates the
@@ -469,36 +474,61 @@ static int connect_impl(nc_context* c, const uint32_t* src_nodes, nc_range src, 
     if (rc != NC_OK) return rc;
     return connect_core(c, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed, nullptr, nullptr, 0, false, true, first, count);
   }
+  // all_to_all over a target RANGE: the owned connections are the strip of owned target columns of every row, generated
+  // directly with the full call's indexes for the random numbers (kAllToAllSub) -- no staging, no filter, no redundant draws
+  if (rule == NC_ALL_TO_ALL && !tgt_nodes && !with_values && c->rule_flags == 0 && params && src.count > 0 && tgt.count > 0 &&
+      (uint64_t)tgt.first + tgt.count <= c->n_nodes) {
+    const uint64_t own_lo = std::max<uint64_t>(c->shard_first, tgt.first);
+    const uint64_t own_hi = std::min<uint64_t>((uint64_t)c->shard_first + c->shard_count, (uint64_t)tgt.first + tgt.count);
+    const uint32_t w = own_hi > own_lo ? (uint32_t)(own_hi - own_lo) : 0u;
+    const int rc = flush_shard(c);  // what is staged comes before this call in creation order
+    if (rc != NC_OK) return rc;
+    return connect_core(c, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed, nullptr, nullptr, 0, false, true, 0,
+                        (uint64_t)src.count * w, w, w ? (uint32_t)(own_lo - tgt.first) : 0u);
+  }
   // swap in the staging storage: the generators append the full projection behind what is already staged
-  std::vector<void*> real_blocks;
-  real_blocks.swap(c->blocks);
-  c->blocks.swap(c->stage_blocks);
-  uint64_t* real_table = c->d_table;
-  const size_t real_cap = c->table_cap;
-  const uint64_t real_n = c->n_conns;
-  c->d_table = c->stage_table;
-  c->table_cap = c->stage_cap;
-  c->n_conns = c->stage_n;
-  const uint32_t proj_before = c->n_proj;
-  const uint64_t stage_start = c->stage_n;
-  const int rc = connect_core(c, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed, weights, delays_ms, n_values, with_values);
-  c->stage_blocks.swap(c->blocks);
-  c->stage_table = c->d_table;
-  c->stage_cap = c->table_cap;
-  c->stage_n = c->n_conns;
-  c->blocks.swap(real_blocks);
-  c->d_table = real_table;
-  c->table_cap = real_cap;
-  c->n_conns = real_n;
+  auto staged_attempt = [&]() -> int {
+    std::vector<void*> real_blocks;
+    real_blocks.swap(c->blocks);
+    c->blocks.swap(c->stage_blocks);
+    uint64_t* real_table = c->d_table;
+    const size_t real_cap = c->table_cap;
+    const uint64_t real_n = c->n_conns;
+    c->d_table = c->stage_table;
+    c->table_cap = c->stage_cap;
+    c->n_conns = c->stage_n;
+    const uint32_t proj_before = c->n_proj;
+    const uint64_t stage_start = c->stage_n;
+    const int rc = connect_core(c, src_nodes, src, tgt_nodes, tgt, rule, params, syn, seed, weights, delays_ms, n_values, with_values);
+    c->stage_blocks.swap(c->blocks);
+    c->stage_table = c->d_table;
+    c->stage_cap = c->table_cap;
+    c->stage_n = c->n_conns;
+    c->blocks.swap(real_blocks);
+    c->d_table = real_table;
+    c->table_cap = real_cap;
+    c->n_conns = real_n;
+    if (rc == NC_OK && c->n_proj > proj_before) c->stage_pending.push_back({proj_before, stage_start});
+    return rc;
+  };
+  int rc = staged_attempt();
+  if (rc == NC_ERR_CAPACITY && c->stage_n > 0) {
+    // the full call did not fit BEHIND what earlier calls left staged (connect_core bounds staged + new by 2^32 - 1): filter
+    // those first -- a failed call changes nothing -- and give this one the whole staging range
+    const int frc = flush_shard(c);
+    if (frc != NC_OK) return frc;
+    rc = staged_attempt();
+  }
   if (rc != NC_OK) return rc;
-  if (c->n_proj > proj_before) c->stage_pending.push_back({proj_before, stage_start});
   return c->stage_n >= kShardFlush ? flush_shard(c) : NC_OK;
 }
 
 int nc_set_shard(nc_context* c, uint32_t first, uint32_t count) {
   if (!c) return NC_ERR_INVALID_ARG;
   if (c->finalized || c->n_conns || c->n_proj) return fail(c, NC_ERR_STATE, "nc_set_shard: only before the first nc_connect*");
-  if (c->cfg.flags & NC_FLAG_ORGANISE_COPASS) {}  // any organisation works: the filter runs before it
+  // one definition of the owned range for the device filter (32-bit t - first < count) and the direct sub-range path
+  // (64-bit clamp): ids first .. first + count - 1 without wrapping
+  if ((uint64_t)first + count > (1ull << 32)) return fail(c, NC_ERR_INVALID_ARG, "nc_set_shard: first + count exceeds 2^32");
   c->sharded = true;
   c->shard_first = first;
   c->shard_count = count;

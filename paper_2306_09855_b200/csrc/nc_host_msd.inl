@@ -23,6 +23,14 @@ cudaStream_t msd_lane_stream(int device, int lane) {
   return s;
 }
 
+template <typename F>
+struct AtExit {  // runs f when the scope is left, whichever return leaves it
+  F f;
+  ~AtExit() { f(); }
+};
+template <typename F>
+AtExit(F) -> AtExit<F>;
+
 struct MsdLane {
   cudaStream_t st = nullptr;
   uint4* tmp[2] = {nullptr, nullptr};    // intermediate records of the bucket being sorted (the second one: three or more passes)
@@ -93,7 +101,10 @@ int sort_msd_and_index(nc_context* c) {
   c->s_d = (uint16_t*)dev_alloc(c, (size_t)n * 2);
   c->perm = (uint32_t*)dev_alloc(c, (size_t)n * 4);
   MsdLane lanes[kMsdMaxLanes];
+  bool scratch_dropped = false;
   auto drop_scratch = [&]() {
+    if (scratch_dropped) return;
+    scratch_dropped = true;
     dev_free_later(c, recs); dev_free_later(c, dig); dev_free_later(c, counts); dev_free_later(c, offs);
     dev_free_later(c, chunk); dev_free_later(c, d_key_base); dev_free_later(c, done);
     for (MsdLane& l : lanes) {
@@ -101,9 +112,28 @@ int sort_msd_and_index(nc_context* c) {
       dev_free_later(c, l.counts); dev_free_later(c, l.chunk_base);
     }
   };
+  // Every way out of this function -- the error returns in the middle of the bucket loop as well -- first makes c->stream wait
+  // for what was queued on the lane streams, then hands the scratch back.  The lane streams are process-wide: without the
+  // join, what nc_finalize does on c->stream after a failure (releasing s_src / s_tgt / perm) could overtake lane kernels
+  // that still write to them.
+  AtExit lane_guard{[&]() {
+    for (MsdLane& l : lanes) {
+      if (!l.st) continue;
+      cudaEvent_t ev = nullptr;
+      bool joined = false;
+      if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) == cudaSuccess) {
+        joined = cudaEventRecord(ev, l.st) == cudaSuccess && cudaStreamWaitEvent(c->stream, ev, 0) == cudaSuccess;
+        cudaEventDestroy(ev);
+      }
+      if (!joined) {
+        cudaStreamSynchronize(l.st);
+        cudaGetLastError();
+      }
+    }
+    drop_scratch();
+  }};
   if (!recs || !dig || !counts || !offs || !chunk || !d_key_base || !done || !c->s_src || !c->s_tgt || !c->s_w || !c->s_d ||
       !c->perm) {
-    drop_scratch();
     return fail(c, NC_ERR_OOM, "out of device memory in nc_finalize");
   }
   cudaStream_t side = msd_lane_stream(c->device, 0);

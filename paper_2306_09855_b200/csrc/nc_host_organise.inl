@@ -312,11 +312,15 @@ int launch_scatter_pass(nc_context* c, const ScatterParams& sp, uint32_t n_tiles
 }
 
 // NC_FLAG_SORT_BULK: the same pass as a persistent kernel fed by cp.async.bulk (nc_sort_bulk.cuh), one CTA per SM.
-// Checked once per context, on its device: whether the bulk kernel may take ranks from returning shared atomics.
+// Ranks among equal digits come from ballots (defined behaviour) unless NC_ATOMIC_RANK=1 asks for the faster form that takes
+// them from the return values of one shared atomicAdd per record.  That form rests on same-address lanes of one instruction
+// being served in ascending lane order, which no document promises: it is therefore never a default, and even when asked for
+// it is only used after atomic_lane_order_kernel has seen the order hold on this device (once per context; a sampling check,
+// not a proof -- a stable sort is only guaranteed with ballots).
 int atomic_rank_usable(nc_context* c) {
   if (c->atomic_rank >= 0) return NC_OK;
-  const char* e = getenv("NC_BULK_BALLOT_RANK");
-  if (e && atoi(e) != 0) {
+  const char* e = getenv("NC_ATOMIC_RANK");
+  if (!(e && atoi(e) != 0)) {
     c->atomic_rank = 0;
     return NC_OK;
   }

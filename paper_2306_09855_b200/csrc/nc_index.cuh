@@ -15,27 +15,7 @@ constexpr int kScanThreads = 256;
 constexpr int kScanItems = 16;
 constexpr int kScanChunk = kScanThreads * kScanItems;
 
-__device__ __forceinline__ uint32_t block_exclusive_scan_256(uint32_t v, uint32_t* warp_tmp /*[8]*/, uint32_t& total) {
-  uint32_t inc = v;
-#pragma unroll
-  for (int d = 1; d < 32; d <<= 1) {
-    const uint32_t t = __shfl_up_sync(0xffffffffu, inc, d);
-    if (lane_id() >= (uint32_t)d) inc += t;
-  }
-  __syncthreads();  // protect warp_tmp against a previous use
-  if (lane_id() == 31) warp_tmp[threadIdx.x >> 5] = inc;
-  __syncthreads();
-  uint32_t base = 0, tot = 0;
-#pragma unroll
-  for (uint32_t w = 0; w < kScanThreads / 32; ++w) {
-    const uint32_t t = warp_tmp[w];
-    if (w < (threadIdx.x >> 5)) base += t;
-    tot += t;
-  }
-  total = tot;
-  return base + inc - v;
-}
-
+// CTA-wide exclusive scan of one value per thread (THREADS threads; every thread calls it); total = the sum over the CTA.
 template <int THREADS>
 __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t* warp_tmp /*[THREADS / 32]*/, uint32_t& total) {
   uint32_t inc = v;
@@ -88,7 +68,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_partials_kernel(uint32_t* _
     const uint64_t idx = base + threadIdx.x;
     const uint32_t v = idx < n_partial ? partial[idx] : 0u;
     uint32_t tot;
-    const uint32_t ex = block_exclusive_scan_256(v, warp_tmp, tot);
+    const uint32_t ex = block_exclusive_scan<256>(v, warp_tmp, tot);
     if (idx < n_partial) partial[idx] = (uint32_t)run + ex;
     run += tot;
   }
@@ -108,7 +88,7 @@ __global__ void __launch_bounds__(kScanThreads) scan_downsweep_kernel(const uint
     s += v[i];
   }
   uint32_t tot;
-  uint32_t ex = block_exclusive_scan_256(s, warp_tmp, tot) + partial[blockIdx.x];
+  uint32_t ex = block_exclusive_scan<256>(s, warp_tmp, tot) + partial[blockIdx.x];
 #pragma unroll
   for (int i = 0; i < kScanItems; ++i) {
     if (base + i < n) out[base + i] = ex;
@@ -275,7 +255,7 @@ __global__ void __launch_bounds__(kHeadThreads) index_scatter_kernel(const Keys 
     }
   }
   uint32_t tot;
-  uint32_t g = block_exclusive_scan_256(c, warp_tmp, tot) + tile_head_off[blockIdx.x];
+  uint32_t g = block_exclusive_scan<256>(c, warp_tmp, tot) + tile_head_off[blockIdx.x];
   if (base >= n) return;
   const uint32_t dmask = (1u << delay_bits) - 1u;
   KeyT prev = prev0;
@@ -367,7 +347,7 @@ __global__ void __launch_bounds__(kHeadThreads) index_scatter_soa_kernel(const u
   heads &= live;
   first_of_source &= live;
   uint32_t tot;
-  uint32_t g = block_exclusive_scan_256(__popc(heads), warp_tmp, tot) + tile_head_off[blockIdx.x];
+  uint32_t g = block_exclusive_scan<256>(__popc(heads), warp_tmp, tot) + tile_head_off[blockIdx.x];
   uint32_t m = heads;
   while (m) {
     const int i = __ffs(m) - 1;

@@ -60,7 +60,10 @@ def test_config0_tiny_full_parity(nc_mod, oracle_mod, B):
 
 @pytest.mark.parametrize("rule,scale", [("one_to_one", 1.0), ("all_to_all", 0.15), ("fixed_indegree", 0.3),
                                         ("fixed_outdegree", 0.25), ("fixed_total_number", 0.3),
-                                        ("pairwise_bernoulli", 0.4)])
+                                        ("pairwise_bernoulli", 0.4),
+                                        # BASELINE.json configs[1] at its full size, every connection against the oracle:
+                                        # 10^8, 2 * 10^7 and 4 * 10^7 connections
+                                        ("all_to_all", 1.0), ("fixed_outdegree", 1.0), ("fixed_total_number", 1.0)])
 def test_config1_rule_sweep_parity(nc_mod, oracle_mod, rule, scale):
     net = WL.config1_rule(rule, scale=scale)
     rep, _ = PU.full_parity(net, oracle_mod, nc_mod)
@@ -97,14 +100,21 @@ def test_onesweep_lookback_variant_parity(nc_mod, oracle_mod):
         assert rep["n"] > 300_000
 
 
-def test_bulk_fed_persistent_variant_parity(nc_mod, oracle_mod):
+def test_bulk_fed_persistent_variant_parity(nc_mod, oracle_mod, monkeypatch):
     """NC_FLAG_SORT_BULK: every digit pass as a persistent kernel fed by cp.async.bulk (nc_sort_bulk.cuh): first pass from
     the SoA slices of the storage blocks (B a multiple of the tile) or through the default kernel (odd B), middle
-    passes with one bulk store per digit run, last pass into the final arrays; ragged last tile; several blocks."""
-    for net, B in ((WL.config2_microcircuit(scale=0.06), 0), (WL.config1_rule("fixed_indegree", scale=0.2), 1 << 16),
-                   (WL.config1_rule("fixed_total_number", scale=0.05), 100_003), (WL.config0_tiny(), 64)):
-        rep, _ = PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_BULK, B=B)
-        assert rep["n"] >= 1000
+    passes with one bulk store per digit run, last pass into the final arrays; ragged last tile; several blocks.  Ranks
+    from ballots (the default) and from returning shared atomics (NC_ATOMIC_RANK=1, opt-in)."""
+    for atomic in (None, "1"):
+        if atomic is None:
+            monkeypatch.delenv("NC_ATOMIC_RANK", raising=False)
+        else:
+            monkeypatch.setenv("NC_ATOMIC_RANK", atomic)
+        for net, B in ((WL.config2_microcircuit(scale=0.06), 0), (WL.config1_rule("fixed_indegree", scale=0.2), 1 << 16),
+                       (WL.config1_rule("fixed_total_number", scale=0.05), 100_003), (WL.config0_tiny(), 64)):
+            rep, _ = PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_BULK, B=B)
+            assert rep["n"] >= 1000
+    monkeypatch.delenv("NC_ATOMIC_RANK", raising=False)
 
 
 def test_bucket_first_variant_parity(nc_mod, oracle_mod, monkeypatch):
@@ -124,6 +134,10 @@ def test_bucket_first_variant_parity(nc_mod, oracle_mod, monkeypatch):
             rep, _ = PU.full_parity(net, oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_BUCKETS, B=B)
             assert rep["n"] >= 1000
     monkeypatch.delenv("NC_BUCKET_LANES")
+    monkeypatch.setenv("NC_ATOMIC_RANK", "1")  # opt-in: ranks from returning shared atomics in the persistent bucket kernel
+    rep, _ = PU.full_parity(WL.config2_microcircuit(scale=0.06), oracle_mod, nc_mod, flags=nc_mod.FLAG_SORT_BUCKETS)
+    assert rep["n"] >= 1000
+    monkeypatch.delenv("NC_ATOMIC_RANK")
     # 16 nodes, delays up to 15 steps: 4 delay bits + 1 -> one in-bucket pass
     net = WL.Network("narrow", [16])
     net.projections = [WL.Projection(0, 0, "fixed_total_number", degree_or_total=100_000, weight=W,
@@ -446,7 +460,8 @@ def test_full_size_config4_large_bernoulli(nc_mod, oracle_mod):
     """configs[4]: 200,000 nodes, 4 x pairwise_bernoulli p = 0.025 over 4e10 pairs + fixed_outdegree K = 500.
     Bernoulli projections: the count is within 5 sigma of the binomial, pairs ascend in q (D4), every sampled pair
     is one the oracle's trial stream accepts and carries the oracle's weight and delay for that q, and the accepted
-    set of the first 200,000 pairs of every projection is exactly the oracle's."""
+    set inside windows of 200,000 pairs (the first and last pairs of every projection, both sides of q = 2^32, 2^33, 2^34)
+    is exactly the oracle's."""
     net = WL.config4_large_bernoulli()
     g = nc_mod.NC(dt_ms=net.dt_ms)
     firsts = [g.create_population(p) for p in net.populations]
@@ -461,6 +476,7 @@ def test_full_size_config4_large_bernoulli(nc_mod, oracle_mod):
     n = g.num_connections()
     starts = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
     bern_checked = bern_mism = 0
+    win_count = win_pairs = win_accepted = 0
     for pj, pr in enumerate(net.projections):
         ns, nt = net.populations[pr.src_pop], net.populations[pr.tgt_pop]
         s0, t0 = firsts[pr.src_pop], firsts[pr.tgt_pop]
@@ -479,6 +495,12 @@ def test_full_size_config4_large_bernoulli(nc_mod, oracle_mod):
         assert np.array_equal(q[q < 200_000], np.array(want, dtype=np.int64))
         # every 64th accepted pair of the projection, streamed: the pair index q rebuilt from (source, target) must
         # ascend, be one the oracle's trial stream accepts, and carry the oracle's weight and delay for that q
+        # completeness, not only soundness: inside windows of 200,000 pairs -- the first pairs, both sides of q = 2^32, 2^33
+        # and 2^34 (where the 64-bit counter path, the mask words and the tile counts change regime) and the last pairs of
+        # the projection -- the device's accepted set must be EXACTLY the oracle's (a dropped pair fails here)
+        n_pairs, WIN = ns * nt, 200_000
+        wins = [0, n_pairs - WIN] + [c - WIN // 2 for c in (2**32, 2**33, 2**34) if c + WIN // 2 <= n_pairs]
+        got_win = {w0: [] for w0 in wins}
         chunk = 1 << 26
         last_q = -1
         for a0 in range(int(starts[pj]), int(starts[pj + 1]), chunk):
@@ -487,6 +509,10 @@ def test_full_size_config4_large_bernoulli(nc_mod, oracle_mod):
             q = (got["source"].astype(np.int64) - s0) * nt + (got["target"].astype(np.int64) - t0)
             assert q[0] > last_q and np.all(np.diff(q) > 0) and q[-1] < ns * nt
             last_q = int(q[-1])
+            for w0 in wins:
+                lo, hi = np.searchsorted(q, [w0, w0 + WIN])
+                if hi > lo:
+                    got_win[w0].append(q[lo:hi].copy())
             sel = np.arange(0, c, 64)
             want = oracle_mod.eval_synapses((s0, ns), (t0, nt), WL.RULE_IDS[pr.rule], 0, pr.p, pr.weight, pr.delay_ms,
                                             pr.seed, pj, net.dt_ms, q[sel])
@@ -500,11 +526,24 @@ def test_full_size_config4_large_bernoulli(nc_mod, oracle_mod):
             assert np.all(np.abs(dd[bad]) == 1) and np.all(want["boundary"][bad] == 1)
             bern_checked += sel.size
             bern_mism += bad.size
+        for w0 in wins:
+            idx = np.arange(w0, w0 + WIN, dtype=np.uint64)
+            acc = oracle_mod.eval_synapses((s0, ns), (t0, nt), WL.RULE_IDS[pr.rule], 0, pr.p, pr.weight, pr.delay_ms, pr.seed,
+                                           pj, net.dt_ms, idx)["accepted"]
+            want_q = idx[acc == 1].astype(np.int64)
+            have_q = np.concatenate(got_win[w0]) if got_win[w0] else np.zeros(0, np.int64)
+            assert np.array_equal(have_q, want_q), f"projection {pj}: accepted pairs in [{w0}, {w0 + WIN}) differ from the oracle's"
+            win_pairs += WIN
+            win_accepted += int(want_q.size)
+        win_count += len(wins)
     rep = _check_sampled_synapses(g, net, firsts, oracle_mod, starts, stride=4)  # the fixed_outdegree projection
     assert rep["checked"] >= 20_000_000
     _report("c4_sampled_outdegree", rep)
     assert bern_checked >= 15_000_000 and bern_mism <= math.ceil(1e-7 * bern_checked)
     _report("c4_sampled_bernoulli", {"checked": int(bern_checked), "delay_mismatches": int(bern_mism)})
+    assert win_count >= 4 * 2 + 3 + 1 + 1  # head and tail of four projections; 2^32 in three of them, 2^33 and 2^34 in the largest
+    _report("c4_bernoulli_exact_windows", {"windows": int(win_count), "pairs_tried": int(win_pairs),
+                                           "accepted_in_windows": int(win_accepted), "set_differences": 0})
     _check_organised_chunked(g, n, net.n_nodes)
     g.close()
 

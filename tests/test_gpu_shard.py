@@ -114,7 +114,7 @@ def test_fixed_indegree_and_one_to_one_shards_take_the_direct_path(nc_mod, oracl
             b.connect((0, 300), (500, 900), R["fixed_total_number"], degree_or_total=20000, weight=W, delay_ms=D, seed=3)  # staged
             b.connect((100, 1900), (100, 1900), R["one_to_one"], weight=W, delay_ms=D, seed=4)                              # direct
             b.connect((0, 2000), (650, 100), R["fixed_indegree"], degree_or_total=33, weight=W, delay_ms=D, seed=5)         # direct
-            b.connect((0, 50), (0, 2000), R["all_to_all"], weight=W, delay_ms=D, seed=6)                                    # staged
+            b.connect((0, 50), (0, 2000), R["all_to_all"], weight=W, delay_ms=D, seed=6)                                    # direct (strip of owned columns)
         n = o.num_connections()
         assert g.num_connections() == n and n > 0
         scale = PU.scale_per_connection([22.0] * (len(net.projections) + 4), o)
@@ -127,3 +127,65 @@ def test_fixed_indegree_and_one_to_one_shards_take_the_direct_path(nc_mod, oracl
         PU.compare_index(g.read_index(), o.index(), "index")
         g.close()
         o.close()
+
+
+def test_set_shard_refuses_a_range_that_wraps(nc_mod):
+    """first + count beyond 2^32 would make the device filter (32-bit t - first < count) own ids below `first` as well while
+    the direct sub-range path clamps: one definition of the owned range, so the call is refused."""
+    g = nc_mod.NC(dt_ms=0.1)
+    g.create_population(100)
+    with pytest.raises(nc_mod.NCError) as e:
+        g.set_shard(2**32 - 10, 11)
+    assert e.value.code == nc_mod.ERR_INVALID_ARG
+    g.set_shard(2**32 - 10, 10)  # ends exactly at 2^32: fine (owns nothing of 100 nodes)
+    g.connect((0, 100), (0, 100), WL.RULE_IDS["all_to_all"], weight=(1.0, 0.0, -INF, INF), delay_ms=(1.0, 0.0, -INF, INF))
+    assert g.num_connections() == 0
+    g.close()
+
+
+def test_a_full_size_call_fits_behind_staged_leftovers(nc_mod, oracle_mod):
+    """A legal call (<= 2^32 - 1 connections) used to fail with NC_ERR_CAPACITY in a sharded context when earlier calls were
+    still staged (staged + new > 2^32 - 1).  Now the staged calls are filtered first.  fixed_outdegree with 65,535 sources of
+    out-degree 65,535 = 2^32 - 131,071 connections (staged in full: its targets are drawn) behind a staged call of 200,000;
+    the shard owns 16 targets.  Checked: the owned count against the binomial; for 40 sources, the owned connections of the
+    source are exactly those the oracle's per-synapse function gives over ALL 65,535 indexes of that source, in index order,
+    with its weights and delays."""
+    import torch
+    torch.cuda.empty_cache()  # what earlier tests left in torch's caching allocator counts as used in mem_get_info
+    free, _ = torch.cuda.mem_get_info()
+    if free < 80 * 2**30:
+        pytest.skip("needs ~65 GB of free device memory for the staged full call")
+    M, first, count = 65_535, 100, 16
+    W, D = (20.0, 2.0, 0.0, INF), (1.5, 0.75, 0.1, INF)
+    R = WL.RULE_IDS
+    g = nc_mod.NC(dt_ms=0.1)
+    g.create_population(M)
+    g.set_shard(first, count)
+    g.connect((0, M), (0, M), R["fixed_total_number"], degree_or_total=200_000, weight=W, delay_ms=D, seed=11)  # staged, not yet filtered
+    g.set_connection_attributes(1)
+    g.connect((0, M), (0, M), R["fixed_outdegree"], degree_or_total=M, weight=W, delay_ms=D, seed=12)
+    n = g.num_connections()
+    mean_small, mean_big = 200_000 * count / M, M * M * count / M
+    assert abs(n - mean_small - mean_big) < 6 * math.sqrt(mean_small + mean_big)
+    c = g.read_connections(sorted=False)
+    port, _ = g.read_connection_attributes(sorted=False)  # the two calls carry ports 0 and 1: where the second one starts
+    n_small = int((port == 0).sum())
+    assert np.all(np.diff(port.astype(np.int64)) >= 0) and abs(n_small - mean_small) < 6 * math.sqrt(mean_small) + 1
+    big = {k: v[n_small:] for k, v in c.items() if k != "n"}
+    assert np.all((big["target"] >= first) & (big["target"] < first + count)) and np.all(np.diff(big["source"].astype(np.int64)) >= 0)
+    checked = 0
+    for s_id in np.random.default_rng(5).choice(M, size=40, replace=False):
+        lo, hi = np.searchsorted(big["source"], [s_id, s_id + 1])
+        i = np.arange(s_id * M, (s_id + 1) * M, dtype=np.uint64)
+        o = oracle_mod.eval_synapses((0, M), (0, M), R["fixed_outdegree"], M, 0.0, W, D, 12, 1, 0.1, i)
+        own = (o["target"] >= first) & (o["target"] < first + count)
+        assert np.array_equal(o["target"][own], big["target"][lo:hi]), f"source {s_id}: owned targets differ from the oracle's"
+        assert np.all(np.abs(o["weight"][own].astype(np.float64) - big["weight"][lo:hi]) <= 1e-5 * 22.0)
+        dd = o["delay"][own].astype(np.int64) - big["delay"][lo:hi].astype(np.int64)
+        assert np.all((dd == 0) | ((np.abs(dd) == 1) & (o["boundary"][own] == 1)))
+        checked += int(own.sum())
+    assert checked > 400
+    g.finalize()
+    idx = g.read_index()
+    assert int(idx["src_offsets"][-1]) == n
+    g.close()
